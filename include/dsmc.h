@@ -1,0 +1,166 @@
+/*
+ * dsmc.h -- C ABI of the B200-native hot path of arXiv 1211.6234 (Stamps & Ambrose):
+ * periodic long-range dipole field h = W (*) s on an L x L lattice of Heisenberg
+ * spins, batched over R temperature replicas, coupled to a fused checkerboard
+ * Metropolis half-sweep that uses the paper's frozen-field approximation.
+ *
+ * Every step of the path runs in hand-written sm_100a CUDA kernels inside
+ * libdsmc.so; there is no CPU fallback.  The library NEVER allocates device
+ * memory: the caller (PyTorch in this repo) allocates one workspace and lends
+ * it with dsmc_bind().  All calls on one context are ordered on the bound CUDA
+ * stream and asynchronous, except the calls that return data to HOST memory.
+ *
+ * Citations: PAPER.md:<line> = /root/reference/PAPER.md; R<n> = DESIGN.md section 2.
+ *
+ * Notation: N = L*L; site n = (x, y), n = y*L + x; k_B = 1.
+ * External ("canonical") layouts, all fp32, C order:
+ *   W[4][L][L]    components xx, xy, yy, zz;  W[c][rho_y][rho_x], rho = (m - n) mod L
+ *   s[R][3][L][L] unit spins, component planes x, y, z
+ *   h[R][3][L][L] dipole field in lattice units (no factor g)
+ * The internal HBM layout (colour-split, replica-innermost) is the library's
+ * business; see DESIGN.md section 5.
+ *
+ * Energy convention (PAPER.md:150 eq. 11, :160 eq. 12, R7, R8):
+ *   E = -J sum_bonds s.s - sum_n (K2 s_z^2 + K4 s_z^4) + (g/2) sum_n s_n.h_n
+ *
+ * Error behaviour: every int-returning call returns DSMC_OK (0) or a negative
+ * code; no exceptions, no abort, no global state.  dsmc_last_error() returns a
+ * message owned by the context (valid until the next call on that context).
+ */
+#ifndef DSMC_H
+#define DSMC_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dsmc_ctx dsmc_ctx;
+
+enum {
+    DSMC_OK = 0,
+    DSMC_EINVAL = -1, /* bad L/R/T/colour/flag, null pointer                          */
+    DSMC_ESTATE = -2, /* workspace not bound, tensor not built, spins not set         */
+    DSMC_ECUDA = -3,  /* CUDA runtime / launch failure (message kept)                 */
+    DSMC_ENOMEM = -4  /* workspace lent by the caller is too small / host malloc fail */
+};
+
+/* where a caller-supplied buffer lives */
+enum { DSMC_HOST = 0, DSMC_DEVICE = 1 };
+
+/* dsmc_build_tensor methods */
+enum { DSMC_W_IMAGE = 0, DSMC_W_EWALD = 1 };
+
+/* dsmc_halfsweep_ex flags */
+enum {
+    DSMC_REUSE_FIELD = 1 /* skip the field step: reuse h kept from the previous field call of
+                            the same colour (for timing the Metropolis kernel alone)         */
+};
+
+/* dsmc_init_spins modes */
+enum { DSMC_INIT_RANDOM = 0, DSMC_INIT_UP = 1 };
+
+/* Create a context for an L x L lattice (L even, L >= 4: the checkerboard needs even L and
+ * L = 2 makes the +x and -x neighbours coincide) and R >= 1 replicas with couplings J, g = C_D/J,
+ * K2, K4 (same for all replicas; see dsmc_set_anisotropy).  Host-only; touches no GPU state.
+ * *out is owned by the caller and released with dsmc_destroy.                                 */
+int dsmc_create(dsmc_ctx **out, int L, int R, float J, float g, float K2, float K4);
+
+/* Per-replica anisotropy constants (HOST arrays of length R), e.g. BASELINE config 3's two K4
+ * values in one R = 16 batch (eq. 12 with K2 = -K(1-a), K4 = -Ka, R7).            */
+int dsmc_set_anisotropy(dsmc_ctx *ctx, const float *K2_r, const float *K4_r);
+
+/* Bytes of device workspace a context of this shape needs (0 if the shape is invalid).        */
+size_t dsmc_workspace_bytes(int L, int R);
+
+/* Lend `bytes` of DEVICE memory (256-byte aligned) and the CUDA stream (a cudaStream_t passed as
+ * void*, NULL = default stream) every later call runs on.  The context borrows both; the caller
+ * frees the memory after dsmc_destroy.  DSMC_ENOMEM if bytes < dsmc_workspace_bytes(L, R).      */
+int dsmc_bind(dsmc_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream);
+
+/* a0. Build the lattice-summed interaction table once (eq. 1-5):
+ *   W^{ab}(rho) = sum_G T^{ab}(rho + G), T = (delta_ab - 3 rhat_a rhat_b)/r^3, G = (aL, bL);
+ *   W(0) omits G = 0 (self-image term of eq. 2, coefficient 1/2: R2).
+ * method DSMC_W_EWALD: 2-D Ewald split of eq. 3-5 (cutoff_A and tail ignored; converged to fp64
+ *   rounding); DSMC_W_IMAGE: square image cutoff |a|,|b| <= cutoff_A centred on rho reduced to
+ *   (-L/2, L/2], plus the continuum tail if tail != 0 (R6).  fp64 arithmetic on the device,
+ *   rounded once to fp32.                                                                      */
+int dsmc_build_tensor(dsmc_ctx *ctx, int method, int cutoff_A, int tail);
+
+/* Copy the table out / in, canonical layout W[4][L][L]; `where` = DSMC_HOST or DSMC_DEVICE.
+ * dsmc_set_tensor replaces the built table (tests use it to isolate the field kernel).        */
+int dsmc_get_tensor(dsmc_ctx *ctx, float *W_out, int where);
+int dsmc_set_tensor(dsmc_ctx *ctx, const float *W_in, int where);
+
+/* Spins in canonical layout s[R][3][L][L].  set does not renormalise: |s| = 1 is the caller's
+ * contract.  Host variants copy through a staging area inside the workspace; get to HOST
+ * synchronises the stream.                                                                    */
+int dsmc_set_spins(dsmc_ctx *ctx, const float *s, int where);
+int dsmc_get_spins(dsmc_ctx *ctx, float *s, int where);
+
+/* a4. Initial spins on the device: DSMC_INIT_RANDOM = uniform on S^2 from Philox4x32-10 keyed by
+ * (seed; site, replica, tag 1) with the same map as the trial move (R9, R10);
+ * DSMC_INIT_UP = all +z.                                                                      */
+int dsmc_init_spins(dsmc_ctx *ctx, int mode, uint64_t seed);
+
+/* a1. Dipole field of the CURRENT spins (App. A :331-350):
+ *   h_n^x = sum_m [W^xx(rho_nm) s_m^x + W^xy(rho_nm) s_m^y],  h_n^y = sum_m [W^xy s_m^x + W^yy s_m^y],
+ *   h_n^z = sum_m W^zz(rho_nm) s_m^z,   every m including m = n.
+ * colour = 0 / 1: only targets with (x + y) mod 2 == colour; -1: all targets.  The result is
+ * kept in the context for the next half-sweep of that colour.  h_out (nullable) receives the
+ * canonical h[R][3][L][L]; entries of inactive targets are left untouched.                     */
+int dsmc_dipole_field(dsmc_ctx *ctx, int colour, float *h_out, int where);
+
+/* a2. One checkerboard Metropolis half-sweep (PAPER.md:60-72 eq. 7; :98; :102-118; R11-R14):
+ *   colour c = step & 1.  (i) h <- dipole field of colour c from the state at entry (frozen for
+ *   the whole half-sweep).  (ii) for every active site n and replica r, in one fused kernel:
+ *   trial s' uniform on S^2 and u in (0,1) from Philox4x32-10(seed; n, r, step); delta = s' - s;
+ *     dE = -J delta.(sum of 4 nn) - K2 (s'_z^2 - s_z^2) - K4 (s'_z^4 - s_z^4)
+ *          + g [delta.h_n + (1/2) delta.W(0).delta];
+ *   accept  <=>  dE / T_r + ln u < 0;  accepted sites take s'.
+ * T: HOST array of R temperatures, all > 0 (else DSMC_EINVAL); uploaded only when it changes;
+ * NULL reuses the last one.  One sweep (MC step) = steps 2k and 2k+1.            */
+int dsmc_halfsweep(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t step);
+
+/* Same with flags (DSMC_REUSE_FIELD) and parity hooks, both nullable DEVICE
+ * buffers in canonical site order, written at active sites only:
+ *   accept_out[R][L][L] bytes (0/1),  margin_out[R][L][L] floats (dE/T + ln u as the kernel saw it). */
+int dsmc_halfsweep_ex(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t step, int flags,
+                      uint8_t *accept_out, float *margin_out);
+
+/* n_half consecutive half-sweeps (steps first_step .. first_step + n_half - 1) without returning
+ * to the caller in between.                                                                    */
+int dsmc_run(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_step, uint64_t n_half);
+
+/* a3. Observables of the current state, out[R][4] doubles in HOST memory:
+ *   E/N (eq. 11 with a freshly computed full field), m_z = N^-1 sum s^z,
+ *   M_par = (M_x^2 + M_y^2)^(1/2) (eq. 16),
+ *   eta = (2/pi) (N^-1 sum_i (arccos s_i^z - pi/2)^2)^(1/2) (eq. 17, R15).
+ * Synchronises the stream.                                                                      */
+int dsmc_observables(dsmc_ctx *ctx, double *out);
+
+/* Device time in milliseconds of the last field / Metropolis / reduction launches made by the
+ * last dsmc_halfsweep* call, measured with CUDA events on the bound stream when timing was
+ * enabled with dsmc_set_timing(ctx, 1); synchronises.  out[3] = {field, metropolis, total}.      */
+int dsmc_set_timing(dsmc_ctx *ctx, int on);
+int dsmc_last_timing(dsmc_ctx *ctx, float *out_ms);
+
+/* Number of kernels this context has launched since creation (bench.py's gpu_launches).       */
+uint64_t dsmc_launch_count(dsmc_ctx *ctx);
+
+/* Which field kernel runs: 0 = generic (any even L, any R), 1 = tiled (register-tiled,
+ * TMA-staged; needs L % 16 == 0 and R % 4 == 0).  dsmc_select_field_kernel: kind -1 = automatic
+ * (tiled when the shape allows), 0 = force generic, 1 = tiled (DSMC_EINVAL if unsupported).     */
+int dsmc_field_kernel_kind(dsmc_ctx *ctx);
+int dsmc_select_field_kernel(dsmc_ctx *ctx, int kind);
+
+int dsmc_destroy(dsmc_ctx *ctx);
+const char *dsmc_last_error(dsmc_ctx *ctx);
+const char *dsmc_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DSMC_H */

@@ -1,0 +1,6 @@
+"""B200-native hot path of arXiv 1211.6234: dipole field + fused checkerboard Metropolis half-sweep.
+
+`Dsmc` is a thin ctypes binding over libdsmc.so (include/dsmc.h); every step runs in CUDA kernels.
+"""
+from .dsmc import Dsmc, DsmcError, load_library, DSMC_W_IMAGE, DSMC_W_EWALD, \
+    DSMC_REUSE_FIELD, DSMC_INIT_RANDOM, DSMC_INIT_UP  # noqa: F401

@@ -1,0 +1,393 @@
+// dsmc_api.cu -- the C ABI of include/dsmc.h: argument checks, workspace carving, stream-ordered
+// launches.  No device memory is allocated here; no step of the path runs on the host.
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "dsmc_internal.cuh"
+
+namespace {
+
+size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
+
+bool shape_ok(int L, int R) { return L >= 4 && (L & 1) == 0 && L <= 4096 && R >= 1 && R <= 65535; }
+
+int fail(dsmc_ctx *c, int code, const char *msg) {
+    if (c) c->err = msg;
+    return code;
+}
+
+int cuda_fail(dsmc_ctx *c, cudaError_t e, const char *what) {
+    if (c) {
+        c->err = std::string(what) + ": " + cudaGetErrorString(e);
+    }
+    return DSMC_ECUDA;
+}
+
+#define CU(call, what)                                       \
+    do {                                                     \
+        cudaError_t e__ = (call);                            \
+        if (e__ != cudaSuccess) return cuda_fail(ctx, e__, what); \
+    } while (0)
+
+int need_bound(dsmc_ctx *ctx) {
+    if (!ctx) return DSMC_EINVAL;
+    if (!ctx->ws) return fail(ctx, DSMC_ESTATE, "workspace not bound (call dsmc_bind)");
+    return DSMC_OK;
+}
+
+int upload_params(dsmc_ctx *ctx, const float *T) {
+    const int R = ctx->R;
+    if (T) {
+        for (int r = 0; r < R; ++r)
+            if (!(T[r] > 0.0f)) return fail(ctx, DSMC_EINVAL, "temperatures must be > 0");
+        if (!ctx->T_valid || std::memcmp(T, ctx->T.data(), sizeof(float) * R) != 0) {
+            std::memcpy(ctx->T.data(), T, sizeof(float) * R);
+            std::vector<float> inv(R);
+            for (int r = 0; r < R; ++r) inv[r] = 1.0f / T[r];
+            CU(cudaMemcpyAsync(ctx->invT(), inv.data(), sizeof(float) * R, cudaMemcpyHostToDevice, ctx->stream),
+               "upload T");
+            CU(cudaStreamSynchronize(ctx->stream), "upload T sync");  // inv is a stack-lifetime buffer
+            ctx->T_valid = true;
+        }
+    } else if (!ctx->T_valid) {
+        return fail(ctx, DSMC_EINVAL, "T is NULL and no temperatures were set before");
+    }
+    if (ctx->aniso_dirty) {
+        CU(cudaMemcpyAsync(ctx->K2d(), ctx->K2.data(), sizeof(float) * R, cudaMemcpyHostToDevice, ctx->stream),
+           "upload K2");
+        CU(cudaMemcpyAsync(ctx->K4d(), ctx->K4.data(), sizeof(float) * R, cudaMemcpyHostToDevice, ctx->stream),
+           "upload K4");
+        CU(cudaStreamSynchronize(ctx->stream), "upload K sync");
+        ctx->aniso_dirty = false;
+    }
+    return DSMC_OK;
+}
+
+bool use_tiled(const dsmc_ctx *ctx) { return ctx->force_generic ? false : dsmc_tiled_supported(ctx->L, ctx->R); }
+
+int run_field(dsmc_ctx *ctx, int colour) {
+    cudaError_t e;
+    if (use_tiled(ctx))
+        e = launch_field_tiled(ctx->S(), ctx->Wk(), ctx->Hpart(), ctx->H(), ctx->L, ctx->R, colour, ctx->sm_count,
+                               ctx->stream, &ctx->launches);
+    else
+        e = launch_field_generic(ctx->S(), ctx->Wc(), ctx->H(), ctx->L, ctx->R, colour, ctx->stream,
+                                 &ctx->launches);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "dipole field launch");
+    ctx->field_valid[colour] = true;
+    return DSMC_OK;
+}
+
+int after_tensor_change(dsmc_ctx *ctx) {
+    // W(0) for the self term of dE, and the kernel-layout copy for the tiled field kernel
+    const size_t N = (size_t)ctx->L * ctx->L;
+    for (int c = 0; c < 4; ++c)
+        CU(cudaMemcpyAsync(&ctx->w0[c], ctx->Wc() + c * N, sizeof(float), cudaMemcpyDeviceToHost, ctx->stream),
+           "read W(0)");
+    if (dsmc_tiled_supported(ctx->L, ctx->R))
+        CU(launch_make_wk(ctx->Wc(), ctx->Wk(), ctx->L, ctx->stream, &ctx->launches), "W kernel layout");
+    CU(cudaStreamSynchronize(ctx->stream), "tensor sync");
+    ctx->tensor_built = true;
+    ctx->field_valid[0] = ctx->field_valid[1] = false;
+    return DSMC_OK;
+}
+
+}  // namespace
+
+DsmcLayout dsmc_make_layout(int L, int R) {
+    DsmcLayout l;
+    const size_t N = (size_t)L * L, Nh = N / 2;
+    size_t o = 0;
+    l.off_Wc = o; o = align256(o + sizeof(float) * 4 * N);
+    l.off_Wk = o; o = align256(o + sizeof(float) * dsmc_wk_floats(L));
+    l.off_S = o; o = align256(o + sizeof(float) * 6 * Nh * R);
+    l.off_H = o; o = align256(o + sizeof(float) * 6 * Nh * R);
+    l.off_Hpart = o;
+    o = align256(o + (dsmc_tiled_supported(L, R) ? sizeof(float) * DSMC_KS_MAX * 3 * Nh * R : 0));
+    l.off_stage = o; o = align256(o + sizeof(float) * 3 * N * R);
+    l.off_T = o; o = align256(o + sizeof(float) * 3 * R);
+    l.off_obs = o; o = align256(o + sizeof(double) * 8 * R);
+    l.total = o;
+    return l;
+}
+
+extern "C" {
+
+const char *dsmc_version(void) { return "dsmc 0.1 (sm_100a)"; }
+
+int dsmc_create(dsmc_ctx **out, int L, int R, float J, float g, float K2, float K4) {
+    if (!out) return DSMC_EINVAL;
+    *out = nullptr;
+    if (!shape_ok(L, R)) return DSMC_EINVAL;
+    dsmc_ctx *c = new (std::nothrow) dsmc_ctx();
+    if (!c) return DSMC_ENOMEM;
+    c->L = L;
+    c->R = R;
+    c->J = J;
+    c->g = g;
+    c->K2.assign(R, K2);
+    c->K4.assign(R, K4);
+    c->T.assign(R, 0.0f);
+    c->lay = dsmc_make_layout(L, R);
+    *out = c;
+    return DSMC_OK;
+}
+
+int dsmc_set_anisotropy(dsmc_ctx *ctx, const float *K2_r, const float *K4_r) {
+    if (!ctx || !K2_r || !K4_r) return fail(ctx, DSMC_EINVAL, "null argument");
+    ctx->K2.assign(K2_r, K2_r + ctx->R);
+    ctx->K4.assign(K4_r, K4_r + ctx->R);
+    ctx->aniso_dirty = true;
+    return DSMC_OK;
+}
+
+size_t dsmc_workspace_bytes(int L, int R) {
+    if (!shape_ok(L, R)) return 0;
+    return dsmc_make_layout(L, R).total;
+}
+
+int dsmc_bind(dsmc_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream) {
+    if (!ctx || !dev_workspace) return fail(ctx, DSMC_EINVAL, "null argument");
+    if (((uintptr_t)dev_workspace & 255) != 0) return fail(ctx, DSMC_EINVAL, "workspace must be 256-byte aligned");
+    if (bytes < ctx->lay.total) return fail(ctx, DSMC_ENOMEM, "workspace smaller than dsmc_workspace_bytes");
+    cudaPointerAttributes attr;
+    CU(cudaPointerGetAttributes(&attr, dev_workspace), "cudaPointerGetAttributes");
+    if (attr.type != cudaMemoryTypeDevice && attr.type != cudaMemoryTypeManaged)
+        return fail(ctx, DSMC_EINVAL, "workspace is not device memory");
+    int dev = 0;
+    CU(cudaGetDevice(&dev), "cudaGetDevice");
+    CU(cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, dev), "SM count");
+    ctx->ws = (char *)dev_workspace;
+    ctx->ws_bytes = bytes;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    ctx->tensor_built = ctx->spins_set = false;
+    ctx->field_valid[0] = ctx->field_valid[1] = false;
+    ctx->T_valid = false;
+    ctx->aniso_dirty = true;
+    for (int i = 0; i < 3; ++i)
+        if (!ctx->ev[i]) CU(cudaEventCreate(&ctx->ev[i]), "cudaEventCreate");
+    return DSMC_OK;
+}
+
+int dsmc_build_tensor(dsmc_ctx *ctx, int method, int cutoff_A, int tail) {
+    if (int rc = need_bound(ctx)) return rc;
+    if (method != DSMC_W_IMAGE && method != DSMC_W_EWALD) return fail(ctx, DSMC_EINVAL, "unknown method");
+    if (method == DSMC_W_IMAGE && (cutoff_A < 0 || cutoff_A > 4096)) return fail(ctx, DSMC_EINVAL, "bad cutoff");
+    CU(launch_build_tensor(nullptr, ctx->Wc(), ctx->L, method, cutoff_A, tail, ctx->stream, &ctx->launches),
+       "build tensor");
+    return after_tensor_change(ctx);
+}
+
+int dsmc_get_tensor(dsmc_ctx *ctx, float *W_out, int where) {
+    if (int rc = need_bound(ctx)) return rc;
+    if (!W_out) return fail(ctx, DSMC_EINVAL, "null argument");
+    if (!ctx->tensor_built) return fail(ctx, DSMC_ESTATE, "tensor not built");
+    const size_t bytes = sizeof(float) * 4 * (size_t)ctx->L * ctx->L;
+    CU(cudaMemcpyAsync(W_out, ctx->Wc(), bytes, where == DSMC_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice,
+                       ctx->stream),
+       "get tensor");
+    if (where == DSMC_HOST) CU(cudaStreamSynchronize(ctx->stream), "get tensor sync");
+    return DSMC_OK;
+}
+
+int dsmc_set_tensor(dsmc_ctx *ctx, const float *W_in, int where) {
+    if (int rc = need_bound(ctx)) return rc;
+    if (!W_in) return fail(ctx, DSMC_EINVAL, "null argument");
+    const size_t bytes = sizeof(float) * 4 * (size_t)ctx->L * ctx->L;
+    CU(cudaMemcpyAsync(ctx->Wc(), W_in, bytes, where == DSMC_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice,
+                       ctx->stream),
+       "set tensor");
+    return after_tensor_change(ctx);
+}
+
+int dsmc_set_spins(dsmc_ctx *ctx, const float *s, int where) {
+    if (int rc = need_bound(ctx)) return rc;
+    if (!s) return fail(ctx, DSMC_EINVAL, "null argument");
+    const float *src = s;
+    if (where == DSMC_HOST) {
+        CU(cudaMemcpyAsync(ctx->stage(), s, sizeof(float) * 3 * (size_t)ctx->L * ctx->L * ctx->R,
+                           cudaMemcpyHostToDevice, ctx->stream),
+           "spins H2D");
+        src = ctx->stage();
+    }
+    CU(launch_canon_to_internal(src, ctx->S(), ctx->L, ctx->R, ctx->stream, &ctx->launches), "set spins");
+    ctx->spins_set = true;
+    ctx->field_valid[0] = ctx->field_valid[1] = false;
+    return DSMC_OK;
+}
+
+int dsmc_get_spins(dsmc_ctx *ctx, float *s, int where) {
+    if (int rc = need_bound(ctx)) return rc;
+    if (!s) return fail(ctx, DSMC_EINVAL, "null argument");
+    if (!ctx->spins_set) return fail(ctx, DSMC_ESTATE, "spins not set");
+    float *dst = where == DSMC_HOST ? ctx->stage() : s;
+    CU(launch_internal_to_canon(ctx->S(), dst, ctx->L, ctx->R, -1, ctx->stream, &ctx->launches), "get spins");
+    if (where == DSMC_HOST) {
+        CU(cudaMemcpyAsync(s, dst, sizeof(float) * 3 * (size_t)ctx->L * ctx->L * ctx->R, cudaMemcpyDeviceToHost,
+                           ctx->stream),
+           "spins D2H");
+        CU(cudaStreamSynchronize(ctx->stream), "spins D2H sync");
+    }
+    return DSMC_OK;
+}
+
+int dsmc_init_spins(dsmc_ctx *ctx, int mode, uint64_t seed) {
+    if (int rc = need_bound(ctx)) return rc;
+    if (mode != DSMC_INIT_RANDOM && mode != DSMC_INIT_UP) return fail(ctx, DSMC_EINVAL, "unknown init mode");
+    CU(launch_init_spins(ctx->S(), ctx->L, ctx->R, mode, seed, ctx->stream, &ctx->launches), "init spins");
+    ctx->spins_set = true;
+    ctx->field_valid[0] = ctx->field_valid[1] = false;
+    return DSMC_OK;
+}
+
+int dsmc_dipole_field(dsmc_ctx *ctx, int colour, float *h_out, int where) {
+    if (int rc = need_bound(ctx)) return rc;
+    if (colour < -1 || colour > 1) return fail(ctx, DSMC_EINVAL, "colour must be -1, 0 or 1");
+    if (!ctx->tensor_built) return fail(ctx, DSMC_ESTATE, "tensor not built");
+    if (!ctx->spins_set) return fail(ctx, DSMC_ESTATE, "spins not set");
+    for (int q = 0; q < 2; ++q)
+        if (colour < 0 || colour == q)
+            if (int rc = run_field(ctx, q)) return rc;
+    if (h_out) {
+        const size_t bytes = sizeof(float) * 3 * (size_t)ctx->L * ctx->L * ctx->R;
+        float *dst = h_out;
+        if (where == DSMC_HOST) {
+            // inactive entries must stay untouched: bring the caller's buffer in first
+            CU(cudaMemcpyAsync(ctx->stage(), h_out, bytes, cudaMemcpyHostToDevice, ctx->stream), "h H2D");
+            dst = ctx->stage();
+        }
+        CU(launch_internal_to_canon(ctx->H(), dst, ctx->L, ctx->R, colour, ctx->stream, &ctx->launches), "get field");
+        if (where == DSMC_HOST) {
+            CU(cudaMemcpyAsync(h_out, dst, bytes, cudaMemcpyDeviceToHost, ctx->stream), "h D2H");
+            CU(cudaStreamSynchronize(ctx->stream), "h D2H sync");
+        }
+    }
+    return DSMC_OK;
+}
+
+int dsmc_halfsweep_ex(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t step, int flags, uint8_t *accept_out,
+                      float *margin_out) {
+    if (int rc = need_bound(ctx)) return rc;
+    if (!ctx->tensor_built) return fail(ctx, DSMC_ESTATE, "tensor not built");
+    if (!ctx->spins_set) return fail(ctx, DSMC_ESTATE, "spins not set");
+    if (flags & ~DSMC_REUSE_FIELD) return fail(ctx, DSMC_EINVAL, "unknown flag");
+    if (int rc = upload_params(ctx, T)) return rc;
+    const int colour = (int)(step & 1u);
+    if (ctx->timing) CU(cudaEventRecord(ctx->ev[0], ctx->stream), "event");
+    if (!(flags & DSMC_REUSE_FIELD)) {
+        if (int rc = run_field(ctx, colour)) return rc;
+    } else if (!ctx->field_valid[colour]) {
+        return fail(ctx, DSMC_ESTATE, "DSMC_REUSE_FIELD without a field of this colour");
+    }
+    if (ctx->timing) CU(cudaEventRecord(ctx->ev[1], ctx->stream), "event");
+    MetropolisArgs a;
+    a.S = ctx->S();
+    a.H = ctx->H();
+    a.invT = ctx->invT();
+    a.K2 = ctx->K2d();
+    a.K4 = ctx->K4d();
+    a.L = ctx->L;
+    a.R = ctx->R;
+    a.colour = colour;
+    a.J = ctx->J;
+    a.g = ctx->g;
+    a.w0xx = ctx->w0[0];
+    a.w0xy = ctx->w0[1];
+    a.w0yy = ctx->w0[2];
+    a.w0zz = ctx->w0[3];
+    a.seed_lo = (uint32_t)(seed & 0xFFFFFFFFu);
+    a.seed_hi = (uint32_t)(seed >> 32);
+    a.step_lo = (uint32_t)(step & 0xFFFFFFFFu);
+    a.step_hi = (uint32_t)(step >> 32) & 0x7FFFFFFFu;  // bit 31 is the init tag
+    a.accept_out = accept_out;
+    a.margin_out = margin_out;
+    CU(launch_metropolis(a, ctx->stream, &ctx->launches), "metropolis launch");
+    if (ctx->timing) {
+        CU(cudaEventRecord(ctx->ev[2], ctx->stream), "event");
+        ctx->ev_recorded = true;
+    }
+    // the spins of this colour changed: both colours' fields are stale for observables, but the
+    // field of this colour stays "valid" only in the DSMC_REUSE_FIELD (timing) sense
+    ctx->field_valid[1 - colour] = false;
+    return DSMC_OK;
+}
+
+int dsmc_halfsweep(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t step) {
+    return dsmc_halfsweep_ex(ctx, T, seed, step, 0, nullptr, nullptr);
+}
+
+int dsmc_run(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_step, uint64_t n_half) {
+    for (uint64_t k = 0; k < n_half; ++k)
+        if (int rc = dsmc_halfsweep_ex(ctx, k == 0 ? T : nullptr, seed, first_step + k, 0, nullptr, nullptr)) return rc;
+    return DSMC_OK;
+}
+
+int dsmc_observables(dsmc_ctx *ctx, double *out) {
+    if (int rc = need_bound(ctx)) return rc;
+    if (!out) return fail(ctx, DSMC_EINVAL, "null argument");
+    if (!ctx->tensor_built) return fail(ctx, DSMC_ESTATE, "tensor not built");
+    if (!ctx->spins_set) return fail(ctx, DSMC_ESTATE, "spins not set");
+    if (int rc = upload_params(ctx, ctx->T_valid ? nullptr : std::vector<float>(ctx->R, 1.0f).data())) return rc;
+    for (int q = 0; q < 2; ++q)
+        if (int rc = run_field(ctx, q)) return rc;
+    CU(launch_observables(ctx->S(), ctx->H(), ctx->K2d(), ctx->K4d(), ctx->obs(), ctx->L, ctx->R, ctx->J, ctx->g,
+                          ctx->stream, &ctx->launches),
+       "observables launch");
+    std::vector<double> raw(8 * (size_t)ctx->R);
+    CU(cudaMemcpyAsync(raw.data(), ctx->obs(), sizeof(double) * raw.size(), cudaMemcpyDeviceToHost, ctx->stream),
+       "observables D2H");
+    CU(cudaStreamSynchronize(ctx->stream), "observables sync");
+    const double N = (double)ctx->L * ctx->L;
+    for (int r = 0; r < ctx->R; ++r) {
+        const double *s = &raw[8 * (size_t)r];
+        const double mx = s[0] / N, my = s[1] / N;
+        out[4 * r + 0] = (-(double)ctx->J * s[4] - s[5] + 0.5 * (double)ctx->g * s[6]) / N;
+        out[4 * r + 1] = s[2] / N;
+        out[4 * r + 2] = sqrt(mx * mx + my * my);
+        out[4 * r + 3] = (2.0 / 3.14159265358979323846) * sqrt(s[3] / N);
+    }
+    return DSMC_OK;
+}
+
+int dsmc_set_timing(dsmc_ctx *ctx, int on) {
+    if (!ctx) return DSMC_EINVAL;
+    ctx->timing = on ? 1 : 0;
+    ctx->ev_recorded = false;
+    return DSMC_OK;
+}
+
+int dsmc_last_timing(dsmc_ctx *ctx, float *out_ms) {
+    if (int rc = need_bound(ctx)) return rc;
+    if (!out_ms) return fail(ctx, DSMC_EINVAL, "null argument");
+    if (!ctx->ev_recorded) return fail(ctx, DSMC_ESTATE, "no timed half-sweep yet");
+    CU(cudaEventSynchronize(ctx->ev[2]), "event sync");
+    CU(cudaEventElapsedTime(&out_ms[0], ctx->ev[0], ctx->ev[1]), "elapsed");
+    CU(cudaEventElapsedTime(&out_ms[1], ctx->ev[1], ctx->ev[2]), "elapsed");
+    CU(cudaEventElapsedTime(&out_ms[2], ctx->ev[0], ctx->ev[2]), "elapsed");
+    return DSMC_OK;
+}
+
+uint64_t dsmc_launch_count(dsmc_ctx *ctx) { return ctx ? ctx->launches : 0; }
+
+int dsmc_field_kernel_kind(dsmc_ctx *ctx) { return ctx && use_tiled(ctx) ? 1 : 0; }
+
+int dsmc_select_field_kernel(dsmc_ctx *ctx, int kind) {
+    if (!ctx || kind < -1 || kind > 1) return fail(ctx, DSMC_EINVAL, "kind must be -1, 0 or 1");
+    if (kind == 1 && !dsmc_tiled_supported(ctx->L, ctx->R)) return fail(ctx, DSMC_EINVAL, "tiled kernel needs L % 16 == 0, R % 4 == 0");
+    ctx->force_generic = (kind == 0);
+    ctx->field_valid[0] = ctx->field_valid[1] = false;
+    return DSMC_OK;
+}
+
+int dsmc_destroy(dsmc_ctx *ctx) {
+    if (!ctx) return DSMC_EINVAL;
+    for (int i = 0; i < 3; ++i)
+        if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
+    delete ctx;
+    return DSMC_OK;
+}
+
+const char *dsmc_last_error(dsmc_ctx *ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+}  // extern "C"

@@ -1,0 +1,108 @@
+// dsmc_internal.cuh -- context, HBM layout and launcher prototypes shared by the translation
+// units of libdsmc.so.  Not part of the public boundary (include/dsmc.h is).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include <string>
+#include <vector>
+
+#include "../../include/dsmc.h"
+
+// ---------------------------------------------------------------------------------------------
+// Internal HBM layout.  Nh = N/2 sites per colour, Lh = L/2 per row.
+//   site (x, y): colour q = (x + y) & 1, in-row index i = x >> 1, colour-site index a = y*Lh + i
+//   spins  S[q][c][a][r]   c in {x,y,z}, replica r innermost      (6*Nh*R floats)
+//   field  H[q][c][a][r]   same shape
+// Replica-innermost makes every per-site access of the Metropolis kernel a contiguous run of R
+// floats and lets the field kernel fetch 4 replicas of one source with one 128-bit load; the
+// colour split makes the active colour of a half-sweep a dense array and turns the stride-2
+// structure of checkerboard targets into a unit-stride sliding window over W (section 5).
+// ---------------------------------------------------------------------------------------------
+
+#define DSMC_KS_MAX 16  // maximum source split (partial-field slabs) of the tiled field kernel
+
+struct DsmcLayout {
+    size_t off_Wc;     // canonical W fp32 [4][L][L]
+    size_t off_Wk;     // kernel-layout W for the tiled field kernel
+    size_t off_S;      // spins, internal layout
+    size_t off_H;      // field, internal layout (both colours)
+    size_t off_Hpart;  // partial fields [KS][3][Nh][R] of the tiled kernel
+    size_t off_stage;  // canonical staging [R][3][L][L] floats
+    size_t off_T;      // invT[R], K2[R], K4[R] floats
+    size_t off_obs;    // R*8 doubles
+    size_t total;
+};
+
+struct dsmc_ctx {
+    int L, R;
+    float J, g;
+    std::vector<float> K2, K4, T;  // host copies
+    bool aniso_dirty = true, T_valid = false;
+    char *ws = nullptr;
+    size_t ws_bytes = 0;
+    cudaStream_t stream = nullptr;
+    DsmcLayout lay;
+    bool tensor_built = false, spins_set = false;
+    bool field_valid[2] = {false, false};
+    float w0[4] = {0, 0, 0, 0};  // W(0) components (fp32, as stored)
+    bool force_generic = false;
+    int timing = 0;
+    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
+    bool ev_recorded = false;
+    uint64_t launches = 0;
+    int sm_count = 148;
+    std::string err;
+
+    float *Wc() const { return (float *)(ws + lay.off_Wc); }
+    float *Wk() const { return (float *)(ws + lay.off_Wk); }
+    float *S() const { return (float *)(ws + lay.off_S); }
+    float *H() const { return (float *)(ws + lay.off_H); }
+    float *Hpart() const { return (float *)(ws + lay.off_Hpart); }
+    float *stage() const { return (float *)(ws + lay.off_stage); }
+    float *invT() const { return (float *)(ws + lay.off_T); }
+    float *K2d() const { return invT() + R; }
+    float *K4d() const { return invT() + 2 * R; }
+    double *obs() const { return (double *)(ws + lay.off_obs); }
+    size_t Nh() const { return (size_t)L * (L / 2); }
+    size_t plane() const { return Nh() * (size_t)R; }  // floats in one [a][r] plane
+};
+
+DsmcLayout dsmc_make_layout(int L, int R);
+
+// tiled-kernel W layout size in floats (field_tiled.cu)
+size_t dsmc_wk_floats(int L);
+bool dsmc_tiled_supported(int L, int R);
+
+// ---- launchers (each returns the cudaError_t of its launch(es); all async on `st`) ----------
+cudaError_t launch_build_tensor(double *scratch_unused, float *Wc, int L, int method, int A, int tail,
+                                cudaStream_t st, uint64_t *launches);
+cudaError_t launch_make_wk(const float *Wc, float *Wk, int L, cudaStream_t st, uint64_t *launches);
+
+cudaError_t launch_canon_to_internal(const float *canon, float *S, int L, int R, cudaStream_t st,
+                                     uint64_t *launches);
+// colour = -1: both colours; else only that colour's sites are written to canon
+cudaError_t launch_internal_to_canon(const float *S, float *canon, int L, int R, int colour,
+                                     cudaStream_t st, uint64_t *launches);
+
+cudaError_t launch_field_generic(const float *S, const float *Wc, float *H, int L, int R, int colour,
+                                 cudaStream_t st, uint64_t *launches);
+cudaError_t launch_field_tiled(const float *S, const float *Wk, float *Hpart, float *H, int L, int R,
+                               int colour, int sm_count, cudaStream_t st, uint64_t *launches);
+
+struct MetropolisArgs {
+    float *S;
+    const float *H;
+    const float *invT, *K2, *K4;
+    int L, R, colour;
+    float J, g, w0xx, w0yy, w0zz, w0xy;
+    uint32_t seed_lo, seed_hi, step_lo, step_hi;
+    uint8_t *accept_out;  // canonical [R][L][L] or null
+    float *margin_out;    // canonical [R][L][L] or null
+};
+cudaError_t launch_metropolis(const MetropolisArgs &a, cudaStream_t st, uint64_t *launches);
+cudaError_t launch_init_spins(float *S, int L, int R, int mode, uint64_t seed, cudaStream_t st,
+                              uint64_t *launches);
+cudaError_t launch_observables(const float *S, const float *H, const float *K2, const float *K4,
+                               double *obs, int L, int R, float J, float g, cudaStream_t st,
+                               uint64_t *launches);

@@ -1,0 +1,217 @@
+"""Thin Python binding of the C ABI in include/dsmc.h (argument marshalling only).
+
+PyTorch supplies device memory (one workspace tensor) and the CUDA stream; all arithmetic of the
+path runs inside libdsmc.so.  There is no CPU fallback: a missing library or GPU raises.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+DSMC_HOST, DSMC_DEVICE = 0, 1
+DSMC_W_IMAGE, DSMC_W_EWALD = 0, 1
+DSMC_REUSE_FIELD = 1
+DSMC_INIT_RANDOM, DSMC_INIT_UP = 0, 1
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libdsmc.so")
+_lib = None
+
+# every symbol include/dsmc.h declares: (name, restype, argtypes)
+_vp, _i, _f, _u64, _sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_float, ctypes.c_uint64, ctypes.c_size_t
+ABI = [
+    ("dsmc_create", _i, [ctypes.POINTER(_vp), _i, _i, _f, _f, _f, _f]),
+    ("dsmc_set_anisotropy", _i, [_vp, _vp, _vp]),
+    ("dsmc_workspace_bytes", _sz, [_i, _i]),
+    ("dsmc_bind", _i, [_vp, _vp, _sz, _vp]),
+    ("dsmc_build_tensor", _i, [_vp, _i, _i, _i]),
+    ("dsmc_get_tensor", _i, [_vp, _vp, _i]),
+    ("dsmc_set_tensor", _i, [_vp, _vp, _i]),
+    ("dsmc_set_spins", _i, [_vp, _vp, _i]),
+    ("dsmc_get_spins", _i, [_vp, _vp, _i]),
+    ("dsmc_init_spins", _i, [_vp, _i, _u64]),
+    ("dsmc_dipole_field", _i, [_vp, _i, _vp, _i]),
+    ("dsmc_halfsweep", _i, [_vp, _vp, _u64, _u64]),
+    ("dsmc_halfsweep_ex", _i, [_vp, _vp, _u64, _u64, _i, _vp, _vp]),
+    ("dsmc_run", _i, [_vp, _vp, _u64, _u64, _u64]),
+    ("dsmc_observables", _i, [_vp, _vp]),
+    ("dsmc_set_timing", _i, [_vp, _i]),
+    ("dsmc_last_timing", _i, [_vp, _vp]),
+    ("dsmc_launch_count", _u64, [_vp]),
+    ("dsmc_field_kernel_kind", _i, [_vp]),
+    ("dsmc_select_field_kernel", _i, [_vp, _i]),
+    ("dsmc_destroy", _i, [_vp]),
+    ("dsmc_last_error", ctypes.c_char_p, [_vp]),
+    ("dsmc_version", ctypes.c_char_p, []),
+]
+
+
+class DsmcError(RuntimeError):
+    pass
+
+
+def load_library(path=None):
+    """dlopen libdsmc.so and set the prototypes; raises if it has not been built."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    p = path or _LIB_PATH
+    if not os.path.exists(p):
+        raise DsmcError(f"{p} not found: build it with `python -m paper_1211_6234_b200.build` "
+                        "(there is no CPU fallback)")
+    lib = ctypes.CDLL(p)
+    for name, res, args in ABI:
+        fn = getattr(lib, name)
+        fn.restype = res
+        fn.argtypes = args
+    if path is None:
+        _lib = lib
+    return lib
+
+
+def _np_f32(a, shape=None):
+    a = np.ascontiguousarray(a, dtype=np.float32)
+    if shape is not None and tuple(a.shape) != tuple(shape):
+        raise ValueError(f"expected shape {shape}, got {a.shape}")
+    return a
+
+
+class Dsmc:
+    """One simulation context: L x L lattice, R replicas.  Mirrors the dsmc_* calls one to one."""
+
+    def __init__(self, L, R, J=1.0, g=0.1, K2=0.6, K4=0.0, device="cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise DsmcError("no CUDA device: the dsmc path has no CPU fallback")
+        self._torch = torch
+        self.lib = load_library()
+        self.L, self.R = int(L), int(R)
+        self.device = torch.device(device)
+        self._h = _vp()
+        rc = self.lib.dsmc_create(ctypes.byref(self._h), self.L, self.R, J, g,
+                                  float(np.atleast_1d(K2)[0]), float(np.atleast_1d(K4)[0]))
+        if rc != 0:
+            raise DsmcError(f"dsmc_create({L}, {R}) failed: {rc}")
+        nbytes = self.lib.dsmc_workspace_bytes(self.L, self.R)
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            base = self.workspace.data_ptr()
+            self._ws_ptr = (base + 255) & ~255
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            self._check(self.lib.dsmc_bind(self._h, self._ws_ptr, nbytes, self.stream.cuda_stream))
+        if np.ndim(K2) > 0 or np.ndim(K4) > 0:
+            self.set_anisotropy(K2, K4)
+
+    # -- helpers -------------------------------------------------------------------------------
+    def _check(self, rc):
+        if rc != 0:
+            raise DsmcError(f"dsmc error {rc}: {self.lib.dsmc_last_error(self._h).decode()}")
+
+    def _ptr(self, a):
+        """(pointer, where) for a numpy array (host) or torch CUDA tensor (device)."""
+        torch = self._torch
+        if isinstance(a, torch.Tensor):
+            assert a.is_contiguous()
+            return a.data_ptr(), (DSMC_DEVICE if a.is_cuda else DSMC_HOST)
+        assert isinstance(a, np.ndarray) and a.flags.c_contiguous
+        return a.ctypes.data, DSMC_HOST
+
+    def close(self):
+        if self._h:
+            self._torch.cuda.synchronize(self.device)
+            self.lib.dsmc_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- the calls of include/dsmc.h -----------------------------------------------------------
+    def set_anisotropy(self, K2, K4):
+        k2 = np.empty(self.R, dtype=np.float32)
+        k4 = np.empty(self.R, dtype=np.float32)
+        k2[:] = K2
+        k4[:] = K4
+        self._check(self.lib.dsmc_set_anisotropy(self._h, k2.ctypes.data, k4.ctypes.data))
+
+    def build_tensor(self, method=DSMC_W_EWALD, cutoff_A=64, tail=1):
+        self._check(self.lib.dsmc_build_tensor(self._h, method, cutoff_A, tail))
+
+    def get_tensor(self):
+        W = np.empty((4, self.L, self.L), dtype=np.float32)
+        self._check(self.lib.dsmc_get_tensor(self._h, W.ctypes.data, DSMC_HOST))
+        return W
+
+    def set_tensor(self, W):
+        W = _np_f32(W, (4, self.L, self.L))
+        self._check(self.lib.dsmc_set_tensor(self._h, W.ctypes.data, DSMC_HOST))
+
+    def set_spins(self, s):
+        if isinstance(s, np.ndarray):
+            s = _np_f32(s, (self.R, 3, self.L, self.L))
+        p, where = self._ptr(s)
+        self._check(self.lib.dsmc_set_spins(self._h, p, where))
+
+    def get_spins(self, out=None):
+        if out is None:
+            out = np.empty((self.R, 3, self.L, self.L), dtype=np.float32)
+        p, where = self._ptr(out)
+        self._check(self.lib.dsmc_get_spins(self._h, p, where))
+        return out
+
+    def init_spins(self, mode=DSMC_INIT_RANDOM, seed=0):
+        self._check(self.lib.dsmc_init_spins(self._h, mode, seed))
+
+    def dipole_field(self, colour=-1, out=None, want_output=True):
+        if not want_output:
+            self._check(self.lib.dsmc_dipole_field(self._h, colour, None, DSMC_HOST))
+            return None
+        if out is None:
+            out = np.zeros((self.R, 3, self.L, self.L), dtype=np.float32)
+        p, where = self._ptr(out)
+        self._check(self.lib.dsmc_dipole_field(self._h, colour, p, where))
+        return out
+
+    def _T(self, T):
+        if T is None:
+            return None, None
+        t = np.empty(self.R, dtype=np.float32)
+        t[:] = T
+        return t, t.ctypes.data
+
+    def halfsweep(self, T, seed, step, flags=0, accept_out=None, margin_out=None):
+        t, tp = self._T(T)
+        if flags == 0 and accept_out is None and margin_out is None:
+            self._check(self.lib.dsmc_halfsweep(self._h, tp, seed, step))
+            return
+        ap = accept_out.data_ptr() if accept_out is not None else None
+        mp = margin_out.data_ptr() if margin_out is not None else None
+        self._check(self.lib.dsmc_halfsweep_ex(self._h, tp, seed, step, flags, ap, mp))
+
+    def run(self, T, seed, first_step, n_half):
+        t, tp = self._T(T)
+        self._check(self.lib.dsmc_run(self._h, tp, seed, first_step, n_half))
+
+    def observables(self):
+        out = np.empty((self.R, 4), dtype=np.float64)
+        self._check(self.lib.dsmc_observables(self._h, out.ctypes.data))
+        return out
+
+    def set_timing(self, on=True):
+        self._check(self.lib.dsmc_set_timing(self._h, int(on)))
+
+    def last_timing(self):
+        out = np.empty(3, dtype=np.float32)
+        self._check(self.lib.dsmc_last_timing(self._h, out.ctypes.data))
+        return out
+
+    def launch_count(self):
+        return int(self.lib.dsmc_launch_count(self._h))
+
+    def field_kernel_kind(self):
+        return int(self.lib.dsmc_field_kernel_kind(self._h))
+
+    def select_field_kernel(self, kind):
+        self._check(self.lib.dsmc_select_field_kernel(self._h, kind))

@@ -1,0 +1,280 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the fp64 oracle, element by element
+on the same seeded inputs.  Tolerances are BASELINE.json's north_star:
+  field: relative L2 <= 1e-5 and max abs <= 1e-4 (h in lattice units, i.e. 1e-4*g on g*h);
+  decisions: identical outside |dE/T + ln u| < 1e-4, the ambiguous ones counted, < 1e-4 of trials.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+FIELD_REL_L2 = 1e-5
+FIELD_MAX_ABS = 1e-4
+BAND = 1e-4
+BAND_FRACTION = 1e-4
+
+
+@pytest.fixture(scope="module")
+def dsmc_mod():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_1211_6234_b200 as m
+    from paper_1211_6234_b200 import build
+    build.build()
+    return m
+
+
+def make_ctx(m, cfg_id, inputs, R=None):
+    c = inputs.CONFIGS[cfg_id]
+    K2, K4 = inputs.anisotropy(cfg_id)
+    R = R or c["R"]
+    ctx = m.Dsmc(c["L"], R, J=1.0, g=c["g"], K2=K2[:R], K4=K4[:R])
+    ctx.build_tensor(m.DSMC_W_EWALD)
+    return ctx
+
+
+def field_errors(h_gpu, h_ref, mask=None):
+    d = h_gpu.astype(np.float64) - h_ref
+    if mask is not None:
+        d = d[..., mask]
+        h_ref = h_ref[..., mask]
+    return np.sqrt((d ** 2).sum() / (h_ref ** 2).sum()), np.abs(d).max()
+
+
+@pytest.mark.parametrize("L", [4, 8, 32, 64])
+@pytest.mark.parametrize("method", ["ewald", "image"])
+def test_tensor_parity(dsmc_mod, oracle, L, method):
+    ctx = dsmc_mod.Dsmc(L, 1)
+    if method == "ewald":
+        ctx.build_tensor(dsmc_mod.DSMC_W_EWALD)
+        ref = oracle.build_tensor_ewald(L)
+    else:
+        ctx.build_tensor(dsmc_mod.DSMC_W_IMAGE, 64, 1)
+        ref = oracle.build_tensor_image(L, 64, 1)
+    W = ctx.get_tensor()
+    # fp64 on both sides, one rounding to fp32 on the GPU side: half an fp32 ulp of each entry
+    assert np.all(np.abs(W.astype(np.float64) - ref) <= 6.1e-8 * np.abs(ref) + 1e-12)
+    ctx.close()
+
+
+def test_tensor_parity_L256(dsmc_mod, oracle):
+    ctx = dsmc_mod.Dsmc(256, 1)
+    ctx.build_tensor(dsmc_mod.DSMC_W_EWALD)
+    W = ctx.get_tensor()
+    ref = oracle.build_tensor_ewald(256)
+    assert np.all(np.abs(W.astype(np.float64) - ref) <= 6.1e-8 * np.abs(ref) + 1e-12)
+    ctx.close()
+
+
+@pytest.mark.parametrize("cfg_id", [1, 2, 3, 4])
+@pytest.mark.parametrize("generic", [False, True])
+def test_field_parity_full(dsmc_mod, oracle, cfg_id, generic):
+    from paper_1211_6234_b200 import inputs
+    c = inputs.CONFIGS[cfg_id]
+    L, R = c["L"], c["R"]
+    ctx = make_ctx(dsmc_mod, cfg_id, inputs)
+    if generic and ctx.field_kernel_kind() == 0:
+        pytest.skip("shape already uses the generic kernel")
+    W = oracle.build_tensor_ewald(L)
+    x = np.arange(L)
+    par = (x[:, None] + x[None, :]) % 2
+    if generic:
+        ctx.select_field_kernel(0)
+        assert ctx.field_kernel_kind() == 0
+    states = [inputs.initial_spins(cfg_id), inputs.up_spins(L, R), inputs.random_spins(L, R, 99)]
+    for s in states:
+        ctx.set_spins(s)
+        ref = oracle.dipole_field(W, s.astype(np.float64))
+        h = ctx.dipole_field(-1)
+        rel, mx = field_errors(h, ref)
+        assert rel <= FIELD_REL_L2 and mx <= FIELD_MAX_ABS, (cfg_id, rel, mx)
+        for colour in (0, 1):
+            hc = np.full((R, 3, L, L), 7.0, dtype=np.float32)
+            ctx.dipole_field(colour, out=hc)
+            assert np.all(hc[..., par != colour] == 7.0)            # inactive targets untouched
+            rel, mx = field_errors(hc, ref, par == colour)
+            assert rel <= FIELD_REL_L2 and mx <= FIELD_MAX_ABS, (cfg_id, colour, rel, mx)
+    ctx.close()
+
+
+def test_field_parity_L256_sampled(dsmc_mod, oracle):
+    """Config 5 at full size, in the launch configuration bench.py times: sampled targets on all
+    replicas by the oracle's direct sum."""
+    from paper_1211_6234_b200 import inputs
+    c = inputs.CONFIGS[5]
+    L, R = c["L"], c["R"]
+    ctx = make_ctx(dsmc_mod, 5, inputs)
+    W = oracle.build_tensor_ewald(L)
+    rng = np.random.default_rng(7)
+    targets = rng.choice(L * L, size=48, replace=False).astype(np.int32)
+    for s in (inputs.initial_spins(5), inputs.up_spins(L, R)):
+        ctx.set_spins(s)
+        h = ctx.dipole_field(-1)
+        got = h.reshape(R, 3, L * L)[:, :, targets]                      # [R][3][nt]
+        ref = np.stack([oracle.dipole_field_sampled(W, s[r].astype(np.float64), targets).T for r in range(R)])
+        d = got.astype(np.float64) - ref
+        rel = np.sqrt((d ** 2).sum() / (ref ** 2).sum())
+        assert rel <= FIELD_REL_L2 and np.abs(d).max() <= FIELD_MAX_ABS, (rel, np.abs(d).max())
+    # a property that holds at any size: all +z -> h_z = 4 zeta(3/2) beta(3/2) at every site
+    assert np.max(np.abs(h[:, 2] - 9.033621683100950)) < 5e-5 and np.max(np.abs(h[:, :2])) < 5e-5
+    ctx.close()
+
+
+def lockstep(dsmc_mod, oracle, ctx, W, T, K2, K4, J, g, seed, steps, first_step=0):
+    """Per half-sweep: copy the GPU state into the oracle, run both with the same (seed, step),
+    compare field, decisions and new spins; continue from the GPU's state."""
+    L, R = ctx.L, ctx.R
+    x = np.arange(L)
+    par = (x[:, None] + x[None, :]) % 2
+    acc_d = torch.zeros((R, L, L), dtype=torch.uint8, device="cuda")
+    mar_d = torch.zeros((R, L, L), dtype=torch.float32, device="cuda")
+    ambiguous = trials = 0
+    worst_rel = worst_abs = 0.0
+    for step in range(first_step, first_step + steps):
+        colour = step & 1
+        act = par == colour
+        s_before = ctx.get_spins()
+        s_or = s_before.astype(np.float64)
+        out = oracle.halfsweep(W, s_or, T, seed, step, J, g, K2, K4)
+        ctx.halfsweep(T, seed, step, accept_out=acc_d, margin_out=mar_d)
+        s_after = ctx.get_spins()
+        acc = acc_d.cpu().numpy()
+        mar = mar_d.cpu().numpy()
+        # (1) decisions: identical outside the band
+        m_or = out["margin"][:, act]
+        a_or = out["accept"][:, act].astype(bool)
+        a_gpu = acc[:, act].astype(bool)
+        amb = np.abs(m_or) < BAND
+        assert np.array_equal(a_gpu[~amb], a_or[~amb]), (step, np.sum(a_gpu[~amb] != a_or[~amb]))
+        ambiguous += int(amb.sum())
+        trials += amb.size
+        # the margin the kernel saw agrees with the oracle's to fp32 accuracy
+        dm = np.abs(mar[:, act] - m_or)
+        assert np.all(dm <= 2e-5 + 3e-6 * np.abs(m_or)), (step, dm.max())
+        # (2) new spins: accepted -> the trial spin, rejected -> bit-unchanged, other colour untouched
+        acc_full = np.zeros((R, L, L), dtype=bool)
+        acc_full[:, act] = a_gpu
+        chg = np.broadcast_to(acc_full[:, None], s_after.shape)
+        assert np.array_equal(s_after[~chg], s_before[~chg])
+        assert np.max(np.abs(s_after[chg].astype(np.float64) - out["trial"][chg]), initial=0.0) <= 1e-6
+        # (3) the frozen field the half-sweep used: recompute it on the state at entry
+        h_ref = out["h"]
+        worst = _field_of_state(ctx, s_before, colour)
+        rel, mx = field_errors(worst, h_ref, act)
+        worst_rel, worst_abs = max(worst_rel, rel), max(worst_abs, mx)
+        ctx.set_spins(s_after)
+    assert worst_rel <= FIELD_REL_L2 and worst_abs <= FIELD_MAX_ABS, (worst_rel, worst_abs)
+    assert ambiguous <= max(1, BAND_FRACTION * trials) or ambiguous / trials < BAND_FRACTION, (ambiguous, trials)
+    return ambiguous, trials
+
+
+_scratch = {}
+
+
+def _field_of_state(ctx, s, colour):
+    key = (ctx.L, ctx.R)
+    if key not in _scratch:
+        import paper_1211_6234_b200 as m
+        c2 = m.Dsmc(ctx.L, ctx.R)
+        c2.set_tensor(ctx.get_tensor())
+        _scratch[key] = c2
+    c2 = _scratch[key]
+    c2.set_spins(s)
+    h = np.zeros((ctx.R, 3, ctx.L, ctx.L), dtype=np.float32)
+    return c2.dipole_field(colour, out=h)
+
+
+def test_lockstep_config1(dsmc_mod, oracle):
+    """Config 1 in full: L = 8, R = 1, 100 sweeps, every half-sweep compared (image-sum W, A = 64)."""
+    from paper_1211_6234_b200 import inputs
+    c = inputs.CONFIGS[1]
+    ctx = dsmc_mod.Dsmc(c["L"], c["R"], J=1.0, g=c["g"], K2=c["K2"], K4=c["K4"])
+    ctx.build_tensor(dsmc_mod.DSMC_W_IMAGE, 64, 1)
+    W = oracle.build_tensor_image(c["L"], 64, 1)
+    ctx.set_spins(inputs.initial_spins(1))
+    T = inputs.temperatures(1)
+    lockstep(dsmc_mod, oracle, ctx, W, T, c["K2"], c["K4"], 1.0, c["g"], seed=inputs.SEED_BASE + 1, steps=200)
+    ctx.close()
+
+
+@pytest.mark.parametrize("cfg_id,steps", [(2, 40), (3, 12), (4, 4)])
+def test_lockstep_configs(dsmc_mod, oracle, cfg_id, steps):
+    from paper_1211_6234_b200 import inputs
+    c = inputs.CONFIGS[cfg_id]
+    ctx = make_ctx(dsmc_mod, cfg_id, inputs)
+    W = oracle.build_tensor_ewald(c["L"])
+    K2, K4 = inputs.anisotropy(cfg_id)
+    ctx.set_spins(inputs.initial_spins(cfg_id))
+    T = inputs.temperatures(cfg_id)
+    amb, tr = lockstep(dsmc_mod, oracle, ctx, W, T, K2, K4, 1.0, c["g"], seed=inputs.SEED_BASE + cfg_id, steps=steps)
+    print(f"config {cfg_id}: ambiguous {amb} of {tr} trials")
+    ctx.close()
+
+
+def test_init_spins_parity(dsmc_mod, oracle):
+    for (L, R) in ((8, 1), (32, 8)):
+        ctx = dsmc_mod.Dsmc(L, R)
+        ctx.init_spins(dsmc_mod.DSMC_INIT_RANDOM, seed=4242)
+        s = ctx.get_spins()
+        ref = oracle.init_spins(L, R, 0, 4242)
+        assert np.max(np.abs(s - ref)) <= 1e-6
+        assert np.array_equal(s[:, 2].astype(np.float64), ref[:, 2])      # z = 2u - 1 is exact in fp32
+        ctx.init_spins(dsmc_mod.DSMC_INIT_UP)
+        assert np.array_equal(ctx.get_spins(), oracle.init_spins(L, R, 1, 0).astype(np.float32))
+        ctx.close()
+
+
+@pytest.mark.parametrize("cfg_id", [1, 2, 3])
+def test_observables_parity(dsmc_mod, oracle, cfg_id):
+    from paper_1211_6234_b200 import inputs
+    c = inputs.CONFIGS[cfg_id]
+    ctx = make_ctx(dsmc_mod, cfg_id, inputs)
+    W = oracle.build_tensor_ewald(c["L"])
+    K2, K4 = inputs.anisotropy(cfg_id)
+    for s in (inputs.initial_spins(cfg_id), inputs.random_spins(c["L"], c["R"], 5)):
+        ctx.set_spins(s)
+        got = ctx.observables()
+        ref = oracle.observables(W, s.astype(np.float64), 1.0, c["g"], K2.astype(np.float64), K4.astype(np.float64))
+        assert np.max(np.abs(got - ref)) <= 2e-6, np.abs(got - ref).max(0)
+    ctx.close()
+
+
+def test_set_get_roundtrip_and_errors(dsmc_mod):
+    from paper_1211_6234_b200 import inputs
+    ctx = dsmc_mod.Dsmc(12, 5)                                   # ragged: L not a multiple of 8, odd R
+    s = inputs.random_spins(12, 5, 3)
+    ctx.set_spins(s)
+    assert np.array_equal(ctx.get_spins(), s)
+    d = torch.from_numpy(s).cuda()
+    ctx.set_spins(d)
+    out = torch.empty_like(d)
+    ctx.get_spins(out)
+    assert torch.equal(out, d)
+    with pytest.raises(dsmc_mod.DsmcError):                      # tensor not built
+        ctx.dipole_field(-1)
+    ctx.build_tensor()
+    with pytest.raises(dsmc_mod.DsmcError):                      # T must be > 0
+        ctx.halfsweep(np.zeros(5, np.float32), 1, 0)
+    with pytest.raises(dsmc_mod.DsmcError):                      # bad colour
+        ctx.dipole_field(2)
+    with pytest.raises(dsmc_mod.DsmcError):                      # odd L
+        dsmc_mod.Dsmc(7, 1)
+    ctx.close()
+
+
+def test_ragged_shape_field_and_sweep(dsmc_mod, oracle):
+    """L = 12, R = 5: not a multiple of any tile size; full parity through the generic kernel."""
+    from paper_1211_6234_b200 import inputs
+    L, R, g = 12, 5, 0.3
+    ctx = dsmc_mod.Dsmc(L, R, J=1.0, g=g, K2=0.4, K4=-0.1)
+    ctx.build_tensor()
+    W = oracle.build_tensor_ewald(L)
+    s = inputs.random_spins(L, R, 17)
+    ctx.set_spins(s)
+    rel, mx = field_errors(ctx.dipole_field(-1), oracle.dipole_field(W, s.astype(np.float64)))
+    assert rel <= FIELD_REL_L2 and mx <= FIELD_MAX_ABS
+    T = np.linspace(0.3, 1.5, R).astype(np.float32)
+    lockstep(dsmc_mod, oracle, ctx, W, T, 0.4, -0.1, 1.0, g, seed=77, steps=6)
+    ctx.close()
