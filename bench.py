@@ -1,0 +1,301 @@
+#!/usr/bin/env python
+"""bench.py -- BASELINE.json's metric on BASELINE.json's config 5 (L=256, R=64) on B200.
+
+  python bench.py --gpus N --steps K --warmup W            # the CUDA path (one JSON line, rank 0)
+  python bench.py --impl reference --steps K --warmup W     # the fp64 CPU oracle on host cores
+
+One "step" = one Monte Carlo sweep of the whole hot path: for colour 0 then 1, dipole field
+(a1) + fused Metropolis half-sweep (a2), on all R replicas.  value = spin updates per second
+(N*R updates per step).  Multi-GPU: the path shards by replica with no exchange ("replicas only",
+DESIGN.md section 7): every rank runs the full config-5 workload, weak scaling.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+CFG_ID = 5
+FLOP_PER_PAIR = 10.0           # 5 FMA per (target, source, replica): SURVEY.md section 8(d)
+BYTES_PER_UPDATE = 48.0        # own spin 12 + neighbours 12 (amortised) + h 12 + write 12
+# fp32 FMA peak: 148 SMs x 128 lanes x 2 flop x 1.965 GHz
+FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
+FP32_MEASURED_FFMA_TFLOPS = 70.9   # profiles/r01_ffma_microbench.txt (dependent-free FFMA chains)
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured"
+    return 6650.0, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows = []
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "200"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [t.strip() for t in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample(steps, warmup, n_rep):
+    """The oracle, as it stands, on a bounded sample of config 5: one half-sweep (field for the active
+    colour + Metropolis decisions) restricted to n_rep of the 64 replicas.  -> (updates/s, seconds/step)"""
+    from oracle import oracle as o
+    from paper_1211_6234_b200 import inputs
+    c = inputs.CONFIGS[CFG_ID]
+    L = c["L"]
+    K2, K4 = inputs.anisotropy(CFG_ID)
+    T = inputs.temperatures(CFG_ID)
+    W = o.build_tensor_ewald(L)
+    s = inputs.initial_spins(CFG_ID)[:n_rep].astype(np.float64)
+    times = []
+    for it in range(warmup + steps):
+        t0 = time.perf_counter()
+        o.halfsweep(W, s, T[:n_rep].astype(np.float64), inputs.SEED_BASE + CFG_ID, it, 1.0, c["g"],
+                    K2[:n_rep].astype(np.float64), K4[:n_rep].astype(np.float64), want=())
+        dt = time.perf_counter() - t0
+        if it >= warmup:
+            times.append(dt)
+    sec = float(np.mean(times))
+    updates = (L * L // 2) * n_rep
+    return updates / sec, sec, o.num_threads()
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_1211_6234_b200 import inputs
+    c = inputs.CONFIGS[CFG_ID]
+    n_rep = 2
+    ups, sec, cores = oracle_sample(args.steps, min(args.warmup, 1), n_rep)
+    sample = (f"one checkerboard half-sweep (field of the active colour + Metropolis) of config 5 restricted to "
+              f"{n_rep} of {c['R']} replicas per step (work is linear in R)")
+    line = {
+        "impl": "reference", "metric": "spin_updates_per_s", "value": ups, "unit": "updates/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": min(args.warmup, 1), "ms_per_step": sec * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "config5 L=256 R=64 J=1 g=0.1 K2=0.6 K4=0.1 T=0.1..2.0 (bounded sample)", "L": c["L"],
+                   "R": c["R"], "sample_replicas": n_rep},
+        "cpu_baseline": {"value": ups, "unit": "updates/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": ups, "unit": "updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the dsmc path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    import paper_1211_6234_b200 as m
+    from paper_1211_6234_b200 import build, inputs
+    if rank == 0:
+        build.build()
+    if world > 1:
+        dist.barrier()
+
+    c = inputs.CONFIGS[CFG_ID]
+    L, R = c["L"], c["R"]
+    N = L * L
+    K2, K4 = inputs.anisotropy(CFG_ID)
+    T = inputs.temperatures(CFG_ID)
+    seed = inputs.SEED_BASE + CFG_ID + 1000 * rank
+    ctx = m.Dsmc(L, R, J=1.0, g=c["g"], K2=K2, K4=K4, device=dev)
+    ctx.build_tensor(m.DSMC_W_EWALD)
+    s_host = torch.from_numpy(inputs.random_spins(L, R, seed)).pin_memory()
+    ctx.set_spins(s_host.numpy())
+    out_host = torch.empty_like(s_host).pin_memory()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    def sweep(k):
+        ctx.halfsweep(T, seed, 2 * k)
+        ctx.halfsweep(None, seed, 2 * k + 1)
+
+    # ---- whole-path throughput, inputs resident in HBM ---------------------------------------------
+    for k in range(args.warmup):
+        sweep(k)
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    l0 = ctx.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for k in range(args.steps):
+        sweep(args.warmup + k)
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = ctx.launch_count() - l0
+
+    # ---- per-kernel device times on the launching stream (CUDA events inside the library) ----------
+    ctx.set_timing(True)
+    f_ms, m_ms = [], []
+    for k in range(max(args.steps, 3)):
+        for h in (0, 1):
+            ctx.halfsweep(None, seed, 2 * (args.warmup + args.steps + k) + h)
+            t = ctx.last_timing()
+            f_ms.append(float(t[0]))
+            m_ms.append(float(t[1]))
+    ctx.set_timing(False)
+    clocks = sampler.stop() if sampler else None
+
+    # Metropolis kernel alone, L2 flushed before every launch (its working set would fit in L2)
+    flush = torch.empty(512 * 1024 * 1024, dtype=torch.uint8, device=dev)
+    ctx.dipole_field(-1, want_output=False)
+    ctx.set_timing(True)
+    mm = []
+    for k in range(12):
+        flush.zero_()
+        ctx.halfsweep(None, seed, 10_000 + k, flags=m.DSMC_REUSE_FIELD)
+        mm.append(float(ctx.last_timing()[1]))
+    ctx.set_timing(False)
+    metro_cold_ms = float(np.median(mm[2:]))
+    del flush
+
+    # ---- end to end through the public API with HOST buffers ----------------------------------------
+    def e2e_step(k):
+        ctx.set_spins(s_host.numpy())                 # H2D from pinned memory
+        sweep(k)
+        ctx.get_spins(out_host.numpy())               # D2H of the step's result (synchronises)
+    e2e_step(0)
+    barrier()
+    t0 = time.perf_counter()
+    n_e2e = max(2, min(args.steps, 5))
+    for k in range(n_e2e):
+        e2e_step(k)
+    barrier()
+    e2e_s = (time.perf_counter() - t0) / n_e2e
+
+    # ---- max over ranks ----------------------------------------------------------------------------
+    if world > 1:
+        tt = torch.tensor([ms, e2e_s], device=dev, dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms, e2e_s = float(tt[0]), float(tt[1])
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    updates_per_step = N * R
+    ms_per_step = ms / args.steps
+    value = world * updates_per_step / (ms_per_step * 1e-3)
+    field_ms = float(np.mean(f_ms))
+    metro_ms = float(np.mean(m_ms))
+    flop_per_field = FLOP_PER_PAIR * (N // 2) * N * R
+    field_tflops = flop_per_field / (field_ms * 1e-3) / 1e12
+    hbm_peak, hbm_kind = measured_peaks()
+    metro_bytes = BYTES_PER_UPDATE * (N // 2) * R
+    metro_gbs = metro_bytes / (metro_cold_ms * 1e-3) / 1e9
+
+    line = {
+        "metric": "spin_updates_per_s", "value": value, "unit": "updates/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "config5 L=256 R=64 J=1 g=0.1 K2=0.6 K4=0.1 T=0.1..2.0, 1 step = 1 sweep "
+                               "(2 x [dipole field + Metropolis half-sweep])",
+                   "L": L, "R": R, "parallelism": f"replicas only x{world}",
+                   "l2": "working set per step (spins 50 MB + h 25 MB + split-K partials 201 MB) exceeds the 126 MB L2; "
+                         "the Metropolis-only figure flushes L2 (512 MB memset) before every launch",
+                   "field_kernel": "tiled" if ctx.field_kernel_kind() == 1 else "generic"},
+        "clocks": clocks,
+        "e2e": {"value": world * updates_per_step / e2e_s, "unit": "updates/s",
+                "h2d_bytes_per_step": int(s_host.numel() * 4), "d2h_bytes_per_step": int(out_host.numel() * 4)},
+        "gpu_launches": int(launches),
+        "roofline": {"kernel": "field_tiled_kernel (+ reduce_partials)", "bound": "alu", "achieved": field_tflops,
+                     "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": field_tflops / FP32_PEAK_TFLOPS,
+                     "peak_kind": "derived: 148 SM x 128 fp32 lanes x 2 x 1.965 GHz (DESIGN.md section 6)",
+                     "frac_of_measured_ffma_peak": field_tflops / FP32_MEASURED_FFMA_TFLOPS,
+                     "traffic": None, "ms_per_launch": field_ms, "flop_per_launch": flop_per_field},
+        "dipole_field_gflops": field_tflops * 1e3,
+        "roofline_metropolis": {"kernel": "metropolis_kernel", "bound": "hbm", "achieved": metro_gbs, "peak": hbm_peak,
+                                "unit": "GB/s", "frac": metro_gbs / hbm_peak, "peak_kind": hbm_kind,
+                                "frac_of_8TBs": metro_gbs / 8000.0, "ms_per_launch_cold_l2": metro_cold_ms,
+                                "ms_per_launch_in_sweep": metro_ms, "bytes_per_launch": metro_bytes,
+                                "updates_per_s": (N // 2) * R / (metro_cold_ms * 1e-3), "traffic": None},
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        ups, sec, cores = oracle_sample(1, 0, 8)
+        line["cpu_baseline"] = {"value": ups, "unit": "updates/s", "cores": cores, "kind": "oracle",
+                                "sample": "one checkerboard half-sweep of config 5 on 8 of 64 replicas "
+                                          f"({sec:.1f} s; work is linear in R)"}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_cuda(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -290,6 +290,7 @@ int dsmc_halfsweep_ex(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t ste
     a.L = ctx->L;
     a.R = ctx->R;
     a.colour = colour;
+    a.rq_shift = -1;
     a.J = ctx->J;
     a.g = ctx->g;
     a.w0xx = ctx->w0[0];
@@ -307,9 +308,8 @@ int dsmc_halfsweep_ex(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t ste
         CU(cudaEventRecord(ctx->ev[2], ctx->stream), "event");
         ctx->ev_recorded = true;
     }
-    // the spins of this colour changed: both colours' fields are stale for observables, but the
-    // field of this colour stays "valid" only in the DSMC_REUSE_FIELD (timing) sense
-    ctx->field_valid[1 - colour] = false;
+    // field_valid only records that H holds a field of that colour computed since the spins were
+    // last set (what DSMC_REUSE_FIELD needs for timing); observables always recompute both colours
     return DSMC_OK;
 }
 

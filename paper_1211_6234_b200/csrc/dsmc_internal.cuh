@@ -95,6 +95,7 @@ struct MetropolisArgs {
     const float *H;
     const float *invT, *K2, *K4;
     int L, R, colour;
+    int rq_shift;  // log2(R/4) when R/4 is a power of two, else -1 (set by the launcher)
     float J, g, w0xx, w0yy, w0zz, w0xy;
     uint32_t seed_lo, seed_hi, step_lo, step_hi;
     uint8_t *accept_out;  // canonical [R][L][L] or null
