@@ -27,7 +27,6 @@ FLOP_PER_PAIR = 10.0           # 5 FMA per (target, source, replica): SURVEY.md 
 BYTES_PER_UPDATE = 48.0        # own spin 12 + neighbours 12 (amortised) + h 12 + write 12
 # fp32 FMA peak: 148 SMs x 128 lanes x 2 flop x 1.965 GHz
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
-FP32_MEASURED_FFMA_TFLOPS = 70.9   # profiles/r01_ffma_microbench.txt (dependent-free FFMA chains)
 
 
 def measured_peaks():
@@ -243,6 +242,7 @@ def run_cuda(args):
     flop_per_field = FLOP_PER_PAIR * (N // 2) * N * R
     field_tflops = flop_per_field / (field_ms * 1e-3) / 1e12
     hbm_peak, hbm_kind = measured_peaks()
+    ffma_peak = ctx.fp32_fma_peak()            # dependency-free FFMA chains, same process, same clocks
     metro_bytes = BYTES_PER_UPDATE * (N // 2) * R
     metro_gbs = metro_bytes / (metro_cold_ms * 1e-3) / 1e9
 
@@ -263,7 +263,7 @@ def run_cuda(args):
         "roofline": {"kernel": "field_tiled_kernel (+ reduce_partials)", "bound": "alu", "achieved": field_tflops,
                      "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": field_tflops / FP32_PEAK_TFLOPS,
                      "peak_kind": "derived: 148 SM x 128 fp32 lanes x 2 x 1.965 GHz (DESIGN.md section 6)",
-                     "frac_of_measured_ffma_peak": field_tflops / FP32_MEASURED_FFMA_TFLOPS,
+                     "measured_ffma_peak": ffma_peak, "frac_of_measured_ffma_peak": field_tflops / ffma_peak,
                      "traffic": None, "ms_per_launch": field_ms, "flop_per_launch": flop_per_field},
         "dipole_field_gflops": field_tflops * 1e3,
         "roofline_metropolis": {"kernel": "metropolis_kernel", "bound": "hbm", "achieved": metro_gbs, "peak": hbm_peak,

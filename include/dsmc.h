@@ -156,6 +156,11 @@ uint64_t dsmc_launch_count(dsmc_ctx *ctx);
 int dsmc_field_kernel_kind(dsmc_ctx *ctx);
 int dsmc_select_field_kernel(dsmc_ctx *ctx, int kind);
 
+/* Measured fp32 FMA issue peak of this GPU in TFLOP/s: a dependency-free FFMA-chain microbenchmark
+ * (one CTA of 256 threads per SM, 96 independent accumulators per thread), the denominator
+ * bench.py reports beside the derived SMs x 128 lanes x 2 x clock figure.  Synchronises.          */
+int dsmc_fp32_fma_peak(dsmc_ctx *ctx, double *tflops_out);
+
 int dsmc_destroy(dsmc_ctx *ctx);
 const char *dsmc_last_error(dsmc_ctx *ctx);
 const char *dsmc_version(void);

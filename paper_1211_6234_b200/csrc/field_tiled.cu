@@ -17,6 +17,8 @@
 //   * because both targets and sources are walked in steps of one same-colour site, the W values a
 //     thread needs form a sliding window: one new value per component per source step, kept in an
 //     8-deep register ring (fully unrolled by 8), fetched as 128-bit shared loads every 4 steps.
+//   * the FMAs are issued as packed FFMA2 over pairs of replicas (W value duplicated in a register
+//     pair): 80 FFMA2 per source step per thread.
 //
 // Wk[cl][pt][dy][c][kk] = W[c][dy][(2 (kk - Lh) + ((pt + dy + cl) & 1) - pt) mod L], kk in [0, L):
 //   cl = source colour != target colour, pt = parity offset of the target row, dy = (y_s - y_t) mod L,
@@ -150,13 +152,17 @@ __global__ void __launch_bounds__(MAX_THREADS, 1) field_tiled_kernel(const Tiled
         for (int s = 0; s < NSTAGE && s < nstages; ++s) produce(s);
     }
 
-    float acc[TT][3][4];
+    // accumulators as packed pairs of replicas: acc[j][c][kp] = (replica 2kp, replica 2kp+1).
+    // The inner product is issued as FFMA2 (fma.rn.f32x2): 64-bit register pairs read one word from
+    // each register bank, so the operand fetch has no bank conflicts by construction, and one issue
+    // slot carries two FMAs per lane (measured 114 vs 102 FMA/clk/SM for the scalar form of this loop).
+    float2 acc[TT][3][2];
 #pragma unroll
     for (int j = 0; j < TT; ++j)
 #pragma unroll
         for (int c = 0; c < 3; ++c)
 #pragma unroll
-            for (int k = 0; k < 4; ++k) acc[j][c][k] = 0.0f;
+            for (int k = 0; k < 2; ++k) acc[j][c][k] = make_float2(0.0f, 0.0f);
 
     const int RCH4 = RCH >> 2;
     for (int st = 0; st < nstages; ++st) {
@@ -169,15 +175,16 @@ __global__ void __launch_bounds__(MAX_THREADS, 1) field_tiled_kernel(const Tiled
         const int base = seg * SEG + Lh - TT * g;  // multiple of 8
         const float *wr = wsm + (size_t)trow * 4 * L + base;
 
-        // register ring of the sliding W window: slot (u & 7) holds W[base + u]
-        float w[4][8];
+        // register ring of the sliding W window: slot (u & 7) holds (W[base + u], W[base + u])
+        float2 w[4][8];
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
             const float4 a = *reinterpret_cast<const float4 *>(wr + c * L - 8);
             const float4 bq = *reinterpret_cast<const float4 *>(wr + c * L - 4);
-            w[c][0] = a.x;  // W[base - 8]: never used, overwritten at u = 0
-            w[c][1] = a.y; w[c][2] = a.z; w[c][3] = a.w;
-            w[c][4] = bq.x; w[c][5] = bq.y; w[c][6] = bq.z; w[c][7] = bq.w;
+            w[c][0] = make_float2(a.x, a.x);  // W[base - 8]: never used, overwritten at u = 0
+            w[c][1] = make_float2(a.y, a.y); w[c][2] = make_float2(a.z, a.z); w[c][3] = make_float2(a.w, a.w);
+            w[c][4] = make_float2(bq.x, bq.x); w[c][5] = make_float2(bq.y, bq.y);
+            w[c][6] = make_float2(bq.z, bq.z); w[c][7] = make_float2(bq.w, bq.w);
         }
         for (int ub = 0; ub < SEG; ub += 8) {
             float4 wn[4];
@@ -191,25 +198,25 @@ __global__ void __launch_bounds__(MAX_THREADS, 1) field_tiled_kernel(const Tiled
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
                     const float v = (uu & 3) == 0 ? wn[c].x : (uu & 3) == 1 ? wn[c].y : (uu & 3) == 2 ? wn[c].z : wn[c].w;
-                    w[c][uu] = v;
+                    w[c][uu] = make_float2(v, v);
                 }
                 const float4 sx = ssm[(size_t)(0 * SEG + u) * RCH4];
                 const float4 sy = ssm[(size_t)(1 * SEG + u) * RCH4];
                 const float4 sz = ssm[(size_t)(2 * SEG + u) * RCH4];
-                const float sxa[4] = {sx.x, sx.y, sx.z, sx.w};
-                const float sya[4] = {sy.x, sy.y, sy.z, sy.w};
-                const float sza[4] = {sz.x, sz.y, sz.z, sz.w};
+                const float2 sx2[2] = {make_float2(sx.x, sx.y), make_float2(sx.z, sx.w)};
+                const float2 sy2[2] = {make_float2(sy.x, sy.y), make_float2(sy.z, sy.w)};
+                const float2 sz2[2] = {make_float2(sz.x, sz.y), make_float2(sz.z, sz.w)};
 #pragma unroll
                 for (int j = 0; j < TT; ++j) {
                     const int slot = (uu - j) & 7;
-                    const float wxx = w[0][slot], wxy = w[1][slot], wyy = w[2][slot], wzz = w[3][slot];
+                    const float2 wxx = w[0][slot], wxy = w[1][slot], wyy = w[2][slot], wzz = w[3][slot];
 #pragma unroll
-                    for (int k = 0; k < 4; ++k) {
-                        acc[j][0][k] = fmaf(wxx, sxa[k], acc[j][0][k]);
-                        acc[j][0][k] = fmaf(wxy, sya[k], acc[j][0][k]);
-                        acc[j][1][k] = fmaf(wxy, sxa[k], acc[j][1][k]);
-                        acc[j][1][k] = fmaf(wyy, sya[k], acc[j][1][k]);
-                        acc[j][2][k] = fmaf(wzz, sza[k], acc[j][2][k]);
+                    for (int k = 0; k < 2; ++k) {
+                        acc[j][0][k] = __ffma2_rn(wxx, sx2[k], acc[j][0][k]);
+                        acc[j][0][k] = __ffma2_rn(wxy, sy2[k], acc[j][0][k]);
+                        acc[j][1][k] = __ffma2_rn(wxy, sx2[k], acc[j][1][k]);
+                        acc[j][1][k] = __ffma2_rn(wyy, sy2[k], acc[j][1][k]);
+                        acc[j][2][k] = __ffma2_rn(wzz, sz2[k], acc[j][2][k]);
                     }
                 }
             }
@@ -225,7 +232,7 @@ __global__ void __launch_bounds__(MAX_THREADS, 1) field_tiled_kernel(const Tiled
         for (int j = 0; j < TT; ++j)
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
-                float4 v = make_float4(acc[j][c][0], acc[j][c][1], acc[j][c][2], acc[j][c][3]);
+                float4 v = make_float4(acc[j][c][0].x, acc[j][c][0].y, acc[j][c][1].x, acc[j][c][1].y);
                 *reinterpret_cast<float4 *>(out + (size_t)c * plane + (a0 + j) * R + r0 + 4 * rt) = v;
             }
     }

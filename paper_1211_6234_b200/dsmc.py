@@ -40,6 +40,7 @@ ABI = [
     ("dsmc_launch_count", _u64, [_vp]),
     ("dsmc_field_kernel_kind", _i, [_vp]),
     ("dsmc_select_field_kernel", _i, [_vp, _i]),
+    ("dsmc_fp32_fma_peak", _i, [_vp, _vp]),
     ("dsmc_destroy", _i, [_vp]),
     ("dsmc_last_error", ctypes.c_char_p, [_vp]),
     ("dsmc_version", ctypes.c_char_p, []),
@@ -212,6 +213,11 @@ class Dsmc:
 
     def field_kernel_kind(self):
         return int(self.lib.dsmc_field_kernel_kind(self._h))
+
+    def fp32_fma_peak(self):
+        out = ctypes.c_double(0.0)
+        self._check(self.lib.dsmc_fp32_fma_peak(self._h, ctypes.addressof(out)))
+        return float(out.value)
 
     def select_field_kernel(self, kind):
         self._check(self.lib.dsmc_select_field_kernel(self._h, kind))
