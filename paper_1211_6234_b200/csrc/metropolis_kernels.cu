@@ -93,66 +93,202 @@ __device__ __forceinline__ Trial decide(const MetropolisArgs &p, const RoundKeys
     return t;
 }
 
-// R % 4 == 0: one thread = one active site x 4 consecutive replicas.  grid.y = lattice row.
+// ---- packed fp32 pairs (FFMA2 / FMUL2 / FADD2 of sm_100a): one instruction works on the same
+// quantity of two replicas.  A scalar operand written f2_bc(x) is folded by ptxas into the
+// instruction's broadcast / immediate operand form, so constants cost nothing.
+typedef unsigned long long f2;
+__device__ __forceinline__ f2 f2_make(float lo, float hi) {
+    f2 d;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "f"(lo), "f"(hi));
+    return d;
+}
+__device__ __forceinline__ f2 f2_bc(float a) { return f2_make(a, a); }
+__device__ __forceinline__ void f2_split(f2 v, float &lo, float &hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f2 f2_fma(f2 a, f2 b, f2 c) {
+    f2 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ f2 f2_mul(f2 a, f2 b) {
+    f2 d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ f2 f2_add(f2 a, f2 b) {
+    f2 d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ f2 f2_sub(f2 a, f2 b) { return f2_fma(b, f2_bc(-1.0f), a); }  // a - b, exact like FADD
+__device__ __forceinline__ float rsqrt_approx(float x) {
+    float r;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ float lg2_approx(float x) {
+    float r;
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
+// word -> y = 1 + (x >> 9) 2^-23 in [1, 2) by writing the mantissa field (no int->float conversion)
+__device__ __forceinline__ float mant(uint32_t x) { return __uint_as_float(0x3F800000u | (x >> 9)); }
+
+// Two Metropolis decisions at once (replicas r, r+1 of one site).  Same arithmetic as decide() with
+// two differences, both within the parity tolerances:
+//   * u = (2k+1) 2^-24 with k = x >> 9: z = 2u0 - 1 = 2 (y - 1.5) + 2^-23 and v = 2u1 - 1 likewise are
+//     exact in fp32 (y - 1.5 is a multiple of 2^-23 in [-1/2, 1/2); the fma rounds once to a
+//     representable odd multiple of 2^-23), so the trial z is bit-identical to the oracle's;
+//   * azimuth phi = 2 pi u1 = pi v + pi.  With S = sin(pi v / 2) = v P(v^2), C = cos(pi v / 2) = Q(v^2)
+//     (the polynomials of sphere_point, valid on [-1, 1] by parity):
+//       cos phi = -cos(pi v) = (S - C)(S + C),   sin phi = -sin(pi v) = (-2 S) C,
+//     no quadrant selects; max abs error 4.5e-7.
+struct Pair {
+    f2 tx, ty, tz, margin;
+};
+__device__ __forceinline__ Pair decide2(const MetropolisArgs &p, uint4 ra, uint4 rb, f2 sx, f2 sy, f2 sz, f2 nx, f2 ny,
+                                        f2 nz, f2 hx, f2 hy, f2 hz, f2 invT, f2 K2, f2 K4) {
+    Pair t;
+    const f2 c2 = f2_bc(2.0f), cm15 = f2_bc(-1.5f), ulp = f2_bc(1.1920928955078125e-7f);
+    const f2 z = f2_fma(c2, f2_add(f2_make(mant(ra.x), mant(rb.x)), cm15), ulp);
+    const f2 v = f2_fma(c2, f2_add(f2_make(mant(ra.y), mant(rb.y)), cm15), ulp);
+    // u = (y - 1) + 2^-24, exact
+    const f2 u = f2_add(f2_add(f2_make(mant(ra.z), mant(rb.z)), f2_bc(-1.0f)), f2_bc(5.9604644775390625e-8f));
+    const f2 q = f2_mul(v, v);
+    f2 ps = f2_fma(f2_bc(1.516751217423007e-4f), q, f2_bc(-4.674150608479977e-3f));
+    ps = f2_fma(ps, q, f2_bc(7.968991994857788e-2f));
+    ps = f2_fma(ps, q, f2_bc(-6.459637880325317e-1f));
+    ps = f2_fma(ps, q, f2_bc(1.5707963705062866f));
+    const f2 S = f2_mul(ps, v);
+    f2 C = f2_fma(f2_bc(-2.3824535674066283e-5f), q, f2_bc(9.177238680422306e-4f));
+    C = f2_fma(C, q, f2_bc(-2.086268737912178e-2f));
+    C = f2_fma(C, q, f2_bc(2.536693215370178e-1f));
+    C = f2_fma(C, q, f2_bc(-1.2337005138397217f));
+    C = f2_fma(C, q, f2_bc(1.0f));
+    const f2 cs = f2_mul(f2_sub(S, C), f2_add(S, C));
+    const f2 sn = f2_mul(f2_mul(S, f2_bc(-2.0f)), C);
+    const f2 w = f2_mul(f2_sub(f2_bc(1.0f), z), f2_add(z, f2_bc(1.0f)));  // > 0: |z| <= 1 - 2^-23
+    float w0, w1;
+    f2_split(w, w0, w1);
+    const f2 rho = f2_mul(w, f2_make(rsqrt_approx(w0), rsqrt_approx(w1)));
+    t.tx = f2_mul(rho, cs);
+    t.ty = f2_mul(rho, sn);
+    t.tz = z;
+    const f2 dx = f2_sub(t.tx, sx), dy = f2_sub(t.ty, sy), dz = f2_sub(z, sz);
+    const f2 dz2 = f2_mul(dz, f2_add(z, sz));                              // s'_z^2 - s_z^2
+    const f2 z2sum = f2_fma(z, z, f2_mul(sz, sz));
+    f2 dE = f2_mul(f2_fma(dx, nx, f2_fma(dy, ny, f2_mul(dz, nz))), f2_bc(-p.J));
+    dE = f2_fma(f2_mul(dz2, f2_bc(-1.0f)), f2_fma(K4, z2sum, K2), dE);     // -K2 d(z^2) - K4 d(z^4)
+    // g [ delta.h + (1/2) delta.W(0).delta ] = g delta.(h + W(0) delta / 2)
+    const f2 ex = f2_fma(f2_bc(p.w0xy), dy, f2_fma(f2_bc(0.5f * p.w0xx), dx, hx));
+    const f2 ey = f2_fma(f2_bc(0.5f * p.w0yy), dy, hy);
+    const f2 ez = f2_fma(f2_bc(0.5f * p.w0zz), dz, hz);
+    const f2 dip = f2_fma(dx, ex, f2_fma(dy, ey, f2_mul(dz, ez)));
+    dE = f2_fma(f2_bc(p.g), dip, dE);
+    float u0, u1;
+    f2_split(u, u0, u1);
+    t.margin = f2_fma(f2_make(lg2_approx(u0), lg2_approx(u1)), f2_bc(0.693147180559945f), f2_mul(dE, invT));
+    return t;
+}
+
+__device__ __forceinline__ void ld2(const float4 *ptr, f2 &lo, f2 &hi) {
+    const ulonglong2 v = __ldg(reinterpret_cast<const ulonglong2 *>(ptr));
+    lo = v.x;
+    hi = v.y;
+}
+
+// R % 4 == 0: one thread = one active site x 4 consecutive replicas (two packed pairs); grid.y =
+// lattice row.  All 18 128-bit loads are issued first; the four Philox chains and the trial spins
+// do not depend on them and run while they are in flight.  HOOKS = parity outputs requested.
+template <bool HOOKS>
 __global__ void __launch_bounds__(128) metropolis4_kernel(const MetropolisArgs p, const RoundKeys rk) {
     const int Lh = p.L >> 1, RQ = p.R >> 2;
     const int y = blockIdx.y;
+    const uint32_t row4 = (uint32_t)(Lh * RQ);
     const uint32_t e = blockIdx.x * blockDim.x + threadIdx.x;   // (i, replica quad) within the row
-    if (e >= (uint32_t)(Lh * RQ)) return;
+    if (e >= row4) return;
     const int i = p.rq_shift >= 0 ? (int)(e >> p.rq_shift) : (int)(e / (uint32_t)RQ);
     const int rq = (int)e - i * RQ;
     const int par = (y + p.colour) & 1;
     const size_t plane4 = ((size_t)p.L * Lh * p.R) >> 2;      // float4 per [a][r] plane
-    const size_t row4 = (size_t)Lh * RQ;
-
-    float4 *own = reinterpret_cast<float4 *>(p.S) + (size_t)p.colour * 3 * plane4 + (size_t)y * row4 + e;
-    const float4 *oth = reinterpret_cast<const float4 *>(p.S) + (size_t)(1 - p.colour) * 3 * plane4 + rq;
-    const float4 *hf = reinterpret_cast<const float4 *>(p.H) + (size_t)p.colour * 3 * plane4 + (size_t)y * row4 + e;
-
-    // the four neighbours all have the other colour (internal layout: same row i or i+-1, rows y+-1 same i)
-    const int ie = par ? (i + 1 == Lh ? 0 : i + 1) : i;
-    const int iw = par ? i : (i == 0 ? Lh - 1 : i - 1);
     const int yn = (y + 1 == p.L) ? 0 : y + 1, ys = (y == 0) ? p.L - 1 : y - 1;
-    const size_t ae = (size_t)y * row4 + (size_t)ie * RQ, aw = (size_t)y * row4 + (size_t)iw * RQ;
-    const size_t an = (size_t)yn * row4 + (size_t)i * RQ, as = (size_t)ys * row4 + (size_t)i * RQ;
 
-    float4 s[3], h[3], nb[3];
+    // Addresses = three per-thread pointers (S + e, H + e, S + e1) plus offsets that depend only on
+    // blockIdx and the parameters (uniform registers).  The four neighbours have the other colour:
+    // rows y+-1 at the same in-row index i (offset e), row y at i (e) and i+-1 (e1).
+    const int i1 = par ? (i + 1 == Lh ? 0 : i + 1) : (i == 0 ? Lh - 1 : i - 1);
+    const uint32_t e1 = (uint32_t)(i1 * RQ + rq);
+    float4 *const Se = reinterpret_cast<float4 *>(p.S) + e;
+    const float4 *const He = reinterpret_cast<const float4 *>(p.H) + e;
+    const float4 *const Se1 = reinterpret_cast<const float4 *>(p.S) + e1;
+    const size_t u_own = (size_t)p.colour * 3 * plane4 + (size_t)y * row4;
+    const size_t u_oth = (size_t)(1 - p.colour) * 3 * plane4;
+    const size_t u_o0 = u_oth + (size_t)y * row4, u_on = u_oth + (size_t)yn * row4, u_os = u_oth + (size_t)ys * row4;
+    float4 *own = Se + u_own;
+    const float4 *hf = He + u_own, *o0 = Se + u_o0, *o1 = Se1 + u_o0, *on = Se + u_on, *os = Se + u_os;
+
+    f2 s[3][2], h[3][2], nb[3][2];
+    {
+        f2 a[3][2], b[3][2], c[3][2], d[3][2];
 #pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        s[c] = own[c * plane4];
-        h[c] = __ldg(hf + c * plane4);
-        const float4 a = __ldg(oth + c * plane4 + ae), b = __ldg(oth + c * plane4 + aw);
-        const float4 cc = __ldg(oth + c * plane4 + an), d = __ldg(oth + c * plane4 + as);
-        nb[c] = make_float4((a.x + b.x) + (cc.x + d.x), (a.y + b.y) + (cc.y + d.y), (a.z + b.z) + (cc.z + d.z),
-                            (a.w + b.w) + (cc.w + d.w));
+        for (int k = 0; k < 3; ++k) {
+            ld2(own + k * plane4, s[k][0], s[k][1]);
+            ld2(hf + k * plane4, h[k][0], h[k][1]);
+            ld2(o0 + k * plane4, a[k][0], a[k][1]);
+            ld2(o1 + k * plane4, b[k][0], b[k][1]);
+            ld2(on + k * plane4, c[k][0], c[k][1]);
+            ld2(os + k * plane4, d[k][0], d[k][1]);
+        }
+#pragma unroll
+        for (int k = 0; k < 3; ++k)
+#pragma unroll
+            for (int j = 0; j < 2; ++j) nb[k][j] = f2_add(f2_add(a[k][j], b[k][j]), f2_add(c[k][j], d[k][j]));
     }
-    const float4 invT = __ldg(reinterpret_cast<const float4 *>(p.invT) + rq);
-    const float4 K2 = __ldg(reinterpret_cast<const float4 *>(p.K2) + rq);
-    const float4 K4 = __ldg(reinterpret_cast<const float4 *>(p.K4) + rq);
+    f2 invT[2], K2[2], K4[2];
+    ld2(reinterpret_cast<const float4 *>(p.invT) + rq, invT[0], invT[1]);
+    ld2(reinterpret_cast<const float4 *>(p.K2) + rq, K2[0], K2[1]);
+    ld2(reinterpret_cast<const float4 *>(p.K4) + rq, K4[0], K4[1]);
 
     const uint32_t n = (uint32_t)(y * p.L + 2 * i + par);
     const uint32_t r0 = 4u * (uint32_t)rq;
-    float *sxp = &s[0].x, *syp = &s[1].x, *szp = &s[2].x;
-    const float *hxp = &h[0].x, *hyp = &h[1].x, *hzp = &h[2].x;
-    const float *nxp = &nb[0].x, *nyp = &nb[1].x, *nzp = &nb[2].x;
-    const float *tp = &invT.x, *k2p = &K2.x, *k4p = &K4.x;
-    bool any = false;
+    uint4 rnd[4];
 #pragma unroll
-    for (int k = 0; k < 4; ++k) {
-        const Trial t = decide(p, rk, n, r0 + k, sxp[k], syp[k], szp[k], nxp[k], nyp[k], nzp[k], hxp[k], hyp[k], hzp[k],
-                               tp[k], k2p[k], k4p[k]);
-        if (t.acc) {
-            sxp[k] = t.tx;
-            syp[k] = t.ty;
-            szp[k] = t.tz;
+    for (int k = 0; k < 4; ++k) rnd[k] = philox4x32_10(make_uint4(n, r0 + k, p.step_lo, p.step_hi), rk);
+
+    bool any = false;
+    float mg[4];
+#pragma unroll
+    for (int j = 0; j < 2; ++j) {
+        const Pair t = decide2(p, rnd[2 * j], rnd[2 * j + 1], s[0][j], s[1][j], s[2][j], nb[0][j], nb[1][j], nb[2][j],
+                               h[0][j], h[1][j], h[2][j], invT[j], K2[j], K4[j]);
+        float m0, m1, a0, a1, b0, b1;
+        f2_split(t.margin, m0, m1);
+        const bool acc0 = m0 < 0.0f, acc1 = m1 < 0.0f;
+        const f2 tr[3] = {t.tx, t.ty, t.tz};
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            f2_split(tr[k], a0, a1);
+            f2_split(s[k][j], b0, b1);
+            s[k][j] = f2_make(acc0 ? a0 : b0, acc1 ? a1 : b1);
         }
-        any |= t.acc;
-        if (p.accept_out) p.accept_out[(size_t)(r0 + k) * p.L * p.L + n] = t.acc ? 1 : 0;
-        if (p.margin_out) p.margin_out[(size_t)(r0 + k) * p.L * p.L + n] = t.margin;
+        any |= acc0 | acc1;
+        mg[2 * j] = m0;
+        mg[2 * j + 1] = m1;
     }
     if (any) {
 #pragma unroll
-        for (int c = 0; c < 3; ++c) own[c * plane4] = s[c];
+        for (int k = 0; k < 3; ++k)
+            *reinterpret_cast<ulonglong2 *>(own + k * plane4) = make_ulonglong2(s[k][0], s[k][1]);
+    }
+    if (HOOKS) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const size_t o = (size_t)(r0 + k) * p.L * p.L + n;
+            if (p.accept_out) p.accept_out[o] = mg[k] < 0.0f ? 1 : 0;
+            if (p.margin_out) p.margin_out[o] = mg[k];
+        }
     }
 }
 
@@ -237,7 +373,8 @@ cudaError_t launch_metropolis(const MetropolisArgs &a, cudaStream_t st, uint64_t
         }
         const unsigned per_row = (unsigned)((a.L / 2) * RQ);
         dim3 grid((per_row + 127) / 128, a.L);
-        metropolis4_kernel<<<grid, 128, 0, st>>>(b, rk);
+        if (a.accept_out || a.margin_out) metropolis4_kernel<true><<<grid, 128, 0, st>>>(b, rk);
+        else metropolis4_kernel<false><<<grid, 128, 0, st>>>(b, rk);
     } else {
         const size_t total = (size_t)a.L * (a.L / 2) * a.R;
         metropolis1_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(a, rk);
