@@ -15,6 +15,7 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", 
 def _deps():
     d = [os.path.join(CSRC, s) for s in SOURCES]
     d.append(os.path.join(CSRC, "dsmc_internal.cuh"))
+    d.append(os.path.join(CSRC, "bulk_copy.cuh"))
     d.append(os.path.join(HERE, "..", "include", "dsmc.h"))
     return d
 

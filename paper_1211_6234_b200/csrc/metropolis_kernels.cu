@@ -145,12 +145,14 @@ __device__ __forceinline__ float mant(uint32_t x) { return __uint_as_float(0x3F8
 //     (the polynomials of sphere_point, valid on [-1, 1] by parity):
 //       cos phi = -cos(pi v) = (S - C)(S + C),   sin phi = -sin(pi v) = (-2 S) C,
 //     no quadrant selects; max abs error 4.5e-7.
+struct Trial2 {
+    f2 tx, ty, tz, lnu;   // trial spins and ln u of two replicas: functions of the random words only
+};
 struct Pair {
     f2 tx, ty, tz, margin;
 };
-__device__ __forceinline__ Pair decide2(const MetropolisArgs &p, uint4 ra, uint4 rb, f2 sx, f2 sy, f2 sz, f2 nx, f2 ny,
-                                        f2 nz, f2 hx, f2 hy, f2 hz, f2 invT, f2 K2, f2 K4) {
-    Pair t;
+__device__ __forceinline__ Trial2 trial2(uint4 ra, uint4 rb) {
+    Trial2 t;
     const f2 c2 = f2_bc(2.0f), cm15 = f2_bc(-1.5f), ulp = f2_bc(1.1920928955078125e-7f);
     const f2 z = f2_fma(c2, f2_add(f2_make(mant(ra.x), mant(rb.x)), cm15), ulp);
     const f2 v = f2_fma(c2, f2_add(f2_make(mant(ra.y), mant(rb.y)), cm15), ulp);
@@ -176,6 +178,15 @@ __device__ __forceinline__ Pair decide2(const MetropolisArgs &p, uint4 ra, uint4
     t.tx = f2_mul(rho, cs);
     t.ty = f2_mul(rho, sn);
     t.tz = z;
+    float u0, u1;
+    f2_split(u, u0, u1);
+    t.lnu = f2_mul(f2_make(lg2_approx(u0), lg2_approx(u1)), f2_bc(0.693147180559945f));
+    return t;
+}
+// margin = dE / T + ln u for the two trials (eq. 7; R12-R14)
+__device__ __forceinline__ f2 margin2(const MetropolisArgs &p, const Trial2 &t, f2 sx, f2 sy, f2 sz, f2 nx, f2 ny, f2 nz,
+                                      f2 hx, f2 hy, f2 hz, f2 invT, f2 K2, f2 K4) {
+    const f2 z = t.tz;
     const f2 dx = f2_sub(t.tx, sx), dy = f2_sub(t.ty, sy), dz = f2_sub(z, sz);
     const f2 dz2 = f2_mul(dz, f2_add(z, sz));                              // s'_z^2 - s_z^2
     const f2 z2sum = f2_fma(z, z, f2_mul(sz, sz));
@@ -187,10 +198,15 @@ __device__ __forceinline__ Pair decide2(const MetropolisArgs &p, uint4 ra, uint4
     const f2 ez = f2_fma(f2_bc(0.5f * p.w0zz), dz, hz);
     const f2 dip = f2_fma(dx, ex, f2_fma(dy, ey, f2_mul(dz, ez)));
     dE = f2_fma(f2_bc(p.g), dip, dE);
-    float u0, u1;
-    f2_split(u, u0, u1);
-    t.margin = f2_fma(f2_make(lg2_approx(u0), lg2_approx(u1)), f2_bc(0.693147180559945f), f2_mul(dE, invT));
-    return t;
+    return f2_fma(dE, invT, t.lnu);
+}
+__device__ __forceinline__ Pair decide2(const MetropolisArgs &p, uint4 ra, uint4 rb, f2 sx, f2 sy, f2 sz, f2 nx, f2 ny,
+                                        f2 nz, f2 hx, f2 hy, f2 hz, f2 invT, f2 K2, f2 K4) {
+    const Trial2 t = trial2(ra, rb);
+    Pair o;
+    o.tx = t.tx, o.ty = t.ty, o.tz = t.tz;
+    o.margin = margin2(p, t, sx, sy, sz, nx, ny, nz, hx, hy, hz, invT, K2, K4);
+    return o;
 }
 
 __device__ __forceinline__ void ld2(const float4 *ptr, f2 &lo, f2 &hi) {
@@ -363,6 +379,7 @@ RoundKeys make_round_keys(uint32_t lo, uint32_t hi) {
 
 cudaError_t launch_metropolis(const MetropolisArgs &a, cudaStream_t st, uint64_t *launches) {
     const RoundKeys rk = make_round_keys(a.seed_lo, a.seed_hi);
+    cudaError_t err = cudaSuccess;
     if (a.R % 4 == 0 && a.L <= 65535) {
         MetropolisArgs b = a;
         const int RQ = a.R / 4;
@@ -375,12 +392,14 @@ cudaError_t launch_metropolis(const MetropolisArgs &a, cudaStream_t st, uint64_t
         dim3 grid((per_row + 127) / 128, a.L);
         if (a.accept_out || a.margin_out) metropolis4_kernel<true><<<grid, 128, 0, st>>>(b, rk);
         else metropolis4_kernel<false><<<grid, 128, 0, st>>>(b, rk);
+        err = cudaGetLastError();
     } else {
         const size_t total = (size_t)a.L * (a.L / 2) * a.R;
         metropolis1_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(a, rk);
+        err = cudaGetLastError();
     }
     ++*launches;
-    return cudaGetLastError();
+    return err;
 }
 
 cudaError_t launch_init_spins(float *S, int L, int R, int mode, uint64_t seed, cudaStream_t st,
