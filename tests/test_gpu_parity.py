@@ -278,3 +278,143 @@ def test_ragged_shape_field_and_sweep(dsmc_mod, oracle):
     T = np.linspace(0.3, 1.5, R).astype(np.float32)
     lockstep(dsmc_mod, oracle, ctx, W, T, 0.4, -0.1, 1.0, g, seed=77, steps=6)
     ctx.close()
+
+
+def test_halfsweep_parity_L256_sampled(dsmc_mod, oracle):
+    """Config 5 at full size, in the launch configuration bench.py times (tiled field kernel +
+    4-replica Metropolis kernel): decisions, margins and new spins at sampled active sites of every
+    replica, each recomputed one by one by the oracle (direct-sum field, trial draw, dE)."""
+    from paper_1211_6234_b200 import inputs
+    c = inputs.CONFIGS[5]
+    L, R, g = c["L"], c["R"], c["g"]
+    K2, K4 = inputs.anisotropy(5)
+    T = inputs.temperatures(5)
+    seed = inputs.SEED_BASE + 5
+    ctx = make_ctx(dsmc_mod, 5, inputs)
+    assert ctx.field_kernel_kind() == 1
+    W = oracle.build_tensor_ewald(L)
+    ctx.set_spins(inputs.initial_spins(5))
+    acc_d = torch.zeros((R, L, L), dtype=torch.uint8, device="cuda")
+    mar_d = torch.zeros((R, L, L), dtype=torch.float32, device="cuda")
+    rng = np.random.default_rng(11)
+    ambiguous = trials = 0
+    for step in (0, 1):
+        s_before = ctx.get_spins()
+        ctx.halfsweep(T, seed, step, accept_out=acc_d, margin_out=mar_d)
+        s_after = ctx.get_spins()
+        acc = acc_d.cpu().numpy().reshape(R, L * L)
+        mar = mar_d.cpu().numpy().reshape(R, L * L)
+        xs, ys = rng.integers(0, L, 24), rng.integers(0, L, 24)
+        xs = (xs - ((xs + ys) % 2 != step)) % L                      # move onto the active colour
+        assert np.all((xs + ys) % 2 == step)
+        # include the lattice corners' neighbourhood (periodic wrap of the neighbour fetch)
+        targets = np.unique(np.concatenate([ys * L + xs, [step * 1, (L - 1) * L + (L - 1 - (1 - step)) % L]])).astype(np.int32)
+        targets = targets[((targets % L) + (targets // L)) % 2 == step]
+        for r in range(R):
+            s_one = s_before[r].astype(np.float64)
+            h = oracle.dipole_field_sampled(W, s_one, targets)
+            for k, n in enumerate(targets):
+                s_new, u, _ = oracle.trial_draw(seed, int(n), r, step)
+                dE = oracle.delta_e(W, s_one, h[k], int(n), s_new, 1.0, g, float(K2[r]), float(K4[r]))
+                m_or = dE / float(T[r]) + np.log(u)
+                trials += 1
+                assert abs(mar[r, n] - m_or) <= 2e-5 + 3e-6 * abs(m_or), (step, r, n, mar[r, n], m_or)
+                if abs(m_or) < BAND:
+                    ambiguous += 1
+                else:
+                    assert bool(acc[r, n]) == (m_or < 0), (step, r, n, m_or)
+                got = s_after[r, :, n // L, n % L]
+                if acc[r, n]:
+                    assert np.max(np.abs(got - s_new)) <= 1e-6
+                else:
+                    assert np.array_equal(got, s_before[r, :, n // L, n % L])
+        # the other colour is untouched at any size
+        x = np.arange(L)
+        par = (x[:, None] + x[None, :]) % 2
+        assert np.array_equal(s_after[..., par != step], s_before[..., par != step])
+        # every spin is still a unit vector
+        assert np.max(np.abs(np.sum(s_after.astype(np.float64) ** 2, axis=1) - 1.0)) < 1e-6
+    assert ambiguous <= max(1, BAND_FRACTION * trials), (ambiguous, trials)
+    ctx.close()
+
+
+def test_observables_parity_L256_one_replica(dsmc_mod, oracle):
+    """Config 5's lattice size through the tiled kernel: observables of 4 replicas on the GPU, the
+    first one recomputed by the oracle (one full direct-sum field at L = 256)."""
+    from paper_1211_6234_b200 import inputs
+    c = inputs.CONFIGS[5]
+    L, g = c["L"], c["g"]
+    ctx = dsmc_mod.Dsmc(L, 4, J=1.0, g=g, K2=c["K2"], K4=c["K4"])
+    ctx.build_tensor(dsmc_mod.DSMC_W_EWALD)
+    assert ctx.field_kernel_kind() == 1
+    s = inputs.random_spins(L, 4, 21)
+    ctx.set_spins(s)
+    got = ctx.observables()
+    W = oracle.build_tensor_ewald(L)
+    ref = oracle.observables(W, s[:1].astype(np.float64), 1.0, g, c["K2"], c["K4"])
+    assert np.max(np.abs(got[:1] - ref)) <= 2e-6, np.abs(got[:1] - ref)
+    ctx.close()
+
+
+def _window_means(obs):
+    """obs[sweep][R][4] -> mean over the second half of the run, [R][4]"""
+    obs = np.asarray(obs)
+    return obs[obs.shape[0] // 2:].mean(axis=0)
+
+
+def _long_run_compare(dsmc_mod, oracle, L, R, g, K2, K4, T, n_sweeps, n_seeds, start):
+    """north_star: 'Observables over long runs: agreement within 3 sigma'.  Independent seeds on the
+    two sides (so the two sets of chains are statistically independent), the same sweep window,
+    sigma from the across-seed scatter (eq. 13)."""
+    from paper_1211_6234_b200 import inputs
+    W = oracle.build_tensor_ewald(L)
+    ctx = dsmc_mod.Dsmc(L, R, J=1.0, g=g, K2=K2, K4=K4)
+    ctx.build_tensor(dsmc_mod.DSMC_W_EWALD)
+    gpu, cpu = [], []
+    for k in range(n_seeds):
+        seed_g, seed_o = 1000 + k, 2000 + k
+        s0 = inputs.up_spins(L, R) if start == "up" else inputs.random_spins(L, R, seed_g)
+        ctx.set_spins(s0)
+        rec = []
+        for sw in range(n_sweeps):
+            ctx.halfsweep(T, seed_g, 2 * sw)
+            ctx.halfsweep(T, seed_g, 2 * sw + 1)
+            rec.append(ctx.observables())
+        gpu.append(_window_means(rec))
+        s = (inputs.up_spins(L, R) if start == "up" else inputs.random_spins(L, R, seed_o)).astype(np.float64)
+        rec = []
+        for sw in range(n_sweeps):
+            oracle.halfsweep(W, s, T, seed_o, 2 * sw, 1.0, g, K2, K4, want=())
+            oracle.halfsweep(W, s, T, seed_o, 2 * sw + 1, 1.0, g, K2, K4, want=())
+            rec.append(oracle.observables(W, s, 1.0, g, K2, K4))
+        cpu.append(_window_means(rec))
+    ctx.close()
+    gpu, cpu = np.array(gpu), np.array(cpu)                       # [seed][R][4]
+    diff = gpu.mean(0) - cpu.mean(0)
+    sigma = np.sqrt(gpu.var(0, ddof=1) / n_seeds + cpu.var(0, ddof=1) / n_seeds)
+    # m_z of a symmetric double-well flips sign between chains: compare |m_z| there
+    zscore = np.abs(diff) / np.maximum(sigma, 1e-7)
+    return zscore, diff, sigma, gpu, cpu
+
+
+def test_long_run_observables_3sigma(dsmc_mod, oracle):
+    """A config-2-shaped run shortened to what the fp64 oracle finishes in about a minute:
+    L = 16, R = 8, T = 0.2 ... 1.6, g = 0.1, K2 = 0.6, 16 independent seeds per side, 300 sweeps,
+    means over sweeps 150-299 of E/N, m_z, M_par, eta per replica."""
+    L, R = 16, 8
+    T = np.linspace(0.2, 1.6, R).astype(np.float32)
+    z, diff, sigma, gpu, cpu = _long_run_compare(dsmc_mod, oracle, L, R, 0.1, 0.6, 0.0, T, 300, 16, "up")
+    print("max z-score", z.max(), "at", np.unravel_index(z.argmax(), z.shape))
+    assert np.all(z <= 3.0), (z, diff, sigma)
+    # and the runs are not trivially frozen: the hottest replica has disordered, the coldest has not
+    assert abs(gpu.mean(0)[-1, 1]) < 0.3 and gpu.mean(0)[0, 1] > 0.8
+
+
+@pytest.mark.skipif(not __import__("os").environ.get("DSMC_LONG"), reason="set DSMC_LONG=1: config 2 in full (minutes of oracle time)")
+def test_long_run_config2_full(dsmc_mod, oracle):
+    """BASELINE config 2 as written: L = 32, R = 8, 2000 sweeps, 8 seeds per side."""
+    from paper_1211_6234_b200 import inputs
+    c = inputs.CONFIGS[2]
+    T = inputs.temperatures(2)
+    z, diff, sigma, _, _ = _long_run_compare(dsmc_mod, oracle, c["L"], c["R"], c["g"], c["K2"], c["K4"], T, 2000, 8, "random")
+    assert np.all(z <= 3.0), (z, diff, sigma)
