@@ -150,9 +150,15 @@ int dsmc_last_timing(dsmc_ctx *ctx, float *out_ms);
 /* Number of kernels this context has launched since creation (bench.py's gpu_launches).       */
 uint64_t dsmc_launch_count(dsmc_ctx *ctx);
 
-/* Which field kernel runs: 0 = generic (any even L, any R), 1 = tiled (register-tiled,
- * TMA-staged; needs L % 16 == 0 and R % 4 == 0).  dsmc_select_field_kernel: kind -1 = automatic
- * (tiled when the shape allows), 0 = force generic, 1 = tiled (DSMC_EINVAL if unsupported).     */
+/* Which field kernel runs (all three compute the same a1 and meet the same tolerances):
+ *   DSMC_FIELD_GENERIC 0  direct sum, any even L, any R;
+ *   DSMC_FIELD_TILED   1  direct sum, register-tiled and TMA-staged; needs L % 16 == 0 and R % 4 == 0;
+ *   DSMC_FIELD_FFT     2  circular convolution by batched 2-D FFT over replica pairs (PAPER.md:295
+ *                         "more efficient parallelization of the dipole sum");
+ *                         needs L in {32, 64, 128, 256, 512} and even R.
+ * dsmc_select_field_kernel: kind -1 = automatic (the direct sum: tiled when the shape allows, else
+ * generic), or one of the three (DSMC_EINVAL if the shape does not support it).                  */
+enum { DSMC_FIELD_AUTO = -1, DSMC_FIELD_GENERIC = 0, DSMC_FIELD_TILED = 1, DSMC_FIELD_FFT = 2 };
 int dsmc_field_kernel_kind(dsmc_ctx *ctx);
 int dsmc_select_field_kernel(dsmc_ctx *ctx, int kind);
 

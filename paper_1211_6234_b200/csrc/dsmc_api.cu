@@ -64,18 +64,34 @@ int upload_params(dsmc_ctx *ctx, const float *T) {
     return DSMC_OK;
 }
 
-bool use_tiled(const dsmc_ctx *ctx) { return ctx->force_generic ? false : dsmc_tiled_supported(ctx->L, ctx->R); }
+// which field kernel runs: 0 generic, 1 tiled, 2 FFT.  Automatic = the direct sum SURVEY.md section 8
+// scopes (tiled when the shape allows, else generic); the FFT route is chosen explicitly.
+int field_kind(const dsmc_ctx *ctx) {
+    if (ctx->field_kind >= 0) return ctx->field_kind;
+    return dsmc_tiled_supported(ctx->L, ctx->R) ? 1 : 0;
+}
 
+// colour = -1: both colours
 int run_field(dsmc_ctx *ctx, int colour) {
-    cudaError_t e;
-    if (use_tiled(ctx))
-        e = launch_field_tiled(ctx->S(), ctx->Wk(), ctx->Hpart(), ctx->H(), ctx->L, ctx->R, colour, ctx->sm_count,
-                               ctx->stream, &ctx->launches);
-    else
-        e = launch_field_generic(ctx->S(), ctx->Wc(), ctx->H(), ctx->L, ctx->R, colour, ctx->stream,
-                                 &ctx->launches);
+    cudaError_t e = cudaSuccess;
+    const int kind = field_kind(ctx);
+    if (kind == 2) {
+        e = launch_field_fft(ctx->S(), ctx->M(), ctx->Z(), ctx->H(), ctx->L, ctx->R, colour, ctx->stream,
+                             &ctx->launches);
+    } else {
+        for (int q = 0; q < 2 && e == cudaSuccess; ++q) {
+            if (colour >= 0 && colour != q) continue;
+            if (kind == 1)
+                e = launch_field_tiled(ctx->S(), ctx->Wk(), ctx->Hpart(), ctx->H(), ctx->L, ctx->R, q, ctx->sm_count,
+                                       ctx->stream, &ctx->launches);
+            else
+                e = launch_field_generic(ctx->S(), ctx->Wc(), ctx->H(), ctx->L, ctx->R, q, ctx->stream,
+                                         &ctx->launches);
+        }
+    }
     if (e != cudaSuccess) return cuda_fail(ctx, e, "dipole field launch");
-    ctx->field_valid[colour] = true;
+    for (int q = 0; q < 2; ++q)
+        if (colour < 0 || colour == q) ctx->field_valid[q] = true;
     return DSMC_OK;
 }
 
@@ -87,6 +103,9 @@ int after_tensor_change(dsmc_ctx *ctx) {
            "read W(0)");
     if (dsmc_tiled_supported(ctx->L, ctx->R))
         CU(launch_make_wk(ctx->Wc(), ctx->Wk(), ctx->L, ctx->stream, &ctx->launches), "W kernel layout");
+    if (dsmc_fft_supported(ctx->L, ctx->R))
+        CU(launch_make_fft_table(ctx->Wc(), ctx->M(), ctx->Z(), ctx->L, ctx->stream, &ctx->launches),
+           "W spectral table");
     CU(cudaStreamSynchronize(ctx->stream), "tensor sync");
     ctx->tensor_built = true;
     ctx->field_valid[0] = ctx->field_valid[1] = false;
@@ -105,6 +124,9 @@ DsmcLayout dsmc_make_layout(int L, int R) {
     l.off_H = o; o = align256(o + sizeof(float) * 6 * Nh * R);
     l.off_Hpart = o;
     o = align256(o + (dsmc_tiled_supported(L, R) ? sizeof(float) * DSMC_KS_MAX * 3 * Nh * R : 0));
+    const bool fft = dsmc_fft_supported(L, R);
+    l.off_M = o; o = align256(o + (fft ? sizeof(float) * dsmc_fft_m_floats(L) : 0));
+    l.off_Z = o; o = align256(o + (fft ? dsmc_fft_scratch_bytes(L, R) : 0));
     l.off_stage = o; o = align256(o + sizeof(float) * 3 * N * R);
     l.off_T = o; o = align256(o + sizeof(float) * 3 * R);
     l.off_obs = o; o = align256(o + sizeof(double) * 8 * R);
@@ -246,9 +268,7 @@ int dsmc_dipole_field(dsmc_ctx *ctx, int colour, float *h_out, int where) {
     if (colour < -1 || colour > 1) return fail(ctx, DSMC_EINVAL, "colour must be -1, 0 or 1");
     if (!ctx->tensor_built) return fail(ctx, DSMC_ESTATE, "tensor not built");
     if (!ctx->spins_set) return fail(ctx, DSMC_ESTATE, "spins not set");
-    for (int q = 0; q < 2; ++q)
-        if (colour < 0 || colour == q)
-            if (int rc = run_field(ctx, q)) return rc;
+    if (int rc = run_field(ctx, colour)) return rc;
     if (h_out) {
         const size_t bytes = sizeof(float) * 3 * (size_t)ctx->L * ctx->L * ctx->R;
         float *dst = h_out;
@@ -329,8 +349,7 @@ int dsmc_observables(dsmc_ctx *ctx, double *out) {
     if (!ctx->tensor_built) return fail(ctx, DSMC_ESTATE, "tensor not built");
     if (!ctx->spins_set) return fail(ctx, DSMC_ESTATE, "spins not set");
     if (int rc = upload_params(ctx, ctx->T_valid ? nullptr : std::vector<float>(ctx->R, 1.0f).data())) return rc;
-    for (int q = 0; q < 2; ++q)
-        if (int rc = run_field(ctx, q)) return rc;
+    if (int rc = run_field(ctx, -1)) return rc;
     CU(launch_observables(ctx->S(), ctx->H(), ctx->K2d(), ctx->K4d(), ctx->obs(), ctx->L, ctx->R, ctx->J, ctx->g,
                           ctx->stream, &ctx->launches),
        "observables launch");
@@ -370,12 +389,13 @@ int dsmc_last_timing(dsmc_ctx *ctx, float *out_ms) {
 
 uint64_t dsmc_launch_count(dsmc_ctx *ctx) { return ctx ? ctx->launches : 0; }
 
-int dsmc_field_kernel_kind(dsmc_ctx *ctx) { return ctx && use_tiled(ctx) ? 1 : 0; }
+int dsmc_field_kernel_kind(dsmc_ctx *ctx) { return ctx ? field_kind(ctx) : 0; }
 
 int dsmc_select_field_kernel(dsmc_ctx *ctx, int kind) {
-    if (!ctx || kind < -1 || kind > 1) return fail(ctx, DSMC_EINVAL, "kind must be -1, 0 or 1");
+    if (!ctx || kind < -1 || kind > 2) return fail(ctx, DSMC_EINVAL, "kind must be -1, 0, 1 or 2");
     if (kind == 1 && !dsmc_tiled_supported(ctx->L, ctx->R)) return fail(ctx, DSMC_EINVAL, "tiled kernel needs L % 16 == 0, R % 4 == 0");
-    ctx->force_generic = (kind == 0);
+    if (kind == 2 && !dsmc_fft_supported(ctx->L, ctx->R)) return fail(ctx, DSMC_EINVAL, "FFT field needs L in {32, 64, 128, 256, 512} and even R");
+    ctx->field_kind = kind;
     ctx->field_valid[0] = ctx->field_valid[1] = false;
     return DSMC_OK;
 }

@@ -28,6 +28,8 @@ struct DsmcLayout {
     size_t off_S;      // spins, internal layout
     size_t off_H;      // field, internal layout (both colours)
     size_t off_Hpart;  // partial fields [KS][3][Nh][R] of the tiled kernel
+    size_t off_M;      // spectral multiplier M[slot_x][slot_y][8] of the FFT field (field_fft.cu)
+    size_t off_Z;      // spectrum scratch Z[3][L][L][R/2] complex of the FFT field
     size_t off_stage;  // canonical staging [R][3][L][L] floats
     size_t off_T;      // invT[R], K2[R], K4[R] floats
     size_t off_obs;    // R*8 doubles
@@ -46,7 +48,7 @@ struct dsmc_ctx {
     bool tensor_built = false, spins_set = false;
     bool field_valid[2] = {false, false};
     float w0[4] = {0, 0, 0, 0};  // W(0) components (fp32, as stored)
-    bool force_generic = false;
+    int field_kind = -1;  // -1 automatic, 0 generic, 1 tiled, 2 FFT (dsmc_select_field_kernel)
     int timing = 0;
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
     bool ev_recorded = false;
@@ -59,6 +61,8 @@ struct dsmc_ctx {
     float *S() const { return (float *)(ws + lay.off_S); }
     float *H() const { return (float *)(ws + lay.off_H); }
     float *Hpart() const { return (float *)(ws + lay.off_Hpart); }
+    float *M() const { return (float *)(ws + lay.off_M); }
+    void *Z() const { return (void *)(ws + lay.off_Z); }
     float *stage() const { return (float *)(ws + lay.off_stage); }
     float *invT() const { return (float *)(ws + lay.off_T); }
     float *K2d() const { return invT() + R; }
@@ -87,6 +91,15 @@ cudaError_t launch_internal_to_canon(const float *S, float *canon, int L, int R,
 
 cudaError_t launch_field_generic(const float *S, const float *Wc, float *H, int L, int R, int colour,
                                  cudaStream_t st, uint64_t *launches);
+// FFT field (field_fft.cu): L in {32, ..., 512}, R even
+bool dsmc_fft_supported(int L, int R);
+size_t dsmc_fft_m_floats(int L);
+size_t dsmc_fft_scratch_bytes(int L, int R);
+cudaError_t launch_make_fft_table(const float *Wc, float *M, void *scratch, int L, cudaStream_t st,
+                                  uint64_t *launches);
+// colour = -1 writes both colours of H with one convolution
+cudaError_t launch_field_fft(const float *S, const float *M, void *scratch, float *H, int L, int R, int colour,
+                             cudaStream_t st, uint64_t *launches);
 cudaError_t launch_field_tiled(const float *S, const float *Wk, float *Hpart, float *H, int L, int R,
                                int colour, int sm_count, cudaStream_t st, uint64_t *launches);
 
