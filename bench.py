@@ -197,6 +197,34 @@ def run_cuda(args):
     ctx.set_timing(False)
     clocks = sampler.stop() if sampler else None
 
+    # ---- the same sweep with the FFT route of the field, reported beside ------
+    fft = None
+    if ctx.fft_supported():
+        ctx.select_field_kernel(m.DSMC_FIELD_FFT)
+        base = 4 * (args.warmup + 2 * args.steps + 8)
+        for k in range(args.warmup):
+            sweep(base + k)
+        torch.cuda.synchronize(dev)
+        n_fft = max(50, args.steps)
+        l0f = ctx.launch_count()
+        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ctx.dipole_field(0, want_output=False)            # the host gets ahead of the GPU (short kernels)
+        f0.record()
+        for k in range(n_fft):
+            sweep(base + args.warmup + k)
+        f1.record()
+        torch.cuda.synchronize(dev)
+        fft_ms = f0.elapsed_time(f1) / n_fft
+        fft_launches = (ctx.launch_count() - l0f - 3) / n_fft
+        ctx.set_timing(True)
+        ff = []
+        for k in range(10):
+            ctx.halfsweep(None, seed, 2 * (base + args.warmup + n_fft) + k)
+            ff.append(float(ctx.last_timing()[0]))
+        ctx.set_timing(False)
+        ctx.select_field_kernel(m.DSMC_FIELD_AUTO)
+        fft = {"ms_per_step": fft_ms, "field_ms_per_launch_group": float(np.median(ff)), "launches_per_step": fft_launches}
+
     # Metropolis kernel alone with a working set larger than L2: three independent contexts are
     # updated in rotation, so the ~100 MB a launch touches were evicted by the ~200 MB the two
     # launches in between touched.  One event pair brackets the whole batch (no per-launch gaps).
@@ -292,6 +320,21 @@ def run_cuda(args):
                                 "ms_per_launch_in_sweep": metro_ms, "bytes_per_launch": metro_bytes,
                                 "updates_per_s": (N // 2) * R / (metro_cold_ms * 1e-3), "traffic": None},
     }
+    if fft is not None:
+        # algorithmic HBM bytes of one half-sweep field by FFT: read every spin (12 B per site and replica),
+        # write h of the active colour (12 B per active site and replica); the spectrum scratch is overhead
+        fft_bytes = 12.0 * N * R + 12.0 * (N // 2) * R
+        gbs = fft_bytes / (fft["field_ms_per_launch_group"] * 1e-3) / 1e9
+        line["fft_path"] = {
+            "what": "the same sweep with dsmc_select_field_kernel(DSMC_FIELD_FFT): the field as a batched 2-D FFT "
+                    "convolution over replica pairs (3 kernels), same parity tolerances; not the path 'value' times",
+            "value": world * updates_per_step / (fft["ms_per_step"] * 1e-3), "unit": "updates/s",
+            "ms_per_step": fft["ms_per_step"], "gpu_launches_per_step": fft["launches_per_step"],
+            "speedup_vs_direct_sum": ms_per_step / fft["ms_per_step"],
+            "roofline": {"kernel": "fft_x_forward + fft_y_multiply + fft_x_inverse", "bound": "hbm", "achieved": gbs,
+                         "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak, "peak_kind": hbm_kind,
+                         "ms_per_launch_group": fft["field_ms_per_launch_group"], "bytes_per_launch_group": fft_bytes,
+                         "traffic": None}}
     if world == 1 and not args.no_cpu_baseline:
         ups, sec, cores = oracle_sample(1, 0, 8)
         line["cpu_baseline"] = {"value": ups, "unit": "updates/s", "cores": cores, "kind": "oracle",

@@ -161,6 +161,8 @@ uint64_t dsmc_launch_count(dsmc_ctx *ctx);
 enum { DSMC_FIELD_AUTO = -1, DSMC_FIELD_GENERIC = 0, DSMC_FIELD_TILED = 1, DSMC_FIELD_FFT = 2 };
 int dsmc_field_kernel_kind(dsmc_ctx *ctx);
 int dsmc_select_field_kernel(dsmc_ctx *ctx, int kind);
+/* 1 if this context's shape supports the kernel `kind` (0, 1, 2), else 0.                         */
+int dsmc_field_kernel_supported(dsmc_ctx *ctx, int kind);
 
 /* Measured fp32 FMA issue peak of this GPU in TFLOP/s: a dependency-free FFMA-chain microbenchmark
  * (one CTA of 256 threads per SM, 96 independent accumulators per thread), the denominator

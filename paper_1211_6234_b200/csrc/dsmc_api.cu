@@ -391,6 +391,14 @@ uint64_t dsmc_launch_count(dsmc_ctx *ctx) { return ctx ? ctx->launches : 0; }
 
 int dsmc_field_kernel_kind(dsmc_ctx *ctx) { return ctx ? field_kind(ctx) : 0; }
 
+int dsmc_field_kernel_supported(dsmc_ctx *ctx, int kind) {
+    if (!ctx) return 0;
+    if (kind == 0) return 1;
+    if (kind == 1) return dsmc_tiled_supported(ctx->L, ctx->R) ? 1 : 0;
+    if (kind == 2) return dsmc_fft_supported(ctx->L, ctx->R) ? 1 : 0;
+    return 0;
+}
+
 int dsmc_select_field_kernel(dsmc_ctx *ctx, int kind) {
     if (!ctx || kind < -1 || kind > 2) return fail(ctx, DSMC_EINVAL, "kind must be -1, 0, 1 or 2");
     if (kind == 1 && !dsmc_tiled_supported(ctx->L, ctx->R)) return fail(ctx, DSMC_EINVAL, "tiled kernel needs L % 16 == 0, R % 4 == 0");

@@ -240,18 +240,21 @@ __device__ __forceinline__ float2 cmac(float2 acc, float2 a, float2 m) {  // acc
 
 // grid (P / LN, L slots), block (LN, 16); shared: twiddles + 3 line buffers
 template <int N2>
-__global__ void __launch_bounds__(256) fft_y_multiply_kernel(const FftParams p) {
+__global__ void __launch_bounds__(256, 2) fft_y_multiply_kernel(const FftParams p) {
     extern __shared__ __align__(16) float2 fsm[];
     const int L = 16 * N2, LN = blockDim.x;
     float2 *tw = fsm;
-    float2 *buf[3] = {fsm + L, fsm + L + (size_t)line_rows<N2>() * LN, fsm + L + 2 * (size_t)line_rows<N2>() * LN};
+    float4 *Msm = reinterpret_cast<float4 *>(fsm + L);     // this column's multiplier, 2 float4 per slot_y
+    float2 *b0 = fsm + L + 4 * L;
+    float2 *buf[3] = {b0, b0 + (size_t)line_rows<N2>() * LN, b0 + 2 * (size_t)line_rows<N2>() * LN};
     const int lane = threadIdx.x, t = threadIdx.y;
     const int pair = blockIdx.x * LN + lane, sx = blockIdx.y;
     fill_twiddles(tw, L);
+    for (int j = t * LN + lane; j < 2 * L; j += 16 * LN) Msm[j] = __ldg(p.M + (size_t)sx * L * 2 + j);
     __syncthreads();
     const size_t rowP = (size_t)L * p.P;                   // one y step in Z
     float2 *col = p.Z + (size_t)sx * p.P + pair;           // + (c * L + y) * rowP
-#pragma unroll
+#pragma unroll 1
     for (int c = 0; c < 3; ++c)
         for (int n2 = t; n2 < N2; n2 += 16) {
             float2 v[16];
@@ -261,31 +264,38 @@ __global__ void __launch_bounds__(256) fft_y_multiply_kernel(const FftParams p) 
         }
     __syncthreads();
     {
-        const float4 *Mrow = p.M + ((size_t)sx * L + N2 * t) * 2;
-        float2 ux[N2], uy[N2];
+        const float4 *Mrow = Msm + (N2 * t) * 2;
+        // The thread owns block t of all three components, so the x spectrum can wait in its own
+        // shared-memory block (natural k2 order) while the y spectrum is transformed: at most one
+        // block lives in registers at a time.
+        float2 ux[N2];
+        float2 *bx = buf[0] + sidx<N2>(t, 0) * LN + lane;
         fwd_step2<N2>(ux, t, buf[0], LN, lane);
-        fwd_step2<N2>(uy, t, buf[1], LN, lane);
+#pragma unroll
+        for (int k2 = 0; k2 < N2; ++k2) bx[k2 * LN] = ux[k2];
+        fwd_step2<N2>(ux, t, buf[1], LN, lane);            // ux now holds the y component
 #pragma unroll
         for (int k2 = 0; k2 < N2; ++k2) {
-            const float4 m0 = __ldg(Mrow + 2 * k2), m1 = __ldg(Mrow + 2 * k2 + 1);
+            const float4 m0 = Mrow[2 * k2], m1 = Mrow[2 * k2 + 1];
             const float2 xx = make_float2(m0.x, m0.y), xy = make_float2(m0.z, m0.w), yy = make_float2(m1.x, m1.y);
-            const float2 hx = cmac(cmul(ux[k2], xx), uy[k2], xy);
-            const float2 hy = cmac(cmul(ux[k2], xy), uy[k2], yy);
-            ux[k2] = hx;
-            uy[k2] = hy;
+            const float2 zx = bx[k2 * LN], zy = ux[k2];
+            bx[k2 * LN] = cmac(cmul(zx, xx), zy, xy);
+            ux[k2] = cmac(cmul(zx, xy), zy, yy);
         }
+        inv_step2<N2>(ux, t, tw, buf[1], LN, lane);
+#pragma unroll
+        for (int k2 = 0; k2 < N2; ++k2) ux[k2] = bx[k2 * LN];
         inv_step2<N2>(ux, t, tw, buf[0], LN, lane);
-        inv_step2<N2>(uy, t, tw, buf[1], LN, lane);
         fwd_step2<N2>(ux, t, buf[2], LN, lane);            // ux reused for the z component
 #pragma unroll
         for (int k2 = 0; k2 < N2; ++k2) {
-            const float4 m1 = __ldg(Mrow + 2 * k2 + 1);
+            const float4 m1 = Mrow[2 * k2 + 1];
             ux[k2] = cmul(ux[k2], make_float2(m1.z, m1.w));
         }
         inv_step2<N2>(ux, t, tw, buf[2], LN, lane);
     }
     __syncthreads();
-#pragma unroll
+#pragma unroll 1
     for (int c = 0; c < 3; ++c)
         for (int n2 = t; n2 < N2; n2 += 16) {
             float2 v[16];
@@ -343,9 +353,11 @@ int pairs_per_cta(int P, int cap) {
 template <int N2>
 cudaError_t launch_fft_n2(const FftParams &p, cudaStream_t st, uint64_t *launches) {
     const int L = 16 * N2;
-    const int LNX = pairs_per_cta(p.P, 32), LNY = pairs_per_cta(p.P, 16);
+    // 16 replica pairs per CTA: 128-byte runs in HBM, and enough CTAs (half rows / half columns) that
+    // the last wave over 148 SMs stays full
+    const int LNX = pairs_per_cta(p.P, 16), LNY = pairs_per_cta(p.P, 16);
     const size_t smx = sizeof(float2) * (L + (size_t)line_rows<N2>() * LNX);
-    const size_t smy = sizeof(float2) * (L + 3 * (size_t)line_rows<N2>() * LNY);
+    const size_t smy = sizeof(float2) * (L + 4 * L + 3 * (size_t)line_rows<N2>() * LNY);
     static bool configured = false;
     if (!configured) {
         cudaError_t e;

@@ -140,7 +140,7 @@ __device__ __forceinline__ float mant(uint32_t x) { return __uint_as_float(0x3F8
 // two differences, both within the parity tolerances:
 //   * u = (2k+1) 2^-24 with k = x >> 9: z = 2u0 - 1 = 2 (y - 1.5) + 2^-23 and v = 2u1 - 1 likewise are
 //     exact in fp32 (y - 1.5 is a multiple of 2^-23 in [-1/2, 1/2); the fma rounds once to a
-//     representable odd multiple of 2^-23), so the trial z is bit-identical to the oracle's;
+//     representable odd multiple of 2^-23), so the trial z carries no rounding error at all;
 //   * azimuth phi = 2 pi u1 = pi v + pi.  With S = sin(pi v / 2) = v P(v^2), C = cos(pi v / 2) = Q(v^2)
 //     (the polynomials of sphere_point, valid on [-1, 1] by parity):
 //       cos phi = -cos(pi v) = (S - C)(S + C),   sin phi = -sin(pi v) = (-2 S) C,

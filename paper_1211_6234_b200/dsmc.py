@@ -41,6 +41,7 @@ ABI = [
     ("dsmc_launch_count", _u64, [_vp]),
     ("dsmc_field_kernel_kind", _i, [_vp]),
     ("dsmc_select_field_kernel", _i, [_vp, _i]),
+    ("dsmc_field_kernel_supported", _i, [_vp, _i]),
     ("dsmc_fp32_fma_peak", _i, [_vp, _vp]),
     ("dsmc_destroy", _i, [_vp]),
     ("dsmc_last_error", ctypes.c_char_p, [_vp]),
@@ -219,6 +220,9 @@ class Dsmc:
         out = ctypes.c_double(0.0)
         self._check(self.lib.dsmc_fp32_fma_peak(self._h, ctypes.addressof(out)))
         return float(out.value)
+
+    def fft_supported(self):
+        return bool(self.lib.dsmc_field_kernel_supported(self._h, DSMC_FIELD_FFT))
 
     def select_field_kernel(self, kind):
         self._check(self.lib.dsmc_select_field_kernel(self._h, kind))
