@@ -570,3 +570,59 @@ int oracle_observables(int L, int R, double J, double g, const double *K2, const
     free(E);
     return 0;
 }
+
+/* ------------------------------------------------------------------------- */
+/* O7. Domain-wall counts (eq. 14) per replica and component */
+/*   n_v^a = sum_i [ 1 - sgn(s_i^a s_{i+y}^a) ],  n_h^a = sum_i [ 1 - sgn(s_i^a s_{i+x}^a) ]  */
+/* with periodic neighbours i+x = ((x+1) mod L, y), i+y = (x, (y+1) mod L), every  */
+/* bond once.  sgn(a b) is taken as sgn(a) sgn(b) (the same number, and immune to   */
+/* the product underflowing), sgn(0) = 0, so every term is 0, 1 or 2 and the sums   */
+/* are integers.  out[r] = { n_h^x, n_v^x, n_h^y, n_v^y, n_h^z, n_v^z }.             */
+/* Derived per snapshot (the thermal averages of eq. 15 and the variances of       */
+/* eq. 18 are statistics the caller takes over snapshots):                         */
+/*   wall density  (n_v^z + n_h^z) / (4N)        */
+/*   O_a = |n_h^a - n_v^a| / (n_h^a + n_v^a)                 (eq. 15, :207);       */
+/*         0 when there is no wall at all (paper silent; R20)            */
+/* ------------------------------------------------------------------------- */
+static int oracle_sgn(double v) { return (v > 0.0) - (v < 0.0); }
+
+int oracle_wall_counts(int L, int R, const double *s, long long *out)
+{
+    if (L < 1 || R < 1 || !s || !out) return -1;
+    size_t N = (size_t)L * L;
+    for (int r = 0; r < R; ++r) {
+        for (int c = 0; c < 3; ++c) {
+            const double *f = s + ((size_t)r * 3 + c) * N;
+            long long nh = 0, nv = 0;
+            for (int y = 0; y < L; ++y) {
+                for (int x = 0; x < L; ++x) {
+                    int si = oracle_sgn(f[(size_t)y * L + x]);
+                    int sx = oracle_sgn(f[(size_t)y * L + (x + 1) % L]);
+                    int sy = oracle_sgn(f[(size_t)((y + 1) % L) * L + x]);
+                    nh += 1 - si * sx;
+                    nv += 1 - si * sy;
+                }
+            }
+            out[6 * r + 2 * c + 0] = nh;
+            out[6 * r + 2 * c + 1] = nv;
+        }
+    }
+    return 0;
+}
+
+/* derived[r] = { wall density, O_x, O_y, O_z } from the counts of oracle_wall_counts */
+int oracle_wall_order(int L, int R, const long long *counts, double *derived)
+{
+    if (L < 1 || R < 1 || !counts || !derived) return -1;
+    double N = (double)L * (double)L;
+    for (int r = 0; r < R; ++r) {
+        const long long *n = counts + 6 * r;
+        derived[4 * r + 0] = (double)(n[4] + n[5]) / (4.0 * N);
+        for (int c = 0; c < 3; ++c) {
+            long long nh = n[2 * c], nv = n[2 * c + 1];
+            long long d = nh > nv ? nh - nv : nv - nh;
+            derived[4 * r + 1 + c] = (nh + nv) > 0 ? (double)d / (double)(nh + nv) : 0.0;
+        }
+    }
+    return 0;
+}

@@ -207,3 +207,23 @@ def observables(W, s, J, g, K2, K4):
                                   _d(W), _d(s), _d(out))
     assert rc == 0, rc
     return out
+
+
+def wall_counts(s):
+    """eq. 14 per replica: int64 [R][6] = n_h^x, n_v^x, n_h^y, n_v^y, n_h^z, n_v^z."""
+    s = _f64(s)
+    R, _, L, _ = s.shape
+    out = np.zeros((R, 6), dtype=np.int64)
+    rc = lib().oracle_wall_counts(L, R, _d(s), out.ctypes.data_as(ctypes.POINTER(ctypes.c_longlong)))
+    assert rc == 0, rc
+    return out
+
+
+def wall_order(L, counts):
+    """[R][4] = wall density, O_x, O_y, O_z (eq. 15, per snapshot)."""
+    counts = np.ascontiguousarray(counts, dtype=np.int64)
+    R = counts.shape[0]
+    out = np.zeros((R, 4), dtype=np.float64)
+    rc = lib().oracle_wall_order(L, R, counts.ctypes.data_as(ctypes.POINTER(ctypes.c_longlong)), _d(out))
+    assert rc == 0, rc
+    return out
