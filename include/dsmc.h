@@ -141,6 +141,16 @@ int dsmc_run(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_step, 
  * Synchronises the stream.                                                                      */
 int dsmc_observables(dsmc_ctx *ctx, double *out);
 
+/* Domain-wall observables of the current state (eq. 14-15), HOST outputs:
+ *   counts_out[R][6] = n_h^x, n_v^x, n_h^y, n_v^y, n_h^z, n_v^z with
+ *     n_h^a = sum_i 1 - sgn(s_i^a s_{i+x}^a),  n_v^a = sum_i 1 - sgn(s_i^a s_{i+y}^a)   (eq. 14),
+ *     periodic neighbours, every bond once, sgn(ab) taken as sgn(a) sgn(b), sgn(0) = 0: exact integers;
+ *   derived_out[R][4] (nullable) = wall density (n_v^z + n_h^z) / (4N) and the
+ *     per-snapshot orientational order O_a = |n_h^a - n_v^a| / (n_h^a + n_v^a), a = x, y, z (eq. 15;
+ *     0 when the component has no wall).  The thermal averages of eq. 15 and the variances of
+ *     eq. 18 are statistics the caller takes over snapshots.  Needs no field; synchronises.        */
+int dsmc_wall_observables(dsmc_ctx *ctx, long long *counts_out, double *derived_out);
+
 /* Device time in milliseconds of the last field / Metropolis / reduction launches made by the
  * last dsmc_halfsweep* call, measured with CUDA events on the bound stream when timing was
  * enabled with dsmc_set_timing(ctx, 1); synchronises.  out[3] = {field, metropolis, total}.      */

@@ -369,6 +369,31 @@ int dsmc_observables(dsmc_ctx *ctx, double *out) {
     return DSMC_OK;
 }
 
+int dsmc_wall_observables(dsmc_ctx *ctx, long long *counts_out, double *derived_out) {
+    if (int rc = need_bound(ctx)) return rc;
+    if (!counts_out) return fail(ctx, DSMC_EINVAL, "null argument");
+    if (!ctx->spins_set) return fail(ctx, DSMC_ESTATE, "spins not set");
+    unsigned long long *dev = reinterpret_cast<unsigned long long *>(ctx->obs());
+    CU(launch_wall_counts(ctx->S(), dev, ctx->L, ctx->R, ctx->stream, &ctx->launches), "wall counts launch");
+    std::vector<unsigned long long> raw(8 * (size_t)ctx->R);
+    CU(cudaMemcpyAsync(raw.data(), dev, sizeof(unsigned long long) * raw.size(), cudaMemcpyDeviceToHost, ctx->stream),
+       "wall counts D2H");
+    CU(cudaStreamSynchronize(ctx->stream), "wall counts sync");
+    const double N = (double)ctx->L * ctx->L;
+    for (int r = 0; r < ctx->R; ++r) {
+        const unsigned long long *n = &raw[8 * (size_t)r];
+        for (int k = 0; k < 6; ++k) counts_out[6 * r + k] = (long long)n[k];
+        if (derived_out) {
+            derived_out[4 * r] = (double)(n[4] + n[5]) / (4.0 * N);
+            for (int c = 0; c < 3; ++c) {
+                const unsigned long long nh = n[2 * c], nv = n[2 * c + 1];
+                derived_out[4 * r + 1 + c] = nh + nv ? (double)(nh > nv ? nh - nv : nv - nh) / (double)(nh + nv) : 0.0;
+            }
+        }
+    }
+    return DSMC_OK;
+}
+
 int dsmc_set_timing(dsmc_ctx *ctx, int on) {
     if (!ctx) return DSMC_EINVAL;
     ctx->timing = on ? 1 : 0;

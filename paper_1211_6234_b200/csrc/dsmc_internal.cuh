@@ -120,3 +120,5 @@ cudaError_t launch_init_spins(float *S, int L, int R, int mode, uint64_t seed, c
 cudaError_t launch_observables(const float *S, const float *H, const float *K2, const float *K4,
                                double *obs, int L, int R, float J, float g, cudaStream_t st,
                                uint64_t *launches);
+cudaError_t launch_wall_counts(const float *S, unsigned long long *counts, int L, int R, cudaStream_t st,
+                               uint64_t *launches);

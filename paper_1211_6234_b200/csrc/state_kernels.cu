@@ -98,6 +98,50 @@ __global__ void __launch_bounds__(256) observables_kernel(const float *__restric
     }
 }
 
+// Domain-wall counts (eq. 14): per replica and component a,
+//   n_h^a = sum_i 1 - sgn(s_i^a) sgn(s_{i+x}^a),   n_v^a = sum_i 1 - sgn(s_i^a) sgn(s_{i+y}^a),
+// every bond once (east and north neighbour of every site), sgn(0) = 0: integer terms 0, 1, 2.
+// Same thread-owns-a-replica walk as observables_kernel; 32-bit per-thread counts, folded per
+// block in shared memory, one 64-bit integer atomicAdd per (replica, count).
+__device__ __forceinline__ int sgnf(float v) { return (v > 0.0f) - (v < 0.0f); }
+
+__global__ void __launch_bounds__(256) wall_counts_kernel(const float *__restrict__ S,
+                                                          unsigned long long *__restrict__ counts, int L, int R) {
+    extern __shared__ unsigned int wsm[];  // [blockDim.x][6]
+    const int Lh = L >> 1;
+    const size_t Nh = (size_t)L * Lh, plane = Nh * (size_t)R;
+    const size_t nthreads = (size_t)gridDim.x * blockDim.x;
+    const size_t gid = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int r = (int)(gid % (size_t)R);
+    unsigned int acc[6] = {0, 0, 0, 0, 0, 0};
+    for (size_t t = gid; t < 2 * plane; t += nthreads) {
+        const size_t qa = t / (size_t)R;
+        const int q = (int)(qa / Nh);
+        const int a = (int)(qa - (size_t)q * Nh);
+        const int y = a / Lh, i = a - y * Lh;
+        const int par = (y + q) & 1;
+        const float *own = S + (size_t)q * 3 * plane + (size_t)a * R + r;
+        const float *oth = S + (size_t)(1 - q) * 3 * plane + r;
+        const int ie = par ? (i + 1 == Lh ? 0 : i + 1) : i;
+        const int yn = (y + 1 == L) ? 0 : y + 1;
+        const size_t ae = ((size_t)y * Lh + ie) * R, an = ((size_t)yn * Lh + i) * R;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const int si = sgnf(own[c * plane]);
+            acc[2 * c + 0] += (unsigned int)(1 - si * sgnf(oth[c * plane + ae]));
+            acc[2 * c + 1] += (unsigned int)(1 - si * sgnf(oth[c * plane + an]));
+        }
+    }
+    for (int k = 0; k < 6; ++k) wsm[threadIdx.x * 6 + k] = acc[k];
+    __syncthreads();
+    if ((int)threadIdx.x < R) {
+        unsigned long long tot[6] = {0, 0, 0, 0, 0, 0};
+        for (int j = threadIdx.x; j < (int)blockDim.x; j += R)
+            for (int k = 0; k < 6; ++k) tot[k] += wsm[j * 6 + k];
+        for (int k = 0; k < 6; ++k) atomicAdd(&counts[(size_t)r * 8 + k], tot[k]);
+    }
+}
+
 }  // namespace
 
 cudaError_t launch_canon_to_internal(const float *canon, float *S, int L, int R, cudaStream_t st,
@@ -116,10 +160,8 @@ cudaError_t launch_internal_to_canon(const float *S, float *canon, int L, int R,
     return cudaGetLastError();
 }
 
-cudaError_t launch_observables(const float *S, const float *H, const float *K2, const float *K4, double *obs,
-                               int L, int R, float, float, cudaStream_t st, uint64_t *launches) {
-    cudaError_t e = cudaMemsetAsync(obs, 0, sizeof(double) * 8 * (size_t)R, st);
-    if (e != cudaSuccess) return e;
+// launch shape of the thread-owns-a-replica walks: grid * block is a multiple of R
+static void replica_walk_shape(int L, int R, int *block_out, unsigned *grid_out) {
     // block size: a multiple of R when R <= 256 (so that every block starts at replica 0),
     // else R threads-per-replica-row blocks of 256 with a grid that keeps gid % R aligned
     int block = 256;
@@ -133,7 +175,30 @@ cudaError_t launch_observables(const float *S, const float *H, const float *K2, 
         const unsigned step = (unsigned)(R / g);
         grid = ((grid + step - 1) / step) * step;
     }
+    *block_out = block;
+    *grid_out = grid;
+}
+
+cudaError_t launch_observables(const float *S, const float *H, const float *K2, const float *K4, double *obs,
+                               int L, int R, float, float, cudaStream_t st, uint64_t *launches) {
+    cudaError_t e = cudaMemsetAsync(obs, 0, sizeof(double) * 8 * (size_t)R, st);
+    if (e != cudaSuccess) return e;
+    int block;
+    unsigned grid;
+    replica_walk_shape(L, R, &block, &grid);
     observables_kernel<<<grid, block, sizeof(double) * 7 * block, st>>>(S, H, K2, K4, obs, L, R);
+    ++*launches;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_wall_counts(const float *S, unsigned long long *counts, int L, int R, cudaStream_t st,
+                               uint64_t *launches) {
+    cudaError_t e = cudaMemsetAsync(counts, 0, sizeof(unsigned long long) * 8 * (size_t)R, st);
+    if (e != cudaSuccess) return e;
+    int block;
+    unsigned grid;
+    replica_walk_shape(L, R, &block, &grid);
+    wall_counts_kernel<<<grid, block, sizeof(unsigned int) * 6 * block, st>>>(S, counts, L, R);
     ++*launches;
     return cudaGetLastError();
 }

@@ -36,6 +36,7 @@ ABI = [
     ("dsmc_halfsweep_ex", _i, [_vp, _vp, _u64, _u64, _i, _vp, _vp]),
     ("dsmc_run", _i, [_vp, _vp, _u64, _u64, _u64]),
     ("dsmc_observables", _i, [_vp, _vp]),
+    ("dsmc_wall_observables", _i, [_vp, _vp, _vp]),
     ("dsmc_set_timing", _i, [_vp, _i]),
     ("dsmc_last_timing", _i, [_vp, _vp]),
     ("dsmc_launch_count", _u64, [_vp]),
@@ -201,6 +202,14 @@ class Dsmc:
         out = np.empty((self.R, 4), dtype=np.float64)
         self._check(self.lib.dsmc_observables(self._h, out.ctypes.data))
         return out
+
+    def wall_observables(self):
+        """-> (counts int64 [R][6] = n_h^x, n_v^x, n_h^y, n_v^y, n_h^z, n_v^z; derived float64 [R][4] =
+        wall density, O_x, O_y, O_z)  (eq. 14-15)"""
+        counts = np.empty((self.R, 6), dtype=np.int64)
+        derived = np.empty((self.R, 4), dtype=np.float64)
+        self._check(self.lib.dsmc_wall_observables(self._h, counts.ctypes.data, derived.ctypes.data))
+        return counts, derived
 
     def set_timing(self, on=True):
         self._check(self.lib.dsmc_set_timing(self._h, int(on)))

@@ -418,3 +418,24 @@ def test_long_run_config2_full(dsmc_mod, oracle):
     T = inputs.temperatures(2)
     z, diff, sigma, _, _ = _long_run_compare(dsmc_mod, oracle, c["L"], c["R"], c["g"], c["K2"], c["K4"], T, 2000, 8, "random")
     assert np.all(z <= 3.0), (z, diff, sigma)
+
+
+@pytest.mark.parametrize("L,R", [(8, 1), (12, 5), (32, 8), (64, 16), (256, 64)])
+def test_wall_observables_parity(dsmc_mod, oracle, L, R):
+    """eq. 14-15: integer wall counts bit-exact against the oracle (random, striped and uniform
+    states, a state with exact zeros), derived ratios to rounding."""
+    from paper_1211_6234_b200 import inputs
+    ctx = dsmc_mod.Dsmc(L, R)
+    x = np.arange(L)
+    stripes = inputs.random_spins(L, R, 8)
+    stripes[:, 2] = np.abs(stripes[:, 2]) * np.where((x // 4) % 2 == 0, 1.0, -1.0)[None, None, :]
+    zeros = inputs.random_spins(L, R, 9)
+    zeros[:, 0, ::3, ::2] = 0.0
+    zeros[:, 2, 1::2, :] = -0.0
+    for s in (inputs.random_spins(L, R, 7), stripes, inputs.up_spins(L, R), zeros):
+        ctx.set_spins(s)
+        counts, derived = ctx.wall_observables()
+        ref = oracle.wall_counts(s.astype(np.float64))
+        assert np.array_equal(counts, ref), (L, R)
+        assert np.max(np.abs(derived - oracle.wall_order(L, ref))) <= 1e-15
+    ctx.close()
