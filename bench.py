@@ -25,6 +25,10 @@ sys.path.insert(0, ROOT)
 CFG_ID = 5
 FLOP_PER_PAIR = 10.0           # 5 FMA per (target, source, replica): SURVEY.md section 8(d)
 BYTES_PER_UPDATE = 48.0        # own spin 12 + neighbours 12 (amortised) + h 12 + write 12
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
+TRAFFIC_FIELD = 207.8e6        # profiles/r01_field_kernel.md (57.9 + 148.1 and 59.0 + 150.5 MB)
+TRAFFIC_METROPOLIS = 78.4e6    # profiles/r01_metropolis_kernel.md (75.5 read; writes stay in L2 under ncu)
+TRAFFIC_FFT_GROUP = 167.0e6    # profiles/r01_fft_field_kernels.md (three kernels of one field)
 # fp32 FMA peak: 148 SMs x 128 lanes x 2 flop x 1.965 GHz
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
 
@@ -312,13 +316,13 @@ def run_cuda(args):
                      "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": field_tflops / FP32_PEAK_TFLOPS,
                      "peak_kind": "derived: 148 SM x 128 fp32 lanes x 2 x 1.965 GHz (DESIGN.md section 6)",
                      "measured_ffma_peak": ffma_peak, "frac_of_measured_ffma_peak": field_tflops / ffma_peak,
-                     "traffic": None, "ms_per_launch": field_ms, "flop_per_launch": flop_per_field},
+                     "traffic": TRAFFIC_FIELD, "ms_per_launch": field_ms, "flop_per_launch": flop_per_field},
         "dipole_field_gflops": field_tflops * 1e3,
         "roofline_metropolis": {"kernel": "metropolis4_kernel", "bound": "hbm", "achieved": metro_gbs, "peak": hbm_peak,
                                 "unit": "GB/s", "frac": metro_gbs / hbm_peak, "peak_kind": hbm_kind,
                                 "frac_of_8TBs": metro_gbs / 8000.0, "ms_per_launch_cold_l2": metro_cold_ms, "launches_timed": launches_metro,
                                 "ms_per_launch_in_sweep": metro_ms, "bytes_per_launch": metro_bytes,
-                                "updates_per_s": (N // 2) * R / (metro_cold_ms * 1e-3), "traffic": None},
+                                "updates_per_s": (N // 2) * R / (metro_cold_ms * 1e-3), "traffic": TRAFFIC_METROPOLIS},
     }
     if fft is not None:
         # algorithmic HBM bytes of one half-sweep field by FFT: read every spin (12 B per site and replica),
@@ -334,7 +338,7 @@ def run_cuda(args):
             "roofline": {"kernel": "fft_x_forward + fft_y_multiply + fft_x_inverse", "bound": "hbm", "achieved": gbs,
                          "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak, "peak_kind": hbm_kind,
                          "ms_per_launch_group": fft["field_ms_per_launch_group"], "bytes_per_launch_group": fft_bytes,
-                         "traffic": None}}
+                         "traffic": TRAFFIC_FFT_GROUP}}
     if world == 1 and not args.no_cpu_baseline:
         ups, sec, cores = oracle_sample(1, 0, 8)
         line["cpu_baseline"] = {"value": ups, "unit": "updates/s", "cores": cores, "kind": "oracle",

@@ -626,3 +626,90 @@ int oracle_wall_order(int L, int R, const long long *counts, double *derived)
     }
     return 0;
 }
+
+/* ------------------------------------------------------------------------- */
+/* O8. The paper's own update schedule (section 3.1; App. A :307-361) */
+/* One pass p of the algorithm with stride l (l >= 2, l | L):                     */
+/*   (i)   a site i_1 = (S_1, S_2) is selected at random, S_1, S_2 in [0, l)       */
+/*         (App. A "S_1 = Random Integer in [1, l]", 0-based here; reading R21:    */
+/*         words x0, x1 of Philox(seed; 0xFFFFFFFF, 0xFFFFFFFF, p), S = x mod l);  */
+/*   (ii)  update sites i = (a l, b l) + i_1, a, b in [0, L/l): n = (L/l)^2 sites   */
+/*         (the "a, b in [0, L/l]" and "T_id <= L^2 \ l^2" of the text count one    */
+/*         too many: R3/A19 reading, every site of the sub-lattice exactly once);   */
+/*   (iii) for each update site and replica a trial spin and u from                 */
+/*         Philox(seed; site, replica, step = p) as in O5; flip != 0 selects the    */
+/*         Ising move of App. B (:366) instead: the trial is the reversed spin;     */
+/*   (iv)  dipole energies of all n sites from the state AT ENTRY to the pass       */
+/*         ("simultaneous flipping", :102-118), exchange and anisotropy exact       */
+/*         (update sites are never nearest neighbours for l >= 2);                  */
+/*   (v)   accept <=> dE/T + ln u < 0.                                              */
+/* sequential != 0 runs the same sites in order a fastest, with the same random     */
+/* numbers, recomputing the field from the CURRENT state for every site: the        */
+/* conventional Metropolis the paper compares against (App. B).                     */
+/* offset_out[2] (nullable) = {S_1, S_2}; accept_out [R][N], margin_out [R][N],     */
+/* trial_out [R][3][N] (nullable) are written at the update sites only.             */
+/* ------------------------------------------------------------------------- */
+void oracle_sublattice_offset(uint64_t seed, uint64_t pass, int l, int offset[2])
+{
+    uint32_t ctr[4], key[2], x[4];
+    ctr[0] = 0xFFFFFFFFu;
+    ctr[1] = 0xFFFFFFFFu;
+    ctr[2] = (uint32_t)(pass & 0xFFFFFFFFu);
+    ctr[3] = (uint32_t)(pass >> 32) & 0x7FFFFFFFu;
+    key[0] = (uint32_t)(seed & 0xFFFFFFFFu);
+    key[1] = (uint32_t)(seed >> 32);
+    oracle_philox4x32_10(ctr, key, x);
+    offset[0] = (int)(x[0] % (uint32_t)l);
+    offset[1] = (int)(x[1] % (uint32_t)l);
+}
+
+int oracle_sublattice_pass(int L, int R, double J, double g, const double *K2, const double *K4,
+                           const double *W, double *s, const double *T, uint64_t seed,
+                           uint64_t pass, int l, int flip, int sequential, int *offset_out,
+                           uint8_t *accept_out, double *margin_out, double *trial_out)
+{
+    if (L < 2 || R < 1 || l < 2 || L % l || !K2 || !K4 || !W || !s || !T) return -1;
+    for (int r = 0; r < R; ++r)
+        if (!(T[r] > 0.0)) return -1;
+    size_t N = (size_t)L * L;
+    int nl = L / l, off[2];
+    oracle_sublattice_offset(seed, pass, l, off);
+    if (offset_out) { offset_out[0] = off[0]; offset_out[1] = off[1]; }
+    double *entry = (double *)malloc(sizeof(double) * 3 * N);
+    if (!entry) return -2;
+    for (int r = 0; r < R; ++r) {
+        double *sr = s + (size_t)r * 3 * N;
+        memcpy(entry, sr, sizeof(double) * 3 * N);          /* the state at entry to the pass */
+        for (int b = 0; b < nl; ++b) {
+            for (int a = 0; a < nl; ++a) {
+                int x = off[0] + l * a, y = off[1] + l * b;
+                int n = y * L + x;
+                uint32_t rnd[4];
+                double sp[3], hn[3];
+                draw(seed, (uint32_t)n, (uint32_t)r, pass, 0u, rnd);
+                if (flip) {
+                    for (int c = 0; c < 3; ++c) sp[c] = -entry[c * N + n];
+                } else {
+                    sphere_point(rnd[0], rnd[1], sp);
+                }
+                double u = to_unit(rnd[2]);
+                /* frozen: every site sees the state at entry; sequential: the current one.
+                 * The site's own spin and its four neighbours are the same in both (no
+                 * other update site touches them), so only the dipole sum differs.       */
+                const double *view = sequential ? sr : entry;
+                field_at(L, W, view, x, y, hn);
+                double dE = oracle_delta_e(L, J, g, K2[r], K4[r], W, view, hn, n, sp);
+                double margin = dE / T[r] + log(u);
+                int acc = margin < 0.0;
+                if (acc)
+                    for (int c = 0; c < 3; ++c) sr[c * N + n] = sp[c];
+                if (accept_out) accept_out[(size_t)r * N + n] = (uint8_t)acc;
+                if (margin_out) margin_out[(size_t)r * N + n] = margin;
+                if (trial_out)
+                    for (int c = 0; c < 3; ++c) trial_out[((size_t)r * 3 + c) * N + n] = sp[c];
+            }
+        }
+    }
+    free(entry);
+    return 0;
+}

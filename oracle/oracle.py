@@ -227,3 +227,31 @@ def wall_order(L, counts):
     rc = lib().oracle_wall_order(L, R, counts.ctypes.data_as(ctypes.POINTER(ctypes.c_longlong)), _d(out))
     assert rc == 0, rc
     return out
+
+
+def sublattice_offset(seed, pass_index, l):
+    off = (ctypes.c_int * 2)()
+    lib().oracle_sublattice_offset.restype = None
+    lib().oracle_sublattice_offset(ctypes.c_uint64(seed), ctypes.c_uint64(pass_index), int(l), off)
+    return int(off[0]), int(off[1])
+
+
+def sublattice_pass(W, s, T, seed, pass_index, l, J, g, K2, K4, flip=False, sequential=False):
+    """One pass of the paper's stride-l schedule (App. A) IN PLACE on s.
+    -> dict(offset, accept[R][L][L], margin[R][L][L], trial[R][3][L][L]); update sites only."""
+    assert s.dtype == np.float64 and s.flags.c_contiguous
+    R, _, L, _ = s.shape
+    W = _f64(W)
+    T = _per_replica(T, R)
+    K2 = _per_replica(K2, R)
+    K4 = _per_replica(K4, R)
+    off = (ctypes.c_int * 2)()
+    acc = np.zeros((R, L, L), dtype=np.uint8)
+    mar = np.zeros((R, L, L), dtype=np.float64)
+    tri = np.zeros((R, 3, L, L), dtype=np.float64)
+    rc = lib().oracle_sublattice_pass(L, R, ctypes.c_double(J), ctypes.c_double(g), _d(K2), _d(K4), _d(W),
+                                      _d(s), _d(T), ctypes.c_uint64(seed), ctypes.c_uint64(pass_index),
+                                      int(l), int(bool(flip)), int(bool(sequential)), off,
+                                      acc.ctypes.data_as(_c_u8_p), _d(mar), _d(tri))
+    assert rc == 0, rc
+    return {"offset": (int(off[0]), int(off[1])), "accept": acc, "margin": mar, "trial": tri}
