@@ -55,8 +55,10 @@ enum { DSMC_W_IMAGE = 0, DSMC_W_EWALD = 1 };
 
 /* dsmc_halfsweep_ex flags */
 enum {
-    DSMC_REUSE_FIELD = 1 /* skip the field step: reuse h kept from the previous field call of
-                            the same colour (for timing the Metropolis kernel alone)         */
+    DSMC_REUSE_FIELD = 1, /* skip the field step: reuse h kept from the previous field call of
+                             the same colour (for timing the Metropolis kernel alone)         */
+    DSMC_TRIAL_FLIP = 2   /* the trial is the reversed spin s' = -s instead of a point uniform on
+                             S^2: the Ising move of App. B; u is drawn as usual   */
 };
 
 /* dsmc_init_spins modes */
@@ -129,6 +131,21 @@ int dsmc_halfsweep(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t step);
  *   accept_out[R][L][L] bytes (0/1),  margin_out[R][L][L] floats (dE/T + ln u as the kernel saw it). */
 int dsmc_halfsweep_ex(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t step, int flags,
                       uint8_t *accept_out, float *margin_out);
+
+/* The paper's own update schedule (section 3.1; App. A :307-361).
+ * One pass: an offset (S_1, S_2) in [0, l)^2 is drawn from Philox4x32-10(seed; 0xFFFFFFFF, 0xFFFFFFFF,
+ * pass) as (x0 mod l, x1 mod l) (R21); the n = (L/l)^2 sites (S_1 + a l, S_2 + b l) are updated
+ * simultaneously, each with the trial and u of Philox(seed; site, replica, step = pass), the dipole
+ * field of ALL of them taken from the state at entry to the pass (section 3.2), exchange, anisotropy
+ * and the self-term exact as in dsmc_halfsweep.  l >= 2 and l | L (DSMC_EINVAL otherwise); l = L is
+ * conventional single-spin Metropolis.  One MC step (N attempted updates) = l*l passes.
+ * flags: DSMC_TRIAL_FLIP.  accept_out / margin_out: nullable DEVICE buffers [R][L][L], written at
+ * the update sites only.  offset_out: nullable HOST int[2] = {S_1, S_2}.                          */
+int dsmc_sublattice_pass(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t pass, int l, int flags,
+                         uint8_t *accept_out, float *margin_out, int *offset_out);
+/* n_passes consecutive passes first_pass .. first_pass + n_passes - 1 (two kernel launches each).   */
+int dsmc_sublattice_run(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_pass, uint64_t n_passes, int l,
+                        int flags);
 
 /* n_half consecutive half-sweeps (steps first_step .. first_step + n_half - 1) without returning
  * to the caller in between.                                                                    */

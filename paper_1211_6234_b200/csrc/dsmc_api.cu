@@ -112,6 +112,34 @@ int after_tensor_change(dsmc_ctx *ctx) {
     return DSMC_OK;
 }
 
+MetropolisArgs metropolis_args(dsmc_ctx *ctx, int colour, uint64_t seed, uint64_t step, int flags, uint8_t *accept_out,
+                               float *margin_out) {
+    MetropolisArgs a;
+    a.S = ctx->S();
+    a.H = ctx->H();
+    a.invT = ctx->invT();
+    a.K2 = ctx->K2d();
+    a.K4 = ctx->K4d();
+    a.L = ctx->L;
+    a.R = ctx->R;
+    a.colour = colour;
+    a.rq_shift = -1;
+    a.flip = (flags & DSMC_TRIAL_FLIP) ? 1 : 0;
+    a.J = ctx->J;
+    a.g = ctx->g;
+    a.w0xx = ctx->w0[0];
+    a.w0xy = ctx->w0[1];
+    a.w0yy = ctx->w0[2];
+    a.w0zz = ctx->w0[3];
+    a.seed_lo = (uint32_t)(seed & 0xFFFFFFFFu);
+    a.seed_hi = (uint32_t)(seed >> 32);
+    a.step_lo = (uint32_t)(step & 0xFFFFFFFFu);
+    a.step_hi = (uint32_t)(step >> 32) & 0x7FFFFFFFu;  // bit 31 is the init tag
+    a.accept_out = accept_out;
+    a.margin_out = margin_out;
+    return a;
+}
+
 }  // namespace
 
 DsmcLayout dsmc_make_layout(int L, int R) {
@@ -291,7 +319,7 @@ int dsmc_halfsweep_ex(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t ste
     if (int rc = need_bound(ctx)) return rc;
     if (!ctx->tensor_built) return fail(ctx, DSMC_ESTATE, "tensor not built");
     if (!ctx->spins_set) return fail(ctx, DSMC_ESTATE, "spins not set");
-    if (flags & ~DSMC_REUSE_FIELD) return fail(ctx, DSMC_EINVAL, "unknown flag");
+    if (flags & ~(DSMC_REUSE_FIELD | DSMC_TRIAL_FLIP)) return fail(ctx, DSMC_EINVAL, "unknown flag");
     if (int rc = upload_params(ctx, T)) return rc;
     const int colour = (int)(step & 1u);
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[0], ctx->stream), "event");
@@ -301,28 +329,7 @@ int dsmc_halfsweep_ex(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t ste
         return fail(ctx, DSMC_ESTATE, "DSMC_REUSE_FIELD without a field of this colour");
     }
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[1], ctx->stream), "event");
-    MetropolisArgs a;
-    a.S = ctx->S();
-    a.H = ctx->H();
-    a.invT = ctx->invT();
-    a.K2 = ctx->K2d();
-    a.K4 = ctx->K4d();
-    a.L = ctx->L;
-    a.R = ctx->R;
-    a.colour = colour;
-    a.rq_shift = -1;
-    a.J = ctx->J;
-    a.g = ctx->g;
-    a.w0xx = ctx->w0[0];
-    a.w0xy = ctx->w0[1];
-    a.w0yy = ctx->w0[2];
-    a.w0zz = ctx->w0[3];
-    a.seed_lo = (uint32_t)(seed & 0xFFFFFFFFu);
-    a.seed_hi = (uint32_t)(seed >> 32);
-    a.step_lo = (uint32_t)(step & 0xFFFFFFFFu);
-    a.step_hi = (uint32_t)(step >> 32) & 0x7FFFFFFFu;  // bit 31 is the init tag
-    a.accept_out = accept_out;
-    a.margin_out = margin_out;
+    const MetropolisArgs a = metropolis_args(ctx, colour, seed, step, flags, accept_out, margin_out);
     CU(launch_metropolis(a, ctx->stream, &ctx->launches), "metropolis launch");
     if (ctx->timing) {
         CU(cudaEventRecord(ctx->ev[2], ctx->stream), "event");
@@ -335,6 +342,35 @@ int dsmc_halfsweep_ex(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t ste
 
 int dsmc_halfsweep(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t step) {
     return dsmc_halfsweep_ex(ctx, T, seed, step, 0, nullptr, nullptr);
+}
+
+int dsmc_sublattice_pass(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t pass, int l, int flags,
+                         uint8_t *accept_out, float *margin_out, int *offset_out) {
+    if (int rc = need_bound(ctx)) return rc;
+    if (!ctx->tensor_built) return fail(ctx, DSMC_ESTATE, "tensor not built");
+    if (!ctx->spins_set) return fail(ctx, DSMC_ESTATE, "spins not set");
+    if (flags & ~DSMC_TRIAL_FLIP) return fail(ctx, DSMC_EINVAL, "unknown flag");
+    if (l < 2 || ctx->L % l) return fail(ctx, DSMC_EINVAL, "l must be >= 2 and divide L");
+    if (int rc = upload_params(ctx, T)) return rc;
+    int ox, oy;
+    dsmc_sublattice_offset(seed, pass, l, &ox, &oy);
+    if (offset_out) {
+        offset_out[0] = ox;
+        offset_out[1] = oy;
+    }
+    const MetropolisArgs a = metropolis_args(ctx, 0, seed, pass, flags, accept_out, margin_out);
+    CU(launch_sublattice_pass(a, ctx->Wc(), l, ox, oy, ctx->stream, &ctx->launches), "sub-lattice pass launch");
+    ctx->field_valid[0] = ctx->field_valid[1] = false;
+    return DSMC_OK;
+}
+
+int dsmc_sublattice_run(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_pass, uint64_t n_passes, int l,
+                        int flags) {
+    for (uint64_t k = 0; k < n_passes; ++k)
+        if (int rc = dsmc_sublattice_pass(ctx, k == 0 ? T : nullptr, seed, first_pass + k, l, flags, nullptr, nullptr,
+                                          nullptr))
+            return rc;
+    return DSMC_OK;
 }
 
 int dsmc_run(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_step, uint64_t n_half) {

@@ -109,12 +109,17 @@ struct MetropolisArgs {
     const float *invT, *K2, *K4;
     int L, R, colour;
     int rq_shift;  // log2(R/4) when R/4 is a power of two, else -1 (set by the launcher)
+    int flip;      // 0: trial uniform on S^2; 1: trial = -s (Ising move of App. B)
     float J, g, w0xx, w0yy, w0zz, w0xy;
     uint32_t seed_lo, seed_hi, step_lo, step_hi;
     uint8_t *accept_out;  // canonical [R][L][L] or null
     float *margin_out;    // canonical [R][L][L] or null
 };
 cudaError_t launch_metropolis(const MetropolisArgs &a, cudaStream_t st, uint64_t *launches);
+// the paper's stride-l sub-lattice pass: offset (ox, oy) in [0, l)^2, n = (L/l)^2 update sites
+void dsmc_sublattice_offset(uint64_t seed, uint64_t pass, int l, int *ox, int *oy);
+cudaError_t launch_sublattice_pass(const MetropolisArgs &a, const float *Wc, int l, int ox, int oy, cudaStream_t st,
+                                   uint64_t *launches);
 cudaError_t launch_init_spins(float *S, int L, int R, int mode, uint64_t seed, cudaStream_t st,
                               uint64_t *launches);
 cudaError_t launch_observables(const float *S, const float *H, const float *K2, const float *K4,

@@ -16,7 +16,7 @@ struct RoundKeys {
 };
 
 // Philox4x32-10 (Salmon et al., SC'11) with precomputed round keys
-__device__ __forceinline__ uint4 philox4x32_10(uint4 c, const RoundKeys &rk) {
+__host__ __device__ __forceinline__ uint4 philox4x32_10(uint4 c, const RoundKeys &rk) {
 #pragma unroll
     for (int round = 0; round < 10; ++round) {
         const uint64_t p0 = (uint64_t)0xD2511F53u * c.x;
@@ -78,7 +78,11 @@ __device__ __forceinline__ Trial decide(const MetropolisArgs &p, const RoundKeys
                                         float invT, float K2, float K4) {
     const uint4 rnd = philox4x32_10(make_uint4(n, r, p.step_lo, p.step_hi), rk);
     Trial t;
-    sphere_point(rnd.x, rnd.y, t.tx, t.ty, t.tz);
+    if (p.flip) {                                             // Ising move of App. B: complete reversal
+        t.tx = -sx, t.ty = -sy, t.tz = -sz;
+    } else {
+        sphere_point(rnd.x, rnd.y, t.tx, t.ty, t.tz);
+    }
     const float u = unit24(rnd.z);
     const float dx = t.tx - sx, dy = t.ty - sy, dz = t.tz - sz;
     const float dz2 = dz * (t.tz + sz);                       // s'_z^2 - s_z^2
@@ -148,9 +152,6 @@ __device__ __forceinline__ float mant(uint32_t x) { return __uint_as_float(0x3F8
 struct Trial2 {
     f2 tx, ty, tz, lnu;   // trial spins and ln u of two replicas: functions of the random words only
 };
-struct Pair {
-    f2 tx, ty, tz, margin;
-};
 __device__ __forceinline__ Trial2 trial2(uint4 ra, uint4 rb) {
     Trial2 t;
     const f2 c2 = f2_bc(2.0f), cm15 = f2_bc(-1.5f), ulp = f2_bc(1.1920928955078125e-7f);
@@ -200,15 +201,6 @@ __device__ __forceinline__ f2 margin2(const MetropolisArgs &p, const Trial2 &t, 
     dE = f2_fma(f2_bc(p.g), dip, dE);
     return f2_fma(dE, invT, t.lnu);
 }
-__device__ __forceinline__ Pair decide2(const MetropolisArgs &p, uint4 ra, uint4 rb, f2 sx, f2 sy, f2 sz, f2 nx, f2 ny,
-                                        f2 nz, f2 hx, f2 hy, f2 hz, f2 invT, f2 K2, f2 K4) {
-    const Trial2 t = trial2(ra, rb);
-    Pair o;
-    o.tx = t.tx, o.ty = t.ty, o.tz = t.tz;
-    o.margin = margin2(p, t, sx, sy, sz, nx, ny, nz, hx, hy, hz, invT, K2, K4);
-    return o;
-}
-
 __device__ __forceinline__ void ld2(const float4 *ptr, f2 &lo, f2 &hi) {
     const ulonglong2 v = __ldg(reinterpret_cast<const ulonglong2 *>(ptr));
     lo = v.x;
@@ -219,7 +211,7 @@ __device__ __forceinline__ void ld2(const float4 *ptr, f2 &lo, f2 &hi) {
 // lattice row.  All 18 128-bit loads are issued first; the four Philox chains and the trial spins
 // do not depend on them and run while they are in flight.  HOOKS = parity outputs requested.
 template <bool HOOKS>
-__global__ void __launch_bounds__(128) metropolis4_kernel(const MetropolisArgs p, const RoundKeys rk) {
+__global__ void __launch_bounds__(128, 7) metropolis4_kernel(const MetropolisArgs p, const RoundKeys rk) {
     const int Lh = p.L >> 1, RQ = p.R >> 2;
     const int y = blockIdx.y;
     const uint32_t row4 = (uint32_t)(Lh * RQ);
@@ -277,15 +269,21 @@ __global__ void __launch_bounds__(128) metropolis4_kernel(const MetropolisArgs p
     float mg[4];
 #pragma unroll
     for (int j = 0; j < 2; ++j) {
-        const Pair t = decide2(p, rnd[2 * j], rnd[2 * j + 1], s[0][j], s[1][j], s[2][j], nb[0][j], nb[1][j], nb[2][j],
-                               h[0][j], h[1][j], h[2][j], invT[j], K2[j], K4[j]);
+        Trial2 tr = trial2(rnd[2 * j], rnd[2 * j + 1]);
+        if (p.flip) {                                         // Ising move of App. B: complete reversal
+            tr.tx = f2_mul(s[0][j], f2_bc(-1.0f));
+            tr.ty = f2_mul(s[1][j], f2_bc(-1.0f));
+            tr.tz = f2_mul(s[2][j], f2_bc(-1.0f));
+        }
+        const f2 margin = margin2(p, tr, s[0][j], s[1][j], s[2][j], nb[0][j], nb[1][j], nb[2][j], h[0][j], h[1][j],
+                                  h[2][j], invT[j], K2[j], K4[j]);
         float m0, m1, a0, a1, b0, b1;
-        f2_split(t.margin, m0, m1);
+        f2_split(margin, m0, m1);
         const bool acc0 = m0 < 0.0f, acc1 = m1 < 0.0f;
-        const f2 tr[3] = {t.tx, t.ty, t.tz};
+        const f2 tv[3] = {tr.tx, tr.ty, tr.tz};
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
-            f2_split(tr[k], a0, a1);
+            f2_split(tv[k], a0, a1);
             f2_split(s[k][j], b0, b1);
             s[k][j] = f2_make(acc0 ? a0 : b0, acc1 ? a1 : b1);
         }
@@ -341,6 +339,108 @@ __global__ void __launch_bounds__(256) metropolis1_kernel(const MetropolisArgs p
     }
     if (p.accept_out) p.accept_out[(size_t)r * 2 * Nh + n] = tr.acc ? 1 : 0;
     if (p.margin_out) p.margin_out[(size_t)r * 2 * Nh + n] = tr.margin;
+}
+
+// ---------------------------------------------------------------------------------------------
+// The paper's own schedule (section 3.1, App. A): one pass updates the n = (L/l)^2 sites
+// (ox + a l, oy + b l) of a stride-l sub-lattice simultaneously, every one of them seeing the dipole
+// field of the state at entry to the pass.  Two launches per pass, as the paper's dipole kernel and
+// flip kernel (a grid-wide barrier separates "all fields computed" from "first spin replaced"):
+//   sublattice_field_kernel: one CTA per update site and 32 replicas.  The paper's "P threads per
+//     update site, each a strip of the lattice" becomes 8 warps that each sum the source rows
+//     y = g, g + 8, ... for 32 replicas (lanes = replicas, so the spin loads are coalesced and the four
+//     W values of a source are a warp-wide broadcast), row sums first (two-level fp32 accumulation),
+//     then a fixed-order shared-memory reduction; h goes to the site's slot of the field array H.
+//   sublattice_flip_kernel: one thread per (update site, replica): exchange, anisotropy, self-term,
+//     frozen-field dE and the decision (the paper's exchange and flip kernels fused).
+__device__ __forceinline__ size_t site_index(int x, int y, int Lh, int R, size_t plane, int &q) {
+    q = (x + y) & 1;
+    return (size_t)q * 3 * plane + ((size_t)y * Lh + (x >> 1)) * R;
+}
+
+__global__ void __launch_bounds__(256) sublattice_field_kernel(const float *__restrict__ S, float *__restrict__ H,
+                                                               const float *__restrict__ Wc, int L, int R, int l,
+                                                               int ox, int oy) {
+    __shared__ float part[8][3][32];
+    const int Lh = L >> 1;
+    const size_t N = (size_t)L * L, plane = (size_t)L * Lh * R;
+    const int nl = L / l;
+    const int xt = ox + l * (int)(blockIdx.x % nl), yt = oy + l * (int)(blockIdx.x / nl);
+    const int lane = threadIdx.x & 31, grp = threadIdx.x >> 5;
+    const int r = blockIdx.y * 32 + lane;
+    const int rr = r < R ? r : R - 1;                          // idle lanes load a valid replica
+    float hx = 0.0f, hy = 0.0f, hz = 0.0f;
+    for (int ys = grp; ys < L; ys += 8) {
+        int ry = ys - yt;
+        ry += ry < 0 ? L : 0;
+        const float *Wrow = Wc + (size_t)ry * L;
+        float ax = 0.0f, ay = 0.0f, az = 0.0f;
+        for (int xs = 0; xs < L; ++xs) {
+            int rx = xs - xt;
+            rx += rx < 0 ? L : 0;
+            int q;
+            const float *src = S + site_index(xs, ys, Lh, R, plane, q) + rr;
+            const float sx = src[0], sy = src[plane], sz = src[2 * plane];
+            const float wxx = __ldg(Wrow + rx), wxy = __ldg(Wrow + N + rx), wyy = __ldg(Wrow + 2 * N + rx),
+                        wzz = __ldg(Wrow + 3 * N + rx);
+            ax = fmaf(wxx, sx, fmaf(wxy, sy, ax));
+            ay = fmaf(wxy, sx, fmaf(wyy, sy, ay));
+            az = fmaf(wzz, sz, az);
+        }
+        hx += ax;
+        hy += ay;
+        hz += az;
+    }
+    part[grp][0][lane] = hx;
+    part[grp][1][lane] = hy;
+    part[grp][2][lane] = hz;
+    __syncthreads();
+    if (grp != 0 || r >= R) return;
+    hx = hy = hz = 0.0f;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        hx += part[k][0][lane];
+        hy += part[k][1][lane];
+        hz += part[k][2][lane];
+    }
+    int q;
+    float *dst = H + site_index(xt, yt, Lh, R, plane, q) + r;
+    dst[0] = hx;
+    dst[plane] = hy;
+    dst[2 * plane] = hz;
+}
+
+__global__ void __launch_bounds__(128) sublattice_flip_kernel(const MetropolisArgs p, const RoundKeys rk, int l, int ox,
+                                                              int oy) {
+    const int L = p.L, Lh = L >> 1, R = p.R;
+    const size_t N = (size_t)L * L, plane = (size_t)L * Lh * R;
+    const int nl = L / l;
+    const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (size_t)nl * nl * R) return;
+    const int r = (int)(t % (size_t)R), k = (int)(t / (size_t)R);
+    const int xt = ox + l * (k % nl), yt = oy + l * (k / nl);
+    int q;
+    const size_t at = site_index(xt, yt, Lh, R, plane, q) + r;
+    float *own = p.S + at;
+    const float *hf = p.H + at;
+    const int xe = xt + 1 == L ? 0 : xt + 1, xw = xt == 0 ? L - 1 : xt - 1;
+    const int yn = yt + 1 == L ? 0 : yt + 1, ys = yt == 0 ? L - 1 : yt - 1;
+    const float *ne = p.S + site_index(xe, yt, Lh, R, plane, q) + r, *nw = p.S + site_index(xw, yt, Lh, R, plane, q) + r;
+    const float *nn = p.S + site_index(xt, yn, Lh, R, plane, q) + r, *ns = p.S + site_index(xt, ys, Lh, R, plane, q) + r;
+    const float sx = own[0], sy = own[plane], sz = own[2 * plane];
+    const float nx = (ne[0] + nw[0]) + (nn[0] + ns[0]);
+    const float ny = (ne[plane] + nw[plane]) + (nn[plane] + ns[plane]);
+    const float nz = (ne[2 * plane] + nw[2 * plane]) + (nn[2 * plane] + ns[2 * plane]);
+    const uint32_t n = (uint32_t)(yt * L + xt);
+    const Trial tr = decide(p, rk, n, (uint32_t)r, sx, sy, sz, nx, ny, nz, hf[0], hf[plane], hf[2 * plane], p.invT[r],
+                            p.K2[r], p.K4[r]);
+    if (tr.acc) {
+        own[0] = tr.tx;
+        own[plane] = tr.ty;
+        own[2 * plane] = tr.tz;
+    }
+    if (p.accept_out) p.accept_out[(size_t)r * N + n] = tr.acc ? 1 : 0;
+    if (p.margin_out) p.margin_out[(size_t)r * N + n] = tr.margin;
 }
 
 __global__ void __launch_bounds__(256) init_spins_kernel(float *__restrict__ S, int L, int R, int mode, const RoundKeys rk) {
@@ -409,5 +509,26 @@ cudaError_t launch_init_spins(float *S, int L, int R, int mode, uint64_t seed, c
     init_spins_kernel<<<grid, 256, 0, st>>>(S, L, R, mode,
                                              make_round_keys((uint32_t)(seed & 0xFFFFFFFFu), (uint32_t)(seed >> 32)));
     ++*launches;
+    return cudaGetLastError();
+}
+
+void dsmc_sublattice_offset(uint64_t seed, uint64_t pass, int l, int *ox, int *oy) {
+    // DESIGN.md R21: words x0, x1 of Philox4x32-10(seed; 0xFFFFFFFF, 0xFFFFFFFF, pass) mod l
+    const RoundKeys rk = make_round_keys((uint32_t)(seed & 0xFFFFFFFFu), (uint32_t)(seed >> 32));
+    const uint4 x = philox4x32_10(make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, (uint32_t)(pass & 0xFFFFFFFFu),
+                                             (uint32_t)(pass >> 32) & 0x7FFFFFFFu), rk);
+    *ox = (int)(x.x % (uint32_t)l);
+    *oy = (int)(x.y % (uint32_t)l);
+}
+
+cudaError_t launch_sublattice_pass(const MetropolisArgs &a, const float *Wc, int l, int ox, int oy, cudaStream_t st,
+                                   uint64_t *launches) {
+    const RoundKeys rk = make_round_keys(a.seed_lo, a.seed_hi);
+    const int nl = a.L / l;
+    dim3 grid((unsigned)(nl * nl), (unsigned)((a.R + 31) / 32));
+    sublattice_field_kernel<<<grid, 256, 0, st>>>(a.S, const_cast<float *>(a.H), Wc, a.L, a.R, l, ox, oy);
+    const size_t total = (size_t)nl * nl * a.R;
+    sublattice_flip_kernel<<<(unsigned)((total + 127) / 128), 128, 0, st>>>(a, rk, l, ox, oy);
+    *launches += 2;
     return cudaGetLastError();
 }

@@ -11,6 +11,7 @@ import numpy as np
 DSMC_HOST, DSMC_DEVICE = 0, 1
 DSMC_W_IMAGE, DSMC_W_EWALD = 0, 1
 DSMC_REUSE_FIELD = 1
+DSMC_TRIAL_FLIP = 2
 DSMC_INIT_RANDOM, DSMC_INIT_UP = 0, 1
 DSMC_FIELD_AUTO, DSMC_FIELD_GENERIC, DSMC_FIELD_TILED, DSMC_FIELD_FFT = -1, 0, 1, 2
 
@@ -35,6 +36,8 @@ ABI = [
     ("dsmc_halfsweep", _i, [_vp, _vp, _u64, _u64]),
     ("dsmc_halfsweep_ex", _i, [_vp, _vp, _u64, _u64, _i, _vp, _vp]),
     ("dsmc_run", _i, [_vp, _vp, _u64, _u64, _u64]),
+    ("dsmc_sublattice_pass", _i, [_vp, _vp, _u64, _u64, _i, _i, _vp, _vp, _vp]),
+    ("dsmc_sublattice_run", _i, [_vp, _vp, _u64, _u64, _u64, _i, _i]),
     ("dsmc_observables", _i, [_vp, _vp]),
     ("dsmc_wall_observables", _i, [_vp, _vp, _vp]),
     ("dsmc_set_timing", _i, [_vp, _i]),
@@ -197,6 +200,19 @@ class Dsmc:
     def run(self, T, seed, first_step, n_half):
         t, tp = self._T(T)
         self._check(self.lib.dsmc_run(self._h, tp, seed, first_step, n_half))
+
+    def sublattice_pass(self, T, seed, pass_index, l, flags=0, accept_out=None, margin_out=None):
+        """One pass of the paper's stride-l schedule -> the offset (S_1, S_2)."""
+        t, tp = self._T(T)
+        ap = accept_out.data_ptr() if accept_out is not None else None
+        mp = margin_out.data_ptr() if margin_out is not None else None
+        off = (ctypes.c_int * 2)()
+        self._check(self.lib.dsmc_sublattice_pass(self._h, tp, seed, pass_index, l, flags, ap, mp, off))
+        return int(off[0]), int(off[1])
+
+    def sublattice_run(self, T, seed, first_pass, n_passes, l, flags=0):
+        t, tp = self._T(T)
+        self._check(self.lib.dsmc_sublattice_run(self._h, tp, seed, first_pass, n_passes, l, flags))
 
     def observables(self):
         out = np.empty((self.R, 4), dtype=np.float64)

@@ -1,0 +1,146 @@
+"""GPU parity of the paper's own update schedule (dsmc_sublattice_pass; section 3.1,
+App. A) against the oracle, pass by pass in lock-step with resync (SURVEY.md 8c parity protocol)."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+BAND = 1e-4
+BAND_FRACTION = 1e-4
+
+
+@pytest.fixture(scope="module")
+def dsmc_mod():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_1211_6234_b200 as m
+    from paper_1211_6234_b200 import build
+    build.build()
+    return m
+
+
+def lockstep_passes(m, oracle, ctx, W, T, J, g, K2, K4, seed, l, n_passes, flip=False):
+    L, R = ctx.L, ctx.R
+    acc_d = torch.zeros((R, L, L), dtype=torch.uint8, device="cuda")
+    mar_d = torch.zeros((R, L, L), dtype=torch.float32, device="cuda")
+    flags = m.DSMC_TRIAL_FLIP if flip else 0
+    ambiguous = trials = accepted = 0
+    for p in range(n_passes):
+        s_before = ctx.get_spins()
+        s_or = s_before.astype(np.float64)
+        out = oracle.sublattice_pass(W, s_or, T, seed, p, l, J, g, K2, K4, flip=flip)
+        off = ctx.sublattice_pass(T, seed, p, l, flags=flags, accept_out=acc_d, margin_out=mar_d)
+        assert off == out["offset"]                                    # integer work: bit-exact
+        s_after = ctx.get_spins()
+        ox, oy = off
+        site = np.zeros((L, L), dtype=bool)
+        site[oy::l, ox::l] = True
+        assert site.sum() == (L // l) ** 2
+        acc = acc_d.cpu().numpy()[:, site].astype(bool)
+        mar = mar_d.cpu().numpy()[:, site]
+        m_or = out["margin"][:, site]
+        a_or = out["accept"][:, site].astype(bool)
+        amb = np.abs(m_or) < BAND
+        assert np.array_equal(acc[~amb], a_or[~amb]), (p, int(np.sum(acc[~amb] != a_or[~amb])))
+        # the margin is dE / T: an fp32 dE good to ~2e-5 (field tolerance 1e-4 in h, times g |delta|) gives
+        # a margin good to 2e-5 / T below T = 1
+        tol = 2e-5 / np.minimum(np.asarray(T, dtype=np.float64), 1.0)[:, None] + 3e-6 * np.abs(m_or)
+        assert np.all(np.abs(mar - m_or) <= tol), (p, np.abs(mar - m_or).max())
+        ambiguous += int(amb.sum())
+        trials += amb.size
+        accepted += int(acc.sum())
+        full = np.zeros((R, L, L), dtype=bool)
+        full[:, site] = acc
+        chg = np.broadcast_to(full[:, None], s_after.shape)
+        assert np.array_equal(s_after[~chg], s_before[~chg])           # rejected and all other sites: bit-unchanged
+        assert np.max(np.abs(s_after[chg].astype(np.float64) - out["trial"][chg]), initial=0.0) <= 1e-6
+    assert ambiguous <= max(1, BAND_FRACTION * trials), (ambiguous, trials)
+    return accepted, trials
+
+
+@pytest.mark.parametrize("L,R,l,passes", [(8, 1, 4, 40), (12, 5, 3, 24), (32, 8, 8, 24), (64, 16, 32, 48),
+                                          (64, 40, 2, 6), (16, 3, 16, 12)])
+def test_sublattice_lockstep(dsmc_mod, oracle, L, R, l, passes):
+    """(64, 16, 32) is the paper's own choice L = 64, l = 32; l = 2 is the densest
+    schedule (n = N/4), l = L the conventional single-spin limit; R = 40 spans two replica chunks."""
+    from paper_1211_6234_b200 import inputs
+    J, g, K2, K4 = 1.0, 0.25, 0.6, 0.1
+    ctx = dsmc_mod.Dsmc(L, R, J=J, g=g, K2=K2, K4=K4)
+    ctx.build_tensor(dsmc_mod.DSMC_W_EWALD)
+    W = oracle.build_tensor_ewald(L)
+    ctx.set_spins(inputs.random_spins(L, R, 31))
+    T = np.linspace(0.2, 1.6, R).astype(np.float32)
+    acc, tr = lockstep_passes(dsmc_mod, oracle, ctx, W, T, J, g, K2, K4, 0x5EED, l, passes)
+    assert 0 < acc < tr
+    ctx.close()
+
+
+def test_sublattice_ising_flip(dsmc_mod, oracle):
+    """App. B: L = 64, l = 32, Ising spins, J / C_D = 1.7, T around T_c = 0.85 C_D (PAPER.md:366-372,
+    Table 1), starting from the h = 1 stripe ground state with a few defects."""
+    L, R, l = 64, 8, 32
+    J, g = 1.0, 1.0 / 1.7
+    ctx = dsmc_mod.Dsmc(L, R, J=J, g=g, K2=0.0, K4=0.0)
+    ctx.build_tensor(dsmc_mod.DSMC_W_EWALD)
+    W = oracle.build_tensor_ewald(L)
+    rng = np.random.default_rng(6)
+    s = np.zeros((R, 3, L, L), dtype=np.float32)
+    s[:, 2] = np.where(np.arange(L) % 2 == 0, 1.0, -1.0)[None, None, :]
+    s[:, 2] *= np.where(rng.random((R, L, L)) < 0.2, -1.0, 1.0)
+    ctx.set_spins(s)
+    T = (np.linspace(0.5, 1.2, R) * g).astype(np.float32)
+    acc, tr = lockstep_passes(dsmc_mod, oracle, ctx, W, T, J, g, 0.0, 0.0, 99, l, 64, flip=True)
+    out = ctx.get_spins()
+    assert np.all(np.abs(out[:, 2]) == 1.0) and np.all(out[:, :2] == 0.0)
+    assert acc > 0
+    ctx.close()
+
+
+def test_checkerboard_flip_flag(dsmc_mod, oracle):
+    """DSMC_TRIAL_FLIP on the checkerboard half-sweep: an Ising state stays one, energy changes agree
+    with the oracle's energy of the resulting state (margins are checked through the sub-lattice path)."""
+    L, R = 32, 8
+    J, g = 1.0, 0.5
+    ctx = dsmc_mod.Dsmc(L, R, J=J, g=g, K2=0.0, K4=0.0)
+    ctx.build_tensor(dsmc_mod.DSMC_W_EWALD)
+    rng = np.random.default_rng(8)
+    s = np.zeros((R, 3, L, L), dtype=np.float32)
+    s[:, 2] = rng.choice([-1.0, 1.0], size=(R, L, L))
+    ctx.set_spins(s)
+    T = np.full(R, 0.8, dtype=np.float32)
+    mar_d = torch.zeros((R, L, L), dtype=torch.float32, device="cuda")
+    acc_d = torch.zeros((R, L, L), dtype=torch.uint8, device="cuda")
+    ctx.halfsweep(T, 4, 0, flags=dsmc_mod.DSMC_TRIAL_FLIP, accept_out=acc_d, margin_out=mar_d)
+    out = ctx.get_spins()
+    assert np.all(np.abs(out[:, 2]) == 1.0) and np.all(out[:, :2] == 0.0)
+    x = np.arange(L)
+    par = (x[:, None] + x[None, :]) % 2
+    flipped = out[:, 2] != s[:, 2]
+    assert np.array_equal(flipped[:, par == 0], acc_d.cpu().numpy()[:, par == 0].astype(bool))
+    assert not flipped[:, par == 1].any() and flipped.any()
+    # a flipped site's margin is dE/T + ln u with dE the frozen-field energy change: check one site per replica
+    W = oracle.build_tensor_ewald(L)
+    h = oracle.dipole_field(W, s.astype(np.float64), colour=0)
+    mar = mar_d.cpu().numpy()
+    for r in range(R):
+        n = 2 * r * L + 2 * r                                       # (x, y) = (2r, 2r): colour 0
+        sp = -s[r, :, 2 * r, 2 * r].astype(np.float64)
+        dE = oracle.delta_e(W, s[r].astype(np.float64), h[r, :, 2 * r, 2 * r], n, sp, J, g, 0.0, 0.0)
+        _, u, _ = oracle.trial_draw(4, n, r, 0)
+        m_or = dE / 0.8 + np.log(u)
+        assert abs(mar[r, 2 * r, 2 * r] - m_or) <= 2e-5 + 3e-6 * abs(m_or)
+    ctx.close()
+
+
+def test_sublattice_argument_errors(dsmc_mod):
+    ctx = dsmc_mod.Dsmc(12, 2)
+    ctx.build_tensor()
+    ctx.init_spins(dsmc_mod.DSMC_INIT_RANDOM, seed=1)
+    T = np.ones(2, dtype=np.float32)
+    for bad_l in (1, 5, 24, 0):
+        with pytest.raises(dsmc_mod.DsmcError):
+            ctx.sublattice_pass(T, 1, 0, bad_l)
+    ctx.sublattice_run(T, 1, 0, 9, 3)                               # 9 = l*l passes = one MC step
+    ctx.close()
