@@ -359,7 +359,8 @@ int dsmc_sublattice_pass(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t 
         offset_out[1] = oy;
     }
     const MetropolisArgs a = metropolis_args(ctx, 0, seed, pass, flags, accept_out, margin_out);
-    CU(launch_sublattice_pass(a, ctx->Wc(), l, ox, oy, ctx->stream, &ctx->launches), "sub-lattice pass launch");
+    CU(launch_sublattice_pass(a, ctx->Wc(), ctx->stage(), ctx->sm_count, l, ox, oy, ctx->stream, &ctx->launches),
+       "sub-lattice pass launch");
     ctx->field_valid[0] = ctx->field_valid[1] = false;
     return DSMC_OK;
 }

@@ -118,8 +118,9 @@ struct MetropolisArgs {
 cudaError_t launch_metropolis(const MetropolisArgs &a, cudaStream_t st, uint64_t *launches);
 // the paper's stride-l sub-lattice pass: offset (ox, oy) in [0, l)^2, n = (L/l)^2 update sites
 void dsmc_sublattice_offset(uint64_t seed, uint64_t pass, int l, int *ox, int *oy);
-cudaError_t launch_sublattice_pass(const MetropolisArgs &a, const float *Wc, int l, int ox, int oy, cudaStream_t st,
-                                   uint64_t *launches);
+// scratch: 3 N R floats for the per-slab partial fields (the staging buffer)
+cudaError_t launch_sublattice_pass(const MetropolisArgs &a, const float *Wc, float *scratch, int sm_count, int l, int ox,
+                                   int oy, cudaStream_t st, uint64_t *launches);
 cudaError_t launch_init_spins(float *S, int L, int R, int mode, uint64_t seed, cudaStream_t st,
                               uint64_t *launches);
 cudaError_t launch_observables(const float *S, const float *H, const float *K2, const float *K4,

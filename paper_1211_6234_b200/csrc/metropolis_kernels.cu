@@ -8,6 +8,7 @@
 //   * the azimuth 2 pi u1 is reduced to a quadrant exactly in integer arithmetic and sin/cos come
 //     from two short polynomials (abs error 1.5e-7); sqrt and log use the MUFU units.
 #include "dsmc_internal.cuh"
+#include <algorithm>
 
 namespace {
 
@@ -358,9 +359,10 @@ __device__ __forceinline__ size_t site_index(int x, int y, int Lh, int R, size_t
     return (size_t)q * 3 * plane + ((size_t)y * Lh + (x >> 1)) * R;
 }
 
-__global__ void __launch_bounds__(256) sublattice_field_kernel(const float *__restrict__ S, float *__restrict__ H,
+// grid (n sites, replica chunks of 32, KS source slabs); part[ks][site][c][r] receives the slab's sum
+__global__ void __launch_bounds__(256) sublattice_field_kernel(const float *__restrict__ S, float *__restrict__ part_out,
                                                                const float *__restrict__ Wc, int L, int R, int l,
-                                                               int ox, int oy) {
+                                                               int ox, int oy, int rows_per_slab) {
     __shared__ float part[8][3][32];
     const int Lh = L >> 1;
     const size_t N = (size_t)L * L, plane = (size_t)L * Lh * R;
@@ -369,25 +371,31 @@ __global__ void __launch_bounds__(256) sublattice_field_kernel(const float *__re
     const int lane = threadIdx.x & 31, grp = threadIdx.x >> 5;
     const int r = blockIdx.y * 32 + lane;
     const int rr = r < R ? r : R - 1;                          // idle lanes load a valid replica
+    const int y0 = blockIdx.z * rows_per_slab, y1 = min(L, y0 + rows_per_slab);
     float hx = 0.0f, hy = 0.0f, hz = 0.0f;
-    for (int ys = grp; ys < L; ys += 8) {
+    for (int ys = y0 + grp; ys < y1; ys += 8) {
         int ry = ys - yt;
         ry += ry < 0 ? L : 0;
         const float *Wrow = Wc + (size_t)ry * L;
+        // sources of row ys in internal order: colour q, in-row index i  ->  x = 2 i + ((ys + q) & 1)
         float ax = 0.0f, ay = 0.0f, az = 0.0f;
-        for (int xs = 0; xs < L; ++xs) {
-            int rx = xs - xt;
-            rx += rx < 0 ? L : 0;
-            int q;
-            const float *src = S + site_index(xs, ys, Lh, R, plane, q) + rr;
-            const float sx = src[0], sy = src[plane], sz = src[2 * plane];
-            const float wxx = __ldg(Wrow + rx), wxy = __ldg(Wrow + N + rx), wyy = __ldg(Wrow + 2 * N + rx),
-                        wzz = __ldg(Wrow + 3 * N + rx);
-            ax = fmaf(wxx, sx, fmaf(wxy, sy, ax));
-            ay = fmaf(wxy, sx, fmaf(wyy, sy, ay));
-            az = fmaf(wzz, sz, az);
+#pragma unroll
+        for (int q = 0; q < 2; ++q) {
+            const float *row = S + (size_t)q * 3 * plane + (size_t)ys * Lh * R + rr;
+            const int x0 = (ys + q) & 1;
+#pragma unroll 4
+            for (int i = 0; i < Lh; ++i) {
+                int rx = 2 * i + x0 - xt;
+                rx += rx < 0 ? L : 0;
+                const float sx = row[(size_t)i * R], sy = row[plane + (size_t)i * R], sz = row[2 * plane + (size_t)i * R];
+                const float wxx = __ldg(Wrow + rx), wxy = __ldg(Wrow + N + rx), wyy = __ldg(Wrow + 2 * N + rx),
+                            wzz = __ldg(Wrow + 3 * N + rx);
+                ax = fmaf(wxx, sx, fmaf(wxy, sy, ax));
+                ay = fmaf(wxy, sx, fmaf(wyy, sy, ay));
+                az = fmaf(wzz, sz, az);
+            }
         }
-        hx += ax;
+        hx += ax;                                              // row sums first: two-level fp32 accumulation
         hy += ay;
         hz += az;
     }
@@ -403,14 +411,14 @@ __global__ void __launch_bounds__(256) sublattice_field_kernel(const float *__re
         hy += part[k][1][lane];
         hz += part[k][2][lane];
     }
-    int q;
-    float *dst = H + site_index(xt, yt, Lh, R, plane, q) + r;
+    float *dst = part_out + (((size_t)blockIdx.z * gridDim.x + blockIdx.x) * 3) * R + r;
     dst[0] = hx;
-    dst[plane] = hy;
-    dst[2 * plane] = hz;
+    dst[R] = hy;
+    dst[2 * R] = hz;
 }
 
-__global__ void __launch_bounds__(128) sublattice_flip_kernel(const MetropolisArgs p, const RoundKeys rk, int l, int ox,
+__global__ void __launch_bounds__(128) sublattice_flip_kernel(const MetropolisArgs p, const RoundKeys rk,
+                                                              const float *__restrict__ part, int KS, int l, int ox,
                                                               int oy) {
     const int L = p.L, Lh = L >> 1, R = p.R;
     const size_t N = (size_t)L * L, plane = (size_t)L * Lh * R;
@@ -422,7 +430,13 @@ __global__ void __launch_bounds__(128) sublattice_flip_kernel(const MetropolisAr
     int q;
     const size_t at = site_index(xt, yt, Lh, R, plane, q) + r;
     float *own = p.S + at;
-    const float *hf = p.H + at;
+    float hx = 0.0f, hy = 0.0f, hz = 0.0f;                     // slab partials in fixed order
+    for (int ks = 0; ks < KS; ++ks) {
+        const float *ph = part + (((size_t)ks * nl * nl + k) * 3) * R + r;
+        hx += ph[0];
+        hy += ph[R];
+        hz += ph[2 * R];
+    }
     const int xe = xt + 1 == L ? 0 : xt + 1, xw = xt == 0 ? L - 1 : xt - 1;
     const int yn = yt + 1 == L ? 0 : yt + 1, ys = yt == 0 ? L - 1 : yt - 1;
     const float *ne = p.S + site_index(xe, yt, Lh, R, plane, q) + r, *nw = p.S + site_index(xw, yt, Lh, R, plane, q) + r;
@@ -432,8 +446,7 @@ __global__ void __launch_bounds__(128) sublattice_flip_kernel(const MetropolisAr
     const float ny = (ne[plane] + nw[plane]) + (nn[plane] + ns[plane]);
     const float nz = (ne[2 * plane] + nw[2 * plane]) + (nn[2 * plane] + ns[2 * plane]);
     const uint32_t n = (uint32_t)(yt * L + xt);
-    const Trial tr = decide(p, rk, n, (uint32_t)r, sx, sy, sz, nx, ny, nz, hf[0], hf[plane], hf[2 * plane], p.invT[r],
-                            p.K2[r], p.K4[r]);
+    const Trial tr = decide(p, rk, n, (uint32_t)r, sx, sy, sz, nx, ny, nz, hx, hy, hz, p.invT[r], p.K2[r], p.K4[r]);
     if (tr.acc) {
         own[0] = tr.tx;
         own[plane] = tr.ty;
@@ -521,14 +534,20 @@ void dsmc_sublattice_offset(uint64_t seed, uint64_t pass, int l, int *ox, int *o
     *oy = (int)(x.y % (uint32_t)l);
 }
 
-cudaError_t launch_sublattice_pass(const MetropolisArgs &a, const float *Wc, int l, int ox, int oy, cudaStream_t st,
-                                   uint64_t *launches) {
+cudaError_t launch_sublattice_pass(const MetropolisArgs &a, const float *Wc, float *scratch, int sm_count, int l, int ox,
+                                   int oy, cudaStream_t st, uint64_t *launches) {
     const RoundKeys rk = make_round_keys(a.seed_lo, a.seed_hi);
-    const int nl = a.L / l;
-    dim3 grid((unsigned)(nl * nl), (unsigned)((a.R + 31) / 32));
-    sublattice_field_kernel<<<grid, 256, 0, st>>>(a.S, const_cast<float *>(a.H), Wc, a.L, a.R, l, ox, oy);
-    const size_t total = (size_t)nl * nl * a.R;
-    sublattice_flip_kernel<<<(unsigned)((total + 127) / 128), 128, 0, st>>>(a, rk, l, ox, oy);
+    const int nl = a.L / l, n = nl * nl, chunks = (a.R + 31) / 32;
+    // source slabs: enough CTAs to fill the GPU about four times over, at least 8 rows per slab (one per
+    // warp), and KS * n <= N so that the partials fit the 3 N R floats of the staging buffer
+    int KS = (4 * sm_count + n * chunks - 1) / (n * chunks);
+    KS = std::max(1, std::min(KS, std::min(a.L / 8, l * l)));
+    const int rows = (a.L + KS - 1) / KS;
+    KS = (a.L + rows - 1) / rows;
+    sublattice_field_kernel<<<dim3((unsigned)n, (unsigned)chunks, (unsigned)KS), 256, 0, st>>>(a.S, scratch, Wc, a.L, a.R,
+                                                                                               l, ox, oy, rows);
+    const size_t total = (size_t)n * a.R;
+    sublattice_flip_kernel<<<(unsigned)((total + 127) / 128), 128, 0, st>>>(a, rk, scratch, KS, l, ox, oy);
     *launches += 2;
     return cudaGetLastError();
 }
