@@ -16,6 +16,7 @@ def _deps():
     d = [os.path.join(CSRC, s) for s in SOURCES]
     d.append(os.path.join(CSRC, "dsmc_internal.cuh"))
     d.append(os.path.join(CSRC, "bulk_copy.cuh"))
+    d.append(os.path.join(CSRC, "packed_f32x2.cuh"))
     d.append(os.path.join(HERE, "..", "include", "dsmc.h"))
     return d
 

@@ -8,6 +8,7 @@
 //   * the azimuth 2 pi u1 is reduced to a quadrant exactly in integer arithmetic and sin/cos come
 //     from two short polynomials (abs error 1.5e-7); sqrt and log use the MUFU units.
 #include "dsmc_internal.cuh"
+#include "packed_f32x2.cuh"
 #include <algorithm>
 
 namespace {
@@ -98,35 +99,6 @@ __device__ __forceinline__ Trial decide(const MetropolisArgs &p, const RoundKeys
     return t;
 }
 
-// ---- packed fp32 pairs (FFMA2 / FMUL2 / FADD2 of sm_100a): one instruction works on the same
-// quantity of two replicas.  A scalar operand written f2_bc(x) is folded by ptxas into the
-// instruction's broadcast / immediate operand form, so constants cost nothing.
-typedef unsigned long long f2;
-__device__ __forceinline__ f2 f2_make(float lo, float hi) {
-    f2 d;
-    asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "f"(lo), "f"(hi));
-    return d;
-}
-__device__ __forceinline__ f2 f2_bc(float a) { return f2_make(a, a); }
-__device__ __forceinline__ void f2_split(f2 v, float &lo, float &hi) {
-    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
-}
-__device__ __forceinline__ f2 f2_fma(f2 a, f2 b, f2 c) {
-    f2 d;
-    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
-    return d;
-}
-__device__ __forceinline__ f2 f2_mul(f2 a, f2 b) {
-    f2 d;
-    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
-    return d;
-}
-__device__ __forceinline__ f2 f2_add(f2 a, f2 b) {
-    f2 d;
-    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
-    return d;
-}
-__device__ __forceinline__ f2 f2_sub(f2 a, f2 b) { return f2_fma(b, f2_bc(-1.0f), a); }  // a - b, exact like FADD
 __device__ __forceinline__ float rsqrt_approx(float x) {
     float r;
     asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
