@@ -136,9 +136,8 @@ def run_reference(args):
 def run_cuda(args):
     import torch
     import torch.distributed as dist
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_1211_6234_b200 import multirank
+    rank, world, local = multirank.env()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the dsmc path has no CPU fallback)")
     torch.cuda.set_device(local)
@@ -158,7 +157,7 @@ def run_cuda(args):
     N = L * L
     K2, K4 = inputs.anisotropy(CFG_ID)
     T = inputs.temperatures(CFG_ID)
-    seed = inputs.SEED_BASE + CFG_ID + 1000 * rank
+    seed = multirank.rank_seed(inputs.SEED_BASE + CFG_ID, rank)
     ctx = m.Dsmc(L, R, J=1.0, g=c["g"], K2=K2, K4=K4, device=dev)
     ctx.build_tensor(m.DSMC_W_EWALD)
     s_host = torch.from_numpy(inputs.random_spins(L, R, seed)).pin_memory()
@@ -277,10 +276,7 @@ def run_cuda(args):
     e2e_s = (time.perf_counter() - t0) / n_e2e
 
     # ---- max over ranks ----------------------------------------------------------------------------
-    if world > 1:
-        tt = torch.tensor([ms, e2e_s], device=dev, dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms, e2e_s = float(tt[0]), float(tt[1])
+    ms, e2e_s = multirank.max_over_ranks([ms, e2e_s], device=dev)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -288,7 +284,7 @@ def run_cuda(args):
 
     updates_per_step = N * R
     ms_per_step = ms / args.steps
-    value = world * updates_per_step / (ms_per_step * 1e-3)
+    value = multirank.whole_job_rate(updates_per_step, world, ms_per_step * 1e-3)
     field_ms = float(np.mean(f_ms))
     metro_ms = float(np.mean(m_ms))
     flop_per_field = FLOP_PER_PAIR * (N // 2) * N * R

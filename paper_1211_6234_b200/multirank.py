@@ -1,0 +1,42 @@
+"""Host-side bookkeeping of the multi-GPU run ("replicas only").
+
+The path shards by replica with no data-path collective: every rank runs its own chains (its own seed),
+and the only exchange is one MAX all-reduce of the ranks' device timings, so that the reported time is
+the slowest rank's.  torch.distributed is plumbing here (NCCL on GPUs, gloo in the CPU tests)."""
+import os
+
+
+def env():
+    """(rank, world_size, local_rank) from the torchrun environment; (0, 1, 0) when run directly."""
+    return (int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")),
+            int(os.environ.get("LOCAL_RANK", "0")))
+
+
+def rank_seed(seed, rank):
+    """Independent chains per rank: Philox keys that differ in the seed never collide."""
+    return int(seed) + 1000 * int(rank)
+
+
+def replica_shard(R, world, rank):
+    """Contiguous block of the R replicas owned by `rank` when ONE ladder is split over the ranks
+    (strong scaling); blocks differ by at most one replica."""
+    base, extra = divmod(int(R), int(world))
+    lo = rank * base + min(rank, extra)
+    return lo, lo + base + (1 if rank < extra else 0)
+
+
+def max_over_ranks(values, device="cpu"):
+    """Element-wise maximum of a list of floats over all ranks (identity when not distributed)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return [float(v) for v in values]
+    t = torch.tensor([float(v) for v in values], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t.cpu()]
+
+
+def whole_job_rate(units_per_rank_step, world, seconds_per_step):
+    """Aggregate throughput of `world` ranks that each process units_per_rank_step per step (weak
+    scaling) in seconds_per_step (the max over ranks)."""
+    return world * units_per_rank_step / seconds_per_step
