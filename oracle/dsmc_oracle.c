@@ -713,3 +713,37 @@ int oracle_sublattice_pass(int L, int R, double J, double g, const double *K2, c
     free(entry);
     return 0;
 }
+
+/* ------------------------------------------------------------------------- */
+/* O9. Staggered magnetisation of App. B (after Binder and Landau [61]) */
+/* for stripes of width h = 1: four sub-lattices of the 2 x 2 plaquette,             */
+/*   1 = (x even, y even), 2 = (x odd, y even), 3 = (x odd, y odd), 4 = (x even, y odd), */
+/*   m_lambda = N^-1 sum_{i in lambda} s_i^z   (so that a perfect stripe state gives 1; */
+/*   the paper does not state the normalisation: DESIGN.md R23),                       */
+/*   m_h = m_1 + m_2 - m_3 - m_4 (horizontal stripes: rows alternate),                 */
+/*   m_v = m_1 + m_4 - m_3 - m_2 (vertical stripes: columns alternate),                */
+/*   m_st = (m_h^2 + m_v^2)^(1/2) per snapshot; <m_st> and chi_st are the caller's.     */
+/* out[r] = { m_h, m_v, m_st }.                                                        */
+/* ------------------------------------------------------------------------- */
+int oracle_staggered(int L, int R, const double *s, double *out)
+{
+    if (L < 2 || (L & 1) || R < 1 || !s || !out) return -1;
+    size_t N = (size_t)L * L;
+    for (int r = 0; r < R; ++r) {
+        const double *sz = s + ((size_t)r * 3 + 2) * N;
+        double m[4] = {0, 0, 0, 0};
+        for (int y = 0; y < L; ++y) {
+            for (int x = 0; x < L; ++x) {
+                int lambda = (y & 1) ? ((x & 1) ? 2 : 3) : ((x & 1) ? 1 : 0);
+                m[lambda] += sz[(size_t)y * L + x];
+            }
+        }
+        for (int k = 0; k < 4; ++k) m[k] /= (double)N;
+        double mh = m[0] + m[1] - m[2] - m[3];
+        double mv = m[0] + m[3] - m[2] - m[1];
+        out[3 * r + 0] = mh;
+        out[3 * r + 1] = mv;
+        out[3 * r + 2] = sqrt(mh * mh + mv * mv);
+    }
+    return 0;
+}

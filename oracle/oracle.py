@@ -255,3 +255,13 @@ def sublattice_pass(W, s, T, seed, pass_index, l, J, g, K2, K4, flip=False, sequ
                                       acc.ctypes.data_as(_c_u8_p), _d(mar), _d(tri))
     assert rc == 0, rc
     return {"offset": (int(off[0]), int(off[1])), "accept": acc, "margin": mar, "trial": tri}
+
+
+def staggered(s):
+    """App. B's staggered magnetisation per replica: [R][3] = m_h, m_v, m_st."""
+    s = _f64(s)
+    R, _, L, _ = s.shape
+    out = np.zeros((R, 3), dtype=np.float64)
+    rc = lib().oracle_staggered(L, R, _d(s), _d(out))
+    assert rc == 0, rc
+    return out

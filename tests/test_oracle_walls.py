@@ -83,3 +83,30 @@ def test_counts_against_numpy_rolls(oracle):
     nv = (1 - sg * np.roll(sg, -1, axis=2)).sum(axis=(2, 3))
     ref = np.stack([nh[:, 0], nv[:, 0], nh[:, 1], nv[:, 1], nh[:, 2], nv[:, 2]], axis=1)
     assert np.array_equal(c, ref.astype(np.int64))
+
+
+def test_staggered_magnetisation_of_stripe_states(oracle):
+    """App. B: width-1 horizontal stripes give |m_h| = 1, m_v = 0; vertical ones the
+    reverse; uniform, checkerboard and width-2 stripe states give m_st = 0; random Ising spins ~ N^-1/2."""
+    L = 8
+    x = np.arange(L)
+    rows = np.where(x % 2 == 0, 1.0, -1.0)[:, None] * np.ones((1, L))        # alternates along y
+    cols = rows.T.copy()
+    for f, expect in ((rows, (1.0, 0.0, 1.0)), (-rows, (-1.0, 0.0, 1.0)), (cols, (0.0, 1.0, 1.0)),
+                      (np.ones((L, L)), (0.0, 0.0, 0.0)),
+                      (np.where((x[:, None] + x[None, :]) % 2 == 0, 1.0, -1.0), (0.0, 0.0, 0.0)),
+                      (np.where((x // 2) % 2 == 0, 1.0, -1.0)[:, None] * np.ones((1, L)), (0.0, 0.0, 0.0))):
+        s = np.zeros((1, 3, L, L))
+        s[0, 2] = f
+        s[0, 0] = 0.5                                                          # in-plane components do not enter
+        assert np.allclose(oracle.staggered(s)[0], expect, atol=1e-15)
+    rng = np.random.default_rng(1)
+    s = np.zeros((4, 3, 64, 64))
+    s[:, 2] = rng.choice([-1.0, 1.0], size=(4, 64, 64))
+    m = oracle.staggered(s)
+    assert np.all(m[:, 2] < 5.0 / 64) and np.allclose(m[:, 2], np.hypot(m[:, 0], m[:, 1]))
+    # one defect in a perfect state lowers m_h by 2/N
+    s1 = np.zeros((1, 3, L, L))
+    s1[0, 2] = rows
+    s1[0, 2, 3, 5] *= -1
+    assert abs(oracle.staggered(s1)[0, 0] - (1.0 - 2.0 / (L * L))) < 1e-15
