@@ -168,6 +168,13 @@ int dsmc_observables(dsmc_ctx *ctx, double *out);
  *     eq. 18 are statistics the caller takes over snapshots.  Needs no field; synchronises.        */
 int dsmc_wall_observables(dsmc_ctx *ctx, long long *counts_out, double *derived_out);
 
+/* Staggered magnetisation of App. B (after Binder and Landau) for stripes of width 1, HOST
+ * out[R][3] = m_h, m_v, m_st with the sub-lattices of the 2 x 2 plaquette 1 = (x even, y even),
+ * 2 = (x odd, y even), 3 = (x odd, y odd), 4 = (x even, y odd), m_lambda = N^-1 sum_{i in lambda} s_i^z (R23),
+ *   m_h = m_1 + m_2 - m_3 - m_4,  m_v = m_1 + m_4 - m_3 - m_2,  m_st = (m_h^2 + m_v^2)^(1/2)
+ * per snapshot; <m_st> and chi_st = L^2 (<m_st^2> - <m_st>^2) / T are the caller's statistics.  Synchronises. */
+int dsmc_staggered_magnetisation(dsmc_ctx *ctx, double *out);
+
 /* Device time in milliseconds of the last field / Metropolis / reduction launches made by the
  * last dsmc_halfsweep* call, measured with CUDA events on the bound stream when timing was
  * enabled with dsmc_set_timing(ctx, 1); synchronises.  out[3] = {field, metropolis, total}.      */

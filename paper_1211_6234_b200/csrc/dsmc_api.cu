@@ -431,6 +431,26 @@ int dsmc_wall_observables(dsmc_ctx *ctx, long long *counts_out, double *derived_
     return DSMC_OK;
 }
 
+int dsmc_staggered_magnetisation(dsmc_ctx *ctx, double *out) {
+    if (int rc = need_bound(ctx)) return rc;
+    if (!out) return fail(ctx, DSMC_EINVAL, "null argument");
+    if (!ctx->spins_set) return fail(ctx, DSMC_ESTATE, "spins not set");
+    CU(launch_staggered(ctx->S(), ctx->obs(), ctx->L, ctx->R, ctx->stream, &ctx->launches), "staggered launch");
+    std::vector<double> raw(8 * (size_t)ctx->R);
+    CU(cudaMemcpyAsync(raw.data(), ctx->obs(), sizeof(double) * raw.size(), cudaMemcpyDeviceToHost, ctx->stream),
+       "staggered D2H");
+    CU(cudaStreamSynchronize(ctx->stream), "staggered sync");
+    const double N = (double)ctx->L * ctx->L;
+    for (int r = 0; r < ctx->R; ++r) {
+        const double *m = &raw[8 * (size_t)r];
+        const double mh = (m[0] + m[1] - m[2] - m[3]) / N, mv = (m[0] + m[3] - m[2] - m[1]) / N;
+        out[3 * r + 0] = mh;
+        out[3 * r + 1] = mv;
+        out[3 * r + 2] = sqrt(mh * mh + mv * mv);
+    }
+    return DSMC_OK;
+}
+
 int dsmc_set_timing(dsmc_ctx *ctx, int on) {
     if (!ctx) return DSMC_EINVAL;
     ctx->timing = on ? 1 : 0;

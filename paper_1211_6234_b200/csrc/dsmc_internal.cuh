@@ -128,3 +128,4 @@ cudaError_t launch_observables(const float *S, const float *H, const float *K2, 
                                uint64_t *launches);
 cudaError_t launch_wall_counts(const float *S, unsigned long long *counts, int L, int R, cudaStream_t st,
                                uint64_t *launches);
+cudaError_t launch_staggered(const float *S, double *sums, int L, int R, cudaStream_t st, uint64_t *launches);

@@ -142,6 +142,38 @@ __global__ void __launch_bounds__(256) wall_counts_kernel(const float *__restric
     }
 }
 
+// Sub-lattice sums of s_z over the 2 x 2 plaquette (App. B): per replica four fp64 sums,
+// index 0 = (x even, y even), 1 = (x odd, y even), 2 = (x odd, y odd), 3 = (x even, y odd).
+__global__ void __launch_bounds__(256) staggered_kernel(const float *__restrict__ S, double *__restrict__ sums, int L,
+                                                        int R) {
+    extern __shared__ double ssm[];  // [blockDim.x][4]
+    const int Lh = L >> 1;
+    const size_t Nh = (size_t)L * Lh, plane = Nh * (size_t)R;
+    const size_t nthreads = (size_t)gridDim.x * blockDim.x;
+    const size_t gid = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int r = (int)(gid % (size_t)R);
+    double acc[4] = {0, 0, 0, 0};
+    for (size_t t = gid; t < 2 * plane; t += nthreads) {
+        const size_t qa = t / (size_t)R;
+        const int q = (int)(qa / Nh);
+        const int a = (int)(qa - (size_t)q * Nh);
+        const int y = a / Lh, i = a - y * Lh;
+        const int x = 2 * i + ((y + q) & 1);
+        const int lambda = (y & 1) ? ((x & 1) ? 2 : 3) : ((x & 1) ? 1 : 0);
+        const float sz = S[((size_t)q * 3 + 2) * plane + (size_t)a * R + r];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) acc[k] += (k == lambda) ? (double)sz : 0.0;
+    }
+    for (int k = 0; k < 4; ++k) ssm[threadIdx.x * 4 + k] = acc[k];
+    __syncthreads();
+    if ((int)threadIdx.x < R) {
+        double tot[4] = {0, 0, 0, 0};
+        for (int j = threadIdx.x; j < (int)blockDim.x; j += R)
+            for (int k = 0; k < 4; ++k) tot[k] += ssm[j * 4 + k];
+        for (int k = 0; k < 4; ++k) atomicAdd(&sums[(size_t)r * 8 + k], tot[k]);
+    }
+}
+
 }  // namespace
 
 cudaError_t launch_canon_to_internal(const float *canon, float *S, int L, int R, cudaStream_t st,
@@ -199,6 +231,17 @@ cudaError_t launch_wall_counts(const float *S, unsigned long long *counts, int L
     unsigned grid;
     replica_walk_shape(L, R, &block, &grid);
     wall_counts_kernel<<<grid, block, sizeof(unsigned int) * 6 * block, st>>>(S, counts, L, R);
+    ++*launches;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_staggered(const float *S, double *sums, int L, int R, cudaStream_t st, uint64_t *launches) {
+    cudaError_t e = cudaMemsetAsync(sums, 0, sizeof(double) * 8 * (size_t)R, st);
+    if (e != cudaSuccess) return e;
+    int block;
+    unsigned grid;
+    replica_walk_shape(L, R, &block, &grid);
+    staggered_kernel<<<grid, block, sizeof(double) * 4 * block, st>>>(S, sums, L, R);
     ++*launches;
     return cudaGetLastError();
 }

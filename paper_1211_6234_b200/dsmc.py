@@ -40,6 +40,7 @@ ABI = [
     ("dsmc_sublattice_run", _i, [_vp, _vp, _u64, _u64, _u64, _i, _i]),
     ("dsmc_observables", _i, [_vp, _vp]),
     ("dsmc_wall_observables", _i, [_vp, _vp, _vp]),
+    ("dsmc_staggered_magnetisation", _i, [_vp, _vp]),
     ("dsmc_set_timing", _i, [_vp, _i]),
     ("dsmc_last_timing", _i, [_vp, _vp]),
     ("dsmc_launch_count", _u64, [_vp]),
@@ -226,6 +227,12 @@ class Dsmc:
         derived = np.empty((self.R, 4), dtype=np.float64)
         self._check(self.lib.dsmc_wall_observables(self._h, counts.ctypes.data, derived.ctypes.data))
         return counts, derived
+
+    def staggered_magnetisation(self):
+        """-> float64 [R][3] = m_h, m_v, m_st of App. B"""
+        out = np.empty((self.R, 3), dtype=np.float64)
+        self._check(self.lib.dsmc_staggered_magnetisation(self._h, out.ctypes.data))
+        return out
 
     def set_timing(self, on=True):
         self._check(self.lib.dsmc_set_timing(self._h, int(on)))

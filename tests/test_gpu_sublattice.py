@@ -144,3 +144,23 @@ def test_sublattice_argument_errors(dsmc_mod):
             ctx.sublattice_pass(T, 1, 0, bad_l)
     ctx.sublattice_run(T, 1, 0, 9, 3)                               # 9 = l*l passes = one MC step
     ctx.close()
+
+
+@pytest.mark.parametrize("L,R", [(8, 1), (12, 5), (64, 16), (256, 64)])
+def test_staggered_magnetisation_parity(dsmc_mod, oracle, L, R):
+    """App. B's order parameter: Ising states (exact sums) and Heisenberg states (fp64 sums of fp32 values)."""
+    from paper_1211_6234_b200 import inputs
+    ctx = dsmc_mod.Dsmc(L, R)
+    rng = np.random.default_rng(12)
+    ising = np.zeros((R, 3, L, L), dtype=np.float32)
+    ising[:, 2] = np.where(np.arange(L) % 2 == 0, 1.0, -1.0)[None, :, None]
+    ising[:, 2] *= np.where(rng.random((R, L, L)) < 0.1, -1.0, 1.0)
+    ctx.set_spins(ising)
+    got, ref = ctx.staggered_magnetisation(), oracle.staggered(ising.astype(np.float64))
+    N = L * L                                                    # the sub-lattice sums are integers: exact
+    assert np.array_equal(np.rint(got[:, :2] * N), np.rint(ref[:, :2] * N)) and np.max(np.abs(got - ref)) <= 1e-15
+    assert np.all(np.abs(got[:, 0]) > 0.7)
+    s = inputs.random_spins(L, R, 4)
+    ctx.set_spins(s)
+    assert np.max(np.abs(ctx.staggered_magnetisation() - oracle.staggered(s.astype(np.float64)))) <= 1e-13
+    ctx.close()
