@@ -225,8 +225,20 @@ def run_cuda(args):
             ctx.halfsweep(None, seed, 2 * (base + args.warmup + n_fft) + k)
             ff.append(float(ctx.last_timing()[0]))
         ctx.set_timing(False)
+        # end to end with HOST buffers, as the e2e key of the main line
+        def fft_e2e_step(k):
+            ctx.set_spins(s_host.numpy())
+            sweep(k)
+            ctx.get_spins(out_host.numpy())
+        fft_e2e_step(0)
+        torch.cuda.synchronize(dev)
+        t0 = time.perf_counter()
+        for k in range(5):
+            fft_e2e_step(k)
+        torch.cuda.synchronize(dev)
+        fft_e2e_s = (time.perf_counter() - t0) / 5
         ctx.select_field_kernel(m.DSMC_FIELD_AUTO)
-        fft = {"ms_per_step": fft_ms, "field_ms_per_launch_group": float(np.median(ff)), "launches_per_step": fft_launches}
+        fft = {"e2e_s": fft_e2e_s, "ms_per_step": fft_ms, "field_ms_per_launch_group": float(np.median(ff)), "launches_per_step": fft_launches}
 
     # Metropolis kernel alone with a working set larger than L2: three independent contexts are
     # updated in rotation, so the ~100 MB a launch touches were evicted by the ~200 MB the two
@@ -331,6 +343,8 @@ def run_cuda(args):
             "value": world * updates_per_step / (fft["ms_per_step"] * 1e-3), "unit": "updates/s",
             "ms_per_step": fft["ms_per_step"], "gpu_launches_per_step": fft["launches_per_step"],
             "speedup_vs_direct_sum": ms_per_step / fft["ms_per_step"],
+            "e2e": {"value": world * updates_per_step / fft["e2e_s"], "unit": "updates/s",
+                    "h2d_bytes_per_step": int(s_host.numel() * 4), "d2h_bytes_per_step": int(out_host.numel() * 4)},
             "roofline": {"kernel": "fft_x_forward + fft_y_multiply + fft_x_inverse", "bound": "hbm", "achieved": gbs,
                          "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak, "peak_kind": hbm_kind,
                          "ms_per_launch_group": fft["field_ms_per_launch_group"], "bytes_per_launch_group": fft_bytes,
