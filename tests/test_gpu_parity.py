@@ -439,3 +439,45 @@ def test_wall_observables_parity(dsmc_mod, oracle, L, R):
         assert np.array_equal(counts, ref), (L, R)
         assert np.max(np.abs(derived - oracle.wall_order(L, ref))) <= 1e-15
     ctx.close()
+
+
+def _fft_field_fp64(W, s):
+    """Harness-only third opinion: the circular correlation h_n = sum_m W(m - n) s_m by
+    numpy's fp64 FFT.  Checked against the oracle's direct sum before it is trusted (below)."""
+    Wh = np.fft.fft2(W, axes=(-2, -1))                      # [4][L][L]
+    sh = np.fft.fft2(s, axes=(-2, -1))                      # [R][3][L][L]
+    M = np.conj(Wh)                                         # correlation: conj of the kernel's transform
+    hx = M[0] * sh[:, 0] + M[1] * sh[:, 1]
+    hy = M[1] * sh[:, 0] + M[2] * sh[:, 1]
+    hz = M[3] * sh[:, 2]
+    return np.real(np.fft.ifft2(np.stack([hx, hy, hz], axis=1), axes=(-2, -1)))
+
+
+def test_field_parity_L256_every_target(dsmc_mod, oracle):
+    """Config 5 at full size, EVERY target of every replica, both direct-sum launch configurations
+    (colour 0 and 1 half-sweep fields of the tiled kernel) and the FFT route, against an fp64 FFT
+    evaluation in the harness that is first pinned to the oracle's direct sum (L = 32 in full, and
+    sampled targets at L = 256)."""
+    from paper_1211_6234_b200 import inputs
+    W32 = oracle.build_tensor_ewald(32)
+    s32 = inputs.random_spins(32, 3, 5).astype(np.float64)
+    assert np.max(np.abs(_fft_field_fp64(W32, s32) - oracle.dipole_field(W32, s32))) < 1e-12
+    c = inputs.CONFIGS[5]
+    L, R = c["L"], c["R"]
+    W = oracle.build_tensor_ewald(L)
+    s = inputs.initial_spins(5)
+    ref = _fft_field_fp64(W, s.astype(np.float64))
+    targets = np.random.default_rng(3).choice(L * L, size=16, replace=False).astype(np.int32)
+    direct = oracle.dipole_field_sampled(W, s[7].astype(np.float64), targets)
+    assert np.max(np.abs(ref[7].reshape(3, L * L)[:, targets].T - direct)) < 1e-11
+    ctx = make_ctx(dsmc_mod, 5, inputs)
+    ctx.set_spins(s)
+    for kind in (dsmc_mod.DSMC_FIELD_TILED, dsmc_mod.DSMC_FIELD_FFT):
+        ctx.select_field_kernel(kind)
+        h = np.zeros((R, 3, L, L), dtype=np.float32)
+        ctx.dipole_field(0, out=h)
+        ctx.dipole_field(1, out=h)
+        rel, mx = field_errors(h, ref)
+        print("kind", kind, "rel L2", rel, "max abs", mx)
+        assert rel <= FIELD_REL_L2 and mx <= FIELD_MAX_ABS, (kind, rel, mx)
+    ctx.close()
