@@ -350,9 +350,9 @@ def run_cuda(args):
                          "ms_per_launch_group": fft["field_ms_per_launch_group"], "bytes_per_launch_group": fft_bytes,
                          "traffic": TRAFFIC_FFT_GROUP}}
     if world == 1 and not args.no_cpu_baseline:
-        ups, sec, cores = oracle_sample(1, 0, 8)
+        ups, sec, cores = oracle_sample(1, 0, 24)
         line["cpu_baseline"] = {"value": ups, "unit": "updates/s", "cores": cores, "kind": "oracle",
-                                "sample": "one checkerboard half-sweep of config 5 on 8 of 64 replicas "
+                                "sample": "one checkerboard half-sweep of config 5 on 24 of 64 replicas "
                                           f"({sec:.1f} s; work is linear in R)"}
     print(json.dumps(line))
     if world > 1:
