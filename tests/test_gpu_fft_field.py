@@ -124,3 +124,26 @@ def test_fft_unsupported_shapes(dsmc_mod):
         with pytest.raises(dsmc_mod.DsmcError):
             ctx.select_field_kernel(dsmc_mod.DSMC_FIELD_FFT)
         ctx.close()
+
+
+def test_largest_transform_L512(dsmc_mod, oracle):
+    """The largest supported lattice of the FFT route (N2 = 32) and the tiled kernel at the same size,
+    every target, against the harness fp64 FFT (pinned to the oracle in test_gpu_parity) plus sampled
+    targets by the oracle's direct sum."""
+    from paper_1211_6234_b200 import inputs
+    from test_gpu_parity import _fft_field_fp64
+    L, R = 512, 4
+    ctx = dsmc_mod.Dsmc(L, R)
+    ctx.build_tensor(dsmc_mod.DSMC_W_EWALD)
+    W = ctx.get_tensor().astype(np.float64)                   # the table itself is checked at L <= 256
+    s = inputs.random_spins(L, R, 2)
+    ctx.set_spins(s)
+    ref = _fft_field_fp64(W, s.astype(np.float64))
+    targets = np.random.default_rng(1).choice(L * L, size=8, replace=False).astype(np.int32)
+    direct = oracle.dipole_field_sampled(W, s[1].astype(np.float64), targets)
+    assert np.max(np.abs(ref[1].reshape(3, L * L)[:, targets].T - direct)) < 1e-10
+    for kind in (dsmc_mod.DSMC_FIELD_FFT, dsmc_mod.DSMC_FIELD_TILED):
+        ctx.select_field_kernel(kind)
+        rel, mx = errs(ctx.dipole_field(-1), ref)
+        assert rel <= FIELD_REL_L2 and mx <= FIELD_MAX_ABS, (kind, rel, mx)
+    ctx.close()
