@@ -78,10 +78,11 @@ def test_sublattice_lockstep(dsmc_mod, oracle, L, R, l, passes):
 
 
 def test_sublattice_ising_flip(dsmc_mod, oracle):
-    """App. B: L = 64, l = 32, Ising spins, J / C_D = 1.7, T around T_c = 0.85 C_D (PAPER.md:366-372,
-    Table 1), starting from the h = 1 stripe ground state with a few defects."""
+    """App. B: L = 64, l = 32, Ising spins, J / C_D = 1.7 in eq. 19's convention (0.85 per bond in ours,
+    DESIGN.md R22), T around the paper's T_c = 0.85 C_D (Table 1), starting from the
+    h = 1 stripe ground state with a few defects."""
     L, R, l = 64, 8, 32
-    J, g = 1.0, 1.0 / 1.7
+    J, g = 0.85, 1.0
     ctx = dsmc_mod.Dsmc(L, R, J=J, g=g, K2=0.0, K4=0.0)
     ctx.build_tensor(dsmc_mod.DSMC_W_EWALD)
     W = oracle.build_tensor_ewald(L)
@@ -164,3 +165,42 @@ def test_staggered_magnetisation_parity(dsmc_mod, oracle, L, R):
     ctx.set_spins(s)
     assert np.max(np.abs(ctx.staggered_magnetisation() - oracle.staggered(s.astype(np.float64)))) <= 1e-13
     ctx.close()
+
+
+def test_simultaneous_flipping_error_is_small(dsmc_mod, oracle):
+    """App. B's question: do the errors of simultaneous flipping compound over many
+    passes?  Dipolar Ising model, J / C_D = 1.7 in eq. 19's convention = 0.85 per bond in ours (DESIGN.md
+    R22: inside the width-1 stripe window 0.43 < J/g < 1.26), L = 16 with l = 8 (four simultaneous
+    flips per pass, a stronger approximation than the paper's l = 32), staggered magnetisation against
+    T / C_D: the GPU's frozen-field schedule versus conventional sequential Metropolis in the oracle
+    (independent seeds).  The paper reports shifts below 8 % in the critical values (Table 1)."""
+    L, l, R = 16, 8, 8
+    J, g = 0.85, 1.0
+    Tn = np.linspace(0.4, 1.4, R)                                   # T / C_D: T_c ~ 0.82-0.85 (Table 1)
+    T = (Tn * g).astype(np.float32)
+    W = oracle.build_tensor_ewald(L)
+    s0 = np.zeros((R, 3, L, L), dtype=np.float32)
+    s0[:, 2] = np.where(np.arange(L) % 2 == 0, 1.0, -1.0)[None, :, None]
+    n_steps, burn, every = 600, 200, 5
+    ctx = dsmc_mod.Dsmc(L, R, J=J, g=g, K2=0.0, K4=0.0)
+    ctx.build_tensor(dsmc_mod.DSMC_W_EWALD)
+    ctx.set_spins(s0)
+    gpu = []
+    for step in range(n_steps):
+        ctx.sublattice_run(T, 4242, step * l * l, l * l, l, flags=dsmc_mod.DSMC_TRIAL_FLIP)
+        if step >= burn and step % every == 0:
+            gpu.append(ctx.staggered_magnetisation()[:, 2])
+    ctx.close()
+    s = s0.astype(np.float64)
+    seq = []
+    for step in range(n_steps):
+        for p in range(step * l * l, (step + 1) * l * l):
+            oracle.sublattice_pass(W, s, T, 1717, p, l, J, g, 0.0, 0.0, flip=True, sequential=True)
+        if step >= burn and step % every == 0:
+            seq.append(oracle.staggered(s)[:, 2])
+    gpu, seq = np.mean(gpu, axis=0), np.mean(seq, axis=0)
+    print("T/C_D      ", np.round(Tn, 2))
+    print("m_st GPU   ", np.round(gpu, 3))
+    print("m_st seq.  ", np.round(seq, 3))
+    assert gpu[0] > 0.75 and seq[0] > 0.75 and gpu[-1] < 0.3 and seq[-1] < 0.3      # ordered -> disordered
+    assert np.max(np.abs(gpu - seq)) < 0.1, np.abs(gpu - seq)                       # measured: 0.03

@@ -111,7 +111,7 @@ def test_ising_flip_move(oracle):
     rng = np.random.default_rng(4)
     L, l, R = 8, 4, 2
     W = oracle.build_tensor_ewald(L)
-    J, g = 1.0, 1.0 / 1.7                                          # J / C_D = 1.7
+    J, g = 0.85, 1.0                                               # J / C_D = 1.7 of eq. 19 = 0.85 per bond (R22)
     s = np.zeros((R, 3, L, L))
     s[:, 2] = rng.choice([-1.0, 1.0], size=(R, L, L))
     for p in range(20):
