@@ -23,6 +23,8 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 CFG_ID = 5
+WORKLOAD = ("config5 L=256 R=64 J=1 g=0.1 K2=0.6 K4=0.1 T=0.1..2.0, 1 step = 1 sweep "
+            "(2 x [dipole field + Metropolis half-sweep])")
 FLOP_PER_PAIR = 10.0           # 5 FMA per (target, source, replica): SURVEY.md section 8(d)
 BYTES_PER_UPDATE = 48.0        # own spin 12 + neighbours 12 (amortised) + h 12 + write 12
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
@@ -124,8 +126,8 @@ def run_reference(args):
         "impl": "reference", "metric": "spin_updates_per_s", "value": ups, "unit": "updates/s", "n_gpus": args.gpus,
         "steps": args.steps, "warmup": min(args.warmup, 1), "ms_per_step": sec * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "config5 L=256 R=64 J=1 g=0.1 K2=0.6 K4=0.1 T=0.1..2.0 (bounded sample)", "L": c["L"],
-                   "R": c["R"], "sample_replicas": n_rep},
+        "config": {"workload": WORKLOAD, "L": c["L"], "R": c["R"], "parallelism": "host cores, rank 0 only",
+                   "sample": f"each step = one half-sweep on {n_rep} of {c['R']} replicas"},
         "cpu_baseline": {"value": ups, "unit": "updates/s", "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": ups, "unit": "updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -310,9 +312,7 @@ def run_cuda(args):
         "metric": "spin_updates_per_s", "value": value, "unit": "updates/s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": "config5 L=256 R=64 J=1 g=0.1 K2=0.6 K4=0.1 T=0.1..2.0, 1 step = 1 sweep "
-                               "(2 x [dipole field + Metropolis half-sweep])",
-                   "L": L, "R": R, "parallelism": f"replicas only x{world}",
+        "config": {"workload": WORKLOAD, "L": L, "R": R, "parallelism": f"replicas only x{world}",
                    "l2": "working set per step (spins 50 MB + h 25 MB + split-K partials 201 MB) exceeds the 126 MB L2; "
                          "the Metropolis-only figure rotates over 3 contexts (300 MB) so every launch starts with its data evicted from L2",
                    "field_kernel": "tiled" if ctx.field_kernel_kind() == 1 else "generic"},
