@@ -747,3 +747,30 @@ int oracle_staggered(int L, int R, const double *s, double *out)
     }
     return 0;
 }
+
+/* ------------------------------------------------------------------------- */
+/* O10. Ensemble statistics over n recorded states:          */
+/*   thermal average <X> = n^-1 sum_t X_t,                                      */
+/*   variance sigma^2(X) = <(X - <X>)^2> = <X^2> - <X>^2          (eq. 18, :265) */
+/*   standard error SE = ((<X^2> - <X>^2) / n)^(1/2)              (eq. 13, :177) */
+/* x[t][k], t < n snapshots, k < K quantities; outputs mean[K], var[K], se[K].  */
+/* ------------------------------------------------------------------------- */
+int oracle_ensemble(int n, int K, const double *x, double *mean, double *var, double *se)
+{
+    if (n < 1 || K < 1 || !x || !mean || !var || !se) return -1;
+    for (int k = 0; k < K; ++k) {
+        double m = 0.0;
+        for (int t = 0; t < n; ++t) m += x[(size_t)t * K + k];
+        m /= (double)n;
+        double v = 0.0;
+        for (int t = 0; t < n; ++t) {
+            double d = x[(size_t)t * K + k] - m;
+            v += d * d;
+        }
+        v /= (double)n;
+        mean[k] = m;
+        var[k] = v;
+        se[k] = sqrt(v / (double)n);
+    }
+    return 0;
+}

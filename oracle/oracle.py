@@ -265,3 +265,15 @@ def staggered(s):
     rc = lib().oracle_staggered(L, R, _d(s), _d(out))
     assert rc == 0, rc
     return out
+
+
+def ensemble(x):
+    """x[n snapshots][...] -> (mean, var, se) over the first axis: eq. 13 and eq. 18."""
+    x = _f64(x)
+    n = x.shape[0]
+    K = int(np.prod(x.shape[1:])) if x.ndim > 1 else 1
+    mean, var, se = np.zeros(K), np.zeros(K), np.zeros(K)
+    rc = lib().oracle_ensemble(int(n), K, _d(x.reshape(n, K)), _d(mean), _d(var), _d(se))
+    assert rc == 0, rc
+    shp = x.shape[1:]
+    return mean.reshape(shp), var.reshape(shp), se.reshape(shp)

@@ -110,3 +110,20 @@ def test_staggered_magnetisation_of_stripe_states(oracle):
     s1[0, 2] = rows
     s1[0, 2, 3, 5] *= -1
     assert abs(oracle.staggered(s1)[0, 0] - (1.0 - 2.0 / (L * L))) < 1e-15
+
+
+def test_ensemble_statistics(oracle):
+    """eq. 13 / eq. 18: closed forms and the library routine."""
+    m, v, se = oracle.ensemble(np.full((7, 3), 2.5))
+    assert np.all(m == 2.5) and np.all(v == 0.0) and np.all(se == 0.0)
+    x = np.array([[1.0], [3.0]] * 50)                              # +-1 around 2: variance 1, SE = 1/sqrt(n)
+    m, v, se = oracle.ensemble(x)
+    assert m[0] == 2.0 and v[0] == 1.0 and abs(se[0] - 0.1) < 1e-16
+    t = np.arange(1, 11, dtype=np.float64)[:, None]                # 1..10: mean 5.5, variance (n^2-1)/12
+    m, v, se = oracle.ensemble(t)
+    assert m[0] == 5.5 and abs(v[0] - 99.0 / 12.0) < 1e-14 and abs(se[0] - np.sqrt(99.0 / 120.0)) < 1e-15
+    rng = np.random.default_rng(0)
+    y = rng.standard_normal((1000, 4, 2))
+    m, v, se = oracle.ensemble(y)
+    assert np.allclose(m, y.mean(0), atol=1e-15) and np.allclose(v, y.var(0), atol=1e-14)
+    assert np.allclose(se, y.std(0) / np.sqrt(1000), atol=1e-15)
