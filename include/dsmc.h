@@ -175,6 +175,19 @@ int dsmc_wall_observables(dsmc_ctx *ctx, long long *counts_out, double *derived_
  * per snapshot; <m_st> and chi_st = L^2 (<m_st^2> - <m_st>^2) / T are the caller's statistics.  Synchronises. */
 int dsmc_staggered_magnetisation(dsmc_ctx *ctx, double *out);
 
+/* Ensemble statistics accumulated on the device (an ensemble of recorded states;
+ * eq. 13 standard error, eq. 18 variance).  dsmc_ensemble_add computes, for the CURRENT state and every
+ * replica, the eight per-snapshot quantities
+ *   0 E/N, 1 m_z, 2 M_par, 3 eta (as dsmc_observables), 4 wall density, 5 O_x, 6 O_y, 7 O_z (as
+ *   dsmc_wall_observables)
+ * and adds x and x^2 to running fp64 sums; it is asynchronous (no host round trip), so a production run is
+ * "sweeps, add, sweeps, add, ..." without synchronisation.  dsmc_ensemble_get returns, as HOST [R][8]
+ * arrays, <x>, sigma^2(x) = <x^2> - <x>^2 (eq. 18) and SE = (sigma^2 / n)^(1/2) (eq. 13) over the n
+ * snapshots added since dsmc_ensemble_reset (n_out nullable); DSMC_ESTATE if n = 0.  Synchronises.      */
+int dsmc_ensemble_reset(dsmc_ctx *ctx);
+int dsmc_ensemble_add(dsmc_ctx *ctx);
+int dsmc_ensemble_get(dsmc_ctx *ctx, double *mean, double *var, double *se, uint64_t *n_out);
+
 /* Device time in milliseconds of the last field / Metropolis / reduction launches made by the
  * last dsmc_halfsweep* call, measured with CUDA events on the bound stream when timing was
  * enabled with dsmc_set_timing(ctx, 1); synchronises.  out[3] = {field, metropolis, total}.      */

@@ -158,6 +158,8 @@ DsmcLayout dsmc_make_layout(int L, int R) {
     l.off_stage = o; o = align256(o + sizeof(float) * 3 * N * R);
     l.off_T = o; o = align256(o + sizeof(float) * 3 * R);
     l.off_obs = o; o = align256(o + sizeof(double) * 8 * R);
+    l.off_walls = o; o = align256(o + sizeof(unsigned long long) * 8 * R);
+    l.off_stats = o; o = align256(o + sizeof(double) * 16 * R);
     l.total = o;
     return l;
 }
@@ -410,7 +412,7 @@ int dsmc_wall_observables(dsmc_ctx *ctx, long long *counts_out, double *derived_
     if (int rc = need_bound(ctx)) return rc;
     if (!counts_out) return fail(ctx, DSMC_EINVAL, "null argument");
     if (!ctx->spins_set) return fail(ctx, DSMC_ESTATE, "spins not set");
-    unsigned long long *dev = reinterpret_cast<unsigned long long *>(ctx->obs());
+    unsigned long long *dev = ctx->walls();
     CU(launch_wall_counts(ctx->S(), dev, ctx->L, ctx->R, ctx->stream, &ctx->launches), "wall counts launch");
     std::vector<unsigned long long> raw(8 * (size_t)ctx->R);
     CU(cudaMemcpyAsync(raw.data(), dev, sizeof(unsigned long long) * raw.size(), cudaMemcpyDeviceToHost, ctx->stream),
@@ -447,6 +449,51 @@ int dsmc_staggered_magnetisation(dsmc_ctx *ctx, double *out) {
         out[3 * r + 0] = mh;
         out[3 * r + 1] = mv;
         out[3 * r + 2] = sqrt(mh * mh + mv * mv);
+    }
+    return DSMC_OK;
+}
+
+int dsmc_ensemble_reset(dsmc_ctx *ctx) {
+    if (int rc = need_bound(ctx)) return rc;
+    CU(cudaMemsetAsync(ctx->stats(), 0, sizeof(double) * 16 * (size_t)ctx->R, ctx->stream), "ensemble reset");
+    ctx->ensemble_n = 0;
+    return DSMC_OK;
+}
+
+int dsmc_ensemble_add(dsmc_ctx *ctx) {
+    if (int rc = need_bound(ctx)) return rc;
+    if (!ctx->tensor_built) return fail(ctx, DSMC_ESTATE, "tensor not built");
+    if (!ctx->spins_set) return fail(ctx, DSMC_ESTATE, "spins not set");
+    if (int rc = upload_params(ctx, ctx->T_valid ? nullptr : std::vector<float>(ctx->R, 1.0f).data())) return rc;
+    if (int rc = run_field(ctx, -1)) return rc;
+    CU(launch_observables(ctx->S(), ctx->H(), ctx->K2d(), ctx->K4d(), ctx->obs(), ctx->L, ctx->R, ctx->J, ctx->g,
+                          ctx->stream, &ctx->launches),
+       "observables launch");
+    CU(launch_wall_counts(ctx->S(), ctx->walls(), ctx->L, ctx->R, ctx->stream, &ctx->launches), "wall counts launch");
+    CU(launch_ensemble_add(ctx->obs(), ctx->walls(), ctx->stats(), ctx->L, ctx->R, (double)ctx->J, (double)ctx->g,
+                           ctx->stream, &ctx->launches),
+       "ensemble launch");
+    ++ctx->ensemble_n;
+    return DSMC_OK;
+}
+
+int dsmc_ensemble_get(dsmc_ctx *ctx, double *mean, double *var, double *se, uint64_t *n_out) {
+    if (int rc = need_bound(ctx)) return rc;
+    if (!mean || !var || !se) return fail(ctx, DSMC_EINVAL, "null argument");
+    if (n_out) *n_out = ctx->ensemble_n;
+    if (ctx->ensemble_n == 0) return fail(ctx, DSMC_ESTATE, "empty ensemble");
+    std::vector<double> raw(16 * (size_t)ctx->R);
+    CU(cudaMemcpyAsync(raw.data(), ctx->stats(), sizeof(double) * raw.size(), cudaMemcpyDeviceToHost, ctx->stream),
+       "ensemble D2H");
+    CU(cudaStreamSynchronize(ctx->stream), "ensemble sync");
+    const double n = (double)ctx->ensemble_n;
+    for (size_t i = 0; i < 8 * (size_t)ctx->R; ++i) {
+        const double m = raw[2 * i] / n;
+        double v = raw[2 * i + 1] / n - m * m;
+        if (v < 0.0) v = 0.0;  // rounding of <x^2> - <x>^2 for a constant series
+        mean[i] = m;
+        var[i] = v;
+        se[i] = sqrt(v / n);
     }
     return DSMC_OK;
 }

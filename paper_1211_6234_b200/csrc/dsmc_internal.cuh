@@ -32,7 +32,9 @@ struct DsmcLayout {
     size_t off_Z;      // spectrum scratch Z[3][L][L][R/2] complex of the FFT field
     size_t off_stage;  // canonical staging [R][3][L][L] floats
     size_t off_T;      // invT[R], K2[R], K4[R] floats
-    size_t off_obs;    // R*8 doubles
+    size_t off_obs;    // R*8 doubles (raw observable sums)
+    size_t off_walls;  // R*8 64-bit wall counts
+    size_t off_stats;  // R*8*2 doubles: ensemble sums of x and x^2
     size_t total;
 };
 
@@ -53,6 +55,7 @@ struct dsmc_ctx {
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
     bool ev_recorded = false;
     uint64_t launches = 0;
+    uint64_t ensemble_n = 0;  // snapshots accumulated since dsmc_ensemble_reset
     int sm_count = 148;
     std::string err;
 
@@ -68,6 +71,8 @@ struct dsmc_ctx {
     float *K2d() const { return invT() + R; }
     float *K4d() const { return invT() + 2 * R; }
     double *obs() const { return (double *)(ws + lay.off_obs); }
+    unsigned long long *walls() const { return (unsigned long long *)(ws + lay.off_walls); }
+    double *stats() const { return (double *)(ws + lay.off_stats); }
     size_t Nh() const { return (size_t)L * (L / 2); }
     size_t plane() const { return Nh() * (size_t)R; }  // floats in one [a][r] plane
 };
@@ -129,3 +134,5 @@ cudaError_t launch_observables(const float *S, const float *H, const float *K2, 
 cudaError_t launch_wall_counts(const float *S, unsigned long long *counts, int L, int R, cudaStream_t st,
                                uint64_t *launches);
 cudaError_t launch_staggered(const float *S, double *sums, int L, int R, cudaStream_t st, uint64_t *launches);
+cudaError_t launch_ensemble_add(const double *obs, const unsigned long long *walls, double *stats, int L, int R, double J,
+                                double g, cudaStream_t st, uint64_t *launches);

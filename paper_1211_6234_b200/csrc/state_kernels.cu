@@ -174,6 +174,35 @@ __global__ void __launch_bounds__(256) staggered_kernel(const float *__restrict_
     }
 }
 
+// Ensemble accumulator (PAPER.md:175-177 eq. 13; :265 eq. 18): one thread per replica turns the raw sums
+// of observables_kernel and the counts of wall_counts_kernel into the eight per-snapshot quantities
+//   E/N, m_z, M_par, eta, wall density, O_x, O_y, O_z
+// and adds x and x^2 to the running sums stats[r][k][2] (fp64), all on the device.
+__global__ void ensemble_add_kernel(const double *__restrict__ obs, const unsigned long long *__restrict__ walls,
+                                    double *__restrict__ stats, int L, int R, double J, double g) {
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= R) return;
+    const double N = (double)L * L;
+    const double *s = obs + 8 * (size_t)r;
+    const unsigned long long *n = walls + 8 * (size_t)r;
+    double x[8];
+    const double mx = s[0] / N, my = s[1] / N;
+    x[0] = (-J * s[4] - s[5] + 0.5 * g * s[6]) / N;
+    x[1] = s[2] / N;
+    x[2] = sqrt(mx * mx + my * my);
+    x[3] = (2.0 / 3.14159265358979323846) * sqrt(s[3] / N);
+    x[4] = (double)(n[4] + n[5]) / (4.0 * N);
+    for (int c = 0; c < 3; ++c) {
+        const unsigned long long nh = n[2 * c], nv = n[2 * c + 1];
+        x[5 + c] = nh + nv ? (double)(nh > nv ? nh - nv : nv - nh) / (double)(nh + nv) : 0.0;
+    }
+    double *dst = stats + 16 * (size_t)r;
+    for (int k = 0; k < 8; ++k) {
+        dst[2 * k] += x[k];
+        dst[2 * k + 1] += x[k] * x[k];
+    }
+}
+
 }  // namespace
 
 cudaError_t launch_canon_to_internal(const float *canon, float *S, int L, int R, cudaStream_t st,
@@ -242,6 +271,13 @@ cudaError_t launch_staggered(const float *S, double *sums, int L, int R, cudaStr
     unsigned grid;
     replica_walk_shape(L, R, &block, &grid);
     staggered_kernel<<<grid, block, sizeof(double) * 4 * block, st>>>(S, sums, L, R);
+    ++*launches;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_ensemble_add(const double *obs, const unsigned long long *walls, double *stats, int L, int R, double J,
+                                double g, cudaStream_t st, uint64_t *launches) {
+    ensemble_add_kernel<<<(R + 127) / 128, 128, 0, st>>>(obs, walls, stats, L, R, J, g);
     ++*launches;
     return cudaGetLastError();
 }

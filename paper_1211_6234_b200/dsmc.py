@@ -41,6 +41,9 @@ ABI = [
     ("dsmc_observables", _i, [_vp, _vp]),
     ("dsmc_wall_observables", _i, [_vp, _vp, _vp]),
     ("dsmc_staggered_magnetisation", _i, [_vp, _vp]),
+    ("dsmc_ensemble_reset", _i, [_vp]),
+    ("dsmc_ensemble_add", _i, [_vp]),
+    ("dsmc_ensemble_get", _i, [_vp, _vp, _vp, _vp, _vp]),
     ("dsmc_set_timing", _i, [_vp, _i]),
     ("dsmc_last_timing", _i, [_vp, _vp]),
     ("dsmc_launch_count", _u64, [_vp]),
@@ -233,6 +236,21 @@ class Dsmc:
         out = np.empty((self.R, 3), dtype=np.float64)
         self._check(self.lib.dsmc_staggered_magnetisation(self._h, out.ctypes.data))
         return out
+
+    def ensemble_reset(self):
+        self._check(self.lib.dsmc_ensemble_reset(self._h))
+
+    def ensemble_add(self):
+        """Accumulate the current state's E/N, m_z, M_par, eta, wall density, O_x, O_y, O_z (asynchronous)."""
+        self._check(self.lib.dsmc_ensemble_add(self._h))
+
+    def ensemble_get(self):
+        """-> (mean, var, se, n): [R][8] each; eq. 13 and eq. 18 (PAPER.md:177, :265)"""
+        mean, var, se = (np.empty((self.R, 8), dtype=np.float64) for _ in range(3))
+        n = ctypes.c_uint64(0)
+        self._check(self.lib.dsmc_ensemble_get(self._h, mean.ctypes.data, var.ctypes.data, se.ctypes.data,
+                                               ctypes.byref(n)))
+        return mean, var, se, int(n.value)
 
     def set_timing(self, on=True):
         self._check(self.lib.dsmc_set_timing(self._h, int(on)))

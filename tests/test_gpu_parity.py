@@ -481,3 +481,39 @@ def test_field_parity_L256_every_target(dsmc_mod, oracle):
         print("kind", kind, "rel L2", rel, "max abs", mx)
         assert rel <= FIELD_REL_L2 and mx <= FIELD_MAX_ABS, (kind, rel, mx)
     ctx.close()
+
+
+@pytest.mark.parametrize("fft", [False, True])
+def test_ensemble_statistics_parity(dsmc_mod, oracle, fft):
+    """eq. 13 / eq. 18 accumulated on the device over a run (config 2's shape, 24 recorded states two
+    sweeps apart) against the oracle: per-snapshot observables and wall order parameters recomputed by
+    the oracle from the recorded states, then its ensemble mean, variance and standard error."""
+    from paper_1211_6234_b200 import inputs
+    c = inputs.CONFIGS[2]
+    L, R, g = c["L"], c["R"], c["g"]
+    K2, K4 = inputs.anisotropy(2)
+    T = inputs.temperatures(2)
+    ctx = make_ctx(dsmc_mod, 2, inputs)
+    if fft:
+        ctx.select_field_kernel(dsmc_mod.DSMC_FIELD_FFT)
+    W = oracle.build_tensor_ewald(L)
+    ctx.set_spins(inputs.initial_spins(2))
+    ctx.ensemble_reset()
+    snaps = []
+    for k in range(24):
+        ctx.run(T, 77, 4 * k, 4)
+        ctx.ensemble_add()
+        s = ctx.get_spins().astype(np.float64)
+        ob = oracle.observables(W, s, 1.0, g, K2.astype(np.float64), K4.astype(np.float64))
+        snaps.append(np.concatenate([ob, oracle.wall_order(L, oracle.wall_counts(s))], axis=1))
+    mean, var, se, n = ctx.ensemble_get()
+    m_ref, v_ref, se_ref = oracle.ensemble(np.array(snaps))
+    assert n == 24
+    assert np.max(np.abs(mean - m_ref)) <= 2e-6                       # the per-snapshot observable tolerance
+    assert np.all(np.abs(var - v_ref) <= 1e-5 * np.sqrt(v_ref) + 1e-10)
+    assert np.all(np.abs(se - se_ref) <= 1e-5 + 1e-3 * se_ref)
+    assert var[:, 0].max() > 1e-6                                     # the run is not frozen
+    ctx.ensemble_reset()
+    with pytest.raises(dsmc_mod.DsmcError):
+        ctx.ensemble_get()
+    ctx.close()
