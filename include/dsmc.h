@@ -148,7 +148,10 @@ int dsmc_sublattice_run(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t f
                         int flags);
 
 /* n_half consecutive half-sweeps (steps first_step .. first_step + n_half - 1) without returning
- * to the caller in between.                                                                    */
+ * to the caller in between.  For n_half >= 8 the bulk is replayed from a CUDA graph of one sweep
+ * (field + Metropolis of colour 0, of colour 1) whose kernels read the step from a counter in the
+ * workspace: one launch per sweep instead of one per kernel; the trajectory is bit-identical to
+ * calling dsmc_halfsweep step by step.                                                         */
 int dsmc_run(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_step, uint64_t n_half);
 
 /* a3. Observables of the current state, out[R][4] doubles in HOST memory:

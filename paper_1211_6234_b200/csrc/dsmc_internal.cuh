@@ -35,6 +35,7 @@ struct DsmcLayout {
     size_t off_obs;    // R*8 doubles (raw observable sums)
     size_t off_walls;  // R*8 64-bit wall counts
     size_t off_stats;  // R*8*2 doubles: ensemble sums of x and x^2
+    size_t off_step;   // one 64-bit step counter (dsmc_run's graph replay)
     size_t total;
 };
 
@@ -56,6 +57,12 @@ struct dsmc_ctx {
     bool ev_recorded = false;
     uint64_t launches = 0;
     uint64_t ensemble_n = 0;  // snapshots accumulated since dsmc_ensemble_reset
+    // one sweep (2 x [field + Metropolis] + step advance) captured as a CUDA graph for dsmc_run
+    cudaStream_t capture_stream = nullptr;
+    cudaGraphExec_t sweep_graph = nullptr;
+    uint64_t graph_seed = 0;
+    int graph_kind = -1, graph_flags = -1;
+    uint64_t graph_launches = 0;
     int sm_count = 148;
     std::string err;
 
@@ -73,6 +80,7 @@ struct dsmc_ctx {
     double *obs() const { return (double *)(ws + lay.off_obs); }
     unsigned long long *walls() const { return (unsigned long long *)(ws + lay.off_walls); }
     double *stats() const { return (double *)(ws + lay.off_stats); }
+    unsigned long long *step_dev() const { return (unsigned long long *)(ws + lay.off_step); }
     size_t Nh() const { return (size_t)L * (L / 2); }
     size_t plane() const { return Nh() * (size_t)R; }  // floats in one [a][r] plane
 };
@@ -117,6 +125,10 @@ struct MetropolisArgs {
     int flip;      // 0: trial uniform on S^2; 1: trial = -s (Ising move of App. B)
     float J, g, w0xx, w0yy, w0zz, w0xy;
     uint32_t seed_lo, seed_hi, step_lo, step_hi;
+    // when non-null the step is *step_dev + step_off instead of (step_lo, step_hi): lets a captured CUDA
+    // graph of one sweep be replayed with a step counter that lives on the device (dsmc_run)
+    const unsigned long long *step_dev;
+    uint32_t step_off;
     uint8_t *accept_out;  // canonical [R][L][L] or null
     float *margin_out;    // canonical [R][L][L] or null
 };
@@ -126,6 +138,9 @@ void dsmc_sublattice_offset(uint64_t seed, uint64_t pass, int l, int *ox, int *o
 // scratch: 3 N R floats for the per-slab partial fields (the staging buffer)
 cudaError_t launch_sublattice_pass(const MetropolisArgs &a, const float *Wc, float *scratch, int sm_count, int l, int ox,
                                    int oy, cudaStream_t st, uint64_t *launches);
+// *step = value (add = 0) or *step += value (add = 1): one thread, stream-ordered
+cudaError_t launch_step_update(unsigned long long *step, unsigned long long value, int add, cudaStream_t st,
+                               uint64_t *launches);
 cudaError_t launch_init_spins(float *S, int L, int R, int mode, uint64_t seed, cudaStream_t st,
                               uint64_t *launches);
 cudaError_t launch_observables(const float *S, const float *H, const float *K2, const float *K4,

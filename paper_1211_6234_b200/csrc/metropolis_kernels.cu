@@ -69,6 +69,17 @@ __device__ __forceinline__ void sphere_point(uint32_t x0, uint32_t x1, float &sx
     sz = z;
 }
 
+// the step words of the Philox counter: kernel parameters, or the device-resident counter of dsmc_run
+__device__ __forceinline__ void step_words(const MetropolisArgs &p, uint32_t &lo, uint32_t &hi) {
+    lo = p.step_lo;
+    hi = p.step_hi;
+    if (p.step_dev) {
+        const unsigned long long st = *p.step_dev + p.step_off;
+        lo = (uint32_t)(st & 0xFFFFFFFFull);
+        hi = (uint32_t)(st >> 32) & 0x7FFFFFFFu;
+    }
+}
+
 struct Trial {
     float tx, ty, tz, margin;
     bool acc;
@@ -78,7 +89,9 @@ struct Trial {
 __device__ __forceinline__ Trial decide(const MetropolisArgs &p, const RoundKeys &rk, uint32_t n, uint32_t r, float sx,
                                         float sy, float sz, float nx, float ny, float nz, float hx, float hy, float hz,
                                         float invT, float K2, float K4) {
-    const uint4 rnd = philox4x32_10(make_uint4(n, r, p.step_lo, p.step_hi), rk);
+    uint32_t step_lo, step_hi;
+    step_words(p, step_lo, step_hi);
+    const uint4 rnd = philox4x32_10(make_uint4(n, r, step_lo, step_hi), rk);
     Trial t;
     if (p.flip) {                                             // Ising move of App. B: complete reversal
         t.tx = -sx, t.ty = -sy, t.tz = -sz;
@@ -234,9 +247,11 @@ __global__ void __launch_bounds__(128, 7) metropolis4_kernel(const MetropolisArg
 
     const uint32_t n = (uint32_t)(y * p.L + 2 * i + par);
     const uint32_t r0 = 4u * (uint32_t)rq;
+    uint32_t step_lo, step_hi;
+    step_words(p, step_lo, step_hi);
     uint4 rnd[4];
 #pragma unroll
-    for (int k = 0; k < 4; ++k) rnd[k] = philox4x32_10(make_uint4(n, r0 + k, p.step_lo, p.step_hi), rk);
+    for (int k = 0; k < 4; ++k) rnd[k] = philox4x32_10(make_uint4(n, r0 + k, step_lo, step_hi), rk);
 
     bool any = false;
     float mg[4];
@@ -451,6 +466,10 @@ __global__ void __launch_bounds__(256) init_spins_kernel(float *__restrict__ S, 
     dst[2 * plane] = sz;
 }
 
+__global__ void step_update_kernel(unsigned long long *step, unsigned long long value, int add) {
+    *step = add ? *step + value : value;
+}
+
 RoundKeys make_round_keys(uint32_t lo, uint32_t hi) {
     RoundKeys rk;
     for (int i = 0; i < 10; ++i) {
@@ -521,5 +540,12 @@ cudaError_t launch_sublattice_pass(const MetropolisArgs &a, const float *Wc, flo
     const size_t total = (size_t)n * a.R;
     sublattice_flip_kernel<<<(unsigned)((total + 127) / 128), 128, 0, st>>>(a, rk, scratch, KS, l, ox, oy);
     *launches += 2;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_step_update(unsigned long long *step, unsigned long long value, int add, cudaStream_t st,
+                               uint64_t *launches) {
+    step_update_kernel<<<1, 1, 0, st>>>(step, value, add);
+    ++*launches;
     return cudaGetLastError();
 }

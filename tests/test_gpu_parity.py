@@ -517,3 +517,33 @@ def test_ensemble_statistics_parity(dsmc_mod, oracle, fft):
     with pytest.raises(dsmc_mod.DsmcError):
         ctx.ensemble_get()
     ctx.close()
+
+
+@pytest.mark.parametrize("L,R,kind", [(32, 8, 1), (32, 8, 2), (12, 5, 0), (64, 16, 2)])
+def test_run_graph_replay_is_bit_identical(dsmc_mod, L, R, kind):
+    """dsmc_run replays a captured CUDA graph of one sweep with the step counter on the device: the
+    trajectory must be bit-identical to calling dsmc_halfsweep step by step (odd first step, ragged
+    tail, a second run with another seed and after switching the field kernel)."""
+    from paper_1211_6234_b200 import inputs
+    T = np.linspace(0.3, 1.5, R).astype(np.float32)
+    a = dsmc_mod.Dsmc(L, R, J=1.0, g=0.2, K2=0.5, K4=0.1)
+    b = dsmc_mod.Dsmc(L, R, J=1.0, g=0.2, K2=0.5, K4=0.1)
+    a.build_tensor(dsmc_mod.DSMC_W_EWALD)
+    b.set_tensor(a.get_tensor())
+    for ctx in (a, b):
+        ctx.select_field_kernel(kind)
+        ctx.set_spins(inputs.random_spins(L, R, 3))
+    for (seed, first, n) in ((11, 7, 25), (12, 100, 16), (12, 116, 9)):
+        a.run(T, seed, first, n)
+        for k in range(n):
+            b.halfsweep(T, seed, first + k)
+        assert np.array_equal(a.get_spins(), b.get_spins()), (seed, first, n)
+    if kind == 2:                                               # the graph is rebuilt when the kernel changes
+        for ctx in (a, b):
+            ctx.select_field_kernel(dsmc_mod.DSMC_FIELD_AUTO)
+        a.run(T, 12, 200, 12)
+        for k in range(12):
+            b.halfsweep(T, 12, 200 + k)
+        assert np.array_equal(a.get_spins(), b.get_spins())
+    a.close()
+    b.close()
