@@ -196,7 +196,9 @@ __device__ __forceinline__ void ld2(const float4 *ptr, f2 &lo, f2 &hi) {
 // R % 4 == 0: one thread = one active site x 4 consecutive replicas (two packed pairs); grid.y =
 // lattice row.  All 18 128-bit loads are issued first; the four Philox chains and the trial spins
 // do not depend on them and run while they are in flight.  HOOKS = parity outputs requested.
-template <bool HOOKS>
+// FLIP: 0 = uniform-sphere trial, 1 = Ising reversal (App. B), 2 = decided at run time from p.flip (parity-hook
+// variant only: a run-time branch here splits the block the scheduler interleaves the two pairs in, +5 %)
+template <bool HOOKS, bool DEVSTEP, int FLIP>
 __global__ void __launch_bounds__(128, 7) metropolis4_kernel(const MetropolisArgs p, const RoundKeys rk) {
     const int Lh = p.L >> 1, RQ = p.R >> 2;
     const int y = blockIdx.y;
@@ -247,8 +249,8 @@ __global__ void __launch_bounds__(128, 7) metropolis4_kernel(const MetropolisArg
 
     const uint32_t n = (uint32_t)(y * p.L + 2 * i + par);
     const uint32_t r0 = 4u * (uint32_t)rq;
-    uint32_t step_lo, step_hi;
-    step_words(p, step_lo, step_hi);
+    uint32_t step_lo = p.step_lo, step_hi = p.step_hi;
+    if (DEVSTEP) step_words(p, step_lo, step_hi);
     uint4 rnd[4];
 #pragma unroll
     for (int k = 0; k < 4; ++k) rnd[k] = philox4x32_10(make_uint4(n, r0 + k, step_lo, step_hi), rk);
@@ -258,7 +260,7 @@ __global__ void __launch_bounds__(128, 7) metropolis4_kernel(const MetropolisArg
 #pragma unroll
     for (int j = 0; j < 2; ++j) {
         Trial2 tr = trial2(rnd[2 * j], rnd[2 * j + 1]);
-        if (p.flip) {                                         // Ising move of App. B: complete reversal
+        if (FLIP == 1 || (FLIP == 2 && p.flip)) {             // Ising move of App. B: complete reversal
             tr.tx = f2_mul(s[0][j], f2_bc(-1.0f));
             tr.ty = f2_mul(s[1][j], f2_bc(-1.0f));
             tr.tz = f2_mul(s[2][j], f2_bc(-1.0f));
@@ -494,8 +496,11 @@ cudaError_t launch_metropolis(const MetropolisArgs &a, cudaStream_t st, uint64_t
         }
         const unsigned per_row = (unsigned)((a.L / 2) * RQ);
         dim3 grid((per_row + 127) / 128, a.L);
-        if (a.accept_out || a.margin_out) metropolis4_kernel<true><<<grid, 128, 0, st>>>(b, rk);
-        else metropolis4_kernel<false><<<grid, 128, 0, st>>>(b, rk);
+        if (a.accept_out || a.margin_out) metropolis4_kernel<true, false, 2><<<grid, 128, 0, st>>>(b, rk);
+        else if (a.step_dev && a.flip) metropolis4_kernel<false, true, 1><<<grid, 128, 0, st>>>(b, rk);
+        else if (a.step_dev) metropolis4_kernel<false, true, 0><<<grid, 128, 0, st>>>(b, rk);
+        else if (a.flip) metropolis4_kernel<false, false, 1><<<grid, 128, 0, st>>>(b, rk);
+        else metropolis4_kernel<false, false, 0><<<grid, 128, 0, st>>>(b, rk);
         err = cudaGetLastError();
     } else {
         const size_t total = (size_t)a.L * (a.L / 2) * a.R;
