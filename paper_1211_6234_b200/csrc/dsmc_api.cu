@@ -424,8 +424,14 @@ int dsmc_sublattice_pass(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t 
         offset_out[0] = ox;
         offset_out[1] = oy;
     }
+    // With the FFT field selected, the whole field costs less than the direct sum over the n update sites
+    // once L is large: compute it (for even l all update sites have the colour of the offset) and let the
+    // flip kernel read it.
+    const bool fft = field_kind(ctx) == 2;
+    if (fft)
+        if (int rc = run_field(ctx, (l & 1) ? -1 : ((ox + oy) & 1))) return rc;
     const MetropolisArgs a = metropolis_args(ctx, 0, seed, pass, flags, accept_out, margin_out);
-    CU(launch_sublattice_pass(a, ctx->Wc(), ctx->stage(), ctx->sm_count, l, ox, oy, ctx->stream, &ctx->launches),
+    CU(launch_sublattice_pass(a, ctx->Wc(), ctx->stage(), ctx->sm_count, l, ox, oy, fft, ctx->stream, &ctx->launches),
        "sub-lattice pass launch");
     ctx->field_valid[0] = ctx->field_valid[1] = false;
     return DSMC_OK;

@@ -136,8 +136,9 @@ cudaError_t launch_metropolis(const MetropolisArgs &a, cudaStream_t st, uint64_t
 // the paper's stride-l sub-lattice pass: offset (ox, oy) in [0, l)^2, n = (L/l)^2 update sites
 void dsmc_sublattice_offset(uint64_t seed, uint64_t pass, int l, int *ox, int *oy);
 // scratch: 3 N R floats for the per-slab partial fields (the staging buffer)
+// field_in_H: h of the update sites is already in the field array H (FFT route); else it is summed here
 cudaError_t launch_sublattice_pass(const MetropolisArgs &a, const float *Wc, float *scratch, int sm_count, int l, int ox,
-                                   int oy, cudaStream_t st, uint64_t *launches);
+                                   int oy, bool field_in_H, cudaStream_t st, uint64_t *launches);
 // *step = value (add = 0) or *step += value (add = 1): one thread, stream-ordered
 cudaError_t launch_step_update(unsigned long long *step, unsigned long long value, int add, cudaStream_t st,
                                uint64_t *launches);

@@ -420,6 +420,11 @@ __global__ void __launch_bounds__(128) sublattice_flip_kernel(const MetropolisAr
     const size_t at = site_index(xt, yt, Lh, R, plane, q) + r;
     float *own = p.S + at;
     float hx = 0.0f, hy = 0.0f, hz = 0.0f;                     // slab partials in fixed order
+    if (KS == 0) {                                             // the field array holds h (FFT route)
+        hx = p.H[at];
+        hy = p.H[at + plane];
+        hz = p.H[at + 2 * plane];
+    }
     for (int ks = 0; ks < KS; ++ks) {
         const float *ph = part + (((size_t)ks * nl * nl + k) * 3) * R + r;
         hx += ph[0];
@@ -531,20 +536,24 @@ void dsmc_sublattice_offset(uint64_t seed, uint64_t pass, int l, int *ox, int *o
 }
 
 cudaError_t launch_sublattice_pass(const MetropolisArgs &a, const float *Wc, float *scratch, int sm_count, int l, int ox,
-                                   int oy, cudaStream_t st, uint64_t *launches) {
+                                   int oy, bool field_in_H, cudaStream_t st, uint64_t *launches) {
     const RoundKeys rk = make_round_keys(a.seed_lo, a.seed_hi);
     const int nl = a.L / l, n = nl * nl, chunks = (a.R + 31) / 32;
-    // source slabs: enough CTAs to fill the GPU about four times over, at least 8 rows per slab (one per
-    // warp), and KS * n <= N so that the partials fit the 3 N R floats of the staging buffer
-    int KS = (4 * sm_count + n * chunks - 1) / (n * chunks);
-    KS = std::max(1, std::min(KS, std::min(a.L / 8, l * l)));
-    const int rows = (a.L + KS - 1) / KS;
-    KS = (a.L + rows - 1) / rows;
-    sublattice_field_kernel<<<dim3((unsigned)n, (unsigned)chunks, (unsigned)KS), 256, 0, st>>>(a.S, scratch, Wc, a.L, a.R,
-                                                                                               l, ox, oy, rows);
+    int KS = 0;
+    if (!field_in_H) {
+        // source slabs: enough CTAs to fill the GPU about four times over, at least 8 rows per slab (one per
+        // warp), and KS * n <= N so that the partials fit the 3 N R floats of the staging buffer
+        KS = (4 * sm_count + n * chunks - 1) / (n * chunks);
+        KS = std::max(1, std::min(KS, std::min(a.L / 8, l * l)));
+        const int rows = (a.L + KS - 1) / KS;
+        KS = (a.L + rows - 1) / rows;
+        sublattice_field_kernel<<<dim3((unsigned)n, (unsigned)chunks, (unsigned)KS), 256, 0, st>>>(a.S, scratch, Wc, a.L,
+                                                                                                   a.R, l, ox, oy, rows);
+        ++*launches;
+    }
     const size_t total = (size_t)n * a.R;
     sublattice_flip_kernel<<<(unsigned)((total + 127) / 128), 128, 0, st>>>(a, rk, scratch, KS, l, ox, oy);
-    *launches += 2;
+    ++*launches;
     return cudaGetLastError();
 }
 

@@ -60,15 +60,18 @@ def lockstep_passes(m, oracle, ctx, W, T, J, g, K2, K4, seed, l, n_passes, flip=
     return accepted, trials
 
 
-@pytest.mark.parametrize("L,R,l,passes", [(8, 1, 4, 40), (12, 5, 3, 24), (32, 8, 8, 24), (64, 16, 32, 48),
-                                          (64, 40, 2, 6), (16, 3, 16, 12)])
-def test_sublattice_lockstep(dsmc_mod, oracle, L, R, l, passes):
+@pytest.mark.parametrize("L,R,l,passes,fft", [(8, 1, 4, 40, False), (12, 5, 3, 24, False), (32, 8, 8, 24, False),
+                                              (64, 16, 32, 48, False), (64, 40, 2, 6, False), (16, 3, 16, 12, False),
+                                              (64, 16, 32, 48, True), (32, 8, 8, 24, True), (32, 6, 2, 8, True)])
+def test_sublattice_lockstep(dsmc_mod, oracle, L, R, l, passes, fft):
     """(64, 16, 32) is the paper's own choice L = 64, l = 32; l = 2 is the densest
     schedule (n = N/4), l = L the conventional single-spin limit; R = 40 spans two replica chunks."""
     from paper_1211_6234_b200 import inputs
     J, g, K2, K4 = 1.0, 0.25, 0.6, 0.1
     ctx = dsmc_mod.Dsmc(L, R, J=J, g=g, K2=K2, K4=K4)
     ctx.build_tensor(dsmc_mod.DSMC_W_EWALD)
+    if fft:                                                     # the field of the pass through the FFT route
+        ctx.select_field_kernel(dsmc_mod.DSMC_FIELD_FFT)
     W = oracle.build_tensor_ewald(L)
     ctx.set_spins(inputs.random_spins(L, R, 31))
     T = np.linspace(0.2, 1.6, R).astype(np.float32)
