@@ -143,13 +143,15 @@ int dsmc_halfsweep_ex(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t ste
  * the update sites only.  offset_out: nullable HOST int[2] = {S_1, S_2}.                          */
 int dsmc_sublattice_pass(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t pass, int l, int flags,
                          uint8_t *accept_out, float *margin_out, int *offset_out);
-/* n_passes consecutive passes first_pass .. first_pass + n_passes - 1 (two kernel launches each).   */
+/* n_passes consecutive passes first_pass .. first_pass + n_passes - 1; long runs are replayed from a
+ * captured CUDA graph whose kernels recompute the offset from a pass counter on the device
+ * (bit-identical to calling dsmc_sublattice_pass pass by pass).                                    */
 int dsmc_sublattice_run(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_pass, uint64_t n_passes, int l,
                         int flags);
 
 /* n_half consecutive half-sweeps (steps first_step .. first_step + n_half - 1) without returning
- * to the caller in between.  For n_half >= 8 the bulk is replayed from a CUDA graph of one sweep
- * (field + Metropolis of colour 0, of colour 1) whose kernels read the step from a counter in the
+ * to the caller in between.  Long runs are replayed from a CUDA graph of 8 sweeps (each: field +
+ * Metropolis of colour 0, of colour 1) whose kernels read the step from a counter in the
  * workspace: one launch per sweep instead of one per kernel; the trajectory is bit-identical to
  * calling dsmc_halfsweep step by step.                                                         */
 int dsmc_run(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_step, uint64_t n_half);

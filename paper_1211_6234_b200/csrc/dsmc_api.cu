@@ -148,9 +148,77 @@ MetropolisArgs metropolis_args(dsmc_ctx *ctx, int colour, uint64_t seed, uint64_
 void drop_sweep_graph(dsmc_ctx *ctx) {
     if (ctx->sweep_graph) cudaGraphExecDestroy(ctx->sweep_graph);
     ctx->sweep_graph = nullptr;
+    if (ctx->pass_graph) cudaGraphExecDestroy(ctx->pass_graph);
+    ctx->pass_graph = nullptr;
 }
 
-// Capture one sweep -- field + Metropolis of colour 0, of colour 1, step counter += 2 -- as a CUDA graph
+// enqueue one stride-l pass; pass_dev != null: offset and step come from the device counter (graph capture)
+int enqueue_pass(dsmc_ctx *ctx, uint64_t seed, uint64_t pass, int l, int flags, uint8_t *accept_out, float *margin_out,
+                 int *offset_out, const unsigned long long *pass_dev) {
+    int ox = 0, oy = 0;
+    if (!pass_dev) dsmc_sublattice_offset(seed, pass, l, &ox, &oy);
+    if (offset_out) {
+        offset_out[0] = ox;
+        offset_out[1] = oy;
+    }
+    // With the FFT field selected, the whole field costs less than the direct sum over the n update sites
+    // once L is large: compute it (for even l all update sites have the colour of the offset, which is
+    // only known here when the offset is) and let the flip kernel read it.
+    const bool fft = field_kind(ctx) == 2;
+    if (fft)
+        if (int rc = run_field(ctx, ((l & 1) || pass_dev) ? -1 : ((ox + oy) & 1))) return rc;
+    MetropolisArgs a = metropolis_args(ctx, 0, seed, pass, flags, accept_out, margin_out);
+    a.step_dev = pass_dev;
+    CU(launch_sublattice_pass(a, ctx->Wc(), ctx->stage(), ctx->sm_count, l, ox, oy, fft, ctx->stream, &ctx->launches),
+       "sub-lattice pass launch");
+    ctx->field_valid[0] = ctx->field_valid[1] = false;
+    return DSMC_OK;
+}
+
+int build_pass_graph(dsmc_ctx *ctx, uint64_t seed, int l, int flags) {
+    const int kind = field_kind(ctx);
+    if (ctx->pass_graph && ctx->pgraph_seed == seed && ctx->pgraph_kind == kind && ctx->pgraph_flags == flags &&
+        ctx->pgraph_l == l)
+        return DSMC_OK;
+    if (ctx->pass_graph) cudaGraphExecDestroy(ctx->pass_graph);
+    ctx->pass_graph = nullptr;
+    if (!ctx->capture_stream)
+        CU(cudaStreamCreateWithFlags(&ctx->capture_stream, cudaStreamNonBlocking), "capture stream");
+    cudaStream_t saved = ctx->stream;
+    const uint64_t l0 = ctx->launches;
+    ctx->stream = ctx->capture_stream;
+    cudaGraph_t graph = nullptr;
+    cudaError_t e = cudaStreamBeginCapture(ctx->capture_stream, cudaStreamCaptureModeThreadLocal);
+    int rc = DSMC_OK;
+    if (e == cudaSuccess) {
+        for (int rep = 0; rep < DSMC_GRAPH_UNROLL && rc == DSMC_OK && e == cudaSuccess; ++rep) {
+            rc = enqueue_pass(ctx, seed, 0, l, flags, nullptr, nullptr, nullptr, ctx->step_dev());
+            if (rc == DSMC_OK) e = launch_step_update(ctx->step_dev(), 1, 1, ctx->stream, &ctx->launches);
+        }
+        cudaError_t e2 = cudaStreamEndCapture(ctx->capture_stream, &graph);
+        if (e == cudaSuccess) e = e2;
+    }
+    ctx->stream = saved;
+    ctx->pgraph_launches = ctx->launches - l0;
+    ctx->launches = l0;
+    if (rc != DSMC_OK || e != cudaSuccess) {
+        if (graph) cudaGraphDestroy(graph);
+        return rc != DSMC_OK ? rc : cuda_fail(ctx, e, "pass graph capture");
+    }
+    e = cudaGraphInstantiate(&ctx->pass_graph, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e != cudaSuccess) {
+        ctx->pass_graph = nullptr;
+        return cuda_fail(ctx, e, "pass graph instantiate");
+    }
+    ctx->pgraph_seed = seed;
+    ctx->pgraph_kind = kind;
+    ctx->pgraph_flags = flags;
+    ctx->pgraph_l = l;
+    return DSMC_OK;
+}
+
+// Capture DSMC_GRAPH_UNROLL sweeps -- each field + Metropolis of colour 0, of colour 1, step counter += 2 -- as a CUDA graph
 // whose Metropolis kernels read the step from the device-resident counter, so that dsmc_run replays
 // it with one launch per sweep instead of one per kernel (small lattices are launch-bound).
 int build_sweep_graph(dsmc_ctx *ctx, uint64_t seed, int flags) {
@@ -166,16 +234,19 @@ int build_sweep_graph(dsmc_ctx *ctx, uint64_t seed, int flags) {
     cudaError_t e = cudaStreamBeginCapture(ctx->capture_stream, cudaStreamCaptureModeThreadLocal);
     int rc = DSMC_OK;
     if (e == cudaSuccess) {
-        for (int colour = 0; colour < 2 && rc == DSMC_OK; ++colour) {
-            rc = run_field(ctx, colour);
-            if (rc != DSMC_OK) break;
-            MetropolisArgs a = metropolis_args(ctx, colour, seed, 0, flags, nullptr, nullptr);
-            a.step_dev = ctx->step_dev();
-            a.step_off = (uint32_t)colour;
-            e = launch_metropolis(a, ctx->stream, &ctx->launches);
-            if (e != cudaSuccess) break;
+        for (int rep = 0; rep < DSMC_GRAPH_UNROLL && rc == DSMC_OK && e == cudaSuccess; ++rep) {
+            for (int colour = 0; colour < 2 && rc == DSMC_OK; ++colour) {
+                rc = run_field(ctx, colour);
+                if (rc != DSMC_OK) break;
+                MetropolisArgs a = metropolis_args(ctx, colour, seed, 0, flags, nullptr, nullptr);
+                a.step_dev = ctx->step_dev();
+                a.step_off = (uint32_t)colour;
+                e = launch_metropolis(a, ctx->stream, &ctx->launches);
+                if (e != cudaSuccess) break;
+            }
+            if (e == cudaSuccess && rc == DSMC_OK)
+                e = launch_step_update(ctx->step_dev(), 2, 1, ctx->stream, &ctx->launches);
         }
-        if (e == cudaSuccess && rc == DSMC_OK) e = launch_step_update(ctx->step_dev(), 2, 1, ctx->stream, &ctx->launches);
         cudaError_t e2 = cudaStreamEndCapture(ctx->capture_stream, &graph);
         if (e == cudaSuccess) e = e2;
     }
@@ -418,32 +489,31 @@ int dsmc_sublattice_pass(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t 
     if (flags & ~DSMC_TRIAL_FLIP) return fail(ctx, DSMC_EINVAL, "unknown flag");
     if (l < 2 || ctx->L % l) return fail(ctx, DSMC_EINVAL, "l must be >= 2 and divide L");
     if (int rc = upload_params(ctx, T)) return rc;
-    int ox, oy;
-    dsmc_sublattice_offset(seed, pass, l, &ox, &oy);
-    if (offset_out) {
-        offset_out[0] = ox;
-        offset_out[1] = oy;
-    }
-    // With the FFT field selected, the whole field costs less than the direct sum over the n update sites
-    // once L is large: compute it (for even l all update sites have the colour of the offset) and let the
-    // flip kernel read it.
-    const bool fft = field_kind(ctx) == 2;
-    if (fft)
-        if (int rc = run_field(ctx, (l & 1) ? -1 : ((ox + oy) & 1))) return rc;
-    const MetropolisArgs a = metropolis_args(ctx, 0, seed, pass, flags, accept_out, margin_out);
-    CU(launch_sublattice_pass(a, ctx->Wc(), ctx->stage(), ctx->sm_count, l, ox, oy, fft, ctx->stream, &ctx->launches),
-       "sub-lattice pass launch");
-    ctx->field_valid[0] = ctx->field_valid[1] = false;
-    return DSMC_OK;
+    return enqueue_pass(ctx, seed, pass, l, flags, accept_out, margin_out, offset_out, nullptr);
 }
 
 int dsmc_sublattice_run(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_pass, uint64_t n_passes, int l,
                         int flags) {
-    for (uint64_t k = 0; k < n_passes; ++k)
-        if (int rc = dsmc_sublattice_pass(ctx, k == 0 ? T : nullptr, seed, first_pass + k, l, flags, nullptr, nullptr,
-                                          nullptr))
-            return rc;
-    return DSMC_OK;
+    uint64_t k = 0;
+    auto plain = [&](uint64_t count) -> int {
+        for (uint64_t j = 0; j < count; ++j, ++k)
+            if (int rc = dsmc_sublattice_pass(ctx, k == 0 ? T : nullptr, seed, first_pass + k, l, flags, nullptr, nullptr,
+                                              nullptr))
+                return rc;
+        return DSMC_OK;
+    };
+    if (n_passes >= 1 + 2 * DSMC_GRAPH_UNROLL) {
+        // the first pass runs launch by launch (argument checks, kernel configuration), the rest is replayed
+        // from a captured graph of DSMC_GRAPH_UNROLL passes whose kernels derive offset and step from a device counter
+        if (int rc = plain(1)) return rc;
+        if (int rc = build_pass_graph(ctx, seed, l, flags)) return rc;
+        CU(launch_step_update(ctx->step_dev(), first_pass + k, 0, ctx->stream, &ctx->launches), "pass counter");
+        const uint64_t reps = (n_passes - k) / DSMC_GRAPH_UNROLL;
+        for (uint64_t j = 0; j < reps; ++j) CU(cudaGraphLaunch(ctx->pass_graph, ctx->stream), "pass graph launch");
+        ctx->launches += reps * ctx->pgraph_launches;
+        k += reps * DSMC_GRAPH_UNROLL;
+    }
+    return plain(n_passes - k);
 }
 
 int dsmc_run(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_step, uint64_t n_half) {
@@ -454,18 +524,18 @@ int dsmc_run(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_step, 
             if (int rc = dsmc_halfsweep_ex(ctx, k == 0 ? T : nullptr, seed, first_step + k, 0, nullptr, nullptr)) return rc;
         return DSMC_OK;
     };
-    if (n_half >= 8 && !ctx->timing) {
+    if (n_half >= 4 + 4 * DSMC_GRAPH_UNROLL && !ctx->timing) {
         // an odd first step and one whole sweep run launch by launch (this also configures every kernel
         // before the capture); the bulk is replayed from the captured graph; the tail runs plainly again
         if (int rc = plain((first_step & 1u) + 2)) return rc;
-        const uint64_t n_sweeps = (n_half - k) / 2;
-        if (n_sweeps >= 2) {
+        const uint64_t reps = (n_half - k) / (2 * DSMC_GRAPH_UNROLL);
+        if (reps >= 1) {
             if (int rc = build_sweep_graph(ctx, seed, 0)) return rc;
             CU(launch_step_update(ctx->step_dev(), first_step + k, 0, ctx->stream, &ctx->launches), "step counter");
-            for (uint64_t j = 0; j < n_sweeps; ++j) CU(cudaGraphLaunch(ctx->sweep_graph, ctx->stream), "sweep graph launch");
-            ctx->launches += n_sweeps * ctx->graph_launches;
+            for (uint64_t j = 0; j < reps; ++j) CU(cudaGraphLaunch(ctx->sweep_graph, ctx->stream), "sweep graph launch");
+            ctx->launches += reps * ctx->graph_launches;
             ctx->field_valid[0] = ctx->field_valid[1] = true;
-            k += 2 * n_sweeps;
+            k += 2 * DSMC_GRAPH_UNROLL * reps;
         }
     }
     return plain(n_half - k);

@@ -20,6 +20,7 @@
 // structure of checkerboard targets into a unit-stride sliding window over W (section 5).
 // ---------------------------------------------------------------------------------------------
 
+#define DSMC_GRAPH_UNROLL 8  // sweeps (dsmc_run) or passes (dsmc_sublattice_run) per captured CUDA graph
 #define DSMC_KS_MAX 16  // maximum source split (partial-field slabs) of the tiled field kernel
 
 struct DsmcLayout {
@@ -63,6 +64,11 @@ struct dsmc_ctx {
     uint64_t graph_seed = 0;
     int graph_kind = -1, graph_flags = -1;
     uint64_t graph_launches = 0;
+    // one stride-l pass (field + flip + pass counter += 1) for dsmc_sublattice_run
+    cudaGraphExec_t pass_graph = nullptr;
+    uint64_t pgraph_seed = 0;
+    int pgraph_kind = -1, pgraph_flags = -1, pgraph_l = -1;
+    uint64_t pgraph_launches = 0;
     int sm_count = 148;
     std::string err;
 

@@ -349,9 +349,23 @@ __device__ __forceinline__ size_t site_index(int x, int y, int Lh, int R, size_t
 }
 
 // grid (n sites, replica chunks of 32, KS source slabs); part[ks][site][c][r] receives the slab's sum
+// offset of pass `pass` (R21): words x0, x1 of Philox4x32-10(seed; 0xFFFFFFFF, 0xFFFFFFFF, pass) mod l
+__host__ __device__ __forceinline__ void pass_offset(const RoundKeys &rk, unsigned long long pass, int l, int &ox,
+                                                     int &oy) {
+    const uint4 x = philox4x32_10(make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, (uint32_t)(pass & 0xFFFFFFFFull),
+                                             (uint32_t)(pass >> 32) & 0x7FFFFFFFu), rk);
+    ox = (int)(x.x % (uint32_t)l);
+    oy = (int)(x.y % (uint32_t)l);
+}
+
+// pass_dev (nullable): the pass counter on the device; the offset is then recomputed here, so that a
+// captured graph of one pass can be replayed (dsmc_sublattice_run)
 __global__ void __launch_bounds__(256) sublattice_field_kernel(const float *__restrict__ S, float *__restrict__ part_out,
                                                                const float *__restrict__ Wc, int L, int R, int l,
-                                                               int ox, int oy, int rows_per_slab) {
+                                                               int ox, int oy, int rows_per_slab, int segs,
+                                                               const unsigned long long *__restrict__ pass_dev,
+                                                               const RoundKeys rk) {
+    if (pass_dev) pass_offset(rk, *pass_dev, l, ox, oy);
     __shared__ float part[8][3][32];
     const int Lh = L >> 1;
     const size_t N = (size_t)L * L, plane = (size_t)L * Lh * R;
@@ -361,8 +375,10 @@ __global__ void __launch_bounds__(256) sublattice_field_kernel(const float *__re
     const int r = blockIdx.y * 32 + lane;
     const int rr = r < R ? r : R - 1;                          // idle lanes load a valid replica
     const int y0 = blockIdx.z * rows_per_slab, y1 = min(L, y0 + rows_per_slab);
+    const int iseg = Lh / segs;                                // in-row indices per work item
     float hx = 0.0f, hy = 0.0f, hz = 0.0f;
-    for (int ys = y0 + grp; ys < y1; ys += 8) {
+    for (int item = grp; item < (y1 - y0) * segs; item += 8) { // a warp takes (source row, row segment) items
+        const int ys = y0 + item / segs, i0 = (item % segs) * iseg;
         int ry = ys - yt;
         ry += ry < 0 ? L : 0;
         const float *Wrow = Wc + (size_t)ry * L;
@@ -370,10 +386,10 @@ __global__ void __launch_bounds__(256) sublattice_field_kernel(const float *__re
         float ax = 0.0f, ay = 0.0f, az = 0.0f;
 #pragma unroll
         for (int q = 0; q < 2; ++q) {
-            const float *row = S + (size_t)q * 3 * plane + (size_t)ys * Lh * R + rr;
-            const int x0 = (ys + q) & 1;
+            const float *row = S + (size_t)q * 3 * plane + ((size_t)ys * Lh + i0) * R + rr;
+            const int x0 = 2 * i0 + ((ys + q) & 1);
 #pragma unroll 4
-            for (int i = 0; i < Lh; ++i) {
+            for (int i = 0; i < iseg; ++i) {
                 int rx = 2 * i + x0 - xt;
                 rx += rx < 0 ? L : 0;
                 const float sx = row[(size_t)i * R], sy = row[plane + (size_t)i * R], sz = row[2 * plane + (size_t)i * R];
@@ -384,7 +400,7 @@ __global__ void __launch_bounds__(256) sublattice_field_kernel(const float *__re
                 az = fmaf(wzz, sz, az);
             }
         }
-        hx += ax;                                              // row sums first: two-level fp32 accumulation
+        hx += ax;                                              // item sums first: two-level fp32 accumulation
         hy += ay;
         hz += az;
     }
@@ -409,6 +425,7 @@ __global__ void __launch_bounds__(256) sublattice_field_kernel(const float *__re
 __global__ void __launch_bounds__(128) sublattice_flip_kernel(const MetropolisArgs p, const RoundKeys rk,
                                                               const float *__restrict__ part, int KS, int l, int ox,
                                                               int oy) {
+    if (p.step_dev) pass_offset(rk, *p.step_dev + p.step_off, l, ox, oy);
     const int L = p.L, Lh = L >> 1, R = p.R;
     const size_t N = (size_t)L * L, plane = (size_t)L * Lh * R;
     const int nl = L / l;
@@ -425,11 +442,12 @@ __global__ void __launch_bounds__(128) sublattice_flip_kernel(const MetropolisAr
         hy = p.H[at + plane];
         hz = p.H[at + 2 * plane];
     }
-    for (int ks = 0; ks < KS; ++ks) {
+#pragma unroll 8
+    for (int ks = 0; ks < KS; ++ks) {                          // unrolled: the loads of 8 slabs are in flight together
         const float *ph = part + (((size_t)ks * nl * nl + k) * 3) * R + r;
-        hx += ph[0];
-        hy += ph[R];
-        hz += ph[2 * R];
+        hx += __ldg(ph);
+        hy += __ldg(ph + R);
+        hz += __ldg(ph + 2 * R);
     }
     const int xe = xt + 1 == L ? 0 : xt + 1, xw = xt == 0 ? L - 1 : xt - 1;
     const int yn = yt + 1 == L ? 0 : yt + 1, ys = yt == 0 ? L - 1 : yt - 1;
@@ -527,12 +545,8 @@ cudaError_t launch_init_spins(float *S, int L, int R, int mode, uint64_t seed, c
 }
 
 void dsmc_sublattice_offset(uint64_t seed, uint64_t pass, int l, int *ox, int *oy) {
-    // DESIGN.md R21: words x0, x1 of Philox4x32-10(seed; 0xFFFFFFFF, 0xFFFFFFFF, pass) mod l
     const RoundKeys rk = make_round_keys((uint32_t)(seed & 0xFFFFFFFFu), (uint32_t)(seed >> 32));
-    const uint4 x = philox4x32_10(make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, (uint32_t)(pass & 0xFFFFFFFFu),
-                                             (uint32_t)(pass >> 32) & 0x7FFFFFFFu), rk);
-    *ox = (int)(x.x % (uint32_t)l);
-    *oy = (int)(x.y % (uint32_t)l);
+    pass_offset(rk, pass, l, *ox, *oy);
 }
 
 cudaError_t launch_sublattice_pass(const MetropolisArgs &a, const float *Wc, float *scratch, int sm_count, int l, int ox,
@@ -541,14 +555,16 @@ cudaError_t launch_sublattice_pass(const MetropolisArgs &a, const float *Wc, flo
     const int nl = a.L / l, n = nl * nl, chunks = (a.R + 31) / 32;
     int KS = 0;
     if (!field_in_H) {
-        // source slabs: enough CTAs to fill the GPU about four times over, at least 8 rows per slab (one per
-        // warp), and KS * n <= N so that the partials fit the 3 N R floats of the staging buffer
-        KS = (4 * sm_count + n * chunks - 1) / (n * chunks);
-        KS = std::max(1, std::min(KS, std::min(a.L / 8, l * l)));
-        const int rows = (a.L + KS - 1) / KS;
+        // A CTA's 8 warps share (source row, row segment) items; a row is cut in 4 segments when L allows.
+        // Source slabs: enough CTAs to fill the GPU about four times over, at least 8 items per slab, and
+        // KS * n <= N so that the partials fit the 3 N R floats of the staging buffer.
+        const int segs = (a.L % 8 == 0 && a.L >= 32) ? 4 : 1;
+        const int ks_target = std::max(1, (4 * sm_count + n * chunks - 1) / (n * chunks));
+        int rows = std::max(8 / segs, (a.L + ks_target - 1) / ks_target);
+        rows = std::max(rows, (n + a.L - 1) / a.L);
         KS = (a.L + rows - 1) / rows;
-        sublattice_field_kernel<<<dim3((unsigned)n, (unsigned)chunks, (unsigned)KS), 256, 0, st>>>(a.S, scratch, Wc, a.L,
-                                                                                                   a.R, l, ox, oy, rows);
+        sublattice_field_kernel<<<dim3((unsigned)n, (unsigned)chunks, (unsigned)KS), 256, 0, st>>>(
+            a.S, scratch, Wc, a.L, a.R, l, ox, oy, rows, segs, a.step_dev, rk);
         ++*launches;
     }
     const size_t total = (size_t)n * a.R;

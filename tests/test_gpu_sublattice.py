@@ -207,3 +207,28 @@ def test_simultaneous_flipping_error_is_small(dsmc_mod, oracle):
     print("m_st seq.  ", np.round(seq, 3))
     assert gpu[0] > 0.75 and seq[0] > 0.75 and gpu[-1] < 0.3 and seq[-1] < 0.3      # ordered -> disordered
     assert np.max(np.abs(gpu - seq)) < 0.1, np.abs(gpu - seq)                       # measured: 0.03
+
+
+@pytest.mark.parametrize("L,R,l,fft,flip", [(64, 16, 32, False, False), (64, 16, 32, True, True), (12, 5, 3, False, True),
+                                            (32, 8, 2, True, False)])
+def test_sublattice_run_graph_replay_is_bit_identical(dsmc_mod, L, R, l, fft, flip):
+    """dsmc_sublattice_run replays a captured graph of one pass whose kernels recompute the offset from a
+    pass counter on the device: same trajectory, bit for bit, as pass-by-pass calls."""
+    from paper_1211_6234_b200 import inputs
+    T = np.linspace(0.3, 1.5, R).astype(np.float32)
+    flags = dsmc_mod.DSMC_TRIAL_FLIP if flip else 0
+    a = dsmc_mod.Dsmc(L, R, J=1.0, g=0.3, K2=0.5, K4=0.1)
+    b = dsmc_mod.Dsmc(L, R, J=1.0, g=0.3, K2=0.5, K4=0.1)
+    a.build_tensor(dsmc_mod.DSMC_W_EWALD)
+    b.set_tensor(a.get_tensor())
+    for ctx in (a, b):
+        if fft:
+            ctx.select_field_kernel(dsmc_mod.DSMC_FIELD_FFT)
+        ctx.set_spins(inputs.random_spins(L, R, 3))
+    for (seed, first, n) in ((5, 0, 40), (5, 40, 9), (6, 1000, 17)):
+        a.sublattice_run(T, seed, first, n, l, flags=flags)
+        for k in range(n):
+            b.sublattice_pass(T, seed, first + k, l, flags=flags)
+        assert np.array_equal(a.get_spins(), b.get_spins()), (seed, first, n)
+    a.close()
+    b.close()
