@@ -74,6 +74,13 @@ int dsmc_create(dsmc_ctx **out, int L, int R, float J, float g, float K2, float 
  * values in one R = 16 batch (eq. 12 with K2 = -K(1-a), K4 = -Ka, R7).            */
 int dsmc_set_anisotropy(dsmc_ctx *ctx, const float *K2_r, const float *K4_r);
 
+/* Sharding one ladder of replicas over several contexts (one per GPU): this
+ * context's replica r is replica first_replica + r of the whole ladder in every Philox counter
+ * (trial moves, acceptance, dsmc_init_spins): a sharded run draws the random numbers of the unsharded
+ * one, and reproduces it bit for bit when the shards run the same kernels as the whole (FFT field,
+ * whose arithmetic per replica pair does not depend on R, and R % 4 == 0 on every shard).  Default 0. */
+int dsmc_set_replica_offset(dsmc_ctx *ctx, uint32_t first_replica);
+
 /* Bytes of device workspace a context of this shape needs (0 if the shape is invalid).        */
 size_t dsmc_workspace_bytes(int L, int R);
 

@@ -128,6 +128,7 @@ MetropolisArgs metropolis_args(dsmc_ctx *ctx, int colour, uint64_t seed, uint64_
     a.colour = colour;
     a.rq_shift = -1;
     a.flip = (flags & DSMC_TRIAL_FLIP) ? 1 : 0;
+    a.r_off = ctx->replica_offset;
     a.J = ctx->J;
     a.g = ctx->g;
     a.w0xx = ctx->w0[0];
@@ -328,6 +329,13 @@ int dsmc_set_anisotropy(dsmc_ctx *ctx, const float *K2_r, const float *K4_r) {
     return DSMC_OK;
 }
 
+int dsmc_set_replica_offset(dsmc_ctx *ctx, uint32_t first_replica) {
+    if (!ctx) return DSMC_EINVAL;
+    ctx->replica_offset = first_replica;
+    drop_sweep_graph(ctx);  // the offset is baked into the captured kernel parameters
+    return DSMC_OK;
+}
+
 size_t dsmc_workspace_bytes(int L, int R) {
     if (!shape_ok(L, R)) return 0;
     return dsmc_make_layout(L, R).total;
@@ -422,7 +430,7 @@ int dsmc_get_spins(dsmc_ctx *ctx, float *s, int where) {
 int dsmc_init_spins(dsmc_ctx *ctx, int mode, uint64_t seed) {
     if (int rc = need_bound(ctx)) return rc;
     if (mode != DSMC_INIT_RANDOM && mode != DSMC_INIT_UP) return fail(ctx, DSMC_EINVAL, "unknown init mode");
-    CU(launch_init_spins(ctx->S(), ctx->L, ctx->R, mode, seed, ctx->stream, &ctx->launches), "init spins");
+    CU(launch_init_spins(ctx->S(), ctx->L, ctx->R, mode, seed, ctx->replica_offset, ctx->stream, &ctx->launches), "init spins");
     ctx->spins_set = true;
     ctx->field_valid[0] = ctx->field_valid[1] = false;
     return DSMC_OK;

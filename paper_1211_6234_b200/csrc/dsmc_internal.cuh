@@ -52,6 +52,7 @@ struct dsmc_ctx {
     bool tensor_built = false, spins_set = false;
     bool field_valid[2] = {false, false};
     float w0[4] = {0, 0, 0, 0};  // W(0) components (fp32, as stored)
+    uint32_t replica_offset = 0;  // dsmc_set_replica_offset
     int field_kind = -1;  // -1 automatic, 0 generic, 1 tiled, 2 FFT (dsmc_select_field_kernel)
     int timing = 0;
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
@@ -129,6 +130,7 @@ struct MetropolisArgs {
     int L, R, colour;
     int rq_shift;  // log2(R/4) when R/4 is a power of two, else -1 (set by the launcher)
     int flip;      // 0: trial uniform on S^2; 1: trial = -s (Ising move of App. B)
+    uint32_t r_off;  // index of this context's replica 0 in the whole ladder (Philox counter word 1)
     float J, g, w0xx, w0yy, w0zz, w0xy;
     uint32_t seed_lo, seed_hi, step_lo, step_hi;
     // when non-null the step is *step_dev + step_off instead of (step_lo, step_hi): lets a captured CUDA
@@ -148,7 +150,7 @@ cudaError_t launch_sublattice_pass(const MetropolisArgs &a, const float *Wc, flo
 // *step = value (add = 0) or *step += value (add = 1): one thread, stream-ordered
 cudaError_t launch_step_update(unsigned long long *step, unsigned long long value, int add, cudaStream_t st,
                                uint64_t *launches);
-cudaError_t launch_init_spins(float *S, int L, int R, int mode, uint64_t seed, cudaStream_t st,
+cudaError_t launch_init_spins(float *S, int L, int R, int mode, uint64_t seed, uint32_t r_off, cudaStream_t st,
                               uint64_t *launches);
 cudaError_t launch_observables(const float *S, const float *H, const float *K2, const float *K4,
                                double *obs, int L, int R, float J, float g, cudaStream_t st,

@@ -253,7 +253,7 @@ __global__ void __launch_bounds__(128, 7) metropolis4_kernel(const MetropolisArg
     if (DEVSTEP) step_words(p, step_lo, step_hi);
     uint4 rnd[4];
 #pragma unroll
-    for (int k = 0; k < 4; ++k) rnd[k] = philox4x32_10(make_uint4(n, r0 + k, step_lo, step_hi), rk);
+    for (int k = 0; k < 4; ++k) rnd[k] = philox4x32_10(make_uint4(n, r0 + p.r_off + k, step_lo, step_hi), rk);
 
     bool any = false;
     float mg[4];
@@ -320,7 +320,7 @@ __global__ void __launch_bounds__(256) metropolis1_kernel(const MetropolisArgs p
     const float ny = (oth[plane + ae] + oth[plane + aw]) + (oth[plane + an] + oth[plane + as]);
     const float nz = (oth[2 * plane + ae] + oth[2 * plane + aw]) + (oth[2 * plane + an] + oth[2 * plane + as]);
     const uint32_t n = (uint32_t)(y * p.L + 2 * i + par);
-    const Trial tr = decide(p, rk, n, (uint32_t)r, sx, sy, sz, nx, ny, nz, hf[0], hf[plane], hf[2 * plane], p.invT[r],
+    const Trial tr = decide(p, rk, n, (uint32_t)r + p.r_off, sx, sy, sz, nx, ny, nz, hf[0], hf[plane], hf[2 * plane], p.invT[r],
                             p.K2[r], p.K4[r]);
     if (tr.acc) {
         own[0] = tr.tx;
@@ -458,7 +458,7 @@ __global__ void __launch_bounds__(128) sublattice_flip_kernel(const MetropolisAr
     const float ny = (ne[plane] + nw[plane]) + (nn[plane] + ns[plane]);
     const float nz = (ne[2 * plane] + nw[2 * plane]) + (nn[2 * plane] + ns[2 * plane]);
     const uint32_t n = (uint32_t)(yt * L + xt);
-    const Trial tr = decide(p, rk, n, (uint32_t)r, sx, sy, sz, nx, ny, nz, hx, hy, hz, p.invT[r], p.K2[r], p.K4[r]);
+    const Trial tr = decide(p, rk, n, (uint32_t)r + p.r_off, sx, sy, sz, nx, ny, nz, hx, hy, hz, p.invT[r], p.K2[r], p.K4[r]);
     if (tr.acc) {
         own[0] = tr.tx;
         own[plane] = tr.ty;
@@ -468,7 +468,8 @@ __global__ void __launch_bounds__(128) sublattice_flip_kernel(const MetropolisAr
     if (p.margin_out) p.margin_out[(size_t)r * N + n] = tr.margin;
 }
 
-__global__ void __launch_bounds__(256) init_spins_kernel(float *__restrict__ S, int L, int R, int mode, const RoundKeys rk) {
+__global__ void __launch_bounds__(256) init_spins_kernel(float *__restrict__ S, int L, int R, int mode, uint32_t r_off,
+                                                         const RoundKeys rk) {
     const int Lh = L >> 1;
     const size_t Nh = (size_t)L * Lh;
     const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -481,7 +482,7 @@ __global__ void __launch_bounds__(256) init_spins_kernel(float *__restrict__ S, 
     const int x = 2 * i + ((y + q) & 1);
     float sx = 0.0f, sy = 0.0f, sz = 1.0f;
     if (mode == DSMC_INIT_RANDOM) {
-        const uint4 rnd = philox4x32_10(make_uint4((uint32_t)(y * L + x), (uint32_t)r, 0u, 0x80000000u), rk);
+        const uint4 rnd = philox4x32_10(make_uint4((uint32_t)(y * L + x), (uint32_t)r + r_off, 0u, 0x80000000u), rk);
         sphere_point(rnd.x, rnd.y, sx, sy, sz);
     }
     const size_t plane = Nh * (size_t)R;
@@ -534,11 +535,11 @@ cudaError_t launch_metropolis(const MetropolisArgs &a, cudaStream_t st, uint64_t
     return err;
 }
 
-cudaError_t launch_init_spins(float *S, int L, int R, int mode, uint64_t seed, cudaStream_t st,
+cudaError_t launch_init_spins(float *S, int L, int R, int mode, uint64_t seed, uint32_t r_off, cudaStream_t st,
                               uint64_t *launches) {
     const size_t total = (size_t)L * L * R;
     const unsigned grid = (unsigned)((total + 255) / 256);
-    init_spins_kernel<<<grid, 256, 0, st>>>(S, L, R, mode,
+    init_spins_kernel<<<grid, 256, 0, st>>>(S, L, R, mode, r_off,
                                              make_round_keys((uint32_t)(seed & 0xFFFFFFFFu), (uint32_t)(seed >> 32)));
     ++*launches;
     return cudaGetLastError();

@@ -23,6 +23,7 @@ _lib = None
 _vp, _i, _f, _u64, _sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_float, ctypes.c_uint64, ctypes.c_size_t
 ABI = [
     ("dsmc_create", _i, [ctypes.POINTER(_vp), _i, _i, _f, _f, _f, _f]),
+    ("dsmc_set_replica_offset", _i, [_vp, ctypes.c_uint32]),
     ("dsmc_set_anisotropy", _i, [_vp, _vp, _vp]),
     ("dsmc_workspace_bytes", _sz, [_i, _i]),
     ("dsmc_bind", _i, [_vp, _vp, _sz, _vp]),
@@ -270,6 +271,10 @@ class Dsmc:
         out = ctypes.c_double(0.0)
         self._check(self.lib.dsmc_fp32_fma_peak(self._h, ctypes.addressof(out)))
         return float(out.value)
+
+    def set_replica_offset(self, first_replica):
+        """This context holds replicas first_replica ... of a larger ladder (bit-reproducible sharding)."""
+        self._check(self.lib.dsmc_set_replica_offset(self._h, int(first_replica)))
 
     def fft_supported(self):
         return bool(self.lib.dsmc_field_kernel_supported(self._h, DSMC_FIELD_FFT))

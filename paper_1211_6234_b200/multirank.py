@@ -40,3 +40,24 @@ def whole_job_rate(units_per_rank_step, world, seconds_per_step):
     """Aggregate throughput of `world` ranks that each process units_per_rank_step per step (weak
     scaling) in seconds_per_step (the max over ranks)."""
     return world * units_per_rank_step / seconds_per_step
+
+
+def gather_replica_rows(local, R, device="cpu"):
+    """Concatenate per-rank blocks of per-replica rows (the blocks of replica_shard) on every rank:
+    local is a float64 array [R_local, ...]; returns [R, ...].  The one collective of a sharded run:
+    R x 8 numbers at the end, never inside the sweep loop."""
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    local = np.ascontiguousarray(local, dtype=np.float64)
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return local
+    world, rank = dist.get_world_size(), dist.get_rank()
+    tail = local.shape[1:]
+    width = int(np.prod(tail)) if tail else 1
+    out = torch.zeros((R, width), dtype=torch.float64, device=device)
+    lo, hi = replica_shard(R, world, rank)
+    assert hi - lo == local.shape[0], (lo, hi, local.shape)
+    out[lo:hi] = torch.from_numpy(local.reshape(hi - lo, width)).to(device)
+    dist.all_reduce(out, op=dist.ReduceOp.SUM)              # disjoint blocks: the sum is the concatenation
+    return out.cpu().numpy().reshape((R,) + tail)

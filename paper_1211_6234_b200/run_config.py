@@ -2,6 +2,10 @@
 
   python -m paper_1211_6234_b200.run_config 3 --field fft
   python -m paper_1211_6234_b200.run_config 2 --sweeps 2000 --record-every 1 --equilibrate 0
+  python -m torch.distributed.run --nproc-per-node 8 --master-addr 127.0.0.1 -m paper_1211_6234_b200.run_config 5
+
+Under torchrun the temperature ladder is split over the ranks (one GPU each, contiguous blocks of
+replicas, no exchange inside the run: the chains are independent); rank 0 gathers the R x 8 results.
 
 Everything runs in libdsmc.so (dsmc_run for the sweeps, dsmc_ensemble_add for the recorded states: no
 host round trip inside the loop); this script only marshals arguments and formats the result.
@@ -29,15 +33,25 @@ def main():
     args = ap.parse_args()
 
     import torch
-    from . import Dsmc, DSMC_W_EWALD, DSMC_W_IMAGE, DSMC_FIELD_FFT, DSMC_FIELD_AUTO, DSMC_INIT_UP, inputs
+    import torch.distributed as dist
+    from . import Dsmc, DSMC_W_EWALD, DSMC_W_IMAGE, DSMC_FIELD_FFT, DSMC_FIELD_AUTO, DSMC_INIT_UP, inputs, multirank
     if not torch.cuda.is_available():
         raise SystemExit("run_config: no CUDA device (there is no CPU fallback)")
+    rank, world, local = multirank.env()
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     c = inputs.CONFIGS[args.config]
-    L, R = c["L"], c["R"]
-    K2, K4 = inputs.anisotropy(args.config)
-    T = inputs.temperatures(args.config)
+    L, R_all = c["L"], c["R"]
+    lo, hi = multirank.replica_shard(R_all, world, rank)       # this rank's block of the ladder
+    if hi == lo:
+        raise SystemExit(f"run_config: {world} ranks for {R_all} replicas leaves rank {rank} without work")
+    R = hi - lo
+    K2, K4 = (a[lo:hi] for a in inputs.anisotropy(args.config))
+    T = inputs.temperatures(args.config)[lo:hi]
     seed = inputs.SEED_BASE + args.config
-    ctx = Dsmc(L, R, J=1.0, g=c["g"], K2=K2, K4=K4)
+    ctx = Dsmc(L, R, J=1.0, g=c["g"], K2=K2, K4=K4, device=torch.device("cuda", local))
+    ctx.set_replica_offset(lo)                                 # same random streams as the unsharded ladder
     if args.config == 1:
         ctx.build_tensor(DSMC_W_IMAGE, 64, 1)               # BASELINE config 1: image cutoff |a|,|b| <= 64
     else:
@@ -47,7 +61,7 @@ def main():
     if c["init"] == "up":
         ctx.init_spins(DSMC_INIT_UP)
     else:
-        ctx.set_spins(inputs.initial_spins(args.config))
+        ctx.set_spins(inputs.initial_spins(args.config)[lo:hi])
     sweeps = args.sweeps if args.sweeps is not None else c["sweeps"]
     burn = args.equilibrate if args.equilibrate is not None else sweeps // 2
     every = max(1, args.record_every)
@@ -64,14 +78,25 @@ def main():
         ctx.ensemble_add()
     mean, var, se, n = ctx.ensemble_get()                   # synchronises
     wall = time.perf_counter() - t0
+    kind = ["generic", "tiled", "fft"][ctx.field_kernel_kind()]
+    ctx.close()
+    if world > 1:
+        dev = torch.device("cuda", local)
+        wall = multirank.max_over_ranks([wall], device=dev)[0]
+        mean, var, se = (multirank.gather_replica_rows(a, R_all, device=dev) for a in (mean, var, se))
+        T = multirank.gather_replica_rows(T.astype(np.float64), R_all, device=dev)
+        K4 = multirank.gather_replica_rows(K4.astype(np.float64), R_all, device=dev)
+        dist.destroy_process_group()
+        if rank != 0:
+            return
+    R = R_all
     result = {
-        "config": args.config, "L": L, "R": R, "field_kernel": ["generic", "tiled", "fft"][ctx.field_kernel_kind()],
+        "config": args.config, "L": L, "R": R, "n_gpus": world, "field_kernel": kind,
         "sweeps": sweeps, "equilibrate": burn, "recorded": n, "seconds": wall,
         "sweeps_per_s": sweeps / wall, "updates_per_s": sweeps * L * L * R / wall,
         "T": [float(t) for t in T], "K4": [float(k) for k in K4], "quantities": NAMES,
         "mean": mean.tolist(), "standard_error": se.tolist(), "variance": var.tolist(),
     }
-    ctx.close()
     if args.json:
         print(json.dumps(result))
         return

@@ -547,3 +547,33 @@ def test_run_graph_replay_is_bit_identical(dsmc_mod, L, R, kind):
         assert np.array_equal(a.get_spins(), b.get_spins())
     a.close()
     b.close()
+
+
+def test_sharded_ladder_is_bit_identical(dsmc_mod):
+    """One ladder of 8 replicas run as a whole and as two shards of 4 with dsmc_set_replica_offset (what
+    run_config does under torchrun, one shard per GPU): the random streams are those of the whole ladder, and
+    with the FFT field (whose arithmetic per replica pair does not depend on R) and shards that use the same
+    Metropolis kernel (R % 4 == 0) the trajectories are identical bit for bit -- through dsmc_init_spins and
+    through dsmc_run (graph replay)."""
+    L, R = 32, 8
+    T = np.linspace(0.3, 1.7, R).astype(np.float32)
+    K2 = np.linspace(0.4, 0.8, R).astype(np.float32)
+    K4 = np.linspace(-0.1, 0.1, R).astype(np.float32)
+    whole = dsmc_mod.Dsmc(L, R, J=1.0, g=0.2, K2=K2, K4=K4)
+    whole.build_tensor(dsmc_mod.DSMC_W_EWALD)
+    whole.select_field_kernel(dsmc_mod.DSMC_FIELD_FFT)
+    whole.init_spins(dsmc_mod.DSMC_INIT_RANDOM, seed=9)
+    s0 = whole.get_spins()
+    whole.run(T, 21, 0, 40)
+    ref = whole.get_spins()
+    for (lo, hi) in ((0, 4), (4, 8)):
+        part = dsmc_mod.Dsmc(L, hi - lo, J=1.0, g=0.2, K2=K2[lo:hi], K4=K4[lo:hi])
+        part.set_tensor(whole.get_tensor())
+        part.select_field_kernel(dsmc_mod.DSMC_FIELD_FFT)
+        part.set_replica_offset(lo)
+        part.init_spins(dsmc_mod.DSMC_INIT_RANDOM, seed=9)
+        assert np.array_equal(part.get_spins(), s0[lo:hi])
+        part.run(T[lo:hi], 21, 0, 40)
+        assert np.array_equal(part.get_spins(), ref[lo:hi]), (lo, hi)
+        part.close()
+    whole.close()

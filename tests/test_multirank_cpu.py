@@ -27,6 +27,12 @@ def _worker(rank, world, port, out):
     # every rank times its own work; the job's time is the slowest rank's
     mine = [10.0 + 5.0 * rank, 3.0 - rank]
     got = multirank.max_over_ranks(mine)
+    # a ladder of 5 replicas split over the ranks: every rank ends with all rows, in replica order
+    import numpy as np
+    lo, hi = multirank.replica_shard(5, world, rank)
+    rows = np.arange(lo, hi, dtype=np.float64)[:, None] * np.ones((1, 8)) + 0.25
+    allrows = multirank.gather_replica_rows(rows, 5)
+    assert allrows.shape == (5, 8) and np.array_equal(allrows[:, 0], np.arange(5) + 0.25)
     dist.barrier()
     out.put((rank, got, multirank.rank_seed(0x12116234, rank)))
     dist.destroy_process_group()
