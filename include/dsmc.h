@@ -57,8 +57,10 @@ enum { DSMC_W_IMAGE = 0, DSMC_W_EWALD = 1 };
 enum {
     DSMC_REUSE_FIELD = 1, /* skip the field step: reuse h kept from the previous field call of
                              the same colour (for timing the Metropolis kernel alone)         */
-    DSMC_TRIAL_FLIP = 2   /* the trial is the reversed spin s' = -s instead of a point uniform on
+    DSMC_TRIAL_FLIP = 2,  /* the trial is the reversed spin s' = -s instead of a point uniform on
                              S^2: the Ising move of App. B; u is drawn as usual   */
+    DSMC_NO_RESIDENT = 4  /* dsmc_sublattice_pass / _run only: do not use the kernel that keeps the
+                             lattice in shared memory (two launches per pass instead)            */
 };
 
 /* dsmc_init_spins modes */
@@ -146,13 +148,16 @@ int dsmc_halfsweep_ex(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t ste
  * field of ALL of them taken from the state at entry to the pass (section 3.2), exchange, anisotropy
  * and the self-term exact as in dsmc_halfsweep.  l >= 2 and l | L (DSMC_EINVAL otherwise); l = L is
  * conventional single-spin Metropolis.  One MC step (N attempted updates) = l*l passes.
- * flags: DSMC_TRIAL_FLIP.  accept_out / margin_out: nullable DEVICE buffers [R][L][L], written at
- * the update sites only.  offset_out: nullable HOST int[2] = {S_1, S_2}.                          */
+ * flags: DSMC_TRIAL_FLIP, DSMC_NO_RESIDENT.  accept_out / margin_out: nullable DEVICE buffers
+ * [R][L][L], written at the update sites only.  offset_out: nullable HOST int[2] = {S_1, S_2}.                          */
 int dsmc_sublattice_pass(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t pass, int l, int flags,
                          uint8_t *accept_out, float *margin_out, int *offset_out);
-/* n_passes consecutive passes first_pass .. first_pass + n_passes - 1; long runs are replayed from a
- * captured CUDA graph whose kernels recompute the offset from a pass counter on the device
- * (bit-identical to calling dsmc_sublattice_pass pass by pass).                                    */
+/* n_passes consecutive passes first_pass .. first_pass + n_passes - 1, bit-identical to calling
+ * dsmc_sublattice_pass pass by pass with the same flags.  When L/l is 1 or 2 and 40 L^2 bytes fit one
+ * CTA's shared memory (L <= 74; the paper's L = 64, l = 32) and the FFT field is not selected, one CTA
+ * per replica pair keeps spins and W in shared memory and runs all passes inside one kernel; otherwise
+ * (or with DSMC_NO_RESIDENT) long runs are replayed from a captured CUDA graph whose kernels recompute
+ * the offset from a pass counter on the device.                                                    */
 int dsmc_sublattice_run(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_pass, uint64_t n_passes, int l,
                         int flags);
 

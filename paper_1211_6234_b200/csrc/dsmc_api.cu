@@ -153,6 +153,11 @@ void drop_sweep_graph(dsmc_ctx *ctx) {
     ctx->pass_graph = nullptr;
 }
 
+// the shared-memory-resident kernel serves the pass unless the FFT field was selected or the caller opts out
+bool use_resident(dsmc_ctx *ctx, int l, int flags) {
+    return field_kind(ctx) != 2 && !(flags & DSMC_NO_RESIDENT) && dsmc_resident_supported(ctx->L, l);
+}
+
 // enqueue one stride-l pass; pass_dev != null: offset and step come from the device counter (graph capture)
 int enqueue_pass(dsmc_ctx *ctx, uint64_t seed, uint64_t pass, int l, int flags, uint8_t *accept_out, float *margin_out,
                  int *offset_out, const unsigned long long *pass_dev) {
@@ -166,6 +171,12 @@ int enqueue_pass(dsmc_ctx *ctx, uint64_t seed, uint64_t pass, int l, int flags, 
     // once L is large: compute it (for even l all update sites have the colour of the offset, which is
     // only known here when the offset is) and let the flip kernel read it.
     const bool fft = field_kind(ctx) == 2;
+    if (use_resident(ctx, l, flags) && !pass_dev) {
+        const MetropolisArgs a = metropolis_args(ctx, 0, seed, pass, flags, accept_out, margin_out);
+        CU(launch_sublattice_resident(a, ctx->Wc(), l, pass, 1, ctx->stream, &ctx->launches), "resident pass launch");
+        ctx->field_valid[0] = ctx->field_valid[1] = false;
+        return DSMC_OK;
+    }
     if (fft)
         if (int rc = run_field(ctx, ((l & 1) || pass_dev) ? -1 : ((ox + oy) & 1))) return rc;
     MetropolisArgs a = metropolis_args(ctx, 0, seed, pass, flags, accept_out, margin_out);
@@ -494,7 +505,7 @@ int dsmc_sublattice_pass(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t 
     if (int rc = need_bound(ctx)) return rc;
     if (!ctx->tensor_built) return fail(ctx, DSMC_ESTATE, "tensor not built");
     if (!ctx->spins_set) return fail(ctx, DSMC_ESTATE, "spins not set");
-    if (flags & ~DSMC_TRIAL_FLIP) return fail(ctx, DSMC_EINVAL, "unknown flag");
+    if (flags & ~(DSMC_TRIAL_FLIP | DSMC_NO_RESIDENT)) return fail(ctx, DSMC_EINVAL, "unknown flag");
     if (l < 2 || ctx->L % l) return fail(ctx, DSMC_EINVAL, "l must be >= 2 and divide L");
     if (int rc = upload_params(ctx, T)) return rc;
     return enqueue_pass(ctx, seed, pass, l, flags, accept_out, margin_out, offset_out, nullptr);
@@ -502,6 +513,17 @@ int dsmc_sublattice_pass(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t 
 
 int dsmc_sublattice_run(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_pass, uint64_t n_passes, int l,
                         int flags) {
+    if (int rc = need_bound(ctx)) return rc;
+    if (n_passes >= 2 && l >= 2 && ctx->L % l == 0 && !(flags & ~(DSMC_TRIAL_FLIP | DSMC_NO_RESIDENT)) &&
+        ctx->tensor_built && ctx->spins_set && use_resident(ctx, l, flags)) {
+        // every pass of the run inside one kernel (per 65536 passes), the lattice in shared memory
+        if (int rc = upload_params(ctx, T)) return rc;
+        const MetropolisArgs a = metropolis_args(ctx, 0, seed, first_pass, flags, nullptr, nullptr);
+        CU(launch_sublattice_resident(a, ctx->Wc(), l, first_pass, n_passes, ctx->stream, &ctx->launches),
+           "resident run launch");
+        ctx->field_valid[0] = ctx->field_valid[1] = false;
+        return DSMC_OK;
+    }
     uint64_t k = 0;
     auto plain = [&](uint64_t count) -> int {
         for (uint64_t j = 0; j < count; ++j, ++k)

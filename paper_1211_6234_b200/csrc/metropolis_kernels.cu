@@ -85,20 +85,28 @@ struct Trial {
     bool acc;
 };
 
-// one Metropolis decision: current spin s, neighbour sum nb, frozen field h  (R12-R14)
-__device__ __forceinline__ Trial decide(const MetropolisArgs &p, const RoundKeys &rk, uint32_t n, uint32_t r, float sx,
-                                        float sy, float sz, float nx, float ny, float nz, float hx, float hy, float hz,
-                                        float invT, float K2, float K4) {
-    uint32_t step_lo, step_hi;
-    step_words(p, step_lo, step_hi);
-    const uint4 rnd = philox4x32_10(make_uint4(n, r, step_lo, step_hi), rk);
-    Trial t;
+// the random part of one Metropolis trial: Philox words -> trial spin and ln u.  It depends on the
+// counter only (and on the current spin for the Ising move), not on the field.
+struct Draw {
+    float tx, ty, tz, lnu;
+};
+__device__ __forceinline__ Draw draw_from_words(const MetropolisArgs &p, uint4 rnd, float sx, float sy, float sz) {
+    Draw d;
     if (p.flip) {                                             // Ising move of App. B: complete reversal
-        t.tx = -sx, t.ty = -sy, t.tz = -sz;
+        d.tx = -sx, d.ty = -sy, d.tz = -sz;
     } else {
-        sphere_point(rnd.x, rnd.y, t.tx, t.ty, t.tz);
+        sphere_point(rnd.x, rnd.y, d.tx, d.ty, d.tz);
     }
-    const float u = unit24(rnd.z);
+    d.lnu = __logf(unit24(rnd.z));
+    return d;
+}
+
+// the deterministic part: current spin s, neighbour sum nb, frozen field h  (R12-R14)
+__device__ __forceinline__ Trial decide_drawn(const MetropolisArgs &p, const Draw &d, float sx, float sy, float sz,
+                                              float nx, float ny, float nz, float hx, float hy, float hz, float invT,
+                                              float K2, float K4) {
+    Trial t;
+    t.tx = d.tx, t.ty = d.ty, t.tz = d.tz;
     const float dx = t.tx - sx, dy = t.ty - sy, dz = t.tz - sz;
     const float dz2 = dz * (t.tz + sz);                       // s'_z^2 - s_z^2
     const float z2sum = fmaf(t.tz, t.tz, sz * sz);
@@ -107,9 +115,19 @@ __device__ __forceinline__ Trial decide(const MetropolisArgs &p, const RoundKeys
     float self = fmaf(p.w0xx * dx, dx, fmaf(p.w0yy * dy, dy, p.w0zz * dz * dz));
     self = fmaf(0.5f, self, p.w0xy * dx * dy);
     dE = fmaf(p.g, fmaf(dx, hx, fmaf(dy, hy, fmaf(dz, hz, self))), dE);
-    t.margin = fmaf(dE, invT, __logf(u));
+    t.margin = fmaf(dE, invT, d.lnu);
     t.acc = t.margin < 0.0f;
     return t;
+}
+
+// one Metropolis decision of site n, replica r
+__device__ __forceinline__ Trial decide(const MetropolisArgs &p, const RoundKeys &rk, uint32_t n, uint32_t r, float sx,
+                                        float sy, float sz, float nx, float ny, float nz, float hx, float hy, float hz,
+                                        float invT, float K2, float K4) {
+    uint32_t step_lo, step_hi;
+    step_words(p, step_lo, step_hi);
+    const uint4 rnd = philox4x32_10(make_uint4(n, r, step_lo, step_hi), rk);
+    return decide_drawn(p, draw_from_words(p, rnd, sx, sy, sz), sx, sy, sz, nx, ny, nz, hx, hy, hz, invT, K2, K4);
 }
 
 __device__ __forceinline__ float rsqrt_approx(float x) {
@@ -468,6 +486,213 @@ __global__ void __launch_bounds__(128) sublattice_flip_kernel(const MetropolisAr
     if (p.margin_out) p.margin_out[(size_t)r * N + n] = tr.margin;
 }
 
+// ---------------------------------------------------------------------------------------------
+// The same schedule with the lattice resident in shared memory (sublattice_resident_kernel).
+// One pass is tiny (n = 4 update sites at the paper's L = 64, l = 32: 4 x 4096 x 5 FMAs per replica) and
+// consecutive passes depend on one another, so a launch per pass leaves the run bound by launch
+// latency.  Here one CTA owns two replicas for the WHOLE run of passes: their spins (24 N bytes)
+// and W (16 N bytes) live in shared memory, a pass costs two __syncthreads and no global access, and
+// the R/2 CTAs run side by side on their own SMs.
+//   * 16 summing warps.  For L/l = NL the n = NL^2 update sites are the translates of the offset by
+//     multiples of l, so the sources are taken in cosets {c + (a l, b l)} of the same n translations: the
+//     n x n (source, target) pairs of a coset need only n distinct W entries, rho = c - offset + (u l, v l).
+//     Per coset (NL = 2): 4 LDS.128 of W + 12 LDS.64 of spins feed 80 FFMA2 (two replicas packed, the W
+//     value as broadcast operand) -- 1 byte of shared-memory traffic per FMA, which balances the FMA pipe.
+//   * per-thread sums of a few cosets first, then a fixed-order reduction (two-level fp32 accumulation,
+//     deterministic): a halving exchange over the warp (each step trades half of the values for the
+//     partner's partial sums of the other half: 18 packed shuffles instead of 60), then 16 warp partials.
+//   * one extra warp draws while the others sum: lanes < 2n run Philox for (site, replica, pass) and the
+//     trial spin, lane 31 runs the same Philox code on the offset counter of the NEXT pass (no divergence),
+//     so after the barrier only the 16-term sums, dE and the store of an accepted spin remain.
+// Needs L/l in {1, 2} and 40 N bytes + partials within the 227 KB of one CTA (L <= 74).
+constexpr int kResSumWarps = 16;
+constexpr int kResThreads = 32 * (kResSumWarps + 1);
+
+__host__ __device__ constexpr size_t resident_smem_bytes(int L, int NL) {
+    return (size_t)40 * L * L + sizeof(f2) * kResSumWarps * NL * NL * 3 + 64;
+}
+
+// Reduction helpers for values held as packed pairs.  halve_exchange: lanes with the mask bit clear keep
+// v[0 .. V/2) and receive the partner's partial sums of them, the others keep v[V/2 .. V) (moved to
+// v[0 .. V/2)); butterfly_sum: plain xor butterfly over masks first, first/2, ..., 1.
+template <int V>
+__device__ __forceinline__ void halve_exchange(f2 *v, int lane, int mask) {
+    const bool upper = lane & mask;
+#pragma unroll
+    for (int i = 0; i < V / 2; ++i) {
+        const f2 keep = upper ? v[i + V / 2] : v[i], send = upper ? v[i] : v[i + V / 2];
+        v[i] = f2_add(keep, __shfl_xor_sync(0xFFFFFFFFu, send, mask));
+    }
+}
+template <int V>
+__device__ __forceinline__ void butterfly_sum(f2 *v, int first) {
+#pragma unroll
+    for (int mask = first; mask >= 1; mask >>= 1)
+#pragma unroll
+        for (int i = 0; i < V; ++i) v[i] = f2_add(v[i], __shfl_xor_sync(0xFFFFFFFFu, v[i], mask));
+}
+
+template <int NL>
+__global__ void __launch_bounds__(kResThreads, 1) sublattice_resident_kernel(const MetropolisArgs p, const RoundKeys rk,
+                                                                             const float *__restrict__ Wc, int l,
+                                                                             unsigned long long first_pass,
+                                                                             unsigned n_passes) {
+    constexpr int NN = NL * NL;
+    extern __shared__ __align__(16) unsigned char rsm[];
+    const int L = p.L, Lh = L >> 1, R = p.R, N = L * L;
+    float4 *Wsm = reinterpret_cast<float4 *>(rsm);                     // [N]  (xx, xy, yy, zz) at rho = ry L + rx
+    f2 *Sx = reinterpret_cast<f2 *>(rsm + (size_t)16 * N);             // [N]  replicas (r0, r1) of site n = y L + x
+    f2 *Sy = Sx + N, *Sz = Sy + N;
+    f2 *part = Sz + N;                                                 // [warp][target][c]
+    int *off = reinterpret_cast<int *>(part + kResSumWarps * NN * 3);  // [2][2]: offsets of this and the next pass
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int r0 = 2 * blockIdx.x, r1 = min(r0 + 1, R - 1);            // odd R: the last CTA carries its replica twice
+    const size_t plane = (size_t)L * Lh * R;
+
+    for (int n = tid; n < N; n += kResThreads) {
+        Wsm[n] = make_float4(__ldg(Wc + n), __ldg(Wc + (size_t)N + n), __ldg(Wc + 2 * (size_t)N + n),
+                             __ldg(Wc + 3 * (size_t)N + n));
+        const int x = n % L, y = n / L;
+        int q;
+        const float *src = p.S + site_index(x, y, Lh, R, plane, q);
+        Sx[n] = f2_make(src[r0], src[r1]);
+        Sy[n] = f2_make(src[plane + r0], src[plane + r1]);
+        Sz[n] = f2_make(src[2 * plane + r0], src[2 * plane + r1]);
+    }
+    if (tid == 0) pass_offset(rk, first_pass, l, off[0], off[1]);
+    __syncthreads();
+
+    // the drawing warp's lanes: update site k = lane >> 1, replica half rb = lane & 1
+    const bool flipper = warp == kResSumWarps && lane < 2 * NN;
+    const int fk = lane >> 1, rb = lane & 1, fr = rb ? r1 : r0;
+    float invT = 0.0f, K2 = 0.0f, K4 = 0.0f;
+    if (flipper) invT = p.invT[fr], K2 = p.K2[fr], K4 = p.K4[fr];
+    MetropolisArgs q = p;
+    q.step_dev = nullptr;
+
+    for (unsigned it = 0; it < n_passes; ++it) {
+        const unsigned long long pass = first_pass + it;
+        const int cur = (int)(it & 1u);
+        const int ox = off[2 * cur], oy = off[2 * cur + 1];
+        Draw dr;
+        float sx = 0.0f, sy = 0.0f, sz = 0.0f, nx = 0.0f, ny = 0.0f, nz = 0.0f;
+        int nt = 0;
+        if (warp < kResSumWarps) {
+            f2 acc[NN][3];
+#pragma unroll
+            for (int k = 0; k < NN; ++k) acc[k][0] = acc[k][1] = acc[k][2] = f2_bc(0.0f);
+            for (int c = tid; c < l * l; c += 32 * kResSumWarps) {
+                const int cy = c / l, cx = c - cy * l;
+                int dx[NL], dy[NL];
+                dx[0] = cx - ox + (cx < ox ? L : 0);
+                dy[0] = cy - oy + (cy < oy ? L : 0);
+#pragma unroll
+                for (int u = 1; u < NL; ++u) {
+                    dx[u] = dx[u - 1] + l - (dx[u - 1] + l >= L ? L : 0);
+                    dy[u] = dy[u - 1] + l - (dy[u - 1] + l >= L ? L : 0);
+                }
+                float4 w[NL][NL];
+                f2 ax[NL][NL], ay[NL][NL], az[NL][NL];
+#pragma unroll
+                for (int v = 0; v < NL; ++v)
+#pragma unroll
+                    for (int u = 0; u < NL; ++u) {
+                        w[v][u] = Wsm[dy[v] * L + dx[u]];
+                        const int m = (cy + v * l) * L + cx + u * l;
+                        ax[v][u] = Sx[m], ay[v][u] = Sy[m], az[v][u] = Sz[m];
+                    }
+#pragma unroll
+                for (int k = 0; k < NN; ++k) {                 // target (a', b') = (k % NL, k / NL)
+#pragma unroll
+                    for (int b = 0; b < NL; ++b)
+#pragma unroll
+                        for (int a = 0; a < NL; ++a) {         // source (a, b): rho = c - offset + ((a - a') l, (b - b') l)
+                            const float4 ww = w[(b - k / NL + NL) % NL][(a - k % NL + NL) % NL];
+                            acc[k][0] = f2_fma(f2_bc(ww.x), ax[b][a], f2_fma(f2_bc(ww.y), ay[b][a], acc[k][0]));
+                            acc[k][1] = f2_fma(f2_bc(ww.y), ax[b][a], f2_fma(f2_bc(ww.z), ay[b][a], acc[k][1]));
+                            acc[k][2] = f2_fma(f2_bc(ww.w), az[b][a], acc[k][2]);
+                        }
+                }
+            }
+            // warp reduction of the 3 NN packed values in fixed order
+            f2 *v = &acc[0][0];
+            if constexpr (NL == 2) {
+                halve_exchange<12>(v, lane, 16);
+                halve_exchange<6>(v, lane, 8);
+                butterfly_sum<3>(v, 4);
+                if ((lane & 7) == 0) {                         // lane bits 4, 3 say which 3 of the 12 values it holds
+#pragma unroll
+                    for (int i = 0; i < 3; ++i) part[warp * 12 + (lane >> 3) * 3 + i] = v[i];
+                }
+            } else {
+                butterfly_sum<3>(v, 16);
+                if (lane == 0) {
+#pragma unroll
+                    for (int i = 0; i < 3; ++i) part[warp * 3 + i] = v[i];
+                }
+            }
+        } else {
+            // the drawing warp: lanes < 2 NN take their site's counter, lane 31 the offset counter of the next pass
+            const int xt = ox + l * (fk % NL), yt = oy + l * (fk / NL);
+            nt = yt * L + xt;
+            uint4 ctr = make_uint4((uint32_t)nt, (uint32_t)fr + p.r_off, (uint32_t)(pass & 0xFFFFFFFFull),
+                                   (uint32_t)(pass >> 32) & 0x7FFFFFFFu);
+            if (lane == 31)
+                ctr = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, (uint32_t)((pass + 1) & 0xFFFFFFFFull),
+                                 (uint32_t)((pass + 1) >> 32) & 0x7FFFFFFFu);
+            const uint4 rnd = philox4x32_10(ctr, rk);
+            if (lane == 31) {
+                off[2 * (cur ^ 1)] = (int)(rnd.x % (uint32_t)l);
+                off[2 * (cur ^ 1) + 1] = (int)(rnd.y % (uint32_t)l);
+            }
+            if (flipper) {
+                const int xe = xt + 1 == L ? 0 : xt + 1, xw = xt == 0 ? L - 1 : xt - 1;
+                const int yn = yt + 1 == L ? 0 : yt + 1, ys = yt == 0 ? L - 1 : yt - 1;
+                const float *fx = reinterpret_cast<const float *>(Sx) + rb, *fy = reinterpret_cast<const float *>(Sy) + rb,
+                            *fz = reinterpret_cast<const float *>(Sz) + rb;
+                const int ie = 2 * (yt * L + xe), iw = 2 * (yt * L + xw), in = 2 * (yn * L + xt), is = 2 * (ys * L + xt);
+                sx = fx[2 * nt], sy = fy[2 * nt], sz = fz[2 * nt];
+                nx = (fx[ie] + fx[iw]) + (fx[in] + fx[is]);
+                ny = (fy[ie] + fy[iw]) + (fy[in] + fy[is]);
+                nz = (fz[ie] + fz[iw]) + (fz[in] + fz[is]);
+                dr = draw_from_words(q, rnd, sx, sy, sz);
+            }
+        }
+        __syncthreads();
+        if (flipper) {
+            float h[3] = {0.0f, 0.0f, 0.0f};
+            const float *pf = reinterpret_cast<const float *>(part) + rb;
+#pragma unroll
+            for (int w = 0; w < kResSumWarps; ++w)             // warp partials in fixed order
+#pragma unroll
+                for (int c = 0; c < 3; ++c) h[c] += pf[2 * ((w * NN + fk) * 3 + c)];
+            const Trial tr = decide_drawn(q, dr, sx, sy, sz, nx, ny, nz, h[0], h[1], h[2], invT, K2, K4);
+            if (tr.acc) {
+                reinterpret_cast<float *>(Sx)[2 * nt + rb] = tr.tx;
+                reinterpret_cast<float *>(Sy)[2 * nt + rb] = tr.ty;
+                reinterpret_cast<float *>(Sz)[2 * nt + rb] = tr.tz;
+            }
+            if (r0 + rb < R) {
+                if (p.accept_out) p.accept_out[(size_t)fr * N + nt] = tr.acc ? 1 : 0;
+                if (p.margin_out) p.margin_out[(size_t)fr * N + nt] = tr.margin;
+            }
+        }
+        __syncthreads();
+    }
+
+    for (int n = tid; n < N; n += kResThreads) {
+        const int x = n % L, y = n / L;
+        int qc;
+        float *dst = p.S + site_index(x, y, Lh, R, plane, qc);
+        float a0, a1, b0, b1, c0, c1;
+        f2_split(Sx[n], a0, a1);
+        f2_split(Sy[n], b0, b1);
+        f2_split(Sz[n], c0, c1);
+        dst[r0] = a0, dst[plane + r0] = b0, dst[2 * plane + r0] = c0;
+        if (r0 + 1 < R) dst[r1] = a1, dst[plane + r1] = b1, dst[2 * plane + r1] = c1;
+    }
+}
+
 __global__ void __launch_bounds__(256) init_spins_kernel(float *__restrict__ S, int L, int R, int mode, uint32_t r_off,
                                                          const RoundKeys rk) {
     const int Lh = L >> 1;
@@ -571,6 +796,35 @@ cudaError_t launch_sublattice_pass(const MetropolisArgs &a, const float *Wc, flo
     const size_t total = (size_t)n * a.R;
     sublattice_flip_kernel<<<(unsigned)((total + 127) / 128), 128, 0, st>>>(a, rk, scratch, KS, l, ox, oy);
     ++*launches;
+    return cudaGetLastError();
+}
+
+bool dsmc_resident_supported(int L, int l) {
+    const int nl = L / l;
+    return (nl == 1 || nl == 2) && resident_smem_bytes(L, nl) <= 227 * 1024;
+}
+
+cudaError_t launch_sublattice_resident(const MetropolisArgs &a, const float *Wc, int l, uint64_t first_pass, uint64_t n_passes,
+                                       cudaStream_t st, uint64_t *launches) {
+    const RoundKeys rk = make_round_keys(a.seed_lo, a.seed_hi);
+    const int nl = a.L / l;
+    const size_t smem = resident_smem_bytes(a.L, nl);
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e;
+        if ((e = cudaFuncSetAttribute(sublattice_resident_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024)) != cudaSuccess) return e;
+        if ((e = cudaFuncSetAttribute(sublattice_resident_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024)) != cudaSuccess) return e;
+        configured = true;
+    }
+    const unsigned grid = (unsigned)((a.R + 1) / 2);
+    // one launch per 65536 passes keeps a single kernel well under a second
+    for (uint64_t done = 0; done < n_passes;) {
+        const unsigned chunk = (unsigned)std::min<uint64_t>(n_passes - done, 65536);
+        if (nl == 1) sublattice_resident_kernel<1><<<grid, kResThreads, smem, st>>>(a, rk, Wc, l, first_pass + done, chunk);
+        else sublattice_resident_kernel<2><<<grid, kResThreads, smem, st>>>(a, rk, Wc, l, first_pass + done, chunk);
+        ++*launches;
+        done += chunk;
+    }
     return cudaGetLastError();
 }
 

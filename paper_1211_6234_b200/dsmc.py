@@ -12,6 +12,7 @@ DSMC_HOST, DSMC_DEVICE = 0, 1
 DSMC_W_IMAGE, DSMC_W_EWALD = 0, 1
 DSMC_REUSE_FIELD = 1
 DSMC_TRIAL_FLIP = 2
+DSMC_NO_RESIDENT = 4
 DSMC_INIT_RANDOM, DSMC_INIT_UP = 0, 1
 DSMC_FIELD_AUTO, DSMC_FIELD_GENERIC, DSMC_FIELD_TILED, DSMC_FIELD_FFT = -1, 0, 1, 2
 

@@ -21,11 +21,11 @@ def dsmc_mod():
     return m
 
 
-def lockstep_passes(m, oracle, ctx, W, T, J, g, K2, K4, seed, l, n_passes, flip=False):
+def lockstep_passes(m, oracle, ctx, W, T, J, g, K2, K4, seed, l, n_passes, flip=False, resident=True):
     L, R = ctx.L, ctx.R
     acc_d = torch.zeros((R, L, L), dtype=torch.uint8, device="cuda")
     mar_d = torch.zeros((R, L, L), dtype=torch.float32, device="cuda")
-    flags = m.DSMC_TRIAL_FLIP if flip else 0
+    flags = (m.DSMC_TRIAL_FLIP if flip else 0) | (0 if resident else m.DSMC_NO_RESIDENT)
     ambiguous = trials = accepted = 0
     for p in range(n_passes):
         s_before = ctx.get_spins()
@@ -60,12 +60,16 @@ def lockstep_passes(m, oracle, ctx, W, T, J, g, K2, K4, seed, l, n_passes, flip=
     return accepted, trials
 
 
-@pytest.mark.parametrize("L,R,l,passes,fft", [(8, 1, 4, 40, False), (12, 5, 3, 24, False), (32, 8, 8, 24, False),
-                                              (64, 16, 32, 48, False), (64, 40, 2, 6, False), (16, 3, 16, 12, False),
-                                              (64, 16, 32, 48, True), (32, 8, 8, 24, True), (32, 6, 2, 8, True)])
-def test_sublattice_lockstep(dsmc_mod, oracle, L, R, l, passes, fft):
+@pytest.mark.parametrize("L,R,l,passes,fft,resident", [
+    (8, 1, 4, 40, False, True), (12, 5, 3, 24, False, True), (32, 8, 8, 24, False, True), (64, 16, 32, 48, False, True),
+    (64, 40, 2, 6, False, True), (16, 3, 16, 12, False, True), (64, 16, 32, 48, True, True), (32, 8, 8, 24, True, True),
+    (32, 6, 2, 8, True, True), (8, 1, 4, 40, False, False), (64, 16, 32, 24, False, False), (16, 3, 16, 12, False, False),
+    (12, 5, 6, 24, False, True), (74, 2, 37, 12, False, True), (64, 3, 64, 12, False, True)])
+def test_sublattice_lockstep(dsmc_mod, oracle, L, R, l, passes, fft, resident):
     """(64, 16, 32) is the paper's own choice L = 64, l = 32; l = 2 is the densest
-    schedule (n = N/4), l = L the conventional single-spin limit; R = 40 spans two replica chunks."""
+    schedule (n = N/4), l = L the conventional single-spin limit; R = 40 spans two replica chunks.
+    With L/l in {1, 2} and L <= 74 (and no FFT field) the pass runs in the shared-memory-resident kernel
+    unless resident = False asks for the two-launch path: both are held to the same oracle."""
     from paper_1211_6234_b200 import inputs
     J, g, K2, K4 = 1.0, 0.25, 0.6, 0.1
     ctx = dsmc_mod.Dsmc(L, R, J=J, g=g, K2=K2, K4=K4)
@@ -75,7 +79,7 @@ def test_sublattice_lockstep(dsmc_mod, oracle, L, R, l, passes, fft):
     W = oracle.build_tensor_ewald(L)
     ctx.set_spins(inputs.random_spins(L, R, 31))
     T = np.linspace(0.2, 1.6, R).astype(np.float32)
-    acc, tr = lockstep_passes(dsmc_mod, oracle, ctx, W, T, J, g, K2, K4, 0x5EED, l, passes)
+    acc, tr = lockstep_passes(dsmc_mod, oracle, ctx, W, T, J, g, K2, K4, 0x5EED, l, passes, resident=resident)
     assert 0 < acc < tr
     ctx.close()
 
@@ -209,14 +213,18 @@ def test_simultaneous_flipping_error_is_small(dsmc_mod, oracle):
     assert np.max(np.abs(gpu - seq)) < 0.1, np.abs(gpu - seq)                       # measured: 0.03
 
 
-@pytest.mark.parametrize("L,R,l,fft,flip", [(64, 16, 32, False, False), (64, 16, 32, True, True), (12, 5, 3, False, True),
-                                            (32, 8, 2, True, False)])
-def test_sublattice_run_graph_replay_is_bit_identical(dsmc_mod, L, R, l, fft, flip):
-    """dsmc_sublattice_run replays a captured graph of one pass whose kernels recompute the offset from a
-    pass counter on the device: same trajectory, bit for bit, as pass-by-pass calls."""
+@pytest.mark.parametrize("L,R,l,fft,flip,resident", [
+    (64, 16, 32, False, False, True), (64, 16, 32, True, True, True), (12, 5, 3, False, True, True),
+    (32, 8, 2, True, False, True), (64, 16, 32, False, False, False), (64, 5, 32, False, True, True),
+    (16, 4, 16, False, False, True), (12, 5, 6, False, False, True)])
+def test_sublattice_run_graph_replay_is_bit_identical(dsmc_mod, L, R, l, fft, flip, resident):
+    """dsmc_sublattice_run either keeps the lattice in shared memory for the whole run (one kernel; L/l in
+    {1, 2}, L <= 74, no FFT field, resident = True) or replays a captured graph of passes whose kernels
+    recompute the offset from a pass counter on the device: same trajectory, bit for bit, as pass-by-pass
+    calls with the same flags."""
     from paper_1211_6234_b200 import inputs
     T = np.linspace(0.3, 1.5, R).astype(np.float32)
-    flags = dsmc_mod.DSMC_TRIAL_FLIP if flip else 0
+    flags = (dsmc_mod.DSMC_TRIAL_FLIP if flip else 0) | (0 if resident else dsmc_mod.DSMC_NO_RESIDENT)
     a = dsmc_mod.Dsmc(L, R, J=1.0, g=0.3, K2=0.5, K4=0.1)
     b = dsmc_mod.Dsmc(L, R, J=1.0, g=0.3, K2=0.5, K4=0.1)
     a.build_tensor(dsmc_mod.DSMC_W_EWALD)
