@@ -493,23 +493,26 @@ __global__ void __launch_bounds__(128) sublattice_flip_kernel(const MetropolisAr
 // latency.  Here one CTA owns two replicas for the WHOLE run of passes: their spins (24 N bytes)
 // and W (16 N bytes) live in shared memory, a pass costs two __syncthreads and no global access, and
 // the R/2 CTAs run side by side on their own SMs.
-//   * 16 summing warps.  For L/l = NL the n = NL^2 update sites are the translates of the offset by
+//   * 8 summing warps.  For L/l = NL the n = NL^2 update sites are the translates of the offset by
 //     multiples of l, so the sources are taken in cosets {c + (a l, b l)} of the same n translations: the
 //     n x n (source, target) pairs of a coset need only n distinct W entries, rho = c - offset + (u l, v l).
 //     Per coset (NL = 2): 4 LDS.128 of W + 12 LDS.64 of spins feed 80 FFMA2 (two replicas packed, the W
 //     value as broadcast operand) -- 1 byte of shared-memory traffic per FMA, which balances the FMA pipe.
 //   * per-thread sums of a few cosets first, then a fixed-order reduction (two-level fp32 accumulation,
 //     deterministic): a halving exchange over the warp (each step trades half of the values for the
-//     partner's partial sums of the other half: 18 packed shuffles instead of 60), then 16 warp partials.
+//     partner's partial sums of the other half: 18 packed shuffles instead of 60), then 8 warp partials.
 //   * one extra warp draws while the others sum: lanes < 2n run Philox for (site, replica, pass) and the
 //     trial spin, lane 31 runs the same Philox code on the offset counter of the NEXT pass (no divergence),
-//     so after the barrier only the 16-term sums, dE and the store of an accepted spin remain.
+//     so after the barrier only the 8-term sums, dE and the store of an accepted spin remain.
 // Needs L/l in {1, 2} and 40 N bytes + partials within the 227 KB of one CTA (L <= 74).
-constexpr int kResSumWarps = 16;
+#ifndef DSMC_RES_WARPS
+#define DSMC_RES_WARPS 8
+#endif
+constexpr int kResSumWarps = DSMC_RES_WARPS;
 constexpr int kResThreads = 32 * (kResSumWarps + 1);
 
 __host__ __device__ constexpr size_t resident_smem_bytes(int L, int NL) {
-    return (size_t)40 * L * L + sizeof(f2) * kResSumWarps * NL * NL * 3 + 64;
+    return (size_t)40 * L * L + 16 + sizeof(f2) * kResSumWarps * NL * NL * 3 + 64;
 }
 
 // Reduction helpers for values held as packed pairs.  halve_exchange: lanes with the mask bit clear keep
@@ -540,10 +543,10 @@ __global__ void __launch_bounds__(kResThreads, 1) sublattice_resident_kernel(con
     constexpr int NN = NL * NL;
     extern __shared__ __align__(16) unsigned char rsm[];
     const int L = p.L, Lh = L >> 1, R = p.R, N = L * L;
-    float4 *Wsm = reinterpret_cast<float4 *>(rsm);                     // [N]  (xx, xy, yy, zz) at rho = ry L + rx
-    f2 *Sx = reinterpret_cast<f2 *>(rsm + (size_t)16 * N);             // [N]  replicas (r0, r1) of site n = y L + x
-    f2 *Sy = Sx + N, *Sz = Sy + N;
-    f2 *part = Sz + N;                                                 // [warp][target][c]
+    float4 *Wsm = reinterpret_cast<float4 *>(rsm);                     // [N + 1]  (xx, xy, yy, zz) at rho = ry L + rx; [N] = 0
+    f2 *Ssm = reinterpret_cast<f2 *>(rsm + (size_t)16 * (N + 1));      // [N][3]  replicas (r0, r1) of site n = y L + x
+    float *Sf = reinterpret_cast<float *>(Ssm);                        // the same as [N][3][2] floats
+    f2 *part = Ssm + 3 * (size_t)N;                                    // [warp][target][c]
     int *off = reinterpret_cast<int *>(part + kResSumWarps * NN * 3);  // [2][2]: offsets of this and the next pass
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int r0 = 2 * blockIdx.x, r1 = min(r0 + 1, R - 1);            // odd R: the last CTA carries its replica twice
@@ -555,11 +558,14 @@ __global__ void __launch_bounds__(kResThreads, 1) sublattice_resident_kernel(con
         const int x = n % L, y = n / L;
         int q;
         const float *src = p.S + site_index(x, y, Lh, R, plane, q);
-        Sx[n] = f2_make(src[r0], src[r1]);
-        Sy[n] = f2_make(src[plane + r0], src[plane + r1]);
-        Sz[n] = f2_make(src[2 * plane + r0], src[2 * plane + r1]);
+        Ssm[3 * n] = f2_make(src[r0], src[r1]);
+        Ssm[3 * n + 1] = f2_make(src[plane + r0], src[plane + r1]);
+        Ssm[3 * n + 2] = f2_make(src[2 * plane + r0], src[2 * plane + r1]);
     }
-    if (tid == 0) pass_offset(rk, first_pass, l, off[0], off[1]);
+    if (tid == 0) {
+        Wsm[N] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+        pass_offset(rk, first_pass, l, off[0], off[1]);
+    }
     __syncthreads();
 
     // the drawing warp's lanes: update site k = lane >> 1, replica half rb = lane & 1
@@ -569,8 +575,17 @@ __global__ void __launch_bounds__(kResThreads, 1) sublattice_resident_kernel(con
     if (flipper) invT = p.invT[fr], K2 = p.K2[fr], K4 = p.K4[fr];
     MetropolisArgs q = p;
     q.step_dev = nullptr;
+    const int cy0 = tid / l, cx0 = tid - cy0 * l;                      // this thread's first coset and the stride to the next
+    const int step_y = (32 * kResSumWarps) / l, step_x = 32 * kResSumWarps - step_y * l;
 
+#ifdef DSMC_RES_TIMING
+    long long tacc[6] = {0, 0, 0, 0, 0, 0};
+#define RT(i) const long long rt##i = clock64();
+#else
+#define RT(i)
+#endif
     for (unsigned it = 0; it < n_passes; ++it) {
+        RT(0)
         const unsigned long long pass = first_pass + it;
         const int cur = (int)(it & 1u);
         const int ox = off[2 * cur], oy = off[2 * cur + 1];
@@ -581,39 +596,55 @@ __global__ void __launch_bounds__(kResThreads, 1) sublattice_resident_kernel(con
             f2 acc[NN][3];
 #pragma unroll
             for (int k = 0; k < NN; ++k) acc[k][0] = acc[k][1] = acc[k][2] = f2_bc(0.0f);
-            for (int c = tid; c < l * l; c += 32 * kResSumWarps) {
-                const int cy = c / l, cx = c - cy * l;
-                int dx[NL], dy[NL];
-                dx[0] = cx - ox + (cx < ox ? L : 0);
-                dy[0] = cy - oy + (cy < oy ? L : 0);
+            // UN cosets per trip: all their loads are issued before the first FMA, so the shared-memory latency is
+            // paid once per trip and not once per coset (two warps per scheduler hide little of it)
+            constexpr int UN = NL == 2 ? 2 : 8;
+            int cx = cx0, cy = cy0;                            // coset c = tid, tid + 256, ...: coordinates stepped, not divided
+            for (int c = tid; c < l * l; c += UN * 32 * kResSumWarps) {
+                float4 w[UN][NL][NL];
+                f2 sp[UN][NL][NL][3];
 #pragma unroll
-                for (int u = 1; u < NL; ++u) {
-                    dx[u] = dx[u - 1] + l - (dx[u - 1] + l >= L ? L : 0);
-                    dy[u] = dy[u - 1] + l - (dy[u - 1] + l >= L ? L : 0);
-                }
-                float4 w[NL][NL];
-                f2 ax[NL][NL], ay[NL][NL], az[NL][NL];
+                for (int j = 0; j < UN; ++j) {
+                    if (cx >= l) cx -= l, ++cy;
+                    // past the last coset: W entry N (zeros) and site 0, so the trip contributes exact zeros
+                    const bool valid = c + j * 32 * kResSumWarps < l * l;
+                    int dx[NL], dy[NL];
+                    dx[0] = cx - ox + (cx < ox ? L : 0);
+                    dy[0] = cy - oy + (cy < oy ? L : 0);
 #pragma unroll
-                for (int v = 0; v < NL; ++v)
-#pragma unroll
-                    for (int u = 0; u < NL; ++u) {
-                        w[v][u] = Wsm[dy[v] * L + dx[u]];
-                        const int m = (cy + v * l) * L + cx + u * l;
-                        ax[v][u] = Sx[m], ay[v][u] = Sy[m], az[v][u] = Sz[m];
+                    for (int u = 1; u < NL; ++u) {
+                        dx[u] = dx[u - 1] + l - (dx[u - 1] + l >= L ? L : 0);
+                        dy[u] = dy[u - 1] + l - (dy[u - 1] + l >= L ? L : 0);
                     }
+                    const int m0 = valid ? cy * L + cx : 0;
 #pragma unroll
-                for (int k = 0; k < NN; ++k) {                 // target (a', b') = (k % NL, k / NL)
+                    for (int v = 0; v < NL; ++v)
 #pragma unroll
-                    for (int b = 0; b < NL; ++b)
-#pragma unroll
-                        for (int a = 0; a < NL; ++a) {         // source (a, b): rho = c - offset + ((a - a') l, (b - b') l)
-                            const float4 ww = w[(b - k / NL + NL) % NL][(a - k % NL + NL) % NL];
-                            acc[k][0] = f2_fma(f2_bc(ww.x), ax[b][a], f2_fma(f2_bc(ww.y), ay[b][a], acc[k][0]));
-                            acc[k][1] = f2_fma(f2_bc(ww.y), ax[b][a], f2_fma(f2_bc(ww.z), ay[b][a], acc[k][1]));
-                            acc[k][2] = f2_fma(f2_bc(ww.w), az[b][a], acc[k][2]);
+                        for (int u = 0; u < NL; ++u) {
+                            w[j][v][u] = Wsm[valid ? dy[v] * L + dx[u] : N];
+                            const f2 *src = Ssm + 3 * (m0 + v * l * L + u * l);
+                            sp[j][v][u][0] = src[0], sp[j][v][u][1] = src[1], sp[j][v][u][2] = src[2];
                         }
+                    cx += step_x, cy += step_y;
                 }
+#pragma unroll
+                for (int j = 0; j < UN; ++j)
+#pragma unroll
+                    for (int k = 0; k < NN; ++k)               // target (a', b') = (k % NL, k / NL)
+#pragma unroll
+                        for (int b = 0; b < NL; ++b)
+#pragma unroll
+                            for (int a = 0; a < NL; ++a) {     // source (a, b): rho = c - offset + ((a - a') l, (b - b') l)
+                                const float4 ww = w[j][(b - k / NL + NL) % NL][(a - k % NL + NL) % NL];
+                                const f2 ax = sp[j][b][a][0], ay = sp[j][b][a][1], az = sp[j][b][a][2];
+                                acc[k][0] = f2_fma(f2_bc(ww.x), ax, f2_fma(f2_bc(ww.y), ay, acc[k][0]));
+                                acc[k][1] = f2_fma(f2_bc(ww.y), ax, f2_fma(f2_bc(ww.z), ay, acc[k][1]));
+                                acc[k][2] = f2_fma(f2_bc(ww.w), az, acc[k][2]);
+                            }
             }
+#ifdef DSMC_RES_TIMING
+            tacc[4] += clock64() - rt0;
+#endif
             // warp reduction of the 3 NN packed values in fixed order
             f2 *v = &acc[0][0];
             if constexpr (NL == 2) {
@@ -641,6 +672,9 @@ __global__ void __launch_bounds__(kResThreads, 1) sublattice_resident_kernel(con
                 ctr = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, (uint32_t)((pass + 1) & 0xFFFFFFFFull),
                                  (uint32_t)((pass + 1) >> 32) & 0x7FFFFFFFu);
             const uint4 rnd = philox4x32_10(ctr, rk);
+#ifdef DSMC_RES_TIMING
+            tacc[5] += clock64() - rt0;
+#endif
             if (lane == 31) {
                 off[2 * (cur ^ 1)] = (int)(rnd.x % (uint32_t)l);
                 off[2 * (cur ^ 1) + 1] = (int)(rnd.y % (uint32_t)l);
@@ -648,17 +682,18 @@ __global__ void __launch_bounds__(kResThreads, 1) sublattice_resident_kernel(con
             if (flipper) {
                 const int xe = xt + 1 == L ? 0 : xt + 1, xw = xt == 0 ? L - 1 : xt - 1;
                 const int yn = yt + 1 == L ? 0 : yt + 1, ys = yt == 0 ? L - 1 : yt - 1;
-                const float *fx = reinterpret_cast<const float *>(Sx) + rb, *fy = reinterpret_cast<const float *>(Sy) + rb,
-                            *fz = reinterpret_cast<const float *>(Sz) + rb;
-                const int ie = 2 * (yt * L + xe), iw = 2 * (yt * L + xw), in = 2 * (yn * L + xt), is = 2 * (ys * L + xt);
-                sx = fx[2 * nt], sy = fy[2 * nt], sz = fz[2 * nt];
-                nx = (fx[ie] + fx[iw]) + (fx[in] + fx[is]);
-                ny = (fy[ie] + fy[iw]) + (fy[in] + fy[is]);
-                nz = (fz[ie] + fz[iw]) + (fz[in] + fz[is]);
+                const float *sc = Sf + 6 * nt + rb, *se = Sf + 6 * (yt * L + xe) + rb, *sw = Sf + 6 * (yt * L + xw) + rb,
+                            *sn = Sf + 6 * (yn * L + xt) + rb, *ss = Sf + 6 * (ys * L + xt) + rb;
+                sx = sc[0], sy = sc[2], sz = sc[4];
+                nx = (se[0] + sw[0]) + (sn[0] + ss[0]);
+                ny = (se[2] + sw[2]) + (sn[2] + ss[2]);
+                nz = (se[4] + sw[4]) + (sn[4] + ss[4]);
                 dr = draw_from_words(q, rnd, sx, sy, sz);
             }
         }
+        RT(1)
         __syncthreads();
+        RT(2)
         if (flipper) {
             float h[3] = {0.0f, 0.0f, 0.0f};
             const float *pf = reinterpret_cast<const float *>(part) + rb;
@@ -668,26 +703,36 @@ __global__ void __launch_bounds__(kResThreads, 1) sublattice_resident_kernel(con
                 for (int c = 0; c < 3; ++c) h[c] += pf[2 * ((w * NN + fk) * 3 + c)];
             const Trial tr = decide_drawn(q, dr, sx, sy, sz, nx, ny, nz, h[0], h[1], h[2], invT, K2, K4);
             if (tr.acc) {
-                reinterpret_cast<float *>(Sx)[2 * nt + rb] = tr.tx;
-                reinterpret_cast<float *>(Sy)[2 * nt + rb] = tr.ty;
-                reinterpret_cast<float *>(Sz)[2 * nt + rb] = tr.tz;
+                Sf[6 * nt + rb] = tr.tx;
+                Sf[6 * nt + 2 + rb] = tr.ty;
+                Sf[6 * nt + 4 + rb] = tr.tz;
             }
             if (r0 + rb < R) {
                 if (p.accept_out) p.accept_out[(size_t)fr * N + nt] = tr.acc ? 1 : 0;
                 if (p.margin_out) p.margin_out[(size_t)fr * N + nt] = tr.margin;
             }
         }
+        RT(3)
         __syncthreads();
+#ifdef DSMC_RES_TIMING
+        const long long rt4 = clock64();
+        tacc[0] += rt1 - rt0, tacc[1] += rt2 - rt1, tacc[2] += rt3 - rt2, tacc[3] += rt4 - rt3;
+#endif
     }
+#ifdef DSMC_RES_TIMING
+    if (blockIdx.x == 0 && (tid == 0 || tid == 32 * kResSumWarps))
+        printf("tid %d: work %lld bar1 %lld flip %lld bar2 %lld philox %lld loop %lld (clk per pass)\n", tid, tacc[0] / n_passes,
+               tacc[1] / n_passes, tacc[2] / n_passes, tacc[3] / n_passes, tacc[5] / n_passes, tacc[4] / n_passes);
+#endif
 
     for (int n = tid; n < N; n += kResThreads) {
         const int x = n % L, y = n / L;
         int qc;
         float *dst = p.S + site_index(x, y, Lh, R, plane, qc);
         float a0, a1, b0, b1, c0, c1;
-        f2_split(Sx[n], a0, a1);
-        f2_split(Sy[n], b0, b1);
-        f2_split(Sz[n], c0, c1);
+        f2_split(Ssm[3 * n], a0, a1);
+        f2_split(Ssm[3 * n + 1], b0, b1);
+        f2_split(Ssm[3 * n + 2], c0, c1);
         dst[r0] = a0, dst[plane + r0] = b0, dst[2 * plane + r0] = c0;
         if (r0 + 1 < R) dst[r1] = a1, dst[plane + r1] = b1, dst[2 * plane + r1] = c1;
     }
