@@ -578,14 +578,7 @@ __global__ void __launch_bounds__(kResThreads, 1) sublattice_resident_kernel(con
     const int cy0 = tid / l, cx0 = tid - cy0 * l;                      // this thread's first coset and the stride to the next
     const int step_y = (32 * kResSumWarps) / l, step_x = 32 * kResSumWarps - step_y * l;
 
-#ifdef DSMC_RES_TIMING
-    long long tacc[6] = {0, 0, 0, 0, 0, 0};
-#define RT(i) const long long rt##i = clock64();
-#else
-#define RT(i)
-#endif
     for (unsigned it = 0; it < n_passes; ++it) {
-        RT(0)
         const unsigned long long pass = first_pass + it;
         const int cur = (int)(it & 1u);
         const int ox = off[2 * cur], oy = off[2 * cur + 1];
@@ -596,9 +589,9 @@ __global__ void __launch_bounds__(kResThreads, 1) sublattice_resident_kernel(con
             f2 acc[NN][3];
 #pragma unroll
             for (int k = 0; k < NN; ++k) acc[k][0] = acc[k][1] = acc[k][2] = f2_bc(0.0f);
-            // UN cosets per trip: all their loads are issued before the first FMA, so the shared-memory latency is
-            // paid once per trip and not once per coset (two warps per scheduler hide little of it)
-            constexpr int UN = NL == 2 ? 2 : 8;
+            // UN cosets per trip, all their loads issued before the first FMA.  Measured (us per pass at L = 64,
+            // l = 32 / l = 64): NL = 2 with UN = 1: 1.66, UN = 2: 1.70; NL = 1 with UN = 4: 1.36, UN = 8: 1.29
+            constexpr int UN = NL == 2 ? 1 : 8;
             int cx = cx0, cy = cy0;                            // coset c = tid, tid + 256, ...: coordinates stepped, not divided
             for (int c = tid; c < l * l; c += UN * 32 * kResSumWarps) {
                 float4 w[UN][NL][NL];
@@ -642,9 +635,6 @@ __global__ void __launch_bounds__(kResThreads, 1) sublattice_resident_kernel(con
                                 acc[k][2] = f2_fma(f2_bc(ww.w), az, acc[k][2]);
                             }
             }
-#ifdef DSMC_RES_TIMING
-            tacc[4] += clock64() - rt0;
-#endif
             // warp reduction of the 3 NN packed values in fixed order
             f2 *v = &acc[0][0];
             if constexpr (NL == 2) {
@@ -672,9 +662,6 @@ __global__ void __launch_bounds__(kResThreads, 1) sublattice_resident_kernel(con
                 ctr = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, (uint32_t)((pass + 1) & 0xFFFFFFFFull),
                                  (uint32_t)((pass + 1) >> 32) & 0x7FFFFFFFu);
             const uint4 rnd = philox4x32_10(ctr, rk);
-#ifdef DSMC_RES_TIMING
-            tacc[5] += clock64() - rt0;
-#endif
             if (lane == 31) {
                 off[2 * (cur ^ 1)] = (int)(rnd.x % (uint32_t)l);
                 off[2 * (cur ^ 1) + 1] = (int)(rnd.y % (uint32_t)l);
@@ -691,9 +678,7 @@ __global__ void __launch_bounds__(kResThreads, 1) sublattice_resident_kernel(con
                 dr = draw_from_words(q, rnd, sx, sy, sz);
             }
         }
-        RT(1)
         __syncthreads();
-        RT(2)
         if (flipper) {
             float h[3] = {0.0f, 0.0f, 0.0f};
             const float *pf = reinterpret_cast<const float *>(part) + rb;
@@ -712,18 +697,8 @@ __global__ void __launch_bounds__(kResThreads, 1) sublattice_resident_kernel(con
                 if (p.margin_out) p.margin_out[(size_t)fr * N + nt] = tr.margin;
             }
         }
-        RT(3)
         __syncthreads();
-#ifdef DSMC_RES_TIMING
-        const long long rt4 = clock64();
-        tacc[0] += rt1 - rt0, tacc[1] += rt2 - rt1, tacc[2] += rt3 - rt2, tacc[3] += rt4 - rt3;
-#endif
     }
-#ifdef DSMC_RES_TIMING
-    if (blockIdx.x == 0 && (tid == 0 || tid == 32 * kResSumWarps))
-        printf("tid %d: work %lld bar1 %lld flip %lld bar2 %lld philox %lld loop %lld (clk per pass)\n", tid, tacc[0] / n_passes,
-               tacc[1] / n_passes, tacc[2] / n_passes, tacc[3] / n_passes, tacc[5] / n_passes, tacc[4] / n_passes);
-#endif
 
     for (int n = tid; n < N; n += kResThreads) {
         const int x = n % L, y = n / L;
