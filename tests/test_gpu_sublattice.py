@@ -267,3 +267,42 @@ def test_appendix_b_critical_temperature_matches_table1(dsmc_mod):
     lo, hi = min(rows["T_c"]), max(rows["T_c"])
     assert lo - 0.03 <= tc <= hi + 0.03, tc                                 # measured: 0.846
     assert r["m_st"][0] > 0.85 and r["m_st"][-1] < 0.25                     # ordered -> disordered across the peak
+
+
+def test_section4_production_run_matches_the_papers_statements(dsmc_mod):
+    """The paper's production run (L = 64, l = 32, script-J = 8.9, script-K = 15, striped start) in
+    a shortened protocol, against the numbers its text prints (tests/golden/paper_section4.txt): for a = 0 the
+    in-plane magnetisation peaks at M_par ~ .46 near script-T = 4.5 after the orientational order is lost over
+    1 < script-T < 3 and is gone by script-T = 8; for a = 2 the stripes hold up to script-T = 4 and the system then
+    jumps to an in-plane ferromagnet; for a = -1 the orientational order goes over 1 < script-T < 2.5.  These are
+    the only quantitative statements about Figs. 10-13; they also check the unit map script-T = 2 T / g (R7)."""
+    import os
+    from paper_1211_6234_b200 import section4
+    g = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "paper_section4.txt")) as f:
+        for line in f:
+            if not line.startswith("#"):
+                k, v = line.split()[:2]
+                g[k] = float(v)
+    temps = np.array([1.0, 2.5, 3.0, 3.5, 4.0, 4.5, 5.0, 8.0])
+    r = section4.run(temps, chains=2, equilibrate=10000, steps=4000, every=50, seed=11)
+    mean = r["mean"]                                            # [a][T][quantity]
+    Oz, Mpar, eta = mean[:, :, 7], mean[:, :, 2], mean[:, :, 3]
+    print("script-T   ", temps)
+    for ia, a in enumerate(section4.A_VALUES):
+        print(f"a = {a:+.0f}: O_z  ", np.round(Oz[ia], 3))
+        print(f"        M_par", np.round(Mpar[ia], 3))
+        print(f"        eta  ", np.round(eta[ia], 3))
+    iT = {t: i for i, t in enumerate(temps)}
+    # a = 0 (index 1): ordered at the lower end of the printed window, disordered above it, peak of M_par
+    assert Oz[1, iT[g["a0_Oz_loss_T_lo"]]] > 0.95 and Oz[1, iT[3.5]] < 0.1
+    ipk = int(np.argmax(Mpar[1]))
+    assert abs(temps[ipk] - g["a0_Mpar_peak_T"]) <= 0.5, temps[ipk]
+    assert abs(Mpar[1, ipk] - g["a0_Mpar_peak_value"]) < 0.05, Mpar[1, ipk]           # measured: 0.47
+    assert Mpar[1, iT[g["a0_Mpar_zero_T"]]] < 0.1
+    # a = 2 (index 2): stripes up to script-T = 4, in-plane ferromagnet right above
+    assert Oz[2, iT[3.5]] > 0.4 and Mpar[2, iT[3.5]] < 0.05 and eta[2, iT[3.5]] > 0.75
+    assert Oz[2, iT[4.5]] < 0.05 and Mpar[2, iT[4.5]] > 0.65 and eta[2, iT[4.5]] < 0.4
+    # a = -1 (index 0): canted at every temperature (eta far from 1), order lost across 1 ... 2.5
+    assert Oz[0, iT[g["am1_Oz_loss_T_lo"]]] > 0.9 and Oz[0, iT[3.0]] < 0.15
+    assert np.all(eta[0] < 0.62) and np.all(eta[0] > 0.45)
