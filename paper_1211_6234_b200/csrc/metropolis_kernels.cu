@@ -535,14 +535,15 @@ __device__ __forceinline__ void butterfly_sum(f2 *v, int first) {
         for (int i = 0; i < V; ++i) v[i] = f2_add(v[i], __shfl_xor_sync(0xFFFFFFFFu, v[i], mask));
 }
 
-template <int NL>
+template <int NL, int CPT, int LC>
 __global__ void __launch_bounds__(kResThreads, 1) sublattice_resident_kernel(const MetropolisArgs p, const RoundKeys rk,
-                                                                             const float *__restrict__ Wc, int l,
+                                                                             const float *__restrict__ Wc, int l_arg,
                                                                              unsigned long long first_pass,
                                                                              unsigned n_passes) {
     constexpr int NN = NL * NL;
     extern __shared__ __align__(16) unsigned char rsm[];
-    const int L = p.L, Lh = L >> 1, R = p.R, N = L * L;
+    // LC > 0: lattice size (and with it l = L / NL) known at compile time, index arithmetic in shifts
+    const int L = LC > 0 ? LC : p.L, l = LC > 0 ? LC / NL : l_arg, Lh = L >> 1, R = p.R, N = L * L;
     float4 *Wsm = reinterpret_cast<float4 *>(rsm);                     // [N + 1]  (xx, xy, yy, zz) at rho = ry L + rx; [N] = 0
     f2 *Ssm = reinterpret_cast<f2 *>(rsm + (size_t)16 * (N + 1));      // [N][3]  replicas (r0, r1) of site n = y L + x
     float *Sf = reinterpret_cast<float *>(Ssm);                        // the same as [N][3][2] floats
@@ -590,10 +591,17 @@ __global__ void __launch_bounds__(kResThreads, 1) sublattice_resident_kernel(con
 #pragma unroll
             for (int k = 0; k < NN; ++k) acc[k][0] = acc[k][1] = acc[k][2] = f2_bc(0.0f);
             // UN cosets per trip, all their loads issued before the first FMA.  Measured (us per pass at L = 64,
-            // l = 32 / l = 64): NL = 2 with UN = 1: 1.66, UN = 2: 1.70; NL = 1 with UN = 4: 1.36, UN = 8: 1.29
+            // l = 32 / l = 64, run-time trip count): NL = 2 with UN = 1: 1.66, UN = 2: 1.70; NL = 1 with UN = 4: 1.36,
+            // UN = 8: 1.29.  With the trip count (CPT) and the lattice size (LC) as template parameters: 1.46 / 1.10.
             constexpr int UN = NL == 2 ? 1 : 8;
+            // CPT > 0: the trip count is a compile-time constant and the loop unrolls, so the coset coordinates and
+            // spin addresses become invariants of the pass loop
+            constexpr int UNR = CPT > 0 ? CPT : 1;
+            const int ntrip = CPT > 0 ? CPT : (l * l + UN * 32 * kResSumWarps - 1) / (UN * 32 * kResSumWarps);
             int cx = cx0, cy = cy0;                            // coset c = tid, tid + 256, ...: coordinates stepped, not divided
-            for (int c = tid; c < l * l; c += UN * 32 * kResSumWarps) {
+#pragma unroll UNR
+            for (int trip = 0; trip < ntrip; ++trip) {
+                const int c = tid + trip * UN * 32 * kResSumWarps;
                 float4 w[UN][NL][NL];
                 f2 sp[UN][NL][NL][3];
 #pragma unroll
@@ -829,19 +837,17 @@ cudaError_t launch_sublattice_resident(const MetropolisArgs &a, const float *Wc,
     const RoundKeys rk = make_round_keys(a.seed_lo, a.seed_hi);
     const int nl = a.L / l;
     const size_t smem = resident_smem_bytes(a.L, nl);
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e;
-        if ((e = cudaFuncSetAttribute(sublattice_resident_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024)) != cudaSuccess) return e;
-        if ((e = cudaFuncSetAttribute(sublattice_resident_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024)) != cudaSuccess) return e;
-        configured = true;
-    }
+    // trips of the summing loop per pass: a compile-time constant for the common shapes (0 = run-time count)
+    const int un = nl == 2 ? 1 : 8, trips = (l * l + un * 32 * kResSumWarps - 1) / (un * 32 * kResSumWarps);
+    void (*kern)(const MetropolisArgs, const RoundKeys, const float *, int, unsigned long long, unsigned) = nullptr;
+    if (nl == 2) kern = a.L == 64 ? sublattice_resident_kernel<2, 4, 64> : trips == 4 ? sublattice_resident_kernel<2, 4, 0> : trips == 1 ? sublattice_resident_kernel<2, 1, 0> : sublattice_resident_kernel<2, 0, 0>;
+    else kern = a.L == 64 ? sublattice_resident_kernel<1, 2, 64> : trips == 2 ? sublattice_resident_kernel<1, 2, 0> : trips == 1 ? sublattice_resident_kernel<1, 1, 0> : sublattice_resident_kernel<1, 0, 0>;
+    if (cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024)) return e;
     const unsigned grid = (unsigned)((a.R + 1) / 2);
     // one launch per 65536 passes keeps a single kernel well under a second
     for (uint64_t done = 0; done < n_passes;) {
         const unsigned chunk = (unsigned)std::min<uint64_t>(n_passes - done, 65536);
-        if (nl == 1) sublattice_resident_kernel<1><<<grid, kResThreads, smem, st>>>(a, rk, Wc, l, first_pass + done, chunk);
-        else sublattice_resident_kernel<2><<<grid, kResThreads, smem, st>>>(a, rk, Wc, l, first_pass + done, chunk);
+        kern<<<grid, kResThreads, smem, st>>>(a, rk, Wc, l, first_pass + done, chunk);
         ++*launches;
         done += chunk;
     }
