@@ -64,12 +64,14 @@ def lockstep_passes(m, oracle, ctx, W, T, J, g, K2, K4, seed, l, n_passes, flip=
     (8, 1, 4, 40, False, True), (12, 5, 3, 24, False, True), (32, 8, 8, 24, False, True), (64, 16, 32, 48, False, True),
     (64, 40, 2, 6, False, True), (16, 3, 16, 12, False, True), (64, 16, 32, 48, True, True), (32, 8, 8, 24, True, True),
     (32, 6, 2, 8, True, True), (8, 1, 4, 40, False, False), (64, 16, 32, 24, False, False), (16, 3, 16, 12, False, False),
-    (12, 5, 6, 24, False, True), (74, 2, 37, 12, False, True), (64, 3, 64, 12, False, True)])
+    (12, 5, 6, 24, False, True), (74, 2, 37, 12, False, True), (64, 3, 64, 12, False, True),
+    (64, 296, 32, 6, False, True), (4, 2, 2, 16, False, True), (6, 1, 3, 16, False, True), (6, 2, 6, 16, False, True)])
 def test_sublattice_lockstep(dsmc_mod, oracle, L, R, l, passes, fft, resident):
     """(64, 16, 32) is the paper's own choice L = 64, l = 32; l = 2 is the densest
     schedule (n = N/4), l = L the conventional single-spin limit; R = 40 spans two replica chunks.
     With L/l in {1, 2} and L <= 74 (and no FFT field) the pass runs in the shared-memory-resident kernel
-    unless resident = False asks for the two-launch path: both are held to the same oracle."""
+    unless resident = False asks for the two-launch path: both are held to the same oracle.  (64, 296, 32) is the
+    second launch configuration bench.py times (148 CTAs, one per SM); L = 4 and 6 are the smallest lattices."""
     from paper_1211_6234_b200 import inputs
     J, g, K2, K4 = 1.0, 0.25, 0.6, 0.1
     ctx = dsmc_mod.Dsmc(L, R, J=J, g=g, K2=K2, K4=K4)
