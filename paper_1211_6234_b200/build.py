@@ -6,7 +6,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdsmc.so")
-SOURCES = ["dsmc_api.cu", "tensor_kernels.cu", "state_kernels.cu", "metropolis_kernels.cu",
+SOURCES = ["dsmc_api.cu", "tensor_kernels.cu", "state_kernels.cu", "metropolis_kernels.cu", "sublattice_kernels.cu",
            "field_generic.cu", "field_tiled.cu", "field_fft.cu", "peak_kernels.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--shared", "-cudart", "static"]
@@ -17,6 +17,7 @@ def _deps():
     d.append(os.path.join(CSRC, "dsmc_internal.cuh"))
     d.append(os.path.join(CSRC, "bulk_copy.cuh"))
     d.append(os.path.join(CSRC, "packed_f32x2.cuh"))
+    d.append(os.path.join(CSRC, "metropolis_common.cuh"))
     d.append(os.path.join(HERE, "..", "include", "dsmc.h"))
     return d
 
