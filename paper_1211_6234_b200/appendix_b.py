@@ -9,7 +9,9 @@ of the four sub-lattices (R23), chi_st = (L^2 / k_B T)(<m_st^2> - <m_st>^2), T_c
 l = 32 updates n = 4 sites per pass with the simultaneous-flip approximation of section 3.2; l = L = 64
 updates one random site per pass, i.e. conventional single-spin Metropolis with no approximation: the
 pair of runs is the comparison of the paper's Table 1 (T_c = .85 "GPU algorithm" against .82
-"conventional MC" from its ref. [66]).
+"conventional MC" from its ref. [66]).  Smaller strides (--l 16 8 4 2) make the approximation coarser
+("the error will be increased for decreasing l"); --l 0 is the checkerboard half-sweep of
+north_star (n = N/2 simultaneous sites, the coarsest use of the approximation).
 
 Every pass, the sub-lattice sums of m_st included, runs in libdsmc.so (dsmc_sublattice_run with the lattice
 resident in shared memory, dsmc_staggered_magnetisation); this script marshals arguments and averages the
@@ -26,7 +28,7 @@ import numpy as np
 def scan(l, temps, chains, equilibrate, steps, seed, device="cuda"):
     """-> dict of arrays over temperatures: m_st, chi_st and their standard errors over the chains."""
     import torch
-    from . import Dsmc, DSMC_W_EWALD, DSMC_TRIAL_FLIP
+    from . import Dsmc, DSMC_W_EWALD, DSMC_TRIAL_FLIP, DSMC_FIELD_FFT
     L, g, J = 64, 1.0, 0.85
     nT = len(temps)
     R = nT * chains
@@ -36,14 +38,24 @@ def scan(l, temps, chains, equilibrate, steps, seed, device="cuda"):
     s = np.zeros((R, 3, L, L), dtype=np.float32)
     s[:, 2] = np.where(np.arange(L) % 2 == 0, 1.0, -1.0)[None, :, None]      # h = 1 stripes: the ground state
     ctx.set_spins(s)
-    per_step = l * l                                                       # passes per MC step (N attempted updates)
+    per_step = l * l if l else 2                                           # passes (half-sweeps) per MC step
+    if l == 0:
+        ctx.select_field_kernel(DSMC_FIELD_FFT)
+
+    def advance(first_step, n_steps, Targ):
+        if l:                                                              # stride-l passes (l = L: single-spin Metropolis)
+            ctx.sublattice_run(Targ, seed, first_step * per_step, n_steps * per_step, l, flags=DSMC_TRIAL_FLIP)
+        else:                                                              # checkerboard half-sweeps (north_star's schedule)
+            for h in range(2 * first_step, 2 * (first_step + n_steps)):
+                ctx.halfsweep(Targ if h == 2 * first_step else None, seed, h, flags=DSMC_TRIAL_FLIP)
+
     torch.cuda.synchronize()
     t0 = time.perf_counter()
-    ctx.sublattice_run(T, seed, 0, equilibrate * per_step, l, flags=DSMC_TRIAL_FLIP)
+    advance(0, equilibrate, T)
     s1 = np.zeros(R)
     s2 = np.zeros(R)
     for k in range(steps):
-        ctx.sublattice_run(None, seed, (equilibrate + k) * per_step, per_step, l, flags=DSMC_TRIAL_FLIP)
+        advance(equilibrate + k, 1, None)
         m = ctx.staggered_magnetisation()[:, 2]
         s1 += m
         s2 += m * m
@@ -70,7 +82,8 @@ def peak_temperature(T, chi):
 
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("--l", type=int, nargs="*", default=[32, 64], help="stride(s): 32 = the paper's, 64 = single-spin")
+    ap.add_argument("--l", type=int, nargs="*", default=[32, 64],
+                    help="stride(s): 32 = the paper's, 64 = single-spin, any divisor of 64 >= 2; 0 = checkerboard half-sweeps")
     ap.add_argument("--tmin", type=float, default=0.50)
     ap.add_argument("--tmax", type=float, default=1.22)
     ap.add_argument("--nt", type=int, default=37)
@@ -89,7 +102,7 @@ def main():
         print(json.dumps([{k: (v.tolist() if isinstance(v, np.ndarray) else v) for k, v in r.items()} for r in results]))
         return
     for r in results:
-        n = (64 // r["l"]) ** 2
+        n = (64 // r["l"]) ** 2 if r["l"] else 2048
         print(f"l = {r['l']} (n = {n} simultaneous sites): {args.equilibrate} + {args.steps} MC steps, {args.nt} temperatures x "
               f"{args.chains} chains in {r['seconds']:.1f} s ({r['passes_per_s']:.3e} passes/s); "
               f"T_c (peak of chi_st) = {peak_temperature(r['T'], r['chi_st']):.3f} C_D")
