@@ -153,7 +153,7 @@ int dsmc_halfsweep_ex(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t ste
 int dsmc_sublattice_pass(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t pass, int l, int flags,
                          uint8_t *accept_out, float *margin_out, int *offset_out);
 /* n_passes consecutive passes first_pass .. first_pass + n_passes - 1, bit-identical to calling
- * dsmc_sublattice_pass pass by pass with the same flags.  When L/l is 1 or 2 and 40 L^2 bytes fit one
+ * dsmc_sublattice_pass pass by pass with the same flags.  When L/l is 1, 2 or 4 and 40 L^2 bytes fit one
  * CTA's shared memory (L <= 74; the paper's L = 64, l = 32) and the FFT field is not selected, one CTA
  * per replica pair keeps spins and W in shared memory and runs all passes inside one kernel; otherwise
  * (or with DSMC_NO_RESIDENT) long runs are replayed from a captured CUDA graph whose kernels recompute

@@ -148,7 +148,7 @@ void dsmc_sublattice_offset(uint64_t seed, uint64_t pass, int l, int *ox, int *o
 cudaError_t launch_sublattice_pass(const MetropolisArgs &a, const float *Wc, float *scratch, int sm_count, int l, int ox,
                                    int oy, bool field_in_H, cudaStream_t st, uint64_t *launches);
 // the same schedule with the lattice resident in shared memory: one CTA per replica pair runs all n_passes passes
-// (sublattice_kernels.cu); L/l in {1, 2} and 40 L^2 bytes within one CTA's shared memory
+// (sublattice_kernels.cu); L/l in {1, 2, 4} and 40 L^2 bytes within one CTA's shared memory
 bool dsmc_resident_supported(int L, int l);
 cudaError_t launch_sublattice_resident(const MetropolisArgs &a, const float *Wc, int l, uint64_t first_pass, uint64_t n_passes,
                                        cudaStream_t st, uint64_t *launches);

@@ -1,6 +1,6 @@
 // sublattice_kernels.cu -- the paper's own update schedule (section 3.1, App. A):
 // stride-l sub-lattice passes, as two launches per pass (any shape) and with the lattice resident in shared
-// memory for the whole run (L/l in {1, 2}, L <= 74: the paper's L = 64, l = 32).
+// memory for the whole run (L/l in {1, 2, 4}, L <= 74: the paper's L = 64, l = 32).
 #include "metropolis_common.cuh"
 #include "packed_f32x2.cuh"
 #include <algorithm>
@@ -162,7 +162,9 @@ __global__ void __launch_bounds__(128) sublattice_flip_kernel(const MetropolisAr
 //   * one extra warp draws while the others sum: lanes < 2n run Philox for (site, replica, pass) and the
 //     trial spin, lane 31 runs the same Philox code on the offset counter of the NEXT pass (no divergence),
 //     so after the barrier only the 8-term sums, dE and the store of an accepted spin remain.
-// Needs L/l in {1, 2} and 40 N bytes + partials within the 227 KB of one CTA (L <= 74).
+//   * L/l = 4 (n = 16): the 16 W entries of a coset stay in registers and its 16 sources are streamed against all 16
+//     targets; every lane of the drawing warp then has a site, so lane 0 draws the next offset with a second call.
+// Needs L/l in {1, 2, 4} and 40 N bytes + partials within the 227 KB of one CTA (L <= 74).
 #ifndef DSMC_RES_WARPS
 #define DSMC_RES_WARPS 8
 #endif
@@ -248,6 +250,41 @@ __global__ void __launch_bounds__(kResThreads, 1) sublattice_resident_kernel(con
             f2 acc[NN][3];
 #pragma unroll
             for (int k = 0; k < NN; ++k) acc[k][0] = acc[k][1] = acc[k][2] = f2_bc(0.0f);
+            if constexpr (NL > 2) {
+                // n = NL^2 > 4 update sites: the NL^2 distinct W entries of a coset stay in registers and its sources are
+                // streamed one at a time against all n targets (3 LDS.64 per 5 n FFMA2)
+                for (int c = tid; c < l * l; c += 32 * kResSumWarps) {
+                    const int cy = c / l, cx = c - cy * l;
+                    int dx[NL], dy[NL];
+                    dx[0] = cx - ox + (cx < ox ? L : 0);
+                    dy[0] = cy - oy + (cy < oy ? L : 0);
+#pragma unroll
+                    for (int u = 1; u < NL; ++u) {
+                        dx[u] = dx[u - 1] + l - (dx[u - 1] + l >= L ? L : 0);
+                        dy[u] = dy[u - 1] + l - (dy[u - 1] + l >= L ? L : 0);
+                    }
+                    float4 w[NL][NL];
+#pragma unroll
+                    for (int v = 0; v < NL; ++v)
+#pragma unroll
+                        for (int u = 0; u < NL; ++u) w[v][u] = Wsm[dy[v] * L + dx[u]];
+                    const f2 *src0 = Ssm + 3 * (cy * L + cx);
+#pragma unroll
+                    for (int b = 0; b < NL; ++b)
+#pragma unroll
+                        for (int a = 0; a < NL; ++a) {
+                            const f2 *src = src0 + 3 * (b * l * L + a * l);
+                            const f2 ax = src[0], ay = src[1], az = src[2];
+#pragma unroll
+                            for (int k = 0; k < NN; ++k) {
+                                const float4 ww = w[(b - k / NL + NL) % NL][(a - k % NL + NL) % NL];
+                                acc[k][0] = f2_fma(f2_bc(ww.x), ax, f2_fma(f2_bc(ww.y), ay, acc[k][0]));
+                                acc[k][1] = f2_fma(f2_bc(ww.y), ax, f2_fma(f2_bc(ww.z), ay, acc[k][1]));
+                                acc[k][2] = f2_fma(f2_bc(ww.w), az, acc[k][2]);
+                            }
+                        }
+                }
+            } else {
             // UN cosets per trip, all their loads issued before the first FMA.  Measured (us per pass at L = 64,
             // l = 32 / l = 64, run-time trip count): NL = 2 with UN = 1: 1.66, UN = 2: 1.70; NL = 1 with UN = 4: 1.36,
             // UN = 8: 1.29.  With the trip count (CPT) and the lattice size (LC) as template parameters: 1.46 / 1.10.
@@ -301,9 +338,20 @@ __global__ void __launch_bounds__(kResThreads, 1) sublattice_resident_kernel(con
                                 acc[k][2] = f2_fma(f2_bc(ww.w), az, acc[k][2]);
                             }
             }
+            }
             // warp reduction of the 3 NN packed values in fixed order
             f2 *v = &acc[0][0];
-            if constexpr (NL == 2) {
+            if constexpr (NL == 4) {
+                halve_exchange<48>(v, lane, 16);
+                halve_exchange<24>(v, lane, 8);
+                halve_exchange<12>(v, lane, 4);
+                halve_exchange<6>(v, lane, 2);
+                butterfly_sum<3>(v, 1);
+                if ((lane & 1) == 0) {                         // lane bits 4 .. 1 say which 3 of the 48 values it holds
+#pragma unroll
+                    for (int i = 0; i < 3; ++i) part[warp * 48 + (lane >> 1) * 3 + i] = v[i];
+                }
+            } else if constexpr (NL == 2) {
                 halve_exchange<12>(v, lane, 16);
                 halve_exchange<6>(v, lane, 8);
                 butterfly_sum<3>(v, 4);
@@ -324,13 +372,16 @@ __global__ void __launch_bounds__(kResThreads, 1) sublattice_resident_kernel(con
             nt = yt * L + xt;
             uint4 ctr = make_uint4((uint32_t)nt, (uint32_t)fr + p.r_off, (uint32_t)(pass & 0xFFFFFFFFull),
                                    (uint32_t)(pass >> 32) & 0x7FFFFFFFu);
-            if (lane == 31)
+            if (2 * NN < 32 && lane == 31)
                 ctr = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, (uint32_t)((pass + 1) & 0xFFFFFFFFull),
                                  (uint32_t)((pass + 1) >> 32) & 0x7FFFFFFFu);
             const uint4 rnd = philox4x32_10(ctr, rk);
-            if (lane == 31) {
+            if (2 * NN < 32 && lane == 31) {
                 off[2 * (cur ^ 1)] = (int)(rnd.x % (uint32_t)l);
                 off[2 * (cur ^ 1) + 1] = (int)(rnd.y % (uint32_t)l);
+            }
+            if constexpr (2 * NN >= 32) {                      // every lane has a site: lane 0 draws the next offset as well
+                if (lane == 0) pass_offset(rk, pass + 1, l, off[2 * (cur ^ 1)], off[2 * (cur ^ 1) + 1]);
             }
             if (flipper) {
                 const int xe = xt + 1 == L ? 0 : xt + 1, xw = xt == 0 ? L - 1 : xt - 1;
@@ -412,7 +463,7 @@ cudaError_t launch_sublattice_pass(const MetropolisArgs &a, const float *Wc, flo
 
 bool dsmc_resident_supported(int L, int l) {
     const int nl = L / l;
-    return (nl == 1 || nl == 2) && resident_smem_bytes(L, nl) <= 227 * 1024;
+    return (nl == 1 || nl == 2 || nl == 4) && resident_smem_bytes(L, nl) <= 227 * 1024;
 }
 
 cudaError_t launch_sublattice_resident(const MetropolisArgs &a, const float *Wc, int l, uint64_t first_pass, uint64_t n_passes,
@@ -424,6 +475,7 @@ cudaError_t launch_sublattice_resident(const MetropolisArgs &a, const float *Wc,
     const int un = nl == 2 ? 1 : 8, trips = (l * l + un * 32 * kResSumWarps - 1) / (un * 32 * kResSumWarps);
     void (*kern)(const MetropolisArgs, const RoundKeys, const float *, int, unsigned long long, unsigned) = nullptr;
     if (nl == 2) kern = a.L == 64 ? sublattice_resident_kernel<2, 4, 64> : trips == 4 ? sublattice_resident_kernel<2, 4, 0> : trips == 1 ? sublattice_resident_kernel<2, 1, 0> : sublattice_resident_kernel<2, 0, 0>;
+    else if (nl == 4) kern = a.L == 64 ? sublattice_resident_kernel<4, 0, 64> : sublattice_resident_kernel<4, 0, 0>;
     else kern = a.L == 64 ? sublattice_resident_kernel<1, 2, 64> : trips == 2 ? sublattice_resident_kernel<1, 2, 0> : trips == 1 ? sublattice_resident_kernel<1, 1, 0> : sublattice_resident_kernel<1, 0, 0>;
     if (cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024)) return e;
     const unsigned grid = (unsigned)((a.R + 1) / 2);

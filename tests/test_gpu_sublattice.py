@@ -65,11 +65,11 @@ def lockstep_passes(m, oracle, ctx, W, T, J, g, K2, K4, seed, l, n_passes, flip=
     (64, 40, 2, 6, False, True), (16, 3, 16, 12, False, True), (64, 16, 32, 48, True, True), (32, 8, 8, 24, True, True),
     (32, 6, 2, 8, True, True), (8, 1, 4, 40, False, False), (64, 16, 32, 24, False, False), (16, 3, 16, 12, False, False),
     (12, 5, 6, 24, False, True), (74, 2, 37, 12, False, True), (64, 3, 64, 12, False, True),
-    (64, 296, 32, 6, False, True), (4, 2, 2, 16, False, True), (6, 1, 3, 16, False, True), (6, 2, 6, 16, False, True)])
+    (64, 296, 32, 6, False, True), (64, 16, 16, 24, False, True), (64, 16, 16, 8, False, False), (4, 2, 2, 16, False, True), (6, 1, 3, 16, False, True), (6, 2, 6, 16, False, True)])
 def test_sublattice_lockstep(dsmc_mod, oracle, L, R, l, passes, fft, resident):
     """(64, 16, 32) is the paper's own choice L = 64, l = 32; l = 2 is the densest
     schedule (n = N/4), l = L the conventional single-spin limit; R = 40 spans two replica chunks.
-    With L/l in {1, 2} and L <= 74 (and no FFT field) the pass runs in the shared-memory-resident kernel
+    With L/l in {1, 2, 4} and L <= 74 (and no FFT field) the pass runs in the shared-memory-resident kernel
     unless resident = False asks for the two-launch path: both are held to the same oracle.  (64, 296, 32) is the
     second launch configuration bench.py times (148 CTAs, one per SM); L = 4 and 6 are the smallest lattices."""
     from paper_1211_6234_b200 import inputs
@@ -218,10 +218,10 @@ def test_simultaneous_flipping_error_is_small(dsmc_mod, oracle):
 @pytest.mark.parametrize("L,R,l,fft,flip,resident", [
     (64, 16, 32, False, False, True), (64, 16, 32, True, True, True), (12, 5, 3, False, True, True),
     (32, 8, 2, True, False, True), (64, 16, 32, False, False, False), (64, 5, 32, False, True, True),
-    (16, 4, 16, False, False, True), (12, 5, 6, False, False, True)])
+    (16, 4, 16, False, False, True), (12, 5, 6, False, False, True), (64, 6, 16, False, False, True)])
 def test_sublattice_run_graph_replay_is_bit_identical(dsmc_mod, L, R, l, fft, flip, resident):
     """dsmc_sublattice_run either keeps the lattice in shared memory for the whole run (one kernel; L/l in
-    {1, 2}, L <= 74, no FFT field, resident = True) or replays a captured graph of passes whose kernels
+    {1, 2, 4}, L <= 74, no FFT field, resident = True) or replays a captured graph of passes whose kernels
     recompute the offset from a pass counter on the device: same trajectory, bit for bit, as pass-by-pass
     calls with the same flags."""
     from paper_1211_6234_b200 import inputs
