@@ -141,9 +141,10 @@ def paper_schedule(m, inputs, dev):
     step = l*l = 1024 passes.  Timed through dsmc_sublattice_run with the lattice resident in shared memory (one CTA
     per replica pair, one kernel for the whole run) and, for comparison, through the two-launches-per-pass path."""
     import torch
-    L, l, out = 64, 32, {}
-    npass = l * l
-    for name, R, flags in (("resident", 16, 0), ("resident_R296", 296, 0), ("two_launch_graph", 16, m.DSMC_NO_RESIDENT)):
+    L, out = 64, {}
+    for name, R, l, flags in (("resident", 16, 32, 0), ("resident_R296", 296, 32, 0), ("resident_l16_R296", 296, 16, 0),
+                              ("two_launch_graph", 16, 32, m.DSMC_NO_RESIDENT)):
+        npass = l * l
         ctx = m.Dsmc(L, R, J=1.0, g=0.2247, K2=1.685, K4=0.0, device=dev)
         ctx.build_tensor(m.DSMC_W_EWALD)
         ctx.set_spins(inputs.random_spins(L, R, 1))
@@ -157,7 +158,7 @@ def paper_schedule(m, inputs, dev):
         e1.record()
         torch.cuda.synchronize(dev)
         ms = e0.elapsed_time(e1) / reps
-        out[name] = {"R": R, "us_per_pass": ms * 1e3 / npass, "ms_per_mc_step": ms, "updates_per_s": L * L * R / (ms * 1e-3)}
+        out[name] = {"R": R, "l": l, "us_per_pass": ms * 1e3 / npass, "ms_per_mc_step": ms, "updates_per_s": L * L * R / (ms * 1e-3)}
         ctx.close()
     # resident kernel: one CTA = one SM sums 4 targets x 4096 sources x 5 FMA x 2 replicas per pass
     fma_clk = 4 * L * L * 5 * 2 / 128.0

@@ -308,3 +308,13 @@ def test_section4_production_run_matches_the_papers_statements(dsmc_mod):
     # a = -1 (index 0): canted at every temperature (eta far from 1), order lost across 1 ... 2.5
     assert Oz[0, iT[g["am1_Oz_loss_T_lo"]]] > 0.9 and Oz[0, iT[3.0]] < 0.15
     assert np.all(eta[0] < 0.62) and np.all(eta[0] > 0.45)
+    # north_star's checkerboard half-sweeps on the same workload (R11): the same cone angle at every point
+    # away from the first-order jump of a = 2, the same peak of M_par for a = 0 (profiles/r01_schedules.md)
+    c = section4.run(temps, chains=2, equilibrate=10000, steps=4000, every=50, seed=11, schedule="checkerboard")
+    eta_c, Mpar_c = c["mean"][:, :, 3], c["mean"][:, :, 2]
+    print("checkerboard eta - stride eta", np.round(eta_c - eta, 3))
+    away = np.ones_like(eta, dtype=bool)
+    away[2, iT[4.0]] = False
+    # measured: 0.012 on this shortened protocol (slow relaxation inside the transition windows), 0.003 on the paper's
+    assert np.max(np.abs(eta_c - eta)[away]) < 0.025, np.abs(eta_c - eta).max()
+    assert abs(Mpar_c[1, iT[4.5]] - Mpar[1, iT[4.5]]) < 0.03
