@@ -70,6 +70,42 @@ def scan(l, temps, chains, equilibrate, steps, seed, device="cuda"):
             "passes_per_s": (equilibrate + steps) * per_step / wall}
 
 
+def energy_histograms(temps, chains, equilibrate, steps, seed, l=32, bins=60, device="cuda"):
+    """Fig. 19: distribution of the energy per spin over the recorded states at a few temperatures
+    near the transition.  -> (bin centres [nT][bins], normalised counts [nT][bins])."""
+    import torch
+    from . import Dsmc, DSMC_W_EWALD, DSMC_TRIAL_FLIP
+    L, g, J = 64, 1.0, 0.85
+    nT = len(temps)
+    R = nT * chains
+    T = np.repeat(np.asarray(temps, dtype=np.float32) * g, chains)
+    ctx = Dsmc(L, R, J=J, g=g, K2=0.0, K4=0.0, device=device)
+    ctx.build_tensor(DSMC_W_EWALD)
+    s = np.zeros((R, 3, L, L), dtype=np.float32)
+    s[:, 2] = np.where(np.arange(L) % 2 == 0, 1.0, -1.0)[None, :, None]
+    ctx.set_spins(s)
+    per_step = l * l
+    ctx.sublattice_run(T, seed, 0, equilibrate * per_step, l, flags=DSMC_TRIAL_FLIP)
+    E = np.empty((steps, R))
+    for k in range(steps):
+        ctx.sublattice_run(None, seed, (equilibrate + k) * per_step, per_step, l, flags=DSMC_TRIAL_FLIP)
+        E[k] = ctx.observables()[:, 0]
+    ctx.close()
+    E = E.reshape(steps, nT, chains).transpose(1, 0, 2).reshape(nT, -1)
+    centres, counts = np.empty((nT, bins)), np.empty((nT, bins))
+    for i in range(nT):
+        h, edges = np.histogram(E[i], bins=bins)
+        centres[i], counts[i] = 0.5 * (edges[1:] + edges[:-1]), h / h.sum()
+    return centres, counts
+
+
+def count_modes(counts, smooth=5, floor=0.25):
+    """Number of local maxima of a histogram after a moving average, ignoring bumps below `floor` of the highest."""
+    c = np.convolve(counts, np.ones(smooth) / smooth, mode="same")
+    peaks = [i for i in range(1, len(c) - 1) if c[i] > c[i - 1] and c[i] >= c[i + 1] and c[i] > floor * c.max()]
+    return len(peaks)
+
+
 def peak_temperature(T, chi):
     """Location of the maximum of chi_st: vertex of the parabola through the largest sample and its neighbours."""
     i = int(np.argmax(chi))
@@ -92,10 +128,20 @@ def main():
     ap.add_argument("--steps", type=int, default=8000, help="recorded MC steps (one state per step)")
     ap.add_argument("--seed", type=int, default=0x1211B)
     ap.add_argument("--json", action="store_true")
+    ap.add_argument("--energy-histograms", action="store_true",
+                    help="Fig. 19 instead of the scan: energy distributions at script-T = .833, .85, .867, .884")
     args = ap.parse_args()
     import torch
     if not torch.cuda.is_available():
         raise SystemExit("appendix_b: no CUDA device (there is no CPU fallback)")
+    if args.energy_histograms:
+        script_T = np.array([0.833, 0.85, 0.867, 0.884])                 # PAPER.md:384 (Fig. 19); T / g = script-T / 2
+        centres, counts = energy_histograms(script_T / 2.0, 74, args.equilibrate, args.steps, args.seed)
+        for i, t in enumerate(script_T):
+            print(f"script-T = {t:.3f}: <E/N> = {np.sum(centres[i] * counts[i]):.4f}, modes = {count_modes(counts[i])}")
+            print("   E/N    " + " ".join(f"{x:7.3f}" for x in centres[i][::4]))
+            print("   P      " + " ".join(f"{x:7.4f}" for x in counts[i][::4]))
+        return
     temps = np.linspace(args.tmin, args.tmax, args.nt)
     results = [scan(l, temps, args.chains, args.equilibrate, args.steps, args.seed) for l in args.l]
     if args.json:
