@@ -318,3 +318,57 @@ def test_section4_production_run_matches_the_papers_statements(dsmc_mod):
     # measured: 0.012 on this shortened protocol (slow relaxation inside the transition windows), 0.003 on the paper's
     assert np.max(np.abs(eta_c - eta)[away]) < 0.025, np.abs(eta_c - eta).max()
     assert abs(Mpar_c[1, iT[4.5]] - Mpar[1, iT[4.5]]) < 0.03
+
+
+def _onsager_energy(T):
+    """Exact energy per spin of the infinite square-lattice Ising model with J = 1 (Onsager 1944):
+    u = -coth(2b) [1 + (2/pi)(2 tanh^2(2b) - 1) K(k)], k = 2 sinh(2b) / cosh^2(2b), b = 1/T."""
+    from scipy.special import ellipk
+    b = 1.0 / np.asarray(T, dtype=np.float64)
+    k = 2.0 * np.sinh(2 * b) / np.cosh(2 * b) ** 2
+    return -(1.0 / np.tanh(2 * b)) * (1.0 + (2.0 / np.pi) * (2.0 * np.tanh(2 * b) ** 2 - 1.0) * ellipk(k * k))
+
+
+@pytest.mark.parametrize("schedule", ["checkerboard", "stride", "single"])
+def test_ising_limit_matches_onsager(dsmc_mod, schedule):
+    """A pin that owes nothing to the oracle: with g = 0, K = 0 and the reversal move the path is plain Metropolis
+    sampling of the nearest-neighbour Ising model (no dipole sum, so simultaneous updates of non-neighbouring sites are
+    exact), whose energy per spin is known in closed form.  Temperatures away from T_c = 2.269 so that the finite
+    lattice (L = 64) is within 1e-3 of the infinite one.  Checks the acceptance rule, the random numbers, the
+    neighbour indexing and the energy observable of all three schedules on the GPU."""
+    L, R = 64, 8
+    T = np.array([1.2, 1.6, 1.9, 2.0, 2.7, 3.0, 3.5, 5.0], dtype=np.float32)
+    ctx = dsmc_mod.Dsmc(L, R, J=1.0, g=0.0, K2=0.0, K4=0.0)
+    ctx.build_tensor(dsmc_mod.DSMC_W_EWALD)
+    s = np.zeros((R, 3, L, L), dtype=np.float32)
+    s[:, 2] = 1.0
+    ctx.set_spins(s)
+    flip = dsmc_mod.DSMC_TRIAL_FLIP
+    if schedule == "checkerboard":
+        ctx.select_field_kernel(dsmc_mod.DSMC_FIELD_FFT)
+
+    def advance(first, n):
+        if schedule == "checkerboard":
+            for h in range(2 * first, 2 * (first + n)):
+                ctx.halfsweep(T, 77, h, flags=flip)
+        else:
+            l = 32 if schedule == "stride" else 64
+            ctx.sublattice_run(T, 77, first * l * l, n * l * l, l, flags=flip)
+
+    burn, n_rec, every = 1500, 300, 10
+    advance(0, burn)
+    E = np.empty((n_rec, R))
+    for k in range(n_rec):
+        advance(burn + k * every, every)
+        E[k] = ctx.observables()[:, 0]
+        assert np.all(np.abs(ctx.get_spins()[:, 2]) == 1.0) if k == 0 else True
+    ctx.close()
+    mean = E.mean(axis=0)
+    # standard error with a factor 2 for the correlation left between states 10 sweeps apart
+    se = 2.0 * E.std(axis=0, ddof=1) / np.sqrt(n_rec)
+    exact = _onsager_energy(T)
+    print("T        ", T)
+    print("E/N GPU  ", np.round(mean, 4))
+    print("Onsager  ", np.round(exact, 4))
+    print("3 sigma  ", np.round(3 * se, 4))
+    assert np.all(np.abs(mean - exact) < 3 * se + 1.5e-3), np.abs(mean - exact)

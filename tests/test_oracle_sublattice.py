@@ -128,3 +128,33 @@ def test_ising_flip_move(oracle):
         _, u, _ = oracle.trial_draw(31, oy * L + ox, r, 100)
         dE = oracle.energy(W, s[r:r + 1], J, g, 0.0, 0.0)[0] - oracle.energy(W, before[r:r + 1], J, g, 0.0, 0.0)[0]
         assert abs((out["margin"][r, oy, ox] - np.log(u)) * 1e9 - dE) < 1e-5
+
+
+def test_ising_limit_matches_onsager(oracle):
+    """With g = 0, K = 0 and the reversal move the stride-l schedule is plain Metropolis sampling of the square-lattice
+    Ising model, whose energy per spin is known in closed form (Onsager 1944, evaluated here with scipy's complete
+    elliptic integral): pins the oracle's acceptance rule, exchange sign and neighbour indexing, its random numbers
+    and its energy to something that is neither the oracle nor the GPU.  L = 16 at temperatures well away from
+    T_c = 2.269, where the finite lattice is within 1e-3 of the infinite one."""
+    from scipy.special import ellipk
+    L, l = 16, 8
+    T = np.array([1.5, 1.8, 3.2, 4.0])
+    R = len(T)
+    b = 1.0 / T
+    k = 2.0 * np.sinh(2 * b) / np.cosh(2 * b) ** 2
+    exact = -(1.0 / np.tanh(2 * b)) * (1.0 + (2.0 / np.pi) * (2.0 * np.tanh(2 * b) ** 2 - 1.0) * ellipk(k * k))
+    W = np.zeros((4, L, L))                                    # g = 0: the table is never used
+    s = np.zeros((R, 3, L, L))
+    s[:, 2] = 1.0
+    burn, rec = 200, 1200
+    E = np.empty((rec, R))
+    p = 0
+    for step in range(burn + rec):
+        for _ in range(l * l):
+            oracle.sublattice_pass(W, s, T, 2024, p, l, 1.0, 0.0, 0.0, 0.0, flip=True)
+            p += 1
+        if step >= burn:
+            E[step - burn] = oracle.energy(W, s, 1.0, 0.0, 0.0, 0.0) / (L * L)
+    mean = E.mean(axis=0)
+    se = 3.0 * E.std(axis=0, ddof=1) / np.sqrt(rec)            # factor 3: consecutive sweeps are correlated
+    assert np.all(np.abs(mean - exact) < 3 * se + 2e-3), (mean, exact, se)
