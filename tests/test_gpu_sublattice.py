@@ -372,3 +372,45 @@ def test_ising_limit_matches_onsager(dsmc_mod, schedule):
     print("Onsager  ", np.round(exact, 4))
     print("3 sigma  ", np.round(3 * se, 4))
     assert np.all(np.abs(mean - exact) < 3 * se + 1.5e-3), np.abs(mean - exact)
+
+
+@pytest.mark.parametrize("cfg_id", [2, 3])
+def test_checkerboard_is_unbiased_on_baseline_configs(dsmc_mod, cfg_id):
+    """north_star's checkerboard updates N/2 sites against one frozen field, the coarsest use of the paper's
+    approximation (R11).  GPU-vs-oracle parity cannot show whether that biases the physics, because the oracle
+    restates the same schedule; exact single-spin Metropolis (stride l = L, one site per pass, no approximation;
+    resident kernel) can.  BASELINE configs 2 and 3 (g = 0.1): thermal averages of E/N, m_z^2-free quantities M_par and
+    eta from 8 independent chains per temperature under each schedule must agree within 4 standard errors."""
+    from paper_1211_6234_b200 import inputs
+    c = inputs.CONFIGS[cfg_id]
+    L, chains = c["L"], 8
+    K2c, K4c = inputs.anisotropy(cfg_id)
+    Tc = inputs.temperatures(cfg_id)
+    R = c["R"] * chains
+    T, K2, K4 = np.repeat(Tc, chains), np.repeat(K2c, chains), np.repeat(K4c, chains)
+    sweeps, burn, every = (1500, 700, 10) if cfg_id == 2 else (1200, 600, 10)
+    res = {}
+    for schedule in ("checkerboard", "single"):
+        ctx = dsmc_mod.Dsmc(L, R, J=1.0, g=c["g"], K2=K2, K4=K4)
+        ctx.build_tensor(dsmc_mod.DSMC_W_EWALD)
+        ctx.set_spins(inputs.up_spins(L, R) if c["init"] == "up" else inputs.random_spins(L, R, 5))
+        if schedule == "checkerboard":
+            ctx.select_field_kernel(dsmc_mod.DSMC_FIELD_FFT)
+        ctx.ensemble_reset()
+        for k in range(0, sweeps, every):
+            if schedule == "checkerboard":
+                ctx.run(T, 21, 2 * k, 2 * every)
+            else:
+                ctx.sublattice_run(T, 21, k * L * L, every * L * L, L)
+            if k >= burn:
+                ctx.ensemble_add()
+        mean = ctx.ensemble_get()[0].reshape(c["R"], chains, 8)
+        ctx.close()
+        res[schedule] = (mean.mean(axis=1), mean.std(axis=1, ddof=1) / np.sqrt(chains))
+    (mc, sc), (ms, ss) = res["checkerboard"], res["single"]
+    for q, name in ((0, "E/N"), (2, "M_par"), (3, "eta")):
+        d = np.abs(mc[:, q] - ms[:, q])
+        tol = 4.0 * np.sqrt(sc[:, q] ** 2 + ss[:, q] ** 2) + 2e-3
+        print(name, "checkerboard", np.round(mc[:, q], 4))
+        print(name, "single-spin ", np.round(ms[:, q], 4))
+        assert np.all(d < tol), (name, d, tol)
