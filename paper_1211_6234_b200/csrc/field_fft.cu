@@ -196,17 +196,24 @@ __global__ void __launch_bounds__(512) fft_x_forward_kernel(const FftParams p) {
     float2 *tw = fsm, *buf = fsm + L;
     const int lane = threadIdx.x, t = threadIdx.y;
     const int pair = blockIdx.x * LN + lane, y = blockIdx.y, c = blockIdx.z;
-    fill_twiddles(tw, L);
-    __syncthreads();
     const size_t planeP = (size_t)L * Lh * p.P;
     const float2 *S2 = reinterpret_cast<const float2 *>(p.S);
-    for (int n2 = t; n2 < N2; n2 += 16) {
-        float2 v[16];
+    auto load_line = [&](float2 (&v)[16], int n2) {
 #pragma unroll
         for (int n1 = 0; n1 < 16; ++n1) {
             const int x = N2 * n1 + n2, q = (x + y) & 1;
             v[n1] = __ldg(S2 + (size_t)(q * 3 + c) * planeP + (size_t)(y * Lh + (x >> 1)) * p.P + pair);
         }
+    };
+    // the first sub-sequence's loads are issued before the twiddles are computed: they do not depend on them
+    float2 v0[16];
+    if (t < N2) load_line(v0, t);
+    fill_twiddles(tw, L);
+    __syncthreads();
+    if (t < N2) fwd_step1<N2>(v0, t, tw, buf, LN, lane);
+    for (int n2 = t + 16; n2 < N2; n2 += 16) {
+        float2 v[16];
+        load_line(v, n2);
         fwd_step1<N2>(v, n2, tw, buf, LN, lane);
     }
     __syncthreads();
@@ -225,11 +232,11 @@ __global__ void __launch_bounds__(512) fft_x_inverse_kernel(const FftParams p) {
     float2 *tw = fsm, *buf = fsm + L;
     const int lane = threadIdx.x, t = threadIdx.y;
     const int pair = blockIdx.x * LN + lane, y = blockIdx.y, c = blockIdx.z;
-    fill_twiddles(tw, L);
     float2 u[N2];
     const float2 *src = p.Z + ((size_t)(c * L + y) * L + N2 * t) * p.P + pair;
 #pragma unroll
     for (int k2 = 0; k2 < N2; ++k2) u[k2] = src[(size_t)k2 * p.P];
+    fill_twiddles(tw, L);
     __syncthreads();
     inv_step2<N2>(u, t, tw, buf, LN, lane);
     __syncthreads();
