@@ -165,10 +165,7 @@ __global__ void __launch_bounds__(128) sublattice_flip_kernel(const MetropolisAr
 //   * L/l = 4 (n = 16): the 16 W entries of a coset stay in registers and its 16 sources are streamed against all 16
 //     targets; every lane of the drawing warp then has a site, so lane 0 draws the next offset with a second call.
 // Needs L/l in {1, 2, 4} and 40 N bytes + partials within the 227 KB of one CTA (L <= 74).
-#ifndef DSMC_RES_WARPS
-#define DSMC_RES_WARPS 8
-#endif
-constexpr int kResSumWarps = DSMC_RES_WARPS;
+constexpr int kResSumWarps = 8;   // measured at L = 64, l = 32: 8 warps 1.67, 12 warps 1.78, 16 warps 1.98 us per pass
 constexpr int kResThreads = 32 * (kResSumWarps + 1);
 
 __host__ __device__ constexpr size_t resident_smem_bytes(int L, int NL) {
