@@ -25,12 +25,12 @@ A_VALUES = (-1.0, 0.0, 2.0)
 NAMES = ["E/N", "m_z", "M_par", "eta", "wall_density", "O_x", "O_y", "O_z"]
 
 
-def run(temps, chains, equilibrate, steps, every, seed, device="cuda", schedule="stride"):
-    """schedule: "stride" = the paper's stride-32 passes (n = 4 simultaneous sites), "single" = l = L = 64 (one site per
+def run(temps, chains, equilibrate, steps, every, seed, device="cuda", schedule="stride", stride=32):
+    """schedule: "stride" = stride-l passes (l = `stride`; the paper's l = 32 has n = 4 simultaneous sites), "single" = l = L = 64 (one site per
     pass, no approximation), "checkerboard" = north_star's half-sweeps (n = N/2 simultaneous sites, FFT field)."""
     import torch
     from . import Dsmc, DSMC_W_EWALD, DSMC_FIELD_FFT
-    L, l = 64, 32
+    L, l = 64, stride
     g = 2.0 / 8.9
     K = 7.5 * g
     nT = len(temps)
@@ -84,17 +84,18 @@ def main():
     ap.add_argument("--every", type=int, default=50, help="record a state every this many MC steps (paper: 50)")
     ap.add_argument("--seed", type=int, default=0x5EC4)
     ap.add_argument("--schedule", choices=["stride", "single", "checkerboard"], default="stride")
+    ap.add_argument("--stride", type=int, default=32, help="l of the stride schedule (divides 64; the paper: 32)")
     ap.add_argument("--json", action="store_true")
     args = ap.parse_args()
     import torch
     if not torch.cuda.is_available():
         raise SystemExit("section4: no CUDA device (there is no CPU fallback)")
     temps = np.linspace(args.tmin, args.tmax, args.nt)
-    r = run(temps, args.chains, args.equilibrate, args.steps, args.every, args.seed, schedule=args.schedule)
+    r = run(temps, args.chains, args.equilibrate, args.steps, args.every, args.seed, schedule=args.schedule, stride=args.stride)
     if args.json:
         print(json.dumps({k: (v.tolist() if isinstance(v, np.ndarray) else v) for k, v in r.items()}))
         return
-    print(f"L=64 schedule={args.schedule} script-J=8.9 script-K=15: {r['replicas']} replicas (3 a x {args.nt} script-T x {args.chains} chains), "
+    print(f"L=64 schedule={args.schedule}{args.stride if args.schedule == 'stride' else ''} script-J=8.9 script-K=15: {r['replicas']} replicas (3 a x {args.nt} script-T x {args.chains} chains), "
           f"{args.equilibrate} + {args.steps} MC steps, {r['recorded']} states recorded, {r['seconds']:.1f} s "
           f"({r['mc_steps'] / r['seconds']:.3e} MC steps/s)")
     cols = [4, 7, 3, 2]                                                   # wall density, O_z, eta, M_par
