@@ -242,6 +242,33 @@ __global__ void __launch_bounds__(512) fft_x_inverse_kernel(const FftParams p) {
     __syncthreads();
     const size_t planeP = (size_t)L * Lh * p.P;
     float2 *H2 = reinterpret_cast<float2 *>(p.H);
+    if constexpr (N2 == 16) {
+        // One colour wanted: only the 8 sub-sequences n2 of the right parity are transformed, which would leave every
+        // second t idle.  Instead the 16 t share them in pairs, t < 8 taking the even and t >= 8 the odd outputs n1 of
+        // sub-sequence n2 = par + 2 (t & 7) (a warp holds two consecutive t, so neither half diverges): one radix-2
+        // step by hand, x[2j] = F8^-1[t_k + t_{k+8}](j), x[2j+1] = F8^-1[(t_k - t_{k+8}) w^k](j), w = e^{2 pi i / 16}.
+        if (p.colour >= 0) {
+            const int par = (p.colour + y) & 1, n2 = par + 2 * (t & 7), odd = t >> 3;
+            float2 a[8];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                const float2 lo = buf[sidx<N2>(k, n2) * LN + lane], hi = buf[sidx<N2>(k + 8, n2) * LN + lane];
+                if (odd) {
+                    const float2 d = csub(lo, hi);
+                    a[k] = k == 0 ? d : k == 4 ? make_float2(-d.y, d.x) : cmul(d, make_float2(kTw32.c[2 * k], kTw32.s[2 * k]));
+                } else {
+                    a[k] = cadd(lo, hi);
+                }
+            }
+            fft_reg<8, true>(a);
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                const int x = N2 * (2 * j + odd) + n2;                 // parity of n2: colour p.colour
+                H2[(size_t)(p.colour * 3 + c) * planeP + (size_t)(y * Lh + (x >> 1)) * p.P + pair] = a[bitrev<8>(j)];
+            }
+            return;
+        }
+    }
     for (int n2 = t; n2 < N2; n2 += 16) {
         if (p.colour >= 0 && ((n2 + y) & 1) != p.colour) continue;   // x = N2 n1 + n2 has the parity of n2
         float2 v[16];
