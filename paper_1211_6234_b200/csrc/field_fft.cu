@@ -238,7 +238,33 @@ __global__ void __launch_bounds__(512) fft_x_inverse_kernel(const FftParams p) {
     for (int k2 = 0; k2 < N2; ++k2) u[k2] = src[(size_t)k2 * p.P];
     fill_twiddles(tw, L);
     __syncthreads();
-    inv_step2<N2>(u, t, tw, buf, LN, lane);
+    bool folded = false;
+    if constexpr (N2 == 16) {
+        // One colour wanted: of the N2 outputs n2 of inverse step 2 only those of parity par = (colour + y) & 1 are
+        // used below, so the step is an 8-point transform of the folded input (the same radix-2 step by hand as in the
+        // last step; par is uniform over the CTA)
+        if (p.colour >= 0) {
+            const int par = (p.colour + y) & 1;
+            float2 a[8];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                if (par) {
+                    const float2 d = csub(u[k], u[k + 8]);
+                    a[k] = k == 0 ? d : k == 4 ? make_float2(-d.y, d.x) : cmul(d, make_float2(kTw32.c[2 * k], kTw32.s[2 * k]));
+                } else {
+                    a[k] = cadd(u[k], u[k + 8]);
+                }
+            }
+            fft_reg<8, true>(a);
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                const int n2 = par + 2 * j;
+                buf[sidx<N2>(t, n2) * LN + lane] = cmul(a[bitrev<8>(j)], tw[n2 * t]);
+            }
+            folded = true;
+        }
+    }
+    if (!folded) inv_step2<N2>(u, t, tw, buf, LN, lane);
     __syncthreads();
     const size_t planeP = (size_t)L * Lh * p.P;
     float2 *H2 = reinterpret_cast<float2 *>(p.H);
