@@ -167,6 +167,8 @@ int dsmc_sublattice_run(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t f
  * workspace: one launch per sweep instead of one per kernel; the trajectory is bit-identical to
  * calling dsmc_halfsweep step by step.                                                         */
 int dsmc_run(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_step, uint64_t n_half);
+/* Same with flags: DSMC_TRIAL_FLIP (the Ising reversal move of App. B on the checkerboard half-sweeps). */
+int dsmc_run_ex(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_step, uint64_t n_half, int flags);
 
 /* a3. Observables of the current state, out[R][4] doubles in HOST memory:
  *   E/N (eq. 11 with a freshly computed full field), m_z = N^-1 sum s^z,

@@ -46,8 +46,7 @@ def scan(l, temps, chains, equilibrate, steps, seed, device="cuda"):
         if l:                                                              # stride-l passes (l = L: single-spin Metropolis)
             ctx.sublattice_run(Targ, seed, first_step * per_step, n_steps * per_step, l, flags=DSMC_TRIAL_FLIP)
         else:                                                              # checkerboard half-sweeps (north_star's schedule)
-            for h in range(2 * first_step, 2 * (first_step + n_steps)):
-                ctx.halfsweep(Targ if h == 2 * first_step else None, seed, h, flags=DSMC_TRIAL_FLIP)
+            ctx.run(Targ, seed, 2 * first_step, 2 * n_steps, flags=DSMC_TRIAL_FLIP)
 
     torch.cuda.synchronize()
     t0 = time.perf_counter()

@@ -547,11 +547,16 @@ int dsmc_sublattice_run(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t f
 }
 
 int dsmc_run(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_step, uint64_t n_half) {
+    return dsmc_run_ex(ctx, T, seed, first_step, n_half, 0);
+}
+
+int dsmc_run_ex(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_step, uint64_t n_half, int flags) {
     if (int rc = need_bound(ctx)) return rc;
+    if (flags & ~DSMC_TRIAL_FLIP) return fail(ctx, DSMC_EINVAL, "unknown flag");
     uint64_t k = 0;
     auto plain = [&](uint64_t count) -> int {
         for (uint64_t j = 0; j < count; ++j, ++k)
-            if (int rc = dsmc_halfsweep_ex(ctx, k == 0 ? T : nullptr, seed, first_step + k, 0, nullptr, nullptr)) return rc;
+            if (int rc = dsmc_halfsweep_ex(ctx, k == 0 ? T : nullptr, seed, first_step + k, flags, nullptr, nullptr)) return rc;
         return DSMC_OK;
     };
     if (n_half >= 4 + 4 * DSMC_GRAPH_UNROLL && !ctx->timing) {
@@ -560,7 +565,7 @@ int dsmc_run(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_step, 
         if (int rc = plain((first_step & 1u) + 2)) return rc;
         const uint64_t reps = (n_half - k) / (2 * DSMC_GRAPH_UNROLL);
         if (reps >= 1) {
-            if (int rc = build_sweep_graph(ctx, seed, 0)) return rc;
+            if (int rc = build_sweep_graph(ctx, seed, flags)) return rc;
             CU(launch_step_update(ctx->step_dev(), first_step + k, 0, ctx->stream, &ctx->launches), "step counter");
             for (uint64_t j = 0; j < reps; ++j) CU(cudaGraphLaunch(ctx->sweep_graph, ctx->stream), "sweep graph launch");
             ctx->launches += reps * ctx->graph_launches;

@@ -38,6 +38,7 @@ ABI = [
     ("dsmc_halfsweep", _i, [_vp, _vp, _u64, _u64]),
     ("dsmc_halfsweep_ex", _i, [_vp, _vp, _u64, _u64, _i, _vp, _vp]),
     ("dsmc_run", _i, [_vp, _vp, _u64, _u64, _u64]),
+    ("dsmc_run_ex", _i, [_vp, _vp, _u64, _u64, _u64, _i]),
     ("dsmc_sublattice_pass", _i, [_vp, _vp, _u64, _u64, _i, _i, _vp, _vp, _vp]),
     ("dsmc_sublattice_run", _i, [_vp, _vp, _u64, _u64, _u64, _i, _i]),
     ("dsmc_observables", _i, [_vp, _vp]),
@@ -203,9 +204,12 @@ class Dsmc:
         mp = margin_out.data_ptr() if margin_out is not None else None
         self._check(self.lib.dsmc_halfsweep_ex(self._h, tp, seed, step, flags, ap, mp))
 
-    def run(self, T, seed, first_step, n_half):
+    def run(self, T, seed, first_step, n_half, flags=0):
         t, tp = self._T(T)
-        self._check(self.lib.dsmc_run(self._h, tp, seed, first_step, n_half))
+        if flags == 0:
+            self._check(self.lib.dsmc_run(self._h, tp, seed, first_step, n_half))
+        else:
+            self._check(self.lib.dsmc_run_ex(self._h, tp, seed, first_step, n_half, flags))
 
     def sublattice_pass(self, T, seed, pass_index, l, flags=0, accept_out=None, margin_out=None):
         """One pass of the paper's stride-l schedule -> the offset (S_1, S_2)."""

@@ -519,13 +519,16 @@ def test_ensemble_statistics_parity(dsmc_mod, oracle, fft):
     ctx.close()
 
 
-@pytest.mark.parametrize("L,R,kind", [(32, 8, 1), (32, 8, 2), (12, 5, 0), (64, 16, 2)])
-def test_run_graph_replay_is_bit_identical(dsmc_mod, L, R, kind):
-    """dsmc_run replays a captured CUDA graph of one sweep with the step counter on the device: the
+@pytest.mark.parametrize("L,R,kind,flip", [(32, 8, 1, False), (32, 8, 2, False), (12, 5, 0, False), (64, 16, 2, False),
+                                           (32, 8, 2, True), (12, 5, 0, True)])
+def test_run_graph_replay_is_bit_identical(dsmc_mod, L, R, kind, flip):
+    """dsmc_run / dsmc_run_ex replay a captured CUDA graph of 8 sweeps with the step counter on the device: the
     trajectory must be bit-identical to calling dsmc_halfsweep step by step (odd first step, ragged
-    tail, a second run with another seed and after switching the field kernel)."""
+    tail, runs too short for the graph, a second run with another seed and after switching the field kernel;
+    flip = the reversal move through dsmc_run_ex)."""
     from paper_1211_6234_b200 import inputs
     T = np.linspace(0.3, 1.5, R).astype(np.float32)
+    flags = dsmc_mod.DSMC_TRIAL_FLIP if flip else 0
     a = dsmc_mod.Dsmc(L, R, J=1.0, g=0.2, K2=0.5, K4=0.1)
     b = dsmc_mod.Dsmc(L, R, J=1.0, g=0.2, K2=0.5, K4=0.1)
     a.build_tensor(dsmc_mod.DSMC_W_EWALD)
@@ -533,17 +536,17 @@ def test_run_graph_replay_is_bit_identical(dsmc_mod, L, R, kind):
     for ctx in (a, b):
         ctx.select_field_kernel(kind)
         ctx.set_spins(inputs.random_spins(L, R, 3))
-    for (seed, first, n) in ((11, 7, 25), (12, 100, 16), (12, 116, 9)):
-        a.run(T, seed, first, n)
+    for (seed, first, n) in ((11, 7, 75), (12, 100, 52), (12, 152, 9), (13, 161, 40)):
+        a.run(T, seed, first, n, flags=flags)
         for k in range(n):
-            b.halfsweep(T, seed, first + k)
+            b.halfsweep(T, seed, first + k, flags=flags)
         assert np.array_equal(a.get_spins(), b.get_spins()), (seed, first, n)
     if kind == 2:                                               # the graph is rebuilt when the kernel changes
         for ctx in (a, b):
             ctx.select_field_kernel(dsmc_mod.DSMC_FIELD_AUTO)
-        a.run(T, 12, 200, 12)
-        for k in range(12):
-            b.halfsweep(T, 12, 200 + k)
+        a.run(T, 12, 300, 44, flags=flags)
+        for k in range(44):
+            b.halfsweep(T, 12, 300 + k, flags=flags)
         assert np.array_equal(a.get_spins(), b.get_spins())
     a.close()
     b.close()
