@@ -4,7 +4,18 @@
 #include <cstring>
 #include <new>
 
+#include <cstdlib>
+
 #include "dsmc_internal.cuh"
+
+// programmatic dependent launch of the sweep's kernels (dsmc_internal.cuh); DSMC_NO_PDL=1 turns it off
+bool dsmc_pdl_enabled() {
+    static const bool on = [] {
+        const char *v = getenv("DSMC_NO_PDL");
+        return !(v && v[0] && v[0] != '0');
+    }();
+    return on;
+}
 
 namespace {
 
@@ -143,6 +154,7 @@ MetropolisArgs metropolis_args(dsmc_ctx *ctx, int colour, uint64_t seed, uint64_
     a.step_off = 0;
     a.accept_out = accept_out;
     a.margin_out = margin_out;
+    a.pdl_late = 0;
     return a;
 }
 

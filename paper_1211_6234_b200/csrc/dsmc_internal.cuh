@@ -23,6 +23,38 @@
 #define DSMC_GRAPH_UNROLL 8  // sweeps (dsmc_run) or passes (dsmc_sublattice_run) per captured CUDA graph
 #define DSMC_KS_MAX 16  // maximum source split (partial-field slabs) of the tiled field kernel
 
+// ---------------------------------------------------------------------------------------------
+// Programmatic dependent launch (sm_90+).  The kernels of a sweep form one dependent chain (x-forward -> y-multiply ->
+// x-inverse -> Metropolis -> step counter -> ...) and the small lattices are bound by the ~3 us a kernel-to-kernel edge
+// costs.  A kernel launched through launch_pdl calls pdl_wait() before it touches memory an earlier kernel wrote or
+// read -- it returns once the predecessor grid has completed and its writes are visible; every kernel launched this way
+// calls it, so completion is transitive along the chain -- and pdl_trigger() once its CTA is past the bulk of its work:
+// when every CTA of the grid has triggered (or exited) the successor's CTAs are scheduled into the room that frees
+// up and wait there, so the launch latency of the edge overlaps this grid's tail.  (Triggering at the top instead
+// makes the successor resident while this grid still needs the room: measured slower from L = 128 up, DESIGN.md
+// section 5.2b.)  A kernel launched with <<<>>> keeps plain stream order on both sides.  DSMC_NO_PDL=1 in the
+// environment drops the attribute (A/B timing).
+// ---------------------------------------------------------------------------------------------
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+bool dsmc_pdl_enabled();
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args &&...args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = dsmc_pdl_enabled() ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
+#endif
+
 struct DsmcLayout {
     size_t off_Wc;     // canonical W fp32 [4][L][L]
     size_t off_Wk;     // kernel-layout W for the tiled field kernel
@@ -139,6 +171,8 @@ struct MetropolisArgs {
     uint32_t step_off;
     uint8_t *accept_out;  // canonical [R][L][L] or null
     float *margin_out;    // canonical [R][L][L] or null
+    int pdl_late;  // where the kernel lets its successor be scheduled (set by the launcher): 1 = after its loads and
+                   // random numbers (grids of at most one wave), 0 = at its top (larger grids)
 };
 cudaError_t launch_metropolis(const MetropolisArgs &a, cudaStream_t st, uint64_t *launches);
 // the paper's stride-l sub-lattice pass: offset (ox, oy) in [0, l)^2, n = (L/l)^2 update sites

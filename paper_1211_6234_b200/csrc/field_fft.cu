@@ -205,7 +205,9 @@ __global__ void __launch_bounds__(512) fft_x_forward_kernel(const FftParams p) {
             v[n1] = __ldg(S2 + (size_t)(q * 3 + c) * planeP + (size_t)(y * Lh + (x >> 1)) * p.P + pair);
         }
     };
+    // the twiddles do not depend on the spins: they are computed while the kernel that writes the spins may still run
     // the first sub-sequence's loads are issued before the twiddles are computed: they do not depend on them
+    pdl_wait();                                            // the spins come from the Metropolis kernel before
     float2 v0[16];
     if (t < N2) load_line(v0, t);
     fill_twiddles(tw, L);
@@ -217,6 +219,7 @@ __global__ void __launch_bounds__(512) fft_x_forward_kernel(const FftParams p) {
         fwd_step1<N2>(v, n2, tw, buf, LN, lane);
     }
     __syncthreads();
+    pdl_trigger();                                         // late: a successor resident earlier only takes room (section 5.2b)
     float2 u[N2];
     fwd_step2<N2>(u, t, buf, LN, lane);
     float2 *dst = p.Z + ((size_t)(c * L + y) * L + N2 * t) * p.P + pair;
@@ -234,6 +237,7 @@ __global__ void __launch_bounds__(512) fft_x_inverse_kernel(const FftParams p) {
     const int pair = blockIdx.x * LN + lane, y = blockIdx.y, c = blockIdx.z;
     float2 u[N2];
     const float2 *src = p.Z + ((size_t)(c * L + y) * L + N2 * t) * p.P + pair;
+    pdl_wait();                                            // the spectrum comes from the y pass
 #pragma unroll
     for (int k2 = 0; k2 < N2; ++k2) u[k2] = src[(size_t)k2 * p.P];
     fill_twiddles(tw, L);
@@ -265,6 +269,7 @@ __global__ void __launch_bounds__(512) fft_x_inverse_kernel(const FftParams p) {
         }
     }
     if (!folded) inv_step2<N2>(u, t, tw, buf, LN, lane);
+    pdl_trigger();
     __syncthreads();
     const size_t planeP = (size_t)L * Lh * p.P;
     float2 *H2 = reinterpret_cast<float2 *>(p.H);
@@ -323,7 +328,8 @@ __global__ void __launch_bounds__(256, 2) fft_y_multiply_kernel(const FftParams 
     const int lane = threadIdx.x, t = threadIdx.y;
     const int pair = blockIdx.x * LN + lane, sx = blockIdx.y;
     fill_twiddles(tw, L);
-    for (int j = t * LN + lane; j < 2 * L; j += 16 * LN) Msm[j] = __ldg(p.M + (size_t)sx * L * 2 + j);
+    for (int j = t * LN + lane; j < 2 * L; j += 16 * LN) Msm[j] = __ldg(p.M + (size_t)sx * L * 2 + j);  // constant table
+    pdl_wait();                                            // the spectrum comes from the x pass
     __syncthreads();
     const size_t rowP = (size_t)L * p.P;                   // one y step in Z
     float2 *col = p.Z + (size_t)sx * p.P + pair;           // + (c * L + y) * rowP
@@ -368,6 +374,7 @@ __global__ void __launch_bounds__(256, 2) fft_y_multiply_kernel(const FftParams 
         inv_step2<N2>(ux, t, tw, buf[2], LN, lane);
     }
     __syncthreads();
+    pdl_trigger();
 #pragma unroll 1
     for (int c = 0; c < 3; ++c)
         for (int n2 = t; n2 < N2; n2 += 16) {
@@ -439,9 +446,9 @@ cudaError_t launch_fft_n2(const FftParams &p, cudaStream_t st, uint64_t *launche
         if ((e = cudaFuncSetAttribute(fft_y_multiply_kernel<N2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024)) != cudaSuccess) return e;
         configured = true;
     }
-    fft_x_forward_kernel<N2><<<dim3(p.P / LNX, L, 3), dim3(LNX, 16), smx, st>>>(p);
-    fft_y_multiply_kernel<N2><<<dim3(p.P / LNY, L), dim3(LNY, 16), smy, st>>>(p);
-    fft_x_inverse_kernel<N2><<<dim3(p.P / LNX, L, 3), dim3(LNX, 16), smx, st>>>(p);
+    launch_pdl(fft_x_forward_kernel<N2>, dim3(p.P / LNX, L, 3), dim3(LNX, 16), smx, st, p);
+    launch_pdl(fft_y_multiply_kernel<N2>, dim3(p.P / LNY, L), dim3(LNY, 16), smy, st, p);
+    launch_pdl(fft_x_inverse_kernel<N2>, dim3(p.P / LNX, L, 3), dim3(LNX, 16), smx, st, p);
     *launches += 3;
     return cudaGetLastError();
 }

@@ -105,7 +105,9 @@ __global__ void __launch_bounds__(128, 7) metropolis4_kernel(const MetropolisArg
     const int y = blockIdx.y;
     const uint32_t row4 = (uint32_t)(Lh * RQ);
     const uint32_t e = blockIdx.x * blockDim.x + threadIdx.x;   // (i, replica quad) within the row
+    if (!p.pdl_late) pdl_trigger();
     if (e >= row4) return;
+    pdl_wait();                                                 // spins, field and step counter come from earlier kernels
     const int i = p.rq_shift >= 0 ? (int)(e >> p.rq_shift) : (int)(e / (uint32_t)RQ);
     const int rq = (int)e - i * RQ;
     const int par = (y + p.colour) & 1;
@@ -156,6 +158,7 @@ __global__ void __launch_bounds__(128, 7) metropolis4_kernel(const MetropolisArg
 #pragma unroll
     for (int k = 0; k < 4; ++k) rnd[k] = philox4x32_10(make_uint4(n, r0 + p.r_off + k, step_lo, step_hi), rk);
 
+    if (p.pdl_late) pdl_trigger();
     bool any = false;
     float mg[4];
 #pragma unroll
@@ -257,6 +260,8 @@ __global__ void __launch_bounds__(256) init_spins_kernel(float *__restrict__ S, 
 }
 
 __global__ void step_update_kernel(unsigned long long *step, unsigned long long value, int add) {
+    pdl_trigger();
+    pdl_wait();                                                 // the Metropolis kernel before it reads *step
     *step = add ? *step + value : value;
 }
 
@@ -275,12 +280,15 @@ cudaError_t launch_metropolis(const MetropolisArgs &a, cudaStream_t st, uint64_t
         }
         const unsigned per_row = (unsigned)((a.L / 2) * RQ);
         dim3 grid((per_row + 127) / 128, a.L);
-        if (a.accept_out || a.margin_out) metropolis4_kernel<true, false, 2><<<grid, 128, 0, st>>>(b, rk);
-        else if (a.step_dev && a.flip) metropolis4_kernel<false, true, 1><<<grid, 128, 0, st>>>(b, rk);
-        else if (a.step_dev) metropolis4_kernel<false, true, 0><<<grid, 128, 0, st>>>(b, rk);
-        else if (a.flip) metropolis4_kernel<false, false, 1><<<grid, 128, 0, st>>>(b, rk);
-        else metropolis4_kernel<false, false, 0><<<grid, 128, 0, st>>>(b, rk);
-        err = cudaGetLastError();
+        // measured: a one-wave grid gains from triggering its successor late (L = 128, R = 4:
+        // 18.9 -> 20.8 k sweeps/s), a many-wave grid from triggering at the top (L = 256, R = 64)
+        b.pdl_late = (size_t)grid.x * grid.y <= 1024 ? 1 : 0;
+        if (a.accept_out || a.margin_out) err = launch_pdl(metropolis4_kernel<true, false, 2>, grid, dim3(128), 0, st, b, rk);
+        else if (a.step_dev && a.flip) err = launch_pdl(metropolis4_kernel<false, true, 1>, grid, dim3(128), 0, st, b, rk);
+        else if (a.step_dev) err = launch_pdl(metropolis4_kernel<false, true, 0>, grid, dim3(128), 0, st, b, rk);
+        else if (a.flip) err = launch_pdl(metropolis4_kernel<false, false, 1>, grid, dim3(128), 0, st, b, rk);
+        else err = launch_pdl(metropolis4_kernel<false, false, 0>, grid, dim3(128), 0, st, b, rk);
+        if (err == cudaSuccess) err = cudaGetLastError();
     } else {
         const size_t total = (size_t)a.L * (a.L / 2) * a.R;
         metropolis1_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(a, rk);
@@ -302,7 +310,7 @@ cudaError_t launch_init_spins(float *S, int L, int R, int mode, uint64_t seed, u
 
 cudaError_t launch_step_update(unsigned long long *step, unsigned long long value, int add, cudaStream_t st,
                                uint64_t *launches) {
-    step_update_kernel<<<1, 1, 0, st>>>(step, value, add);
+    const cudaError_t err = launch_pdl(step_update_kernel, dim3(1), dim3(1), 0, st, step, value, add);
     ++*launches;
-    return cudaGetLastError();
+    return err != cudaSuccess ? err : cudaGetLastError();
 }
