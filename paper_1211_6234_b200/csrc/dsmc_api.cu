@@ -242,7 +242,7 @@ int build_pass_graph(dsmc_ctx *ctx, uint64_t seed, int l, int flags) {
     return DSMC_OK;
 }
 
-// Capture DSMC_GRAPH_UNROLL sweeps -- each field + Metropolis of colour 0, of colour 1, step counter += 2 -- as a CUDA graph
+// Capture DSMC_GRAPH_UNROLL sweeps -- each field + Metropolis of colour 0, of colour 1; then step counter += 2 UNROLL -- as a CUDA graph
 // whose Metropolis kernels read the step from the device-resident counter, so that dsmc_run replays
 // it with one launch per sweep instead of one per kernel (small lattices are launch-bound).
 int build_sweep_graph(dsmc_ctx *ctx, uint64_t seed, int flags) {
@@ -264,13 +264,13 @@ int build_sweep_graph(dsmc_ctx *ctx, uint64_t seed, int flags) {
                 if (rc != DSMC_OK) break;
                 MetropolisArgs a = metropolis_args(ctx, colour, seed, 0, flags, nullptr, nullptr);
                 a.step_dev = ctx->step_dev();
-                a.step_off = (uint32_t)colour;
+                a.step_off = (uint32_t)(2 * rep + colour);  // the counter moves once per graph, not once per sweep
                 e = launch_metropolis(a, ctx->stream, &ctx->launches);
                 if (e != cudaSuccess) break;
             }
-            if (e == cudaSuccess && rc == DSMC_OK)
-                e = launch_step_update(ctx->step_dev(), 2, 1, ctx->stream, &ctx->launches);
         }
+        if (e == cudaSuccess && rc == DSMC_OK)
+            e = launch_step_update(ctx->step_dev(), 2 * DSMC_GRAPH_UNROLL, 1, ctx->stream, &ctx->launches);
         cudaError_t e2 = cudaStreamEndCapture(ctx->capture_stream, &graph);
         if (e == cudaSuccess) e = e2;
     }
