@@ -580,3 +580,41 @@ def test_sharded_ladder_is_bit_identical(dsmc_mod):
         assert np.array_equal(part.get_spins(), ref[lo:hi]), (lo, hi)
         part.close()
     whole.close()
+
+
+_PDL_AB_SCRIPT = """
+import hashlib, sys
+import numpy as np
+import paper_1211_6234_b200 as m
+L, R, graph = int(sys.argv[1]), int(sys.argv[2]), int(sys.argv[3])
+T = np.linspace(0.3, 1.7, R).astype(np.float32)
+ctx = m.Dsmc(L, R, J=1.0, g=0.2, K2=np.full(R, 0.6, np.float32), K4=np.full(R, 0.1, np.float32))
+ctx.build_tensor(m.DSMC_W_EWALD)
+ctx.select_field_kernel(m.DSMC_FIELD_FFT)
+ctx.init_spins(m.DSMC_INIT_RANDOM, seed=5)
+if graph:
+    ctx.run(T, 31, 0, 120)                       # bulk replayed from the captured graph
+else:
+    for k in range(60):
+        ctx.halfsweep(T if k == 0 else None, 31, k)
+print(hashlib.sha256(np.ascontiguousarray(ctx.get_spins()).tobytes()).hexdigest())
+"""
+
+
+@pytest.mark.parametrize("L,R,graph", [(32, 8, 0), (32, 8, 1), (64, 16, 1), (128, 4, 1), (256, 8, 0)])
+def test_dependent_launch_is_bit_identical(L, R, graph):
+    """the kernels of a sweep are chained by programmatic dependent launches; each waits for its
+    predecessor before it touches shared state, so nothing but the launch overlaps.  A missing or misplaced wait shows up as a
+    race on spins, field, spectrum scratch or step counter: the same run with plain launches (DSMC_NO_PDL=1, read once
+    per process, hence the subprocesses) must leave the same spins to the last bit -- launch by launch and through
+    the replayed graph, on one-wave and many-wave grids."""
+    import os, subprocess, sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    digest = []
+    for no_pdl in ("0", "1"):
+        env = dict(os.environ, DSMC_NO_PDL=no_pdl)
+        p = subprocess.run([sys.executable, "-c", _PDL_AB_SCRIPT, str(L), str(R), str(graph)], cwd=root, env=env,
+                           capture_output=True, text=True, timeout=600)
+        assert p.returncode == 0, p.stderr[-2000:]
+        digest.append(p.stdout.strip().splitlines()[-1])
+    assert len(digest[0]) == 64 and digest[0] == digest[1]
