@@ -204,6 +204,13 @@ int dsmc_staggered_magnetisation(dsmc_ctx *ctx, double *out);
  * arrays, <x>, sigma^2(x) = <x^2> - <x>^2 (eq. 18) and SE = (sigma^2 / n)^(1/2) (eq. 13) over the n
  * snapshots added since dsmc_ensemble_reset (n_out nullable); DSMC_ESTATE if n = 0.  Synchronises.      */
 int dsmc_ensemble_reset(dsmc_ctx *ctx);
+/* The paper's recording protocol as one call ("the state of the system was recorded every 50 steps"):
+ * n_records times [every whole sweeps, then dsmc_ensemble_add], starting at the even step first_step (T as in
+ * dsmc_halfsweep: HOST [R] or null to keep the last).  The trajectory and the statistics are those of the
+ * equivalent dsmc_run / dsmc_ensemble_add calls; for every <= 16 the sweeps and the record are replayed from one
+ * captured CUDA graph per record.  Asynchronous.  DSMC_EINVAL for every < 1, an odd first_step or an unknown flag. */
+int dsmc_run_recorded(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_step, uint64_t n_records, int every,
+                      int flags);
 int dsmc_ensemble_add(dsmc_ctx *ctx);
 int dsmc_ensemble_get(dsmc_ctx *ctx, double *mean, double *var, double *se, uint64_t *n_out);
 

@@ -242,12 +242,29 @@ int build_pass_graph(dsmc_ctx *ctx, uint64_t seed, int l, int flags) {
     return DSMC_OK;
 }
 
-// Capture DSMC_GRAPH_UNROLL sweeps -- each field + Metropolis of colour 0, of colour 1; then step counter += 2 UNROLL -- as a CUDA graph
+// the kernels of dsmc_ensemble_add: full field of the current state, raw sums, wall counts, running statistics
+int enqueue_record(dsmc_ctx *ctx) {
+    if (int rc = run_field(ctx, -1)) return rc;
+    CU(launch_observables(ctx->S(), ctx->H(), ctx->K2d(), ctx->K4d(), ctx->obs(), ctx->L, ctx->R, ctx->J, ctx->g,
+                          ctx->stream, &ctx->launches),
+       "observables launch");
+    CU(launch_wall_counts(ctx->S(), ctx->walls(), ctx->L, ctx->R, ctx->stream, &ctx->launches), "wall counts launch");
+    CU(launch_ensemble_add(ctx->obs(), ctx->walls(), ctx->stats(), ctx->L, ctx->R, (double)ctx->J, (double)ctx->g,
+                           ctx->stream, &ctx->launches),
+       "ensemble launch");
+    return DSMC_OK;
+}
+
+// Capture n sweeps -- each field + Metropolis of colour 0, of colour 1; then step counter += 2 n -- as a CUDA graph
 // whose Metropolis kernels read the step from the device-resident counter, so that dsmc_run replays
 // it with one launch per sweep instead of one per kernel (small lattices are launch-bound).
-int build_sweep_graph(dsmc_ctx *ctx, uint64_t seed, int flags) {
+// record_every = 0: n = DSMC_GRAPH_UNROLL (dsmc_run); > 0: n = record_every sweeps followed by the kernels of
+// dsmc_ensemble_add (dsmc_run_recorded).
+int build_sweep_graph(dsmc_ctx *ctx, uint64_t seed, int flags, int record_every) {
     const int kind = field_kind(ctx);
-    if (ctx->sweep_graph && ctx->graph_seed == seed && ctx->graph_kind == kind && ctx->graph_flags == flags) return DSMC_OK;
+    if (ctx->sweep_graph && ctx->graph_seed == seed && ctx->graph_kind == kind && ctx->graph_flags == flags &&
+        ctx->graph_every == record_every)
+        return DSMC_OK;
     drop_sweep_graph(ctx);
     if (!ctx->capture_stream)
         CU(cudaStreamCreateWithFlags(&ctx->capture_stream, cudaStreamNonBlocking), "capture stream");
@@ -258,7 +275,8 @@ int build_sweep_graph(dsmc_ctx *ctx, uint64_t seed, int flags) {
     cudaError_t e = cudaStreamBeginCapture(ctx->capture_stream, cudaStreamCaptureModeThreadLocal);
     int rc = DSMC_OK;
     if (e == cudaSuccess) {
-        for (int rep = 0; rep < DSMC_GRAPH_UNROLL && rc == DSMC_OK && e == cudaSuccess; ++rep) {
+        const int n_sweeps = record_every > 0 ? record_every : DSMC_GRAPH_UNROLL;
+        for (int rep = 0; rep < n_sweeps && rc == DSMC_OK && e == cudaSuccess; ++rep) {
             for (int colour = 0; colour < 2 && rc == DSMC_OK; ++colour) {
                 rc = run_field(ctx, colour);
                 if (rc != DSMC_OK) break;
@@ -270,7 +288,8 @@ int build_sweep_graph(dsmc_ctx *ctx, uint64_t seed, int flags) {
             }
         }
         if (e == cudaSuccess && rc == DSMC_OK)
-            e = launch_step_update(ctx->step_dev(), 2 * DSMC_GRAPH_UNROLL, 1, ctx->stream, &ctx->launches);
+            e = launch_step_update(ctx->step_dev(), 2 * (uint64_t)n_sweeps, 1, ctx->stream, &ctx->launches);
+        if (e == cudaSuccess && rc == DSMC_OK && record_every > 0) rc = enqueue_record(ctx);
         cudaError_t e2 = cudaStreamEndCapture(ctx->capture_stream, &graph);
         if (e == cudaSuccess) e = e2;
     }
@@ -294,6 +313,7 @@ int build_sweep_graph(dsmc_ctx *ctx, uint64_t seed, int flags) {
     ctx->graph_seed = seed;
     ctx->graph_kind = kind;
     ctx->graph_flags = flags;
+    ctx->graph_every = record_every;
     return DSMC_OK;
 }
 
@@ -577,7 +597,7 @@ int dsmc_run_ex(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_ste
         if (int rc = plain((first_step & 1u) + 2)) return rc;
         const uint64_t reps = (n_half - k) / (2 * DSMC_GRAPH_UNROLL);
         if (reps >= 1) {
-            if (int rc = build_sweep_graph(ctx, seed, flags)) return rc;
+            if (int rc = build_sweep_graph(ctx, seed, flags, 0)) return rc;
             CU(launch_step_update(ctx->step_dev(), first_step + k, 0, ctx->stream, &ctx->launches), "step counter");
             for (uint64_t j = 0; j < reps; ++j) CU(cudaGraphLaunch(ctx->sweep_graph, ctx->stream), "sweep graph launch");
             ctx->launches += reps * ctx->graph_launches;
@@ -671,15 +691,42 @@ int dsmc_ensemble_add(dsmc_ctx *ctx) {
     if (!ctx->tensor_built) return fail(ctx, DSMC_ESTATE, "tensor not built");
     if (!ctx->spins_set) return fail(ctx, DSMC_ESTATE, "spins not set");
     if (int rc = upload_params(ctx, ctx->T_valid ? nullptr : std::vector<float>(ctx->R, 1.0f).data())) return rc;
-    if (int rc = run_field(ctx, -1)) return rc;
-    CU(launch_observables(ctx->S(), ctx->H(), ctx->K2d(), ctx->K4d(), ctx->obs(), ctx->L, ctx->R, ctx->J, ctx->g,
-                          ctx->stream, &ctx->launches),
-       "observables launch");
-    CU(launch_wall_counts(ctx->S(), ctx->walls(), ctx->L, ctx->R, ctx->stream, &ctx->launches), "wall counts launch");
-    CU(launch_ensemble_add(ctx->obs(), ctx->walls(), ctx->stats(), ctx->L, ctx->R, (double)ctx->J, (double)ctx->g,
-                           ctx->stream, &ctx->launches),
-       "ensemble launch");
+    if (int rc = enqueue_record(ctx)) return rc;
     ++ctx->ensemble_n;
+    return DSMC_OK;
+}
+
+int dsmc_run_recorded(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_step, uint64_t n_records, int every,
+                      int flags) {
+    if (int rc = need_bound(ctx)) return rc;
+    if (flags & ~DSMC_TRIAL_FLIP) return fail(ctx, DSMC_EINVAL, "unknown flag");
+    if (every < 1) return fail(ctx, DSMC_EINVAL, "every must be >= 1");
+    if (first_step & 1u) return fail(ctx, DSMC_EINVAL, "first_step must be even (whole sweeps)");
+    uint64_t done = 0;
+    auto plain = [&]() -> int {                                  // one record launch by launch
+        if (int rc = dsmc_run_ex(ctx, done == 0 ? T : nullptr, seed, first_step + 2 * (uint64_t)every * done,
+                                 2 * (uint64_t)every, flags))
+            return rc;
+        ++done;
+        return dsmc_ensemble_add(ctx);
+    };
+    if (n_records == 0) return T ? upload_params(ctx, T) : DSMC_OK;
+    // the first record runs plainly (uploads T, configures every kernel before a capture); short spacings are then
+    // replayed from a graph of `every` sweeps + the record; long ones go through dsmc_run's own graph
+    if (int rc = plain()) return rc;
+    if (every <= 2 * DSMC_GRAPH_UNROLL && n_records - done >= 4 && !ctx->timing) {
+        if (int rc = build_sweep_graph(ctx, seed, flags, every)) return rc;
+        const uint64_t reps = n_records - done;
+        CU(launch_step_update(ctx->step_dev(), first_step + 2 * (uint64_t)every * done, 0, ctx->stream, &ctx->launches),
+           "step counter");
+        for (uint64_t j = 0; j < reps; ++j) CU(cudaGraphLaunch(ctx->sweep_graph, ctx->stream), "record graph launch");
+        ctx->launches += reps * ctx->graph_launches;
+        ctx->field_valid[0] = ctx->field_valid[1] = true;
+        ctx->ensemble_n += reps;
+        done += reps;
+    }
+    while (done < n_records)
+        if (int rc = plain()) return rc;
     return DSMC_OK;
 }
 

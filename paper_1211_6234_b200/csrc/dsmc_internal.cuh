@@ -95,7 +95,7 @@ struct dsmc_ctx {
     cudaStream_t capture_stream = nullptr;
     cudaGraphExec_t sweep_graph = nullptr;
     uint64_t graph_seed = 0;
-    int graph_kind = -1, graph_flags = -1;
+    int graph_kind = -1, graph_flags = -1, graph_every = -1;  // graph_every > 0: sweeps + record (dsmc_run_recorded)
     uint64_t graph_launches = 0;
     // one stride-l pass (field + flip + pass counter += 1) for dsmc_sublattice_run
     cudaGraphExec_t pass_graph = nullptr;

@@ -39,6 +39,7 @@ ABI = [
     ("dsmc_halfsweep_ex", _i, [_vp, _vp, _u64, _u64, _i, _vp, _vp]),
     ("dsmc_run", _i, [_vp, _vp, _u64, _u64, _u64]),
     ("dsmc_run_ex", _i, [_vp, _vp, _u64, _u64, _u64, _i]),
+    ("dsmc_run_recorded", _i, [_vp, _vp, _u64, _u64, _u64, _i, _i]),
     ("dsmc_sublattice_pass", _i, [_vp, _vp, _u64, _u64, _i, _i, _vp, _vp, _vp]),
     ("dsmc_sublattice_run", _i, [_vp, _vp, _u64, _u64, _u64, _i, _i]),
     ("dsmc_observables", _i, [_vp, _vp]),
@@ -210,6 +211,11 @@ class Dsmc:
             self._check(self.lib.dsmc_run(self._h, tp, seed, first_step, n_half))
         else:
             self._check(self.lib.dsmc_run_ex(self._h, tp, seed, first_step, n_half, flags))
+
+    def run_recorded(self, T, seed, first_step, n_records, every, flags=0):
+        """n_records x [every sweeps, ensemble_add], one native call."""
+        t, tp = self._T(T)
+        self._check(self.lib.dsmc_run_recorded(self._h, tp, seed, first_step, n_records, every, flags))
 
     def sublattice_pass(self, T, seed, pass_index, l, flags=0, accept_out=None, margin_out=None):
         """One pass of the paper's stride-l schedule -> the offset (S_1, S_2)."""

@@ -70,11 +70,11 @@ def main():
     t0 = time.perf_counter()
     ctx.run(T, seed, 0, 2 * burn)
     ctx.ensemble_reset()
-    done = burn
-    while done < sweeps:
-        k = min(every, sweeps - done)
-        ctx.run(None, seed, 2 * done, 2 * k)
-        done += k
+    n_rec = (sweeps - burn) // every
+    ctx.run_recorded(None, seed, 2 * burn, n_rec, every)       # n_rec x [every sweeps, record], one native call
+    done = burn + n_rec * every
+    if done < sweeps:                                          # a last, shorter interval
+        ctx.run(None, seed, 2 * done, 2 * (sweeps - done))
         ctx.ensemble_add()
     mean, var, se, n = ctx.ensemble_get()                   # synchronises
     wall = time.perf_counter() - t0

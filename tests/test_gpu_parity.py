@@ -618,3 +618,43 @@ def test_dependent_launch_is_bit_identical(L, R, graph):
         assert p.returncode == 0, p.stderr[-2000:]
         digest.append(p.stdout.strip().splitlines()[-1])
     assert len(digest[0]) == 64 and digest[0] == digest[1]
+
+
+@pytest.mark.parametrize("L,R,every,fft", [(32, 8, 1, True), (32, 8, 3, True), (64, 4, 20, True), (12, 5, 2, False)])
+def test_run_recorded_matches_separate_calls(dsmc_mod, L, R, every, fft):
+    """dsmc_run_recorded (a state recorded every k steps) = the same dsmc_run / dsmc_ensemble_add calls one by
+    one: identical spins (the graph of `every` sweeps + record replays the same kernels with the same Philox counters),
+    the same number of snapshots, statistics equal up to the rounding of the fp64 atomic sums."""
+    T = np.linspace(0.4, 1.5, R).astype(np.float32)
+    n_rec, first = 9, 6
+    pair = []
+    for _ in range(2):
+        ctx = dsmc_mod.Dsmc(L, R, J=1.0, g=0.15, K2=0.6, K4=0.1)
+        ctx.build_tensor(dsmc_mod.DSMC_W_EWALD)
+        if fft:
+            ctx.select_field_kernel(dsmc_mod.DSMC_FIELD_FFT)
+        ctx.init_spins(dsmc_mod.DSMC_INIT_RANDOM, seed=3)
+        ctx.ensemble_reset()
+        pair.append(ctx)
+    a, b = pair
+    a.run_recorded(T, 17, first, n_rec, every)
+    for k in range(n_rec):
+        b.run(T if k == 0 else None, 17, first + 2 * every * k, 2 * every)
+        b.ensemble_add()
+    assert np.array_equal(a.get_spins(), b.get_spins())
+    ma, va, sa, na = a.ensemble_get()
+    mb, vb, sb, nb = b.ensemble_get()
+    assert na == nb == n_rec
+    np.testing.assert_allclose(ma, mb, rtol=1e-12, atol=1e-14)
+    np.testing.assert_allclose(va, vb, rtol=1e-9, atol=1e-15)
+    # a second call continues the same ensemble and trajectory
+    a.run_recorded(None, 17, first + 2 * every * n_rec, 2, every)
+    b.run(None, 17, first + 2 * every * n_rec, 4 * every)
+    assert np.array_equal(a.get_spins(), b.get_spins())
+    assert a.ensemble_get()[3] == n_rec + 2
+    with pytest.raises(Exception):
+        a.run_recorded(None, 17, 1, 2, every)      # odd first step
+    with pytest.raises(Exception):
+        a.run_recorded(None, 17, 0, 2, 0)          # every < 1
+    a.close()
+    b.close()
