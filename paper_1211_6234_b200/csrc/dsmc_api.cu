@@ -245,11 +245,11 @@ int build_pass_graph(dsmc_ctx *ctx, uint64_t seed, int l, int flags) {
 // the kernels of dsmc_ensemble_add: full field of the current state, raw sums, wall counts, running statistics
 int enqueue_record(dsmc_ctx *ctx) {
     if (int rc = run_field(ctx, -1)) return rc;
-    CU(launch_observables(ctx->S(), ctx->H(), ctx->K2d(), ctx->K4d(), ctx->obs(), ctx->L, ctx->R, ctx->J, ctx->g,
+    CU(launch_observables(ctx->S(), ctx->H(), ctx->K2d(), ctx->K4d(), ctx->robs(), ctx->L, ctx->R, ctx->J, ctx->g, true,
                           ctx->stream, &ctx->launches),
        "observables launch");
-    CU(launch_wall_counts(ctx->S(), ctx->walls(), ctx->L, ctx->R, ctx->stream, &ctx->launches), "wall counts launch");
-    CU(launch_ensemble_add(ctx->obs(), ctx->walls(), ctx->stats(), ctx->L, ctx->R, (double)ctx->J, (double)ctx->g,
+    CU(launch_wall_counts(ctx->S(), ctx->rwalls(), ctx->L, ctx->R, true, ctx->stream, &ctx->launches), "wall counts launch");
+    CU(launch_ensemble_add(ctx->robs(), ctx->rwalls(), ctx->stats(), ctx->L, ctx->R, (double)ctx->J, (double)ctx->g,
                            ctx->stream, &ctx->launches),
        "ensemble launch");
     return DSMC_OK;
@@ -337,6 +337,7 @@ DsmcLayout dsmc_make_layout(int L, int R) {
     l.off_obs = o; o = align256(o + sizeof(double) * 8 * R);
     l.off_walls = o; o = align256(o + sizeof(unsigned long long) * 8 * R);
     l.off_stats = o; o = align256(o + sizeof(double) * 16 * R);
+    l.off_robs = o; o = align256(o + (sizeof(double) + sizeof(unsigned long long)) * 8 * R);
     l.off_step = o; o = align256(o + sizeof(unsigned long long));
     l.total = o;
     return l;
@@ -405,6 +406,11 @@ int dsmc_bind(dsmc_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_strea
     ctx->aniso_dirty = true;
     for (int i = 0; i < 3; ++i)
         if (!ctx->ev[i]) CU(cudaEventCreate(&ctx->ev[i]), "cudaEventCreate");
+    // the ensemble sums start empty, and the raw sums of the record path start (and are kept) zero
+    CU(cudaMemsetAsync(ctx->stats(), 0, sizeof(double) * 16 * (size_t)ctx->R, ctx->stream), "ensemble init");
+    CU(cudaMemsetAsync(ctx->robs(), 0, (sizeof(double) + sizeof(unsigned long long)) * 8 * (size_t)ctx->R, ctx->stream),
+       "ensemble init");
+    ctx->ensemble_n = 0;
     return DSMC_OK;
 }
 
@@ -615,7 +621,7 @@ int dsmc_observables(dsmc_ctx *ctx, double *out) {
     if (!ctx->spins_set) return fail(ctx, DSMC_ESTATE, "spins not set");
     if (int rc = upload_params(ctx, ctx->T_valid ? nullptr : std::vector<float>(ctx->R, 1.0f).data())) return rc;
     if (int rc = run_field(ctx, -1)) return rc;
-    CU(launch_observables(ctx->S(), ctx->H(), ctx->K2d(), ctx->K4d(), ctx->obs(), ctx->L, ctx->R, ctx->J, ctx->g,
+    CU(launch_observables(ctx->S(), ctx->H(), ctx->K2d(), ctx->K4d(), ctx->obs(), ctx->L, ctx->R, ctx->J, ctx->g, false,
                           ctx->stream, &ctx->launches),
        "observables launch");
     std::vector<double> raw(8 * (size_t)ctx->R);
@@ -639,7 +645,7 @@ int dsmc_wall_observables(dsmc_ctx *ctx, long long *counts_out, double *derived_
     if (!counts_out) return fail(ctx, DSMC_EINVAL, "null argument");
     if (!ctx->spins_set) return fail(ctx, DSMC_ESTATE, "spins not set");
     unsigned long long *dev = ctx->walls();
-    CU(launch_wall_counts(ctx->S(), dev, ctx->L, ctx->R, ctx->stream, &ctx->launches), "wall counts launch");
+    CU(launch_wall_counts(ctx->S(), dev, ctx->L, ctx->R, false, ctx->stream, &ctx->launches), "wall counts launch");
     std::vector<unsigned long long> raw(8 * (size_t)ctx->R);
     CU(cudaMemcpyAsync(raw.data(), dev, sizeof(unsigned long long) * raw.size(), cudaMemcpyDeviceToHost, ctx->stream),
        "wall counts D2H");
@@ -682,6 +688,8 @@ int dsmc_staggered_magnetisation(dsmc_ctx *ctx, double *out) {
 int dsmc_ensemble_reset(dsmc_ctx *ctx) {
     if (int rc = need_bound(ctx)) return rc;
     CU(cudaMemsetAsync(ctx->stats(), 0, sizeof(double) * 16 * (size_t)ctx->R, ctx->stream), "ensemble reset");
+    CU(cudaMemsetAsync(ctx->robs(), 0, (sizeof(double) + sizeof(unsigned long long)) * 8 * (size_t)ctx->R, ctx->stream),
+       "ensemble reset");
     ctx->ensemble_n = 0;
     return DSMC_OK;
 }

@@ -68,6 +68,8 @@ struct DsmcLayout {
     size_t off_obs;    // R*8 doubles (raw observable sums)
     size_t off_walls;  // R*8 64-bit wall counts
     size_t off_stats;  // R*8*2 doubles: ensemble sums of x and x^2
+    size_t off_robs;   // R*8 doubles + R*8 64-bit counts: the raw sums of the record path (dsmc_ensemble_add), kept zero
+                       // between records by ensemble_add_kernel
     size_t off_step;   // one 64-bit step counter (dsmc_run's graph replay)
     size_t total;
 };
@@ -119,6 +121,8 @@ struct dsmc_ctx {
     double *obs() const { return (double *)(ws + lay.off_obs); }
     unsigned long long *walls() const { return (unsigned long long *)(ws + lay.off_walls); }
     double *stats() const { return (double *)(ws + lay.off_stats); }
+    double *robs() const { return (double *)(ws + lay.off_robs); }
+    unsigned long long *rwalls() const { return (unsigned long long *)(ws + lay.off_robs + sizeof(double) * 8 * (size_t)R); }
     unsigned long long *step_dev() const { return (unsigned long long *)(ws + lay.off_step); }
     size_t Nh() const { return (size_t)L * (L / 2); }
     size_t plane() const { return Nh() * (size_t)R; }  // floats in one [a][r] plane
@@ -191,11 +195,14 @@ cudaError_t launch_step_update(unsigned long long *step, unsigned long long valu
                                uint64_t *launches);
 cudaError_t launch_init_spins(float *S, int L, int R, int mode, uint64_t seed, uint32_t r_off, cudaStream_t st,
                               uint64_t *launches);
+// chained: the sums are zero on entry and the kernel joins the dependent-launch chain (the record path); else memset +
+// plain launch
 cudaError_t launch_observables(const float *S, const float *H, const float *K2, const float *K4,
-                               double *obs, int L, int R, float J, float g, cudaStream_t st,
+                               double *obs, int L, int R, float J, float g, bool chained, cudaStream_t st,
                                uint64_t *launches);
-cudaError_t launch_wall_counts(const float *S, unsigned long long *counts, int L, int R, cudaStream_t st,
+cudaError_t launch_wall_counts(const float *S, unsigned long long *counts, int L, int R, bool chained, cudaStream_t st,
                                uint64_t *launches);
 cudaError_t launch_staggered(const float *S, double *sums, int L, int R, cudaStream_t st, uint64_t *launches);
-cudaError_t launch_ensemble_add(const double *obs, const unsigned long long *walls, double *stats, int L, int R, double J,
+// consumes obs and walls and leaves them zero
+cudaError_t launch_ensemble_add(double *obs, unsigned long long *walls, double *stats, int L, int R, double J,
                                 double g, cudaStream_t st, uint64_t *launches);

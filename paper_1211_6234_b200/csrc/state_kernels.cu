@@ -55,6 +55,7 @@ __global__ void __launch_bounds__(256) observables_kernel(const float *__restric
                                                           const float *__restrict__ K2, const float *__restrict__ K4,
                                                           double *__restrict__ obs, int L, int R) {
     extern __shared__ double sm[];  // [blockDim.x][7] then folded
+    pdl_wait();                     // spins and field come from earlier kernels (launch_pdl in the record chain)
     const int Lh = L >> 1;
     const size_t Nh = (size_t)L * Lh, plane = Nh * (size_t)R;
     const size_t nthreads = (size_t)gridDim.x * blockDim.x;
@@ -87,6 +88,7 @@ __global__ void __launch_bounds__(256) observables_kernel(const float *__restric
         acc[5] += z2 * (k2 + k4 * z2);
         acc[6] += sx * hf[0] + sy * hf[plane] + sz * hf[2 * plane];
     }
+    pdl_trigger();
     for (int k = 0; k < 7; ++k) sm[threadIdx.x * 7 + k] = acc[k];
     __syncthreads();
     // threads with the same replica inside the block are R apart (blockDim.x*blockIdx.x % R == 0)
@@ -108,6 +110,7 @@ __device__ __forceinline__ int sgnf(float v) { return (v > 0.0f) - (v < 0.0f); }
 __global__ void __launch_bounds__(256) wall_counts_kernel(const float *__restrict__ S,
                                                           unsigned long long *__restrict__ counts, int L, int R) {
     extern __shared__ unsigned int wsm[];  // [blockDim.x][6]
+    pdl_wait();
     const int Lh = L >> 1;
     const size_t Nh = (size_t)L * Lh, plane = Nh * (size_t)R;
     const size_t nthreads = (size_t)gridDim.x * blockDim.x;
@@ -132,6 +135,7 @@ __global__ void __launch_bounds__(256) wall_counts_kernel(const float *__restric
             acc[2 * c + 1] += (unsigned int)(1 - si * sgnf(oth[c * plane + an]));
         }
     }
+    pdl_trigger();
     for (int k = 0; k < 6; ++k) wsm[threadIdx.x * 6 + k] = acc[k];
     __syncthreads();
     if ((int)threadIdx.x < R) {
@@ -178,13 +182,15 @@ __global__ void __launch_bounds__(256) staggered_kernel(const float *__restrict_
 // of observables_kernel and the counts of wall_counts_kernel into the eight per-snapshot quantities
 //   E/N, m_z, M_par, eta, wall density, O_x, O_y, O_z
 // and adds x and x^2 to the running sums stats[r][k][2] (fp64), all on the device.
-__global__ void ensemble_add_kernel(const double *__restrict__ obs, const unsigned long long *__restrict__ walls,
+__global__ void ensemble_add_kernel(double *__restrict__ obs, unsigned long long *__restrict__ walls,
                                     double *__restrict__ stats, int L, int R, double J, double g) {
     const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    pdl_trigger();
     if (r >= R) return;
+    pdl_wait();
     const double N = (double)L * L;
-    const double *s = obs + 8 * (size_t)r;
-    const unsigned long long *n = walls + 8 * (size_t)r;
+    double *s = obs + 8 * (size_t)r;
+    unsigned long long *n = walls + 8 * (size_t)r;
     double x[8];
     const double mx = s[0] / N, my = s[1] / N;
     x[0] = (-J * s[4] - s[5] + 0.5 * g * s[6]) / N;
@@ -200,6 +206,12 @@ __global__ void ensemble_add_kernel(const double *__restrict__ obs, const unsign
     for (int k = 0; k < 8; ++k) {
         dst[2 * k] += x[k];
         dst[2 * k + 1] += x[k] * x[k];
+    }
+    // the raw sums are consumed: leave them zero for the next record, which then needs no memset in front of the
+    // atomics of observables_kernel / wall_counts_kernel (a memset node would cut the dependent-launch chain)
+    for (int k = 0; k < 8; ++k) {
+        s[k] = 0.0;
+        n[k] = 0ull;
     }
 }
 
@@ -241,27 +253,37 @@ static void replica_walk_shape(int L, int R, int *block_out, unsigned *grid_out)
 }
 
 cudaError_t launch_observables(const float *S, const float *H, const float *K2, const float *K4, double *obs,
-                               int L, int R, float, float, cudaStream_t st, uint64_t *launches) {
-    cudaError_t e = cudaMemsetAsync(obs, 0, sizeof(double) * 8 * (size_t)R, st);
-    if (e != cudaSuccess) return e;
+                               int L, int R, float, float, bool chained, cudaStream_t st, uint64_t *launches) {
     int block;
     unsigned grid;
     replica_walk_shape(L, R, &block, &grid);
-    observables_kernel<<<grid, block, sizeof(double) * 7 * block, st>>>(S, H, K2, K4, obs, L, R);
+    cudaError_t e;
+    if (chained) {  // obs is zero on entry (ensemble_add_kernel leaves it so): dependent launch, no memset
+        e = launch_pdl(observables_kernel, dim3(grid), dim3(block), sizeof(double) * 7 * block, st, S, H, K2, K4, obs, L, R);
+    } else {
+        e = cudaMemsetAsync(obs, 0, sizeof(double) * 8 * (size_t)R, st);
+        if (e != cudaSuccess) return e;
+        observables_kernel<<<grid, block, sizeof(double) * 7 * block, st>>>(S, H, K2, K4, obs, L, R);
+    }
     ++*launches;
-    return cudaGetLastError();
+    return e != cudaSuccess ? e : cudaGetLastError();
 }
 
-cudaError_t launch_wall_counts(const float *S, unsigned long long *counts, int L, int R, cudaStream_t st,
+cudaError_t launch_wall_counts(const float *S, unsigned long long *counts, int L, int R, bool chained, cudaStream_t st,
                                uint64_t *launches) {
-    cudaError_t e = cudaMemsetAsync(counts, 0, sizeof(unsigned long long) * 8 * (size_t)R, st);
-    if (e != cudaSuccess) return e;
     int block;
     unsigned grid;
     replica_walk_shape(L, R, &block, &grid);
-    wall_counts_kernel<<<grid, block, sizeof(unsigned int) * 6 * block, st>>>(S, counts, L, R);
+    cudaError_t e;
+    if (chained) {
+        e = launch_pdl(wall_counts_kernel, dim3(grid), dim3(block), sizeof(unsigned int) * 6 * block, st, S, counts, L, R);
+    } else {
+        e = cudaMemsetAsync(counts, 0, sizeof(unsigned long long) * 8 * (size_t)R, st);
+        if (e != cudaSuccess) return e;
+        wall_counts_kernel<<<grid, block, sizeof(unsigned int) * 6 * block, st>>>(S, counts, L, R);
+    }
     ++*launches;
-    return cudaGetLastError();
+    return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 cudaError_t launch_staggered(const float *S, double *sums, int L, int R, cudaStream_t st, uint64_t *launches) {
@@ -275,9 +297,9 @@ cudaError_t launch_staggered(const float *S, double *sums, int L, int R, cudaStr
     return cudaGetLastError();
 }
 
-cudaError_t launch_ensemble_add(const double *obs, const unsigned long long *walls, double *stats, int L, int R, double J,
+cudaError_t launch_ensemble_add(double *obs, unsigned long long *walls, double *stats, int L, int R, double J,
                                 double g, cudaStream_t st, uint64_t *launches) {
-    ensemble_add_kernel<<<(R + 127) / 128, 128, 0, st>>>(obs, walls, stats, L, R, J, g);
+    const cudaError_t e = launch_pdl(ensemble_add_kernel, dim3((R + 127) / 128), dim3(128), 0, st, obs, walls, stats, L, R, J, g);
     ++*launches;
-    return cudaGetLastError();
+    return e != cudaSuccess ? e : cudaGetLastError();
 }
