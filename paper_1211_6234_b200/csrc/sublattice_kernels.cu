@@ -41,6 +41,8 @@ __global__ void __launch_bounds__(256) sublattice_field_kernel(const float *__re
                                                                int ox, int oy, int rows_per_slab, int segs,
                                                                const unsigned long long *__restrict__ pass_dev,
                                                                const RoundKeys rk) {
+    pdl_trigger();
+    pdl_wait();                                                // spins and pass counter come from earlier kernels (section 5.8)
     if (pass_dev) pass_offset(rk, *pass_dev, l, ox, oy);
     __shared__ float part[8][3][32];
     const int Lh = L >> 1;
@@ -101,6 +103,8 @@ __global__ void __launch_bounds__(256) sublattice_field_kernel(const float *__re
 __global__ void __launch_bounds__(128) sublattice_flip_kernel(const MetropolisArgs p, const RoundKeys rk,
                                                               const float *__restrict__ part, int KS, int l, int ox,
                                                               int oy) {
+    pdl_trigger();
+    pdl_wait();                                                // partial fields, spins and pass counter come from earlier kernels
     if (p.step_dev) pass_offset(rk, *p.step_dev + p.step_off, l, ox, oy);
     const int L = p.L, Lh = L >> 1, R = p.R;
     const size_t N = (size_t)L * L, plane = (size_t)L * Lh * R;
@@ -448,14 +452,16 @@ cudaError_t launch_sublattice_pass(const MetropolisArgs &a, const float *Wc, flo
         int rows = std::max(8 / segs, (a.L + ks_target - 1) / ks_target);
         rows = std::max(rows, (n + a.L - 1) / a.L);
         KS = (a.L + rows - 1) / rows;
-        sublattice_field_kernel<<<dim3((unsigned)n, (unsigned)chunks, (unsigned)KS), 256, 0, st>>>(
-            a.S, scratch, Wc, a.L, a.R, l, ox, oy, rows, segs, a.step_dev, rk);
+        const cudaError_t e = launch_pdl(sublattice_field_kernel, dim3((unsigned)n, (unsigned)chunks, (unsigned)KS), dim3(256), 0,
+                                         st, (const float *)a.S, scratch, Wc, a.L, a.R, l, ox, oy, rows, segs, a.step_dev, rk);
         ++*launches;
+        if (e != cudaSuccess) return e;
     }
     const size_t total = (size_t)n * a.R;
-    sublattice_flip_kernel<<<(unsigned)((total + 127) / 128), 128, 0, st>>>(a, rk, scratch, KS, l, ox, oy);
+    const cudaError_t e = launch_pdl(sublattice_flip_kernel, dim3((unsigned)((total + 127) / 128)), dim3(128), 0, st, a, rk,
+                                     (const float *)scratch, KS, l, ox, oy);
     ++*launches;
-    return cudaGetLastError();
+    return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 bool dsmc_resident_supported(int L, int l) {
