@@ -446,11 +446,11 @@ cudaError_t launch_fft_n2(const FftParams &p, cudaStream_t st, uint64_t *launche
         if ((e = cudaFuncSetAttribute(fft_y_multiply_kernel<N2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024)) != cudaSuccess) return e;
         configured = true;
     }
-    launch_pdl(fft_x_forward_kernel<N2>, dim3(p.P / LNX, L, 3), dim3(LNX, 16), smx, st, p);
-    launch_pdl(fft_y_multiply_kernel<N2>, dim3(p.P / LNY, L), dim3(LNY, 16), smy, st, p);
-    launch_pdl(fft_x_inverse_kernel<N2>, dim3(p.P / LNX, L, 3), dim3(LNX, 16), smx, st, p);
+    cudaError_t e = launch_pdl(fft_x_forward_kernel<N2>, dim3(p.P / LNX, L, 3), dim3(LNX, 16), smx, st, p);
+    if (e == cudaSuccess) e = launch_pdl(fft_y_multiply_kernel<N2>, dim3(p.P / LNY, L), dim3(LNY, 16), smy, st, p);
+    if (e == cudaSuccess) e = launch_pdl(fft_x_inverse_kernel<N2>, dim3(p.P / LNX, L, 3), dim3(LNX, 16), smx, st, p);
     *launches += 3;
-    return cudaGetLastError();
+    return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 }  // namespace
