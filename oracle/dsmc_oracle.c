@@ -33,6 +33,9 @@
  *   philox4x32_10   : published known-answer vectors (Salmon et al., SC'11).
  *   delta_e / halfsweep : single-spin dE == full-energy difference; eq. 8 identity;
  *                     g = 0 limit; T -> infinity and T -> 0 limits.
+ *   halfsweep_sequential : g = 0 equals the frozen sweep; g != 0: the eq. 8 terms of the
+ *                     sites updated before, term by term.
+ *   *_given_field   : identical to the plain calls when handed the plain field.
  *   observables     : cone-angle special cases of PAPER.md:241, :255.
  *   eq. 10's "0.14 %" is NOT reproduced: parity unpinned for that
  *   number (context only, nothing on the hot path depends on it).
@@ -272,14 +275,13 @@ int oracle_dipole_field_sampled(int L, const double *W, const double *s /* [3][L
 /* out[r] = total energy (not per spin) of replica r; parts[r][3] optional     */
 /* (exchange, anisotropy, dipole).                                             */
 /* ------------------------------------------------------------------------- */
-int oracle_energy(int L, int R, double J, double g, const double *K2, const double *K4,
-                  const double *W, const double *s, double *out, double *parts)
+/* eq. 11 with the dipole field h[R][3][N] of the state s handed in (h = O2 of s): the form the long-run
+ * harness uses with a field it evaluated itself (SURVEY.md 8c-O2 allows an fp64 FFT there).     */
+int oracle_energy_given_field(int L, int R, double J, double g, const double *K2, const double *K4,
+                              const double *s, const double *h, double *out, double *parts)
 {
-    if (L < 1 || R < 1 || !K2 || !K4 || !W || !s || !out) return -1;
+    if (L < 1 || R < 1 || !K2 || !K4 || !s || !h || !out) return -1;
     size_t N = (size_t)L * L;
-    double *h = (double *)malloc(sizeof(double) * (size_t)R * 3 * N);
-    if (!h) return -2;
-    oracle_dipole_field(L, R, W, s, -1, h);
     for (int r = 0; r < R; ++r) {
         const double *sr = s + (size_t)r * 3 * N, *hr = h + (size_t)r * 3 * N;
         double ex = 0, an = 0, dip = 0;
@@ -302,8 +304,20 @@ int oracle_energy(int L, int R, double J, double g, const double *K2, const doub
             parts[3 * r + 2] = 0.5 * g * dip;
         }
     }
-    free(h);
     return 0;
+}
+
+int oracle_energy(int L, int R, double J, double g, const double *K2, const double *K4,
+                  const double *W, const double *s, double *out, double *parts)
+{
+    if (L < 1 || R < 1 || !K2 || !K4 || !W || !s || !out) return -1;
+    size_t N = (size_t)L * L;
+    double *h = (double *)malloc(sizeof(double) * (size_t)R * 3 * N);
+    if (!h) return -2;
+    oracle_dipole_field(L, R, W, s, -1, h);
+    int rc = oracle_energy_given_field(L, R, J, g, K2, K4, s, h, out, parts);
+    free(h);
+    return rc;
 }
 
 /* ------------------------------------------------------------------------- */
@@ -451,6 +465,11 @@ double oracle_delta_e(int L, double J, double g, double K2, double K4, const dou
  * simultaneously updated sites.
  * Outputs (each nullable): h_out [R][3][N] (active sites written), accept_out
  * [R][N] bytes (active sites written, 0/1), margin_out [R][N], trial_out [R][3][N]. */
+int oracle_halfsweep_given_field(int L, int R, double J, double g, const double *K2, const double *K4,
+                                 const double *W, double *s, const double *T, uint64_t seed,
+                                 uint64_t step, const double *h, double *h_out, uint8_t *accept_out,
+                                 double *margin_out, double *trial_out);
+
 int oracle_halfsweep(int L, int R, double J, double g, const double *K2, const double *K4,
                      const double *W, double *s, const double *T, uint64_t seed, uint64_t step,
                      double *h_out, uint8_t *accept_out, double *margin_out, double *trial_out)
@@ -461,10 +480,31 @@ int oracle_halfsweep(int L, int R, double J, double g, const double *K2, const d
     size_t N = (size_t)L * L;
     int colour = (int)(step & 1u);
     double *h = (double *)malloc(sizeof(double) * (size_t)R * 3 * N);
-    double *snew = (double *)malloc(sizeof(double) * (size_t)R * 3 * N);
-    if (!h || !snew) { free(h); free(snew); return -2; }
+    if (!h) return -2;
     memset(h, 0, sizeof(double) * (size_t)R * 3 * N);
-    oracle_dipole_field(L, R, W, s, colour, h);
+    oracle_dipole_field(L, R, W, s, colour, h);             /* (i): O2 on the state at entry */
+    int rc = oracle_halfsweep_given_field(L, R, J, g, K2, K4, W, s, T, seed, step, h, h_out,
+                                          accept_out, margin_out, trial_out);
+    free(h);
+    return rc;
+}
+
+/* Step (ii) of the half-sweep alone, with the frozen field h[R][3][N] of the state at entry handed in
+ * (only its entries at active sites are read).  oracle_halfsweep is "h <- O2, then this".  The long-run
+ * harness calls it with a field it evaluated by fp64 FFT (allowed in the harness to make
+ * long oracle runs affordable; tests pin that field to O2 first); W is still needed for W(0).    */
+int oracle_halfsweep_given_field(int L, int R, double J, double g, const double *K2, const double *K4,
+                                 const double *W, double *s, const double *T, uint64_t seed,
+                                 uint64_t step, const double *h, double *h_out, uint8_t *accept_out,
+                                 double *margin_out, double *trial_out)
+{
+    if (L < 2 || (L & 1) || R < 1 || !K2 || !K4 || !W || !s || !T || !h) return -1;
+    for (int r = 0; r < R; ++r)
+        if (!(T[r] > 0.0)) return -1;
+    size_t N = (size_t)L * L;
+    int colour = (int)(step & 1u);
+    double *snew = (double *)malloc(sizeof(double) * (size_t)R * 3 * N);
+    if (!snew) return -2;
     memcpy(snew, s, sizeof(double) * (size_t)R * 3 * N);
     long total = (long)R * (long)N;
 #pragma omp parallel for schedule(static)
@@ -494,7 +534,6 @@ int oracle_halfsweep(int L, int R, double J, double g, const double *K2, const d
             for (int c = 0; c < 3; ++c) h_out[((size_t)r * 3 + c) * N + n] = hn[c];
     }
     memcpy(s, snew, sizeof(double) * (size_t)R * 3 * N);
-    free(h);
     free(snew);
     return 0;
 }
@@ -502,10 +541,13 @@ int oracle_halfsweep(int L, int R, double J, double g, const double *K2, const d
 /* Exact sequential single-spin Metropolis over the same sites, in site order,
  * with the same random numbers but the field recomputed after every accepted
  * move (no approximation).  Used only by tests that measure what the frozen-field
- * approximation changes (eq. 8); O(N^2) per site, tiny L only. */
+ * approximation changes (eq. 8); O(N^2) per site, tiny L only.
+ * margin_out (nullable, [R][N], active sites written) = dE/T + ln u as each site saw it.
+ * Pin at g != 0 (tests/test_oracle_physics.py::test_eq8_sequential_minus_frozen_halfsweep):
+ * with every move accepted, margin_seq(k) - margin_frozen(k) = (g/T) sum_{j<k} delta_j.W(rho_jk).delta_k. */
 int oracle_halfsweep_sequential(int L, int R, double J, double g, const double *K2,
                                 const double *K4, const double *W, double *s, const double *T,
-                                uint64_t seed, uint64_t step, uint8_t *accept_out)
+                                uint64_t seed, uint64_t step, uint8_t *accept_out, double *margin_out)
 {
     if (L < 2 || (L & 1) || R < 1 || !K2 || !K4 || !W || !s || !T) return -1;
     size_t N = (size_t)L * L;
@@ -522,10 +564,12 @@ int oracle_halfsweep_sequential(int L, int R, double J, double g, const double *
             double u = to_unit(rnd[2]);
             field_at(L, W, sr, x, y, hn);
             double dE = oracle_delta_e(L, J, g, K2[r], K4[r], W, sr, hn, n, sp);
-            int acc = (dE / T[r] + log(u)) < 0.0;
+            double margin = dE / T[r] + log(u);
+            int acc = margin < 0.0;
             if (acc)
                 for (int c = 0; c < 3; ++c) sr[c * N + n] = sp[c];
             if (accept_out) accept_out[(size_t)r * N + n] = (uint8_t)acc;
+            if (margin_out) margin_out[(size_t)r * N + n] = margin;
         }
     }
     return 0;
@@ -539,6 +583,26 @@ int oracle_halfsweep_sequential(int L, int R, double J, double g, const double *
 /*   eta   : (2/pi) ( N^-1 sum_i (theta_i - pi/2)^2 )^(1/2),                    */
 /*           theta_i = arccos s_i^z   (eq. 17, :232, per-snapshot reading R15)  */
 /* ------------------------------------------------------------------------- */
+static void magnetisation_and_cone(int L, const double *sr, double out[3])
+{
+    size_t N = (size_t)L * L;
+    double mx = 0, my = 0, mz = 0, q = 0;
+    for (size_t n = 0; n < N; ++n) {
+        mx += sr[n];
+        my += sr[N + n];
+        mz += sr[2 * N + n];
+        double cz = sr[2 * N + n];
+        if (cz > 1.0) cz = 1.0;
+        if (cz < -1.0) cz = -1.0;
+        double th = acos(cz) - 0.5 * ORACLE_PI;
+        q += th * th;
+    }
+    mx /= (double)N; my /= (double)N; mz /= (double)N; q /= (double)N;
+    out[0] = mz;
+    out[1] = sqrt(mx * mx + my * my);
+    out[2] = (2.0 / ORACLE_PI) * sqrt(q);
+}
+
 int oracle_observables(int L, int R, double J, double g, const double *K2, const double *K4,
                        const double *W, const double *s, double *out)
 {
@@ -549,23 +613,26 @@ int oracle_observables(int L, int R, double J, double g, const double *K2, const
     int rc = oracle_energy(L, R, J, g, K2, K4, W, s, E, NULL);
     if (rc) { free(E); return rc; }
     for (int r = 0; r < R; ++r) {
-        const double *sr = s + (size_t)r * 3 * N;
-        double mx = 0, my = 0, mz = 0, q = 0;
-        for (size_t n = 0; n < N; ++n) {
-            mx += sr[n];
-            my += sr[N + n];
-            mz += sr[2 * N + n];
-            double cz = sr[2 * N + n];
-            if (cz > 1.0) cz = 1.0;
-            if (cz < -1.0) cz = -1.0;
-            double th = acos(cz) - 0.5 * ORACLE_PI;
-            q += th * th;
-        }
-        mx /= (double)N; my /= (double)N; mz /= (double)N; q /= (double)N;
         out[4 * r + 0] = E[r] / (double)N;
-        out[4 * r + 1] = mz;
-        out[4 * r + 2] = sqrt(mx * mx + my * my);
-        out[4 * r + 3] = (2.0 / ORACLE_PI) * sqrt(q);
+        magnetisation_and_cone(L, s + (size_t)r * 3 * N, out + 4 * r + 1);
+    }
+    free(E);
+    return 0;
+}
+
+/* the same with the field h = O2 of s handed in (see oracle_energy_given_field) */
+int oracle_observables_given_field(int L, int R, double J, double g, const double *K2,
+                                   const double *K4, const double *s, const double *h, double *out)
+{
+    if (L < 1 || R < 1 || !s || !h || !out) return -1;
+    size_t N = (size_t)L * L;
+    double *E = (double *)malloc(sizeof(double) * R);
+    if (!E) return -2;
+    int rc = oracle_energy_given_field(L, R, J, g, K2, K4, s, h, E, NULL);
+    if (rc) { free(E); return rc; }
+    for (int r = 0; r < R; ++r) {
+        out[4 * r + 0] = E[r] / (double)N;
+        magnetisation_and_cone(L, s + (size_t)r * 3 * N, out + 4 * r + 1);
     }
     free(E);
     return 0;

@@ -168,11 +168,13 @@ def halfsweep(W, s, T, seed, step, J, g, K2, K4, want=("h", "accept", "margin", 
     out = {}
     if sequential:
         acc = np.zeros((R, L, L), dtype=np.uint8)
+        mar = np.zeros((R, L, L), dtype=np.float64)
         rc = lib().oracle_halfsweep_sequential(L, R, ctypes.c_double(J), ctypes.c_double(g), _d(K2),
                                                _d(K4), _d(W), _d(s), _d(T), ctypes.c_uint64(seed),
-                                               ctypes.c_uint64(step), acc.ctypes.data_as(_c_u8_p))
+                                               ctypes.c_uint64(step), acc.ctypes.data_as(_c_u8_p), _d(mar))
         assert rc == 0, rc
         out["accept"] = acc
+        out["margin"] = mar
         return out
     h = np.zeros((R, 3, L, L), dtype=np.float64) if "h" in want else None
     acc = np.zeros((R, L, L), dtype=np.uint8) if "accept" in want else None
@@ -193,6 +195,51 @@ def halfsweep(W, s, T, seed, step, J, g, K2, K4, want=("h", "accept", "margin", 
         out["margin"] = mar
     if tri is not None:
         out["trial"] = tri
+    return out
+
+
+def halfsweep_given_field(W, s, h, T, seed, step, J, g, K2, K4, want=()):
+    """Step (ii) of the half-sweep IN PLACE on s with the frozen field h[R][3][L][L] of the state at entry
+    handed in (halfsweep() is "h <- dipole_field(W, s, colour), then this"); W supplies W(0) only."""
+    assert s.dtype == np.float64 and s.flags.c_contiguous
+    R, _, L, _ = s.shape
+    W = _f64(W)
+    h = _f64(h)
+    assert h.shape == s.shape
+    T = _per_replica(T, R)
+    K2 = _per_replica(K2, R)
+    K4 = _per_replica(K4, R)
+    acc = np.zeros((R, L, L), dtype=np.uint8) if "accept" in want else None
+    mar = np.zeros((R, L, L), dtype=np.float64) if "margin" in want else None
+    tri = np.zeros((R, 3, L, L), dtype=np.float64) if "trial" in want else None
+    rc = lib().oracle_halfsweep_given_field(L, R, ctypes.c_double(J), ctypes.c_double(g), _d(K2), _d(K4), _d(W),
+                                            _d(s), _d(T), ctypes.c_uint64(seed), ctypes.c_uint64(step), _d(h), None,
+                                            acc.ctypes.data_as(_c_u8_p) if acc is not None else None,
+                                            _d(mar) if mar is not None else None,
+                                            _d(tri) if tri is not None else None)
+    assert rc == 0, rc
+    out = {}
+    if acc is not None:
+        out["accept"] = acc
+    if mar is not None:
+        out["margin"] = mar
+    if tri is not None:
+        out["trial"] = tri
+    return out
+
+
+def observables_given_field(s, h, J, g, K2, K4):
+    """observables() with the full-lattice field h = dipole_field(W, s) handed in."""
+    s = _f64(s)
+    h = _f64(h)
+    R, _, L, _ = s.shape
+    assert h.shape == s.shape
+    K2 = _per_replica(K2, R)
+    K4 = _per_replica(K4, R)
+    out = np.empty((R, 4), dtype=np.float64)
+    rc = lib().oracle_observables_given_field(L, R, ctypes.c_double(J), ctypes.c_double(g), _d(K2), _d(K4),
+                                              _d(s), _d(h), _d(out))
+    assert rc == 0, rc
     return out
 
 

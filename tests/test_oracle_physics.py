@@ -211,6 +211,67 @@ def test_halfsweep_frozen_vs_sequential_without_dipole(oracle):
     assert np.max(np.abs((a ** 2).sum(1) - 1)) < 1e-14
 
 
+def test_eq8_sequential_minus_frozen_halfsweep(oracle):
+    """PAPER.md:118-125 (section 3.2, eq. 8) on the checkerboard: oracle_halfsweep_sequential differs from the
+    frozen half-sweep only in that the field is recomputed from the CURRENT state.  With every move accepted
+    (T huge) the margin of the k-th active site therefore exceeds the frozen one by the couplings to the
+    sites updated before it (site order), term by term:
+        (m_seq(k) - m_frozen(k)) T = g sum_{j<k} delta_j . W(rho_jk) . delta_k .
+    Dropping the field refresh, refreshing from the wrong state or visiting in another order fails this."""
+    rng = np.random.default_rng(31)
+    L, J, g, K2, K4, T = 6, 1.0, 0.35, 0.4, -0.1, 1e9
+    W = oracle.build_tensor_ewald(L)
+    for step in (0, 1):
+        s0 = rand_spins(rng, 2, L)
+        a, b = s0.copy(), s0.copy()
+        fa = oracle.halfsweep(W, a, T, 5, step, J, g, K2, K4)
+        fb = oracle.halfsweep(W, b, T, 5, step, J, g, K2, K4, sequential=True)
+        x = np.arange(L)
+        act = ((x[:, None] + x[None, :]) % 2) == (step & 1)
+        assert np.all(fa["accept"][:, act] == 1) and np.all(fb["accept"][:, act] == 1)
+        assert np.array_equal(a, b)                                    # same trials, all accepted
+        sites = [(n % L, n // L) for n in range(L * L) if act[n // L, n % L]]
+        worst = 0.0
+        for r in range(2):
+            delta = [fa["trial"][r, :, y, xx] - s0[r, :, y, xx] for (xx, y) in sites]
+            for k, (xk, yk) in enumerate(sites):
+                expect = 0.0
+                for j in range(k):
+                    xj, yj = sites[j]
+                    ry, rx = (yk - yj) % L, (xk - xj) % L
+                    Wm = np.array([[W[0, ry, rx], W[1, ry, rx], 0], [W[1, ry, rx], W[2, ry, rx], 0], [0, 0, W[3, ry, rx]]])
+                    expect += g * delta[j] @ Wm @ delta[k]
+                got = (fb["margin"][r, yk, xk] - fa["margin"][r, yk, xk]) * T
+                assert abs(got - expect) < 1e-6 * max(1.0, abs(expect)), (step, r, k, got, expect)
+                worst = max(worst, abs(expect))
+        assert worst > 1e-2                                            # the test is not vacuous
+    # the first active site sees the state at entry in both: identical margins there
+    assert fb["margin"][0, sites[0][1], sites[0][0]] == fa["margin"][0, sites[0][1], sites[0][0]]
+
+
+def test_given_field_variants_equal_the_plain_calls(oracle):
+    """oracle_halfsweep = "h <- O2, then oracle_halfsweep_given_field"; oracle_observables likewise.  Handing the
+    plain O2 field to the given-field forms reproduces the plain calls bit for bit; a wrong field does not."""
+    rng = np.random.default_rng(32)
+    L, R, J, g = 6, 3, 1.0, 0.3
+    K2, K4 = np.array([0.5, 0.6, 0.7]), np.array([0.1, 0.0, -0.1])
+    T = np.array([0.3, 0.9, 2.0])
+    W = oracle.build_tensor_ewald(L)
+    s0 = rand_spins(rng, R, L)
+    for step in (0, 1):
+        a, b, c = s0.copy(), s0.copy(), s0.copy()
+        fa = oracle.halfsweep(W, a, T, 17, step, J, g, K2, K4)
+        h = oracle.dipole_field(W, s0)                                # all targets; only the active ones are read
+        fb = oracle.halfsweep_given_field(W, b, h, T, 17, step, J, g, K2, K4, want=("accept", "margin", "trial"))
+        assert np.array_equal(a, b)
+        for k in ("accept", "margin", "trial"):
+            assert np.array_equal(fa[k], fb[k]), k
+        fc = oracle.halfsweep_given_field(W, c, 2.0 * h, T, 17, step, J, g, K2, K4, want=("margin",))
+        assert not np.array_equal(fc["margin"], fa["margin"])
+    ob = oracle.observables(W, s0, J, g, K2, K4)
+    assert np.array_equal(ob, oracle.observables_given_field(s0, oracle.dipole_field(W, s0), J, g, K2, K4))
+
+
 def test_detailed_balance_single_spin(oracle):
     # one spin in a fixed anisotropy field only (J = g = 0, L = 2 so the update touches isolated
     # sites): the Metropolis chain must sample exp(K2 s_z^2 / T): <s_z^2> = known 1-D integral
