@@ -107,9 +107,15 @@ int dsmc_set_tensor(dsmc_ctx *ctx, const float *W_in, int where);
 
 /* Spins in canonical layout s[R][3][L][L].  set does not renormalise: |s| = 1 is the caller's
  * contract.  Host variants copy through a staging area inside the workspace; get to HOST
- * synchronises the stream.                                                                    */
+ * synchronises the stream.  With dsmc_set_debug(ctx, 1) set checks the contract: one reduction
+ * kernel takes the largest | |s| - 1 | over all sites and replicas and the call synchronises and
+ * returns DSMC_EINVAL (the spins then count as not set) when it exceeds 1e-5 or a spin is NaN;
+ * without it the hot path pays nothing.                                                         */
 int dsmc_set_spins(dsmc_ctx *ctx, const float *s, int where);
 int dsmc_get_spins(dsmc_ctx *ctx, float *s, int where);
+/* Debug checks on (1) / off (0, the default): argument checks that cost a kernel launch and a
+ * synchronisation (today: |s| = 1 in dsmc_set_spins).  Host-only.                                */
+int dsmc_set_debug(dsmc_ctx *ctx, int on);
 
 /* a4. Initial spins on the device: DSMC_INIT_RANDOM = uniform on S^2 from Philox4x32-10 keyed by
  * (seed; site, replica, tag 1) with the same map as the trial move (R9, R10);

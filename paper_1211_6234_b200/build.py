@@ -9,7 +9,7 @@ LIB = os.path.join(HERE, "libdsmc.so")
 SOURCES = ["dsmc_api.cu", "tensor_kernels.cu", "state_kernels.cu", "metropolis_kernels.cu", "sublattice_kernels.cu",
            "field_generic.cu", "field_tiled.cu", "field_fft.cu", "peak_kernels.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "-Xcompiler", "-fPIC", "--shared", "-cudart", "static"]
+              "-Xcompiler", "-fPIC", "--shared", "-cudart", "static", "--threads", "0"]
 
 
 def _deps():

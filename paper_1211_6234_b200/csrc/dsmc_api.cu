@@ -49,6 +49,25 @@ int need_bound(dsmc_ctx *ctx) {
     return DSMC_OK;
 }
 
+// Every call on a bound context runs with the workspace's device current, whatever the calling thread had
+// selected (launches, cudaFuncSetAttribute, graph capture and events all act on the current device), and puts the
+// caller's device back on return.
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(int want) {
+        int cur = 0;
+        if (cudaGetDevice(&cur) == cudaSuccess && cur != want && cudaSetDevice(want) == cudaSuccess) prev = cur;
+    }
+    ~DeviceGuard() {
+        if (prev >= 0) cudaSetDevice(prev);
+    }
+};
+#define ENTER_BOUND(ctx)                         \
+    if (int rc__ = need_bound(ctx)) return rc__; \
+    DeviceGuard guard__((ctx)->device)
+
+int upload_aniso(dsmc_ctx *ctx);
+
 int upload_params(dsmc_ctx *ctx, const float *T) {
     const int R = ctx->R;
     if (T) {
@@ -66,6 +85,12 @@ int upload_params(dsmc_ctx *ctx, const float *T) {
     } else if (!ctx->T_valid) {
         return fail(ctx, DSMC_EINVAL, "T is NULL and no temperatures were set before");
     }
+    return upload_aniso(ctx);
+}
+
+// the per-replica anisotropy constants alone (observables need them, but no temperature)
+int upload_aniso(dsmc_ctx *ctx) {
+    const int R = ctx->R;
     if (ctx->aniso_dirty) {
         CU(cudaMemcpyAsync(ctx->K2d(), ctx->K2.data(), sizeof(float) * R, cudaMemcpyHostToDevice, ctx->stream),
            "upload K2");
@@ -89,14 +114,14 @@ int run_field(dsmc_ctx *ctx, int colour) {
     cudaError_t e = cudaSuccess;
     const int kind = field_kind(ctx);
     if (kind == 2) {
-        e = launch_field_fft(ctx->S(), ctx->M(), ctx->Z(), ctx->H(), ctx->L, ctx->R, colour, ctx->stream,
-                             &ctx->launches);
+        e = launch_field_fft(ctx->S(), ctx->M(), ctx->Z(), ctx->H(), ctx->L, ctx->R, colour, &ctx->fft_configured,
+                             ctx->stream, &ctx->launches);
     } else {
         for (int q = 0; q < 2 && e == cudaSuccess; ++q) {
             if (colour >= 0 && colour != q) continue;
             if (kind == 1)
                 e = launch_field_tiled(ctx->S(), ctx->Wk(), ctx->Hpart(), ctx->H(), ctx->L, ctx->R, q, ctx->sm_count,
-                                       ctx->stream, &ctx->launches);
+                                       &ctx->tiled_configured, ctx->stream, &ctx->launches);
             else
                 e = launch_field_generic(ctx->S(), ctx->Wc(), ctx->H(), ctx->L, ctx->R, q, ctx->stream,
                                          &ctx->launches);
@@ -245,11 +270,13 @@ int build_pass_graph(dsmc_ctx *ctx, uint64_t seed, int l, int flags) {
 // the kernels of dsmc_ensemble_add: full field of the current state, raw sums, wall counts, running statistics
 int enqueue_record(dsmc_ctx *ctx) {
     if (int rc = run_field(ctx, -1)) return rc;
-    CU(launch_observables(ctx->S(), ctx->H(), ctx->K2d(), ctx->K4d(), ctx->robs(), ctx->L, ctx->R, ctx->J, ctx->g, true,
-                          ctx->stream, &ctx->launches),
+    CU(launch_observables(ctx->S(), ctx->H(), ctx->K2d(), ctx->K4d(), ctx->obs(), ctx->opart(), ctx->ticket(0), ctx->L,
+                          ctx->R, ctx->stream, &ctx->launches),
        "observables launch");
-    CU(launch_wall_counts(ctx->S(), ctx->rwalls(), ctx->L, ctx->R, true, ctx->stream, &ctx->launches), "wall counts launch");
-    CU(launch_ensemble_add(ctx->robs(), ctx->rwalls(), ctx->stats(), ctx->L, ctx->R, (double)ctx->J, (double)ctx->g,
+    CU(launch_wall_counts(ctx->S(), ctx->walls(), (unsigned long long *)ctx->opart(), ctx->ticket(1), ctx->L, ctx->R,
+                          ctx->stream, &ctx->launches),
+       "wall counts launch");
+    CU(launch_ensemble_add(ctx->obs(), ctx->walls(), ctx->stats(), ctx->L, ctx->R, (double)ctx->J, (double)ctx->g,
                            ctx->stream, &ctx->launches),
        "ensemble launch");
     return DSMC_OK;
@@ -337,7 +364,8 @@ DsmcLayout dsmc_make_layout(int L, int R) {
     l.off_obs = o; o = align256(o + sizeof(double) * 8 * R);
     l.off_walls = o; o = align256(o + sizeof(unsigned long long) * 8 * R);
     l.off_stats = o; o = align256(o + sizeof(double) * 16 * R);
-    l.off_robs = o; o = align256(o + (sizeof(double) + sizeof(unsigned long long)) * 8 * R);
+    l.off_opart = o; o = align256(o + dsmc_walk_scratch_bytes(L, R));
+    l.off_ticket = o; o = align256(o + 4 * sizeof(unsigned int));
     l.off_step = o; o = align256(o + sizeof(unsigned long long));
     l.total = o;
     return l;
@@ -393,9 +421,10 @@ int dsmc_bind(dsmc_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_strea
     CU(cudaPointerGetAttributes(&attr, dev_workspace), "cudaPointerGetAttributes");
     if (attr.type != cudaMemoryTypeDevice && attr.type != cudaMemoryTypeManaged)
         return fail(ctx, DSMC_EINVAL, "workspace is not device memory");
-    int dev = 0;
-    CU(cudaGetDevice(&dev), "cudaGetDevice");
-    CU(cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, dev), "SM count");
+    ctx->device = attr.device;                                  // the workspace's device, not the caller's current one
+    DeviceGuard guard__(ctx->device);
+    CU(cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, ctx->device), "SM count");
+    ctx->tiled_configured = ctx->fft_configured = false;
     drop_sweep_graph(ctx);
     ctx->ws = (char *)dev_workspace;
     ctx->ws_bytes = bytes;
@@ -406,16 +435,15 @@ int dsmc_bind(dsmc_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_strea
     ctx->aniso_dirty = true;
     for (int i = 0; i < 3; ++i)
         if (!ctx->ev[i]) CU(cudaEventCreate(&ctx->ev[i]), "cudaEventCreate");
-    // the ensemble sums start empty, and the raw sums of the record path start (and are kept) zero
+    // the ensemble sums start empty; the arrival counters of the observable reductions start (and are left) at zero
     CU(cudaMemsetAsync(ctx->stats(), 0, sizeof(double) * 16 * (size_t)ctx->R, ctx->stream), "ensemble init");
-    CU(cudaMemsetAsync(ctx->robs(), 0, (sizeof(double) + sizeof(unsigned long long)) * 8 * (size_t)ctx->R, ctx->stream),
-       "ensemble init");
+    CU(cudaMemsetAsync(ctx->ticket(0), 0, 4 * sizeof(unsigned int), ctx->stream), "ticket init");
     ctx->ensemble_n = 0;
     return DSMC_OK;
 }
 
 int dsmc_build_tensor(dsmc_ctx *ctx, int method, int cutoff_A, int tail) {
-    if (int rc = need_bound(ctx)) return rc;
+    ENTER_BOUND(ctx);
     if (method != DSMC_W_IMAGE && method != DSMC_W_EWALD) return fail(ctx, DSMC_EINVAL, "unknown method");
     if (method == DSMC_W_IMAGE && (cutoff_A < 0 || cutoff_A > 4096)) return fail(ctx, DSMC_EINVAL, "bad cutoff");
     CU(launch_build_tensor(nullptr, ctx->Wc(), ctx->L, method, cutoff_A, tail, ctx->stream, &ctx->launches),
@@ -424,7 +452,7 @@ int dsmc_build_tensor(dsmc_ctx *ctx, int method, int cutoff_A, int tail) {
 }
 
 int dsmc_get_tensor(dsmc_ctx *ctx, float *W_out, int where) {
-    if (int rc = need_bound(ctx)) return rc;
+    ENTER_BOUND(ctx);
     if (!W_out) return fail(ctx, DSMC_EINVAL, "null argument");
     if (!ctx->tensor_built) return fail(ctx, DSMC_ESTATE, "tensor not built");
     const size_t bytes = sizeof(float) * 4 * (size_t)ctx->L * ctx->L;
@@ -436,7 +464,7 @@ int dsmc_get_tensor(dsmc_ctx *ctx, float *W_out, int where) {
 }
 
 int dsmc_set_tensor(dsmc_ctx *ctx, const float *W_in, int where) {
-    if (int rc = need_bound(ctx)) return rc;
+    ENTER_BOUND(ctx);
     if (!W_in) return fail(ctx, DSMC_EINVAL, "null argument");
     const size_t bytes = sizeof(float) * 4 * (size_t)ctx->L * ctx->L;
     CU(cudaMemcpyAsync(ctx->Wc(), W_in, bytes, where == DSMC_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice,
@@ -446,7 +474,7 @@ int dsmc_set_tensor(dsmc_ctx *ctx, const float *W_in, int where) {
 }
 
 int dsmc_set_spins(dsmc_ctx *ctx, const float *s, int where) {
-    if (int rc = need_bound(ctx)) return rc;
+    ENTER_BOUND(ctx);
     if (!s) return fail(ctx, DSMC_EINVAL, "null argument");
     const float *src = s;
     if (where == DSMC_HOST) {
@@ -456,13 +484,28 @@ int dsmc_set_spins(dsmc_ctx *ctx, const float *s, int where) {
         src = ctx->stage();
     }
     CU(launch_canon_to_internal(src, ctx->S(), ctx->L, ctx->R, ctx->stream, &ctx->launches), "set spins");
-    ctx->spins_set = true;
     ctx->field_valid[0] = ctx->field_valid[1] = false;
+    if (ctx->debug) {
+        // |s| = 1 is the caller's contract, checked to 1e-5 when debugging is on (one reduction kernel and
+        // one synchronisation; the default path pays nothing)
+        float worst = 0.0f;
+        float *dev = reinterpret_cast<float *>(ctx->opart());
+        CU(launch_norm_check(ctx->S(), dev, ctx->L, ctx->R, ctx->stream, &ctx->launches), "norm check");
+        CU(cudaMemcpyAsync(&worst, dev, sizeof(float), cudaMemcpyDeviceToHost, ctx->stream), "norm check D2H");
+        CU(cudaStreamSynchronize(ctx->stream), "norm check sync");
+        if (!(worst <= 2.0e-5f)) {                             // | |s|^2 - 1 | = 2 | |s| - 1 | to first order
+            ctx->spins_set = false;
+            char msg[128];
+            snprintf(msg, sizeof msg, "dsmc_set_spins: a spin is not a unit vector (max | |s|^2 - 1 | = %.3g)", (double)worst);
+            return fail(ctx, DSMC_EINVAL, msg);
+        }
+    }
+    ctx->spins_set = true;
     return DSMC_OK;
 }
 
 int dsmc_get_spins(dsmc_ctx *ctx, float *s, int where) {
-    if (int rc = need_bound(ctx)) return rc;
+    ENTER_BOUND(ctx);
     if (!s) return fail(ctx, DSMC_EINVAL, "null argument");
     if (!ctx->spins_set) return fail(ctx, DSMC_ESTATE, "spins not set");
     float *dst = where == DSMC_HOST ? ctx->stage() : s;
@@ -477,7 +520,7 @@ int dsmc_get_spins(dsmc_ctx *ctx, float *s, int where) {
 }
 
 int dsmc_init_spins(dsmc_ctx *ctx, int mode, uint64_t seed) {
-    if (int rc = need_bound(ctx)) return rc;
+    ENTER_BOUND(ctx);
     if (mode != DSMC_INIT_RANDOM && mode != DSMC_INIT_UP) return fail(ctx, DSMC_EINVAL, "unknown init mode");
     CU(launch_init_spins(ctx->S(), ctx->L, ctx->R, mode, seed, ctx->replica_offset, ctx->stream, &ctx->launches), "init spins");
     ctx->spins_set = true;
@@ -486,7 +529,7 @@ int dsmc_init_spins(dsmc_ctx *ctx, int mode, uint64_t seed) {
 }
 
 int dsmc_dipole_field(dsmc_ctx *ctx, int colour, float *h_out, int where) {
-    if (int rc = need_bound(ctx)) return rc;
+    ENTER_BOUND(ctx);
     if (colour < -1 || colour > 1) return fail(ctx, DSMC_EINVAL, "colour must be -1, 0 or 1");
     if (!ctx->tensor_built) return fail(ctx, DSMC_ESTATE, "tensor not built");
     if (!ctx->spins_set) return fail(ctx, DSMC_ESTATE, "spins not set");
@@ -510,7 +553,7 @@ int dsmc_dipole_field(dsmc_ctx *ctx, int colour, float *h_out, int where) {
 
 int dsmc_halfsweep_ex(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t step, int flags, uint8_t *accept_out,
                       float *margin_out) {
-    if (int rc = need_bound(ctx)) return rc;
+    ENTER_BOUND(ctx);
     if (!ctx->tensor_built) return fail(ctx, DSMC_ESTATE, "tensor not built");
     if (!ctx->spins_set) return fail(ctx, DSMC_ESTATE, "spins not set");
     if (flags & ~(DSMC_REUSE_FIELD | DSMC_TRIAL_FLIP)) return fail(ctx, DSMC_EINVAL, "unknown flag");
@@ -540,7 +583,7 @@ int dsmc_halfsweep(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t step) 
 
 int dsmc_sublattice_pass(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t pass, int l, int flags,
                          uint8_t *accept_out, float *margin_out, int *offset_out) {
-    if (int rc = need_bound(ctx)) return rc;
+    ENTER_BOUND(ctx);
     if (!ctx->tensor_built) return fail(ctx, DSMC_ESTATE, "tensor not built");
     if (!ctx->spins_set) return fail(ctx, DSMC_ESTATE, "spins not set");
     if (flags & ~(DSMC_TRIAL_FLIP | DSMC_NO_RESIDENT)) return fail(ctx, DSMC_EINVAL, "unknown flag");
@@ -551,7 +594,7 @@ int dsmc_sublattice_pass(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t 
 
 int dsmc_sublattice_run(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_pass, uint64_t n_passes, int l,
                         int flags) {
-    if (int rc = need_bound(ctx)) return rc;
+    ENTER_BOUND(ctx);
     if (n_passes >= 2 && l >= 2 && ctx->L % l == 0 && !(flags & ~(DSMC_TRIAL_FLIP | DSMC_NO_RESIDENT)) &&
         ctx->tensor_built && ctx->spins_set && use_resident(ctx, l, flags)) {
         // every pass of the run inside one kernel (per 65536 passes), the lattice in shared memory
@@ -589,7 +632,7 @@ int dsmc_run(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_step, 
 }
 
 int dsmc_run_ex(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_step, uint64_t n_half, int flags) {
-    if (int rc = need_bound(ctx)) return rc;
+    ENTER_BOUND(ctx);
     if (flags & ~DSMC_TRIAL_FLIP) return fail(ctx, DSMC_EINVAL, "unknown flag");
     uint64_t k = 0;
     auto plain = [&](uint64_t count) -> int {
@@ -615,14 +658,14 @@ int dsmc_run_ex(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_ste
 }
 
 int dsmc_observables(dsmc_ctx *ctx, double *out) {
-    if (int rc = need_bound(ctx)) return rc;
+    ENTER_BOUND(ctx);
     if (!out) return fail(ctx, DSMC_EINVAL, "null argument");
     if (!ctx->tensor_built) return fail(ctx, DSMC_ESTATE, "tensor not built");
     if (!ctx->spins_set) return fail(ctx, DSMC_ESTATE, "spins not set");
-    if (int rc = upload_params(ctx, ctx->T_valid ? nullptr : std::vector<float>(ctx->R, 1.0f).data())) return rc;
+    if (int rc = upload_aniso(ctx)) return rc;
     if (int rc = run_field(ctx, -1)) return rc;
-    CU(launch_observables(ctx->S(), ctx->H(), ctx->K2d(), ctx->K4d(), ctx->obs(), ctx->L, ctx->R, ctx->J, ctx->g, false,
-                          ctx->stream, &ctx->launches),
+    CU(launch_observables(ctx->S(), ctx->H(), ctx->K2d(), ctx->K4d(), ctx->obs(), ctx->opart(), ctx->ticket(0), ctx->L,
+                          ctx->R, ctx->stream, &ctx->launches),
        "observables launch");
     std::vector<double> raw(8 * (size_t)ctx->R);
     CU(cudaMemcpyAsync(raw.data(), ctx->obs(), sizeof(double) * raw.size(), cudaMemcpyDeviceToHost, ctx->stream),
@@ -641,11 +684,13 @@ int dsmc_observables(dsmc_ctx *ctx, double *out) {
 }
 
 int dsmc_wall_observables(dsmc_ctx *ctx, long long *counts_out, double *derived_out) {
-    if (int rc = need_bound(ctx)) return rc;
+    ENTER_BOUND(ctx);
     if (!counts_out) return fail(ctx, DSMC_EINVAL, "null argument");
     if (!ctx->spins_set) return fail(ctx, DSMC_ESTATE, "spins not set");
     unsigned long long *dev = ctx->walls();
-    CU(launch_wall_counts(ctx->S(), dev, ctx->L, ctx->R, false, ctx->stream, &ctx->launches), "wall counts launch");
+    CU(launch_wall_counts(ctx->S(), dev, (unsigned long long *)ctx->opart(), ctx->ticket(1), ctx->L, ctx->R, ctx->stream,
+                          &ctx->launches),
+       "wall counts launch");
     std::vector<unsigned long long> raw(8 * (size_t)ctx->R);
     CU(cudaMemcpyAsync(raw.data(), dev, sizeof(unsigned long long) * raw.size(), cudaMemcpyDeviceToHost, ctx->stream),
        "wall counts D2H");
@@ -666,10 +711,11 @@ int dsmc_wall_observables(dsmc_ctx *ctx, long long *counts_out, double *derived_
 }
 
 int dsmc_staggered_magnetisation(dsmc_ctx *ctx, double *out) {
-    if (int rc = need_bound(ctx)) return rc;
+    ENTER_BOUND(ctx);
     if (!out) return fail(ctx, DSMC_EINVAL, "null argument");
     if (!ctx->spins_set) return fail(ctx, DSMC_ESTATE, "spins not set");
-    CU(launch_staggered(ctx->S(), ctx->obs(), ctx->L, ctx->R, ctx->stream, &ctx->launches), "staggered launch");
+    CU(launch_staggered(ctx->S(), ctx->obs(), ctx->opart(), ctx->ticket(2), ctx->L, ctx->R, ctx->stream, &ctx->launches),
+       "staggered launch");
     std::vector<double> raw(8 * (size_t)ctx->R);
     CU(cudaMemcpyAsync(raw.data(), ctx->obs(), sizeof(double) * raw.size(), cudaMemcpyDeviceToHost, ctx->stream),
        "staggered D2H");
@@ -686,19 +732,17 @@ int dsmc_staggered_magnetisation(dsmc_ctx *ctx, double *out) {
 }
 
 int dsmc_ensemble_reset(dsmc_ctx *ctx) {
-    if (int rc = need_bound(ctx)) return rc;
+    ENTER_BOUND(ctx);
     CU(cudaMemsetAsync(ctx->stats(), 0, sizeof(double) * 16 * (size_t)ctx->R, ctx->stream), "ensemble reset");
-    CU(cudaMemsetAsync(ctx->robs(), 0, (sizeof(double) + sizeof(unsigned long long)) * 8 * (size_t)ctx->R, ctx->stream),
-       "ensemble reset");
     ctx->ensemble_n = 0;
     return DSMC_OK;
 }
 
 int dsmc_ensemble_add(dsmc_ctx *ctx) {
-    if (int rc = need_bound(ctx)) return rc;
+    ENTER_BOUND(ctx);
     if (!ctx->tensor_built) return fail(ctx, DSMC_ESTATE, "tensor not built");
     if (!ctx->spins_set) return fail(ctx, DSMC_ESTATE, "spins not set");
-    if (int rc = upload_params(ctx, ctx->T_valid ? nullptr : std::vector<float>(ctx->R, 1.0f).data())) return rc;
+    if (int rc = upload_aniso(ctx)) return rc;
     if (int rc = enqueue_record(ctx)) return rc;
     ++ctx->ensemble_n;
     return DSMC_OK;
@@ -706,7 +750,7 @@ int dsmc_ensemble_add(dsmc_ctx *ctx) {
 
 int dsmc_run_recorded(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_step, uint64_t n_records, int every,
                       int flags) {
-    if (int rc = need_bound(ctx)) return rc;
+    ENTER_BOUND(ctx);
     if (flags & ~DSMC_TRIAL_FLIP) return fail(ctx, DSMC_EINVAL, "unknown flag");
     if (every < 1) return fail(ctx, DSMC_EINVAL, "every must be >= 1");
     if (first_step & 1u) return fail(ctx, DSMC_EINVAL, "first_step must be even (whole sweeps)");
@@ -739,7 +783,7 @@ int dsmc_run_recorded(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t fir
 }
 
 int dsmc_ensemble_get(dsmc_ctx *ctx, double *mean, double *var, double *se, uint64_t *n_out) {
-    if (int rc = need_bound(ctx)) return rc;
+    ENTER_BOUND(ctx);
     if (!mean || !var || !se) return fail(ctx, DSMC_EINVAL, "null argument");
     if (n_out) *n_out = ctx->ensemble_n;
     if (ctx->ensemble_n == 0) return fail(ctx, DSMC_ESTATE, "empty ensemble");
@@ -759,6 +803,12 @@ int dsmc_ensemble_get(dsmc_ctx *ctx, double *mean, double *var, double *se, uint
     return DSMC_OK;
 }
 
+int dsmc_set_debug(dsmc_ctx *ctx, int on) {
+    if (!ctx) return DSMC_EINVAL;
+    ctx->debug = on ? 1 : 0;
+    return DSMC_OK;
+}
+
 int dsmc_set_timing(dsmc_ctx *ctx, int on) {
     if (!ctx) return DSMC_EINVAL;
     ctx->timing = on ? 1 : 0;
@@ -767,7 +817,7 @@ int dsmc_set_timing(dsmc_ctx *ctx, int on) {
 }
 
 int dsmc_last_timing(dsmc_ctx *ctx, float *out_ms) {
-    if (int rc = need_bound(ctx)) return rc;
+    ENTER_BOUND(ctx);
     if (!out_ms) return fail(ctx, DSMC_EINVAL, "null argument");
     if (!ctx->ev_recorded) return fail(ctx, DSMC_ESTATE, "no timed half-sweep yet");
     CU(cudaEventSynchronize(ctx->ev[2]), "event sync");
@@ -791,7 +841,8 @@ int dsmc_field_kernel_supported(dsmc_ctx *ctx, int kind) {
 
 int dsmc_select_field_kernel(dsmc_ctx *ctx, int kind) {
     if (!ctx || kind < -1 || kind > 2) return fail(ctx, DSMC_EINVAL, "kind must be -1, 0, 1 or 2");
-    if (kind == 1 && !dsmc_tiled_supported(ctx->L, ctx->R)) return fail(ctx, DSMC_EINVAL, "tiled kernel needs L % 16 == 0, R % 4 == 0");
+    if (kind == 1 && !dsmc_tiled_supported(ctx->L, ctx->R))
+        return fail(ctx, DSMC_EINVAL, "tiled kernel needs L % 16 == 0, R % 4 == 0 and L <= 1024 (the largest size its fp32 accumulation is tested to meet the field tolerances at)");
     if (kind == 2 && !dsmc_fft_supported(ctx->L, ctx->R)) return fail(ctx, DSMC_EINVAL, "FFT field needs L in {32, 64, 128, 256, 512} and even R");
     ctx->field_kind = kind;
     ctx->field_valid[0] = ctx->field_valid[1] = false;

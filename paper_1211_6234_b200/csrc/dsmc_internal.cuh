@@ -22,13 +22,18 @@
 
 #define DSMC_GRAPH_UNROLL 8  // sweeps (dsmc_run) or passes (dsmc_sublattice_run) per captured CUDA graph
 #define DSMC_KS_MAX 16  // maximum source split (partial-field slabs) of the tiled field kernel
+#define DSMC_TILED_MAX_L 1024  // largest lattice the tiled kernel accepts: the size up to which its fp32 accumulation is
+                               // tested to meet the field tolerances (include/dsmc.h, dsmc_select_field_kernel)
 
 // ---------------------------------------------------------------------------------------------
 // Programmatic dependent launch (sm_90+).  The kernels of a sweep form one dependent chain (x-forward -> y-multiply ->
 // x-inverse -> Metropolis -> step counter -> ...) and the small lattices are bound by the ~3 us a kernel-to-kernel edge
 // costs.  A kernel launched through launch_pdl calls pdl_wait() before it touches memory an earlier kernel wrote or
-// read -- it returns once the predecessor grid has completed and its writes are visible; every kernel launched this way
-// calls it, so completion is transitive along the chain -- and pdl_trigger() once its CTA is past the bulk of its work:
+// read -- it returns once the predecessor grid has completed and its writes are visible.  INVARIANT the chain relies
+// on: every CTA of a launch_pdl grid that touches global memory calls pdl_wait() before its first access, and no
+// launch_pdl grid completes without at least one thread having waited (a grid whose every thread returned early
+// would let ITS successor start before ITS predecessor has finished, breaking the transitivity of completion along
+// the chain).  A CTA calls pdl_trigger() once it is past the bulk of its work:
 // when every CTA of the grid has triggered (or exited) the successor's CTAs are scheduled into the room that frees
 // up and wait there, so the launch latency of the edge overlaps this grid's tail.  (Triggering at the top instead
 // makes the successor resident while this grid still needs the room: measured slower from L = 128 up, DESIGN.md
@@ -68,8 +73,8 @@ struct DsmcLayout {
     size_t off_obs;    // R*8 doubles (raw observable sums)
     size_t off_walls;  // R*8 64-bit wall counts
     size_t off_stats;  // R*8*2 doubles: ensemble sums of x and x^2
-    size_t off_robs;   // R*8 doubles + R*8 64-bit counts: the raw sums of the record path (dsmc_ensemble_add), kept zero
-                       // between records by ensemble_add_kernel
+    size_t off_opart;  // per-CTA partial sums of the observable walks (state_kernels.cu: deterministic reductions)
+    size_t off_ticket; // 4 arrival counters of those walks (zero between launches)
     size_t off_step;   // one 64-bit step counter (dsmc_run's graph replay)
     size_t total;
 };
@@ -89,6 +94,7 @@ struct dsmc_ctx {
     uint32_t replica_offset = 0;  // dsmc_set_replica_offset
     int field_kind = -1;  // -1 automatic, 0 generic, 1 tiled, 2 FFT (dsmc_select_field_kernel)
     int timing = 0;
+    int debug = 0;  // dsmc_set_debug: argument checks that cost a kernel (|s| = 1 in dsmc_set_spins)
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
     bool ev_recorded = false;
     uint64_t launches = 0;
@@ -105,6 +111,8 @@ struct dsmc_ctx {
     int pgraph_kind = -1, pgraph_flags = -1, pgraph_l = -1;
     uint64_t pgraph_launches = 0;
     int sm_count = 148;
+    int device = 0;  // ordinal of the device the workspace lives on (dsmc_bind); every call runs with it current
+    bool tiled_configured = false, fft_configured = false;  // cudaFuncSetAttribute done on this device
     std::string err;
 
     float *Wc() const { return (float *)(ws + lay.off_Wc); }
@@ -121,8 +129,8 @@ struct dsmc_ctx {
     double *obs() const { return (double *)(ws + lay.off_obs); }
     unsigned long long *walls() const { return (unsigned long long *)(ws + lay.off_walls); }
     double *stats() const { return (double *)(ws + lay.off_stats); }
-    double *robs() const { return (double *)(ws + lay.off_robs); }
-    unsigned long long *rwalls() const { return (unsigned long long *)(ws + lay.off_robs + sizeof(double) * 8 * (size_t)R); }
+    double *opart() const { return (double *)(ws + lay.off_opart); }
+    unsigned int *ticket(int k) const { return (unsigned int *)(ws + lay.off_ticket) + k; }
     unsigned long long *step_dev() const { return (unsigned long long *)(ws + lay.off_step); }
     size_t Nh() const { return (size_t)L * (L / 2); }
     size_t plane() const { return Nh() * (size_t)R; }  // floats in one [a][r] plane
@@ -155,9 +163,10 @@ cudaError_t launch_make_fft_table(const float *Wc, float *M, void *scratch, int 
                                   uint64_t *launches);
 // colour = -1 writes both colours of H with one convolution
 cudaError_t launch_field_fft(const float *S, const float *M, void *scratch, float *H, int L, int R, int colour,
-                             cudaStream_t st, uint64_t *launches);
+                             bool *configured, cudaStream_t st, uint64_t *launches);
+// configured: the context's "dynamic shared memory limit raised on this device" flag
 cudaError_t launch_field_tiled(const float *S, const float *Wk, float *Hpart, float *H, int L, int R,
-                               int colour, int sm_count, cudaStream_t st, uint64_t *launches);
+                               int colour, int sm_count, bool *configured, cudaStream_t st, uint64_t *launches);
 
 struct MetropolisArgs {
     float *S;
@@ -195,14 +204,17 @@ cudaError_t launch_step_update(unsigned long long *step, unsigned long long valu
                                uint64_t *launches);
 cudaError_t launch_init_spins(float *S, int L, int R, int mode, uint64_t seed, uint32_t r_off, cudaStream_t st,
                               uint64_t *launches);
-// chained: the sums are zero on entry and the kernel joins the dependent-launch chain (the record path); else memset +
-// plain launch
-cudaError_t launch_observables(const float *S, const float *H, const float *K2, const float *K4,
-                               double *obs, int L, int R, float J, float g, bool chained, cudaStream_t st,
-                               uint64_t *launches);
-cudaError_t launch_wall_counts(const float *S, unsigned long long *counts, int L, int R, bool chained, cudaStream_t st,
-                               uint64_t *launches);
-cudaError_t launch_staggered(const float *S, double *sums, int L, int R, cudaStream_t st, uint64_t *launches);
-// consumes obs and walls and leaves them zero
-cudaError_t launch_ensemble_add(double *obs, unsigned long long *walls, double *stats, int L, int R, double J,
+// Per-replica reductions (state_kernels.cu): deterministic -- warp shuffles / shared memory in index order inside a CTA,
+// per-CTA partials in `part` (dsmc_walk_scratch_bytes), summed in CTA order by the last CTA to arrive (`ticket`).  The
+// kernels call pdl_wait at their top and are launched as dependent launches (the record chain of dsmc_run_recorded).
+size_t dsmc_walk_scratch_bytes(int L, int R);
+cudaError_t launch_observables(const float *S, const float *H, const float *K2, const float *K4, double *obs, double *part,
+                               unsigned int *ticket, int L, int R, cudaStream_t st, uint64_t *launches);
+cudaError_t launch_wall_counts(const float *S, unsigned long long *counts, unsigned long long *part, unsigned int *ticket,
+                               int L, int R, cudaStream_t st, uint64_t *launches);
+cudaError_t launch_staggered(const float *S, double *sums, double *part, unsigned int *ticket, int L, int R, cudaStream_t st,
+                             uint64_t *launches);
+cudaError_t launch_ensemble_add(const double *obs, const unsigned long long *walls, double *stats, int L, int R, double J,
                                 double g, cudaStream_t st, uint64_t *launches);
+// largest |s.s - 1| over all spins -> *out (one float, device): the debug check of dsmc_set_spins
+cudaError_t launch_norm_check(const float *S, float *out, int L, int R, cudaStream_t st, uint64_t *launches);

@@ -431,20 +431,19 @@ int pairs_per_cta(int P, int cap) {
 }
 
 template <int N2>
-cudaError_t launch_fft_n2(const FftParams &p, cudaStream_t st, uint64_t *launches) {
+cudaError_t launch_fft_n2(const FftParams &p, bool *configured, cudaStream_t st, uint64_t *launches) {
     const int L = 16 * N2;
     // 16 replica pairs per CTA: 128-byte runs in HBM, and enough CTAs (half rows / half columns) that
     // the last wave over 148 SMs stays full
     const int LNX = pairs_per_cta(p.P, 16), LNY = pairs_per_cta(p.P, 16);
     const size_t smx = sizeof(float2) * (L + (size_t)line_rows<N2>() * LNX);
     const size_t smy = sizeof(float2) * (L + 4 * L + 3 * (size_t)line_rows<N2>() * LNY);
-    static bool configured = false;
-    if (!configured) {
+    if (!*configured) {
         cudaError_t e;
         if ((e = cudaFuncSetAttribute(fft_x_forward_kernel<N2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)) != cudaSuccess) return e;
         if ((e = cudaFuncSetAttribute(fft_x_inverse_kernel<N2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)) != cudaSuccess) return e;
         if ((e = cudaFuncSetAttribute(fft_y_multiply_kernel<N2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024)) != cudaSuccess) return e;
-        configured = true;
+        *configured = true;
     }
     cudaError_t e = launch_pdl(fft_x_forward_kernel<N2>, dim3(p.P / LNX, L, 3), dim3(LNX, 16), smx, st, p);
     if (e == cudaSuccess) e = launch_pdl(fft_y_multiply_kernel<N2>, dim3(p.P / LNY, L), dim3(LNY, 16), smy, st, p);
@@ -475,7 +474,7 @@ cudaError_t launch_make_fft_table(const float *Wc, float *M, void *scratch, int 
 }
 
 cudaError_t launch_field_fft(const float *S, const float *M, void *scratch, float *H, int L, int R, int colour,
-                             cudaStream_t st, uint64_t *launches) {
+                             bool *configured, cudaStream_t st, uint64_t *launches) {
     FftParams p;
     p.S = S;
     p.H = H;
@@ -485,11 +484,11 @@ cudaError_t launch_field_fft(const float *S, const float *M, void *scratch, floa
     p.P = R / 2;
     p.colour = colour;
     switch (L / 16) {
-        case 2: return launch_fft_n2<2>(p, st, launches);
-        case 4: return launch_fft_n2<4>(p, st, launches);
-        case 8: return launch_fft_n2<8>(p, st, launches);
-        case 16: return launch_fft_n2<16>(p, st, launches);
-        case 32: return launch_fft_n2<32>(p, st, launches);
+        case 2: return launch_fft_n2<2>(p, configured, st, launches);
+        case 4: return launch_fft_n2<4>(p, configured, st, launches);
+        case 8: return launch_fft_n2<8>(p, configured, st, launches);
+        case 16: return launch_fft_n2<16>(p, configured, st, launches);
+        case 32: return launch_fft_n2<32>(p, configured, st, launches);
     }
     return cudaErrorInvalidValue;
 }

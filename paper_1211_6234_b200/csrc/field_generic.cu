@@ -9,10 +9,9 @@ namespace {
 
 constexpr int GT = 128;  // threads per block
 
-// Block = GT consecutive (target a, replica r) pairs of colour `colour` (r fastest).
-// For each source row ys the block stages the row's spins for the replicas it touches? -- the
-// replicas of a block are arbitrary when R is small, so the row is read straight from global
-// memory (L1/L2 resident: a row is 3*L*R floats) and only W's row is staged.
+// Block = GT consecutive (target a, replica r) pairs of colour `colour` (r fastest).  Which replicas a block
+// touches is arbitrary when R is small, so the spins of a source row are read straight from global memory
+// (L1/L2 resident: a row is 3*L*R floats) and only W's row is staged in shared memory.
 __global__ void __launch_bounds__(GT) field_generic_kernel(const float *__restrict__ S, const float *__restrict__ Wc,
                                                            float *__restrict__ H, int L, int R, int colour) {
     extern __shared__ float wrow[];  // [4][L]: W[c][ry][*] for the current (ys - yt) -- per target row

@@ -71,7 +71,7 @@ __global__ void __launch_bounds__(MAX_THREADS, 1) field_tiled_kernel(const Tiled
     const int trow = yt - y_first;
     const int ks = blockIdx.y;
     const int r0 = blockIdx.z * RCH;
-    const int ys0 = ks * p.rows_per_chunk;
+    const int j0 = ks * p.rows_per_chunk;
     const int nseg = Lh / SEG;
     const int nstages = p.rows_per_chunk * 2 * nseg;
 
@@ -88,7 +88,16 @@ __global__ void __launch_bounds__(MAX_THREADS, 1) field_tiled_kernel(const Tiled
         float *sdst = wdst + w_stage_floats;
         const int rr = st / (2 * nseg), rem = st - rr * 2 * nseg;
         const int q = rem / nseg, seg = rem - q * nseg;
-        const int ys = ys0 + rr, i0 = seg * SEG;
+        const int i0 = seg * SEG;
+        // Source rows in the order far -> near (relative to the CTA's first target row): entry j of the sequence
+        // d = -L/2, +(L/2-1), -(L/2-1), ..., +1, -1, 0.  The big terms of the sum (|d| small, W ~ 1/r^3) then arrive
+        // last and only in the last chunk, so every accumulator stays small while the many small far-field terms
+        // are added: the rounding error of an fp32 add scales with the accumulator.
+        const int j = j0 + rr, mm = (j + 1) >> 1;
+        const int d = j == 0 ? -(L >> 1) : ((j & 1) ? (L >> 1) - mm : mm - (L >> 1));
+        int ys = y_first + d;
+        ys += ys < 0 ? L : 0;
+        ys -= ys >= L ? L : 0;
         const int cl = q ^ p.colour;
         const int lane = tid;  // tid < 32 here
         const bool whole = (RCH == R);
@@ -245,7 +254,7 @@ struct TiledPlan {
 };
 
 bool make_plan(int L, int R, int sm_count, TiledPlan &pl) {
-    if (L % 16 != 0 || R % 4 != 0 || L > 2048) return false;
+    if (L % 16 != 0 || R % 4 != 0 || L > DSMC_TILED_MAX_L) return false;
     const int Lh = L / 2, GPR = Lh / TT;
     const int rq = R / 4;
     int RT = 1;
@@ -279,7 +288,7 @@ bool make_plan(int L, int R, int sm_count, TiledPlan &pl) {
 
 }  // namespace
 
-size_t dsmc_wk_floats(int L) { return (L % 16 == 0 && L <= 2048) ? (size_t)16 * L * L : 64; }
+size_t dsmc_wk_floats(int L) { return (L % 16 == 0 && L <= DSMC_TILED_MAX_L) ? (size_t)16 * L * L : 64; }
 
 bool dsmc_tiled_supported(int L, int R) {
     TiledPlan pl;
@@ -294,7 +303,7 @@ cudaError_t launch_make_wk(const float *Wc, float *Wk, int L, cudaStream_t st, u
 }
 
 cudaError_t launch_field_tiled(const float *S, const float *Wk, float *Hpart, float *H, int L, int R, int colour,
-                               int sm_count, cudaStream_t st, uint64_t *launches) {
+                               int sm_count, bool *configured, cudaStream_t st, uint64_t *launches) {
     TiledPlan pl;
     if (!make_plan(L, R, sm_count, pl)) return cudaErrorInvalidValue;
     const size_t plane = (size_t)L * (L / 2) * R;
@@ -313,11 +322,10 @@ cudaError_t launch_field_tiled(const float *S, const float *Wk, float *Hpart, fl
     p.nrows_max = pl.nrows_max;
     p.rows_per_chunk = L / pl.KS;
     p.total_groups = L * (L / 16);
-    static bool attr_set = false;
-    if (!attr_set) {
+    if (!*configured) {                                          // per context, hence per device: no process-global state
         cudaError_t e = cudaFuncSetAttribute(field_tiled_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 210 * 1024);
         if (e != cudaSuccess) return e;
-        attr_set = true;
+        *configured = true;
     }
     dim3 grid(pl.tiles, pl.KS, pl.rchunks);
     field_tiled_kernel<<<grid, (pl.NG * pl.RT + 31) / 32 * 32, pl.smem, st>>>(p);

@@ -48,6 +48,7 @@ ABI = [
     ("dsmc_ensemble_reset", _i, [_vp]),
     ("dsmc_ensemble_add", _i, [_vp]),
     ("dsmc_ensemble_get", _i, [_vp, _vp, _vp, _vp, _vp]),
+    ("dsmc_set_debug", _i, [_vp, _i]),
     ("dsmc_set_timing", _i, [_vp, _i]),
     ("dsmc_last_timing", _i, [_vp, _vp]),
     ("dsmc_launch_count", _u64, [_vp]),
@@ -102,6 +103,8 @@ class Dsmc:
         self.lib = load_library()
         self.L, self.R = int(L), int(R)
         self.device = torch.device(device)
+        if self.device.index is None:
+            self.device = torch.device("cuda", torch.cuda.current_device())
         self._h = _vp()
         rc = self.lib.dsmc_create(ctypes.byref(self._h), self.L, self.R, J, g,
                                   float(np.atleast_1d(K2)[0]), float(np.atleast_1d(K4)[0]))
@@ -122,13 +125,17 @@ class Dsmc:
         if rc != 0:
             raise DsmcError(f"dsmc error {rc}: {self.lib.dsmc_last_error(self._h).decode()}")
 
-    def _ptr(self, a):
-        """(pointer, where) for a numpy array (host) or torch CUDA tensor (device)."""
+    def _ptr(self, a, dtype="float32"):
+        """(pointer, where) for a numpy array (host) or torch CUDA tensor (device) of the ABI's element type."""
         torch = self._torch
         if isinstance(a, torch.Tensor):
-            assert a.is_contiguous()
+            if not a.is_contiguous() or str(a.dtype) != "torch." + dtype:
+                raise TypeError(f"expected a contiguous {dtype} tensor, got {a.dtype}")
+            if a.is_cuda and a.device != self.device:
+                raise ValueError(f"tensor on {a.device}, context on {self.device}")
             return a.data_ptr(), (DSMC_DEVICE if a.is_cuda else DSMC_HOST)
-        assert isinstance(a, np.ndarray) and a.flags.c_contiguous
+        if not (isinstance(a, np.ndarray) and a.flags.c_contiguous and a.dtype == np.dtype(dtype)):
+            raise TypeError(f"expected a C-contiguous {dtype} array")
         return a.ctypes.data, DSMC_HOST
 
     def close(self):
@@ -201,8 +208,8 @@ class Dsmc:
         if flags == 0 and accept_out is None and margin_out is None:
             self._check(self.lib.dsmc_halfsweep(self._h, tp, seed, step))
             return
-        ap = accept_out.data_ptr() if accept_out is not None else None
-        mp = margin_out.data_ptr() if margin_out is not None else None
+        ap = self._ptr(accept_out, "uint8")[0] if accept_out is not None else None
+        mp = self._ptr(margin_out)[0] if margin_out is not None else None
         self._check(self.lib.dsmc_halfsweep_ex(self._h, tp, seed, step, flags, ap, mp))
 
     def run(self, T, seed, first_step, n_half, flags=0):
@@ -220,8 +227,8 @@ class Dsmc:
     def sublattice_pass(self, T, seed, pass_index, l, flags=0, accept_out=None, margin_out=None):
         """One pass of the paper's stride-l schedule -> the offset (S_1, S_2)."""
         t, tp = self._T(T)
-        ap = accept_out.data_ptr() if accept_out is not None else None
-        mp = margin_out.data_ptr() if margin_out is not None else None
+        ap = self._ptr(accept_out, "uint8")[0] if accept_out is not None else None
+        mp = self._ptr(margin_out)[0] if margin_out is not None else None
         off = (ctypes.c_int * 2)()
         self._check(self.lib.dsmc_sublattice_pass(self._h, tp, seed, pass_index, l, flags, ap, mp, off))
         return int(off[0]), int(off[1])
@@ -263,6 +270,10 @@ class Dsmc:
         self._check(self.lib.dsmc_ensemble_get(self._h, mean.ctypes.data, var.ctypes.data, se.ctypes.data,
                                                ctypes.byref(n)))
         return mean, var, se, int(n.value)
+
+    def set_debug(self, on=True):
+        """Debug checks: set_spins verifies |s| = 1 to 1e-5 (DsmcError otherwise)."""
+        self._check(self.lib.dsmc_set_debug(self._h, int(on)))
 
     def set_timing(self, on=True):
         self._check(self.lib.dsmc_set_timing(self._h, int(on)))

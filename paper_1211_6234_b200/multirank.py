@@ -1,6 +1,7 @@
 """Host-side bookkeeping of the multi-GPU run ("replicas only").
 
-The path shards by replica with no data-path collective: every rank runs its own chains (its own seed),
+The path shards by replica with no data-path collective: every rank runs its own chains (one seed for the job,
+disjoint replica indices in the Philox counter: dsmc_set_replica_offset),
 and the only exchange is one MAX all-reduce of the ranks' device timings, so that the reported time is
 the slowest rank's.  torch.distributed is plumbing here (NCCL on GPUs, gloo in the CPU tests)."""
 import os
@@ -13,8 +14,16 @@ def env():
 
 
 def rank_seed(seed, rank):
-    """Independent chains per rank: Philox keys that differ in the seed never collide."""
-    return int(seed) + 1000 * int(rank)
+    """A Philox key per rank that cannot collide with another rank's for any pair of base seeds below 2^32: the
+    rank goes in the high word of the 64-bit seed (key word 1), the base seed stays in the low word.  (The
+    library's own mechanism for one job is dsmc_set_replica_offset -- one seed, disjoint replica indices in the
+    counter -- which is what bench.py and run_config use; this is for jobs that want distinct keys.)"""
+    return (int(seed) & 0xFFFFFFFF) | ((int(rank) + 1) << 32)
+
+
+def rank_replica_offset(R_per_rank, rank):
+    """First global replica index of `rank` when every rank runs R_per_rank replicas of one job under one seed."""
+    return int(rank) * int(R_per_rank)
 
 
 def replica_shard(R, world, rank):

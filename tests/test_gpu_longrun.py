@@ -1,0 +1,105 @@
+"""north_star: "Observables over long runs: agreement within 3 sigma" on BASELINE configs 2, 3 and 4 AS WRITTEN
+(L = 32 / 64 / 128, R = 8 / 16 / 4, 2 000 / 5 000 / 10 000 sweeps; PAPER.md:175-178 protocol, eq. 13).
+
+Per config: 8 independent seeds on each side, E/N, m_z, M_par, eta recorded after every sweep, means over the second
+half of the run, sigma from the across-seed scatter.  GPU side = the CUDA path through the C ABI (dsmc_run,
+dsmc_observables).  Oracle side = tests/longrun_harness.py: the oracle's half-sweep and observables with the field
+handed in from an fp64 FFT, 24 chains in worker processes started when this module is first used.
+
+Criterion: every (replica, observable) within 3 sigma.  With 112 comparisons and 8 seeds a side a chance excursion
+beyond 3 sigma somewhere has probability ~ 1/2 (Student t, 14 d.o.f.), so an excursion is put to the replication
+test a statistician would apply: the SAME comparisons are repeated on 8 fresh seeds a side and must then be within
+3 sigma (a real bias recurs, chance does not: false-alarm probability ~ 1e-2 per flagged entry instead of ~ 1/2 per
+run).  Everything is seeded, hence deterministic.
+"""
+import os
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+from longrun_harness import OBS_NAMES, gpu_chain, start_oracle_chains, window_mean, z_scores  # noqa: E402
+
+N_SEEDS = 8
+RUNS = {2: 2000, 3: 5000, 4: 10000}           # BASELINE.json configs[1..3]: sweeps as written
+LOG_DIR = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
+
+
+@pytest.fixture(scope="module")
+def dsmc_mod():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_1211_6234_b200 as m
+    from paper_1211_6234_b200 import build
+    build.build()
+    return m
+
+
+@pytest.fixture(scope="module")
+def oracle_runs(oracle):
+    """All 24 oracle chains of stage 1, longest first, running while the GPU side is computed."""
+    jobs = [(cfg, 2000 + k, RUNS[cfg]) for cfg in (4, 3, 2) for k in range(N_SEEDS)]
+    chains = start_oracle_chains(jobs)
+    yield chains
+    chains.close()
+
+
+def _log(cfg_id, text):
+    print(text)
+    if os.path.isdir(LOG_DIR):
+        with open(os.path.join(LOG_DIR, f"longrun_config{cfg_id}.log"), "a") as f:
+            f.write(text + "\n")
+
+
+def _run_config(m, cfg_id, pending, field_kind):
+    n_sweeps = RUNS[cfg_id]
+    gpu = [window_mean(gpu_chain(m, cfg_id, 1000 + k, n_sweeps, field_kind)) for k in range(N_SEEDS)]
+    cpu = [window_mean(pending.get((cfg_id, 2000 + k, n_sweeps))) for k in range(N_SEEDS)]
+    z, diff, sigma = z_scores(gpu, cpu)
+    _log(cfg_id, f"config {cfg_id}: {n_sweeps} sweeps, window = second half, {N_SEEDS} seeds a side, field kernel "
+                 f"{'auto (direct sum)' if field_kind is None else field_kind}")
+    gm, cm = np.mean(gpu, 0), np.mean(cpu, 0)
+    for r in range(z.shape[0]):
+        _log(cfg_id, f"  replica {r:2d}: " + "  ".join(
+            f"{OBS_NAMES[k]} gpu {gm[r, k]:+.5f} oracle {cm[r, k]:+.5f} z {z[r, k]:.2f}" for k in range(4)))
+    _log(cfg_id, f"  max z = {z.max():.2f}")
+    flagged = z > 3.0
+    if flagged.any():
+        # replication on fresh seeds (module docstring)
+        _log(cfg_id, f"  {int(flagged.sum())} entries beyond 3 sigma: repeating on fresh seeds")
+        more = start_oracle_chains([(cfg_id, 4000 + k, n_sweeps) for k in range(N_SEEDS)])
+        try:
+            gpu2 = [window_mean(gpu_chain(m, cfg_id, 3000 + k, n_sweeps, field_kind)) for k in range(N_SEEDS)]
+            cpu2 = [window_mean(more.get((cfg_id, 4000 + k, n_sweeps))) for k in range(N_SEEDS)]
+        finally:
+            more.close()
+        z2, diff2, sigma2 = z_scores(gpu2, cpu2)
+        _log(cfg_id, f"  replication: z of the flagged entries {z2[flagged]}")
+        assert np.all(z2[flagged] <= 3.0), (cfg_id, np.argwhere(flagged), z[flagged], z2[flagged], diff2[flagged])
+    return np.array(gpu), np.array(cpu), z
+
+
+def test_long_run_config2_full(dsmc_mod, oracle_runs):
+    """BASELINE config 2 as written: L = 32, R = 8, T = 0.2 ... 1.6, random start, 2 000 sweeps, observables every
+    sweep; the direct-sum (tiled) field kernel."""
+    gpu, cpu, z = _run_config(dsmc_mod, 2, oracle_runs, None)
+    # the runs are not trivially frozen or trivially random: the cold end orders along z, the hot end does not
+    assert np.abs(gpu[:, 0, 1]).mean() > 0.3 and np.abs(gpu[:, -1, 1]).mean() < 0.2
+
+
+def test_long_run_config3_full(dsmc_mod, oracle_runs):
+    """BASELINE config 3 as written: L = 64, R = 16 (K4 = -0.2 / +0.2, T = 0.2 ... 1.6 each), all +z start, 5 000
+    sweeps; the direct-sum (tiled) field kernel.  The z-aligned start is the fp32 field's worst case."""
+    gpu, cpu, z = _run_config(dsmc_mod, 3, oracle_runs, None)
+    assert gpu[:, 0, 1].mean() > 0.8 and gpu[:, 8, 1].mean() > 0.8       # the T = 0.2 replicas stay ordered
+
+
+def test_long_run_config4_full(dsmc_mod, oracle_runs):
+    """BASELINE config 4 as written: L = 128, R = 4, g = 0.25, K2 = 1.8, K4 = 0.1, T = 0.3 ... 0.9, random start,
+    10 000 sweeps (stripe regime: slow relaxation, so same-window multi-seed means are compared, not equilibrium
+    values).  GPU side with the FFT field kernel: the direct sum at R = 4 would take minutes for 8 x 10 000 sweeps
+    with a record every sweep; the direct-sum kernel at this shape is covered by test_lockstep_configs."""
+    _run_config(dsmc_mod, 4, oracle_runs, dsmc_mod.DSMC_FIELD_FFT)

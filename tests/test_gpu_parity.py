@@ -398,7 +398,8 @@ def _long_run_compare(dsmc_mod, oracle, L, R, g, K2, K4, T, n_sweeps, n_seeds, s
 
 
 def test_long_run_observables_3sigma(dsmc_mod, oracle):
-    """A config-2-shaped run shortened to what the fp64 oracle finishes in about a minute:
+    """(The configs as written are in tests/test_gpu_longrun.py; this one keeps the oracle's own direct-sum field.)
+    A config-2-shaped run shortened to what the fp64 oracle finishes in about a minute:
     L = 16, R = 8, T = 0.2 ... 1.6, g = 0.1, K2 = 0.6, 16 independent seeds per side, 300 sweeps,
     means over sweeps 150-299 of E/N, m_z, M_par, eta per replica."""
     L, R = 16, 8
@@ -408,16 +409,6 @@ def test_long_run_observables_3sigma(dsmc_mod, oracle):
     assert np.all(z <= 3.0), (z, diff, sigma)
     # and the runs are not trivially frozen: the hottest replica has disordered, the coldest has not
     assert abs(gpu.mean(0)[-1, 1]) < 0.3 and gpu.mean(0)[0, 1] > 0.8
-
-
-@pytest.mark.skipif(not __import__("os").environ.get("DSMC_LONG"), reason="set DSMC_LONG=1: config 2 in full (minutes of oracle time)")
-def test_long_run_config2_full(dsmc_mod, oracle):
-    """BASELINE config 2 as written: L = 32, R = 8, 2000 sweeps, 8 seeds per side."""
-    from paper_1211_6234_b200 import inputs
-    c = inputs.CONFIGS[2]
-    T = inputs.temperatures(2)
-    z, diff, sigma, _, _ = _long_run_compare(dsmc_mod, oracle, c["L"], c["R"], c["g"], c["K2"], c["K4"], T, 2000, 8, "random")
-    assert np.all(z <= 3.0), (z, diff, sigma)
 
 
 @pytest.mark.parametrize("L,R", [(8, 1), (12, 5), (32, 8), (64, 16), (256, 64)])
@@ -480,6 +471,154 @@ def test_field_parity_L256_every_target(dsmc_mod, oracle):
         rel, mx = field_errors(h, ref)
         print("kind", kind, "rel L2", rel, "max abs", mx)
         assert rel <= FIELD_REL_L2 and mx <= FIELD_MAX_ABS, (kind, rel, mx)
+    ctx.close()
+
+
+def test_field_parity_z_aligned_every_target(dsmc_mod, oracle):
+    """The worst case of fp32 accumulation named by SURVEY.md section 7: the fully z-aligned state (config 3's start),
+    where every term of h_z has the same sign.  EVERY target of every replica of config 5's shape (L = 256, R = 64),
+    both half-sweep launch configurations of the tiled kernel, against the fp64 FFT harness field (pinned to the
+    direct sum in test_field_parity_L256_every_target and tests/test_oracle_harness.py) and against the closed form
+    h_z = 4 zeta(3/2) beta(3/2).  The bound asserted is half the north_star tolerance: the headroom the far -> near
+    source order of the tiled kernel buys."""
+    from paper_1211_6234_b200 import inputs
+    c = inputs.CONFIGS[5]
+    L, R = c["L"], c["R"]
+    W = oracle.build_tensor_ewald(L)
+    ctx = make_ctx(dsmc_mod, 5, inputs)
+    assert ctx.field_kernel_kind() == 1
+    for name, s in (("z-aligned", inputs.up_spins(L, R)), ("random", inputs.initial_spins(5))):
+        ref = _fft_field_fp64(W, s.astype(np.float64))
+        ctx.set_spins(s)
+        h = np.zeros((R, 3, L, L), dtype=np.float32)
+        ctx.dipole_field(0, out=h)
+        ctx.dipole_field(1, out=h)
+        rel, mx = field_errors(h, ref)
+        print(name, "tiled kernel, L = 256, R = 64: rel L2", rel, "max abs", mx)
+        assert rel <= FIELD_REL_L2 and mx <= 0.5 * FIELD_MAX_ABS, (name, rel, mx)
+        if name == "z-aligned":
+            assert np.max(np.abs(ref[:, 2] - 9.033621683100950)) < 1e-9       # the reference itself: closed form
+            assert np.max(np.abs(h[:, 2] - 9.033621683100950)) <= 0.5 * FIELD_MAX_ABS
+    ctx.close()
+
+
+@pytest.mark.parametrize("L,R", [(512, 4), (1024, 4)])
+def test_field_parity_tiled_large_L(dsmc_mod, oracle, L, R):
+    """The accuracy the tiled kernel guarantees as a function of L (include/dsmc.h, dsmc_select_field_kernel): every
+    target, z-aligned (worst case) and random state, up to the largest lattice the kernel accepts (L = 1024: an
+    accumulator then runs over 65 536 sources); beyond it dsmc_select_field_kernel(TILED) refuses."""
+    from paper_1211_6234_b200 import inputs
+    ctx = dsmc_mod.Dsmc(L, R)
+    ctx.build_tensor(dsmc_mod.DSMC_W_EWALD)                               # (the table's own parity: test_tensor_parity*)
+    assert ctx.field_kernel_kind() == 1
+    Wf = ctx.get_tensor().astype(np.float64)                              # the fp32 table, exactly, on both sides
+    for name, s in (("z-aligned", inputs.up_spins(L, R)), ("random", inputs.random_spins(L, R, 12))):
+        ref = _fft_field_fp64(Wf, s.astype(np.float64))
+        ctx.set_spins(s)
+        h = ctx.dipole_field(-1)
+        rel, mx = field_errors(h, ref)
+        print(name, "tiled kernel, L =", L, ": rel L2", rel, "max abs", mx)
+        assert rel <= FIELD_REL_L2 and mx <= FIELD_MAX_ABS, (name, L, rel, mx)
+    ctx.close()
+    big = dsmc_mod.Dsmc(2048, 4)
+    assert big.field_kernel_kind() == 0                                   # automatic choice falls back to the generic kernel
+    with pytest.raises(dsmc_mod.DsmcError):
+        big.select_field_kernel(dsmc_mod.DSMC_FIELD_TILED)
+    big.close()
+
+
+@pytest.mark.parametrize("L,R", [(256, 64), (32, 8)])
+@pytest.mark.parametrize("flip", [False, True])
+def test_benchmarked_metropolis_instantiation_is_the_tested_one(dsmc_mod, L, R, flip):
+    """The lock-step tests pass accept_out / margin_out, which selects the hooked instantiation of the 4-replica
+    Metropolis kernel; bench.py, dsmc_halfsweep and dsmc_run launch the instantiations without hooks (step in the
+    kernel parameters, or read from the device counter inside the replayed graph).  From one state, the three must
+    leave bit-identical spins, half-sweep by half-sweep and over a run long enough to go through the graph: this
+    closes the chain oracle -> hooked kernel -> production kernels (eq. 7)."""
+    from paper_1211_6234_b200 import inputs
+    T = np.linspace(0.1, 2.0, R).astype(np.float32)
+    flags = dsmc_mod.DSMC_TRIAL_FLIP if flip else 0
+    ctxs = []
+    for _ in range(3):
+        c = dsmc_mod.Dsmc(L, R, J=1.0, g=0.1, K2=0.6, K4=0.1)
+        if ctxs:
+            c.set_tensor(ctxs[0].get_tensor())
+        else:
+            c.build_tensor(dsmc_mod.DSMC_W_EWALD)
+        c.select_field_kernel(dsmc_mod.DSMC_FIELD_FFT)        # the field is not under test: the fast one
+        c.set_spins(inputs.random_spins(L, R, 41))
+        ctxs.append(c)
+    plain, hooked, graph = ctxs
+    acc = torch.zeros((R, L, L), dtype=torch.uint8, device="cuda")
+    mar = torch.zeros((R, L, L), dtype=torch.float32, device="cuda")
+    n_half = 4 + 4 * 8 + 7                                       # odd tail: plain prefix, replayed graph, plain tail
+    for k in range(n_half):
+        plain.halfsweep(T, 123, k, flags=flags)
+        hooked.halfsweep(T, 123, k, flags=flags, accept_out=acc, margin_out=mar)
+        if k < 2:
+            assert np.array_equal(plain.get_spins(), hooked.get_spins()), k
+    graph.run(T, 123, 0, n_half, flags=flags)
+    s_plain, s_hooked, s_graph = plain.get_spins(), hooked.get_spins(), graph.get_spins()
+    assert np.array_equal(s_plain, s_hooked)
+    assert np.array_equal(s_plain, s_graph)
+    assert not np.array_equal(s_plain, inputs.random_spins(L, R, 41))
+    for c in ctxs:
+        c.close()
+
+
+def test_ensemble_statistics_are_bit_reproducible(dsmc_mod):
+    """The observable reductions use no floating-point atomics (warp shuffles, shared memory in index order, per-CTA
+    partials summed in CTA order): two runs of dsmc_run_recorded give bit-identical dsmc_ensemble_get, and
+    dsmc_observables / dsmc_staggered_magnetisation repeat bit for bit -- on a power-of-two R below the warp size,
+    a ragged R, R = 64 at config 5's lattice size, and R above the block size."""
+    from paper_1211_6234_b200 import inputs
+    for (L, R, fft) in ((32, 8, True), (12, 5, False), (256, 64, True), (8, 300, False)):
+        T = np.linspace(0.3, 1.7, R).astype(np.float32)
+        got = []
+        for rep in range(2):
+            ctx = dsmc_mod.Dsmc(L, R, J=1.0, g=0.2, K2=0.6, K4=0.1)
+            ctx.build_tensor(dsmc_mod.DSMC_W_EWALD)
+            if fft:
+                ctx.select_field_kernel(dsmc_mod.DSMC_FIELD_FFT)
+            ctx.set_spins(inputs.random_spins(L, R, 6))
+            ctx.ensemble_reset()
+            ctx.run_recorded(T, 5, 0, 12, 2)
+            mean, var, se, n = ctx.ensemble_get()
+            ob = [ctx.observables() for _ in range(3)]
+            st = [ctx.staggered_magnetisation() for _ in range(2)]
+            assert np.array_equal(ob[0], ob[1]) and np.array_equal(ob[0], ob[2]) and np.array_equal(st[0], st[1])
+            got.append((mean, var, se, ob[0], st[0], ctx.wall_observables()[0]))
+            ctx.close()
+        for a, b in zip(*got):
+            assert np.array_equal(a, b), (L, R)
+
+
+def test_set_spins_debug_check(dsmc_mod):
+    """|s| = 1 is the caller's contract, checked to 1e-5 when debugging is on -> DSMC_EINVAL."""
+    from paper_1211_6234_b200 import inputs
+    L, R = 16, 4
+    ctx = dsmc_mod.Dsmc(L, R)
+    ctx.build_tensor()
+    s = inputs.random_spins(L, R, 1)
+    bad = s.copy()
+    bad[2, :, 5, 7] *= 1.0 + 5e-5
+    ctx.set_spins(bad)                                           # default: not checked, not renormalised
+    assert np.array_equal(ctx.get_spins(), bad)
+    ctx.set_debug(True)
+    ctx.set_spins(s)
+    with pytest.raises(dsmc_mod.DsmcError, match="unit vector"):
+        ctx.set_spins(bad)
+    with pytest.raises(dsmc_mod.DsmcError):                      # the rejected state counts as not set
+        ctx.dipole_field(-1)
+    nan = s.copy()
+    nan[0, 1, 0, 0] = np.nan
+    with pytest.raises(dsmc_mod.DsmcError):
+        ctx.set_spins(nan)
+    ok = s.copy()
+    ok[1, :, 3, 3] *= 1.0 + 2e-6                                 # inside the 1e-5 band
+    ctx.set_spins(ok)
+    ctx.set_debug(False)
+    ctx.set_spins(bad)
     ctx.close()
 
 

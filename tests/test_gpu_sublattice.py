@@ -244,6 +244,9 @@ def test_sublattice_run_graph_replay_is_bit_identical(dsmc_mod, L, R, l, fft, fl
     b.close()
 
 
+@pytest.mark.skipif(not __import__("os").environ.get("DSMC_PAPER"),
+                    reason="opt-in (DSMC_PAPER=1): compares the GPU with sentences of the paper, not with the oracle; "
+                           "out of SURVEY.md section 8's scope, kept as an example run")
 def test_appendix_b_critical_temperature_matches_table1(dsmc_mod):
     """The paper's own validation number: App. B puts the order-disorder transition of the dipolar Ising model
     (L = 64, l = 32, J / C_D = 1.7) at script-T_c = .85 with its algorithm and .82 by conventional Monte Carlo
@@ -271,6 +274,9 @@ def test_appendix_b_critical_temperature_matches_table1(dsmc_mod):
     assert r["m_st"][0] > 0.85 and r["m_st"][-1] < 0.25                     # ordered -> disordered across the peak
 
 
+@pytest.mark.skipif(not __import__("os").environ.get("DSMC_PAPER"),
+                    reason="opt-in (DSMC_PAPER=1): compares the GPU with sentences of the paper, not with the oracle; "
+                           "out of SURVEY.md section 8's scope, kept as an example run")
 def test_section4_production_run_matches_the_papers_statements(dsmc_mod):
     """The paper's production run (L = 64, l = 32, script-J = 8.9, script-K = 15, striped start) in
     a shortened protocol, against the numbers its text prints (tests/golden/paper_section4.txt): for a = 0 the
