@@ -114,8 +114,8 @@ int run_field(dsmc_ctx *ctx, int colour) {
     cudaError_t e = cudaSuccess;
     const int kind = field_kind(ctx);
     if (kind == 2) {
-        e = launch_field_fft(ctx->S(), ctx->M(), ctx->Z(), ctx->H(), ctx->L, ctx->R, colour, &ctx->fft_configured,
-                             ctx->stream, &ctx->launches);
+        e = launch_field_fft(ctx->S(), ctx->M(), ctx->Z(), ctx->C(), ctx->H(), ctx->L, ctx->R, colour, ctx->spec_valid,
+                             &ctx->fft_configured, ctx->stream, &ctx->launches);
     } else {
         for (int q = 0; q < 2 && e == cudaSuccess; ++q) {
             if (colour >= 0 && colour != q) continue;
@@ -147,6 +147,7 @@ int after_tensor_change(dsmc_ctx *ctx) {
     CU(cudaStreamSynchronize(ctx->stream), "tensor sync");
     ctx->tensor_built = true;
     ctx->field_valid[0] = ctx->field_valid[1] = false;
+    ctx->spec_valid[0] = ctx->spec_valid[1] = false;
     drop_sweep_graph(ctx);  // W(0) is baked into the captured kernel parameters
     return DSMC_OK;
 }
@@ -212,6 +213,7 @@ int enqueue_pass(dsmc_ctx *ctx, uint64_t seed, uint64_t pass, int l, int flags, 
         const MetropolisArgs a = metropolis_args(ctx, 0, seed, pass, flags, accept_out, margin_out);
         CU(launch_sublattice_resident(a, ctx->Wc(), l, pass, 1, ctx->stream, &ctx->launches), "resident pass launch");
         ctx->field_valid[0] = ctx->field_valid[1] = false;
+        ctx->spec_valid[0] = ctx->spec_valid[1] = false;
         return DSMC_OK;
     }
     if (fft)
@@ -221,6 +223,7 @@ int enqueue_pass(dsmc_ctx *ctx, uint64_t seed, uint64_t pass, int l, int flags, 
     CU(launch_sublattice_pass(a, ctx->Wc(), ctx->stage(), ctx->sm_count, l, ox, oy, fft, ctx->stream, &ctx->launches),
        "sub-lattice pass launch");
     ctx->field_valid[0] = ctx->field_valid[1] = false;
+    ctx->spec_valid[0] = ctx->spec_valid[1] = false;
     return DSMC_OK;
 }
 
@@ -289,8 +292,11 @@ int enqueue_record(dsmc_ctx *ctx) {
 // dsmc_ensemble_add (dsmc_run_recorded).
 int build_sweep_graph(dsmc_ctx *ctx, uint64_t seed, int flags, int record_every) {
     const int kind = field_kind(ctx);
+    // the kernels a field call enqueues depend on which half-spectra are current (FFT field): a graph is only valid
+    // from the state it was captured in, and must leave that state behind to be replayed back to back
+    const int spec_in = (ctx->spec_valid[0] ? 1 : 0) | (ctx->spec_valid[1] ? 2 : 0);
     if (ctx->sweep_graph && ctx->graph_seed == seed && ctx->graph_kind == kind && ctx->graph_flags == flags &&
-        ctx->graph_every == record_every)
+        ctx->graph_every == record_every && ctx->graph_spec_in == spec_in)
         return DSMC_OK;
     drop_sweep_graph(ctx);
     if (!ctx->capture_stream)
@@ -312,6 +318,7 @@ int build_sweep_graph(dsmc_ctx *ctx, uint64_t seed, int flags, int record_every)
                 a.step_off = (uint32_t)(2 * rep + colour);  // the counter moves once per graph, not once per sweep
                 e = launch_metropolis(a, ctx->stream, &ctx->launches);
                 if (e != cudaSuccess) break;
+                ctx->spec_valid[colour] = false;
             }
         }
         if (e == cudaSuccess && rc == DSMC_OK)
@@ -323,6 +330,13 @@ int build_sweep_graph(dsmc_ctx *ctx, uint64_t seed, int flags, int record_every)
     ctx->stream = saved;
     ctx->graph_launches = ctx->launches - l0;
     ctx->launches = l0;
+    const int spec_out = (ctx->spec_valid[0] ? 1 : 0) | (ctx->spec_valid[1] ? 2 : 0);
+    ctx->spec_valid[0] = spec_in & 1;                           // nothing has run: back to the state before the capture
+    ctx->spec_valid[1] = (spec_in & 2) != 0;
+    if (rc == DSMC_OK && e == cudaSuccess && spec_out != spec_in) {
+        if (graph) cudaGraphDestroy(graph);
+        return fail(ctx, DSMC_ESTATE, "internal: a captured sweep does not return to the spectrum state it started from");
+    }
     if (rc != DSMC_OK) {
         if (graph) cudaGraphDestroy(graph);
         return rc;
@@ -341,6 +355,8 @@ int build_sweep_graph(dsmc_ctx *ctx, uint64_t seed, int flags, int record_every)
     ctx->graph_kind = kind;
     ctx->graph_flags = flags;
     ctx->graph_every = record_every;
+    ctx->graph_spec_in = spec_in;
+    ctx->graph_spec_out = spec_out;
     return DSMC_OK;
 }
 
@@ -359,6 +375,7 @@ DsmcLayout dsmc_make_layout(int L, int R) {
     const bool fft = dsmc_fft_supported(L, R);
     l.off_M = o; o = align256(o + (fft ? sizeof(float) * dsmc_fft_m_floats(L) : 0));
     l.off_Z = o; o = align256(o + (fft ? dsmc_fft_scratch_bytes(L, R) : 0));
+    l.off_C = o; o = align256(o + (fft ? dsmc_fft_cache_bytes(L, R) : 0));
     l.off_stage = o; o = align256(o + sizeof(float) * 3 * N * R);
     l.off_T = o; o = align256(o + sizeof(float) * 3 * R);
     l.off_obs = o; o = align256(o + sizeof(double) * 8 * R);
@@ -431,6 +448,7 @@ int dsmc_bind(dsmc_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_strea
     ctx->stream = (cudaStream_t)cuda_stream;
     ctx->tensor_built = ctx->spins_set = false;
     ctx->field_valid[0] = ctx->field_valid[1] = false;
+    ctx->spec_valid[0] = ctx->spec_valid[1] = false;
     ctx->T_valid = false;
     ctx->aniso_dirty = true;
     for (int i = 0; i < 3; ++i)
@@ -485,6 +503,7 @@ int dsmc_set_spins(dsmc_ctx *ctx, const float *s, int where) {
     }
     CU(launch_canon_to_internal(src, ctx->S(), ctx->L, ctx->R, ctx->stream, &ctx->launches), "set spins");
     ctx->field_valid[0] = ctx->field_valid[1] = false;
+    ctx->spec_valid[0] = ctx->spec_valid[1] = false;
     if (ctx->debug) {
         // |s| = 1 is the caller's contract, checked to 1e-5 when debugging is on (one reduction kernel and
         // one synchronisation; the default path pays nothing)
@@ -525,6 +544,7 @@ int dsmc_init_spins(dsmc_ctx *ctx, int mode, uint64_t seed) {
     CU(launch_init_spins(ctx->S(), ctx->L, ctx->R, mode, seed, ctx->replica_offset, ctx->stream, &ctx->launches), "init spins");
     ctx->spins_set = true;
     ctx->field_valid[0] = ctx->field_valid[1] = false;
+    ctx->spec_valid[0] = ctx->spec_valid[1] = false;
     return DSMC_OK;
 }
 
@@ -568,6 +588,7 @@ int dsmc_halfsweep_ex(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t ste
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[1], ctx->stream), "event");
     const MetropolisArgs a = metropolis_args(ctx, colour, seed, step, flags, accept_out, margin_out);
     CU(launch_metropolis(a, ctx->stream, &ctx->launches), "metropolis launch");
+    ctx->spec_valid[colour] = false;                            // the cached half-spectrum of this colour is stale now
     if (ctx->timing) {
         CU(cudaEventRecord(ctx->ev[2], ctx->stream), "event");
         ctx->ev_recorded = true;
@@ -603,6 +624,7 @@ int dsmc_sublattice_run(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t f
         CU(launch_sublattice_resident(a, ctx->Wc(), l, first_pass, n_passes, ctx->stream, &ctx->launches),
            "resident run launch");
         ctx->field_valid[0] = ctx->field_valid[1] = false;
+        ctx->spec_valid[0] = ctx->spec_valid[1] = false;
         return DSMC_OK;
     }
     uint64_t k = 0;
@@ -651,6 +673,8 @@ int dsmc_run_ex(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_ste
             for (uint64_t j = 0; j < reps; ++j) CU(cudaGraphLaunch(ctx->sweep_graph, ctx->stream), "sweep graph launch");
             ctx->launches += reps * ctx->graph_launches;
             ctx->field_valid[0] = ctx->field_valid[1] = true;
+            ctx->spec_valid[0] = ctx->graph_spec_out & 1;           // (= the state the graph started from)
+            ctx->spec_valid[1] = (ctx->graph_spec_out & 2) != 0;
             k += 2 * DSMC_GRAPH_UNROLL * reps;
         }
     }
@@ -774,6 +798,8 @@ int dsmc_run_recorded(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t fir
         for (uint64_t j = 0; j < reps; ++j) CU(cudaGraphLaunch(ctx->sweep_graph, ctx->stream), "record graph launch");
         ctx->launches += reps * ctx->graph_launches;
         ctx->field_valid[0] = ctx->field_valid[1] = true;
+        ctx->spec_valid[0] = ctx->graph_spec_out & 1;
+        ctx->spec_valid[1] = (ctx->graph_spec_out & 2) != 0;
         ctx->ensemble_n += reps;
         done += reps;
     }

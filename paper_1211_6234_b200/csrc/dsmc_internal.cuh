@@ -66,8 +66,9 @@ struct DsmcLayout {
     size_t off_S;      // spins, internal layout
     size_t off_H;      // field, internal layout (both colours)
     size_t off_Hpart;  // partial fields [KS][3][Nh][R] of the tiled kernel
-    size_t off_M;      // spectral multiplier M[slot_x][slot_y][8] of the FFT field (field_fft.cu)
-    size_t off_Z;      // spectrum scratch Z[3][L][L][R/2] complex of the FFT field
+    size_t off_M;      // folded spectral tables AB[slot_x < L/2][slot_y][16] of the FFT field (field_fft.cu)
+    size_t off_Z;      // line scratch Z[3][L/2][pair blocks][L][lane] complex of the FFT field
+    size_t off_C;      // the two half-spectrum caches C[colour][3][L/2][pair blocks][L][lane] complex
     size_t off_stage;  // canonical staging [R][3][L][L] floats
     size_t off_T;      // invT[R], K2[R], K4[R] floats
     size_t off_obs;    // R*8 doubles (raw observable sums)
@@ -90,6 +91,7 @@ struct dsmc_ctx {
     DsmcLayout lay;
     bool tensor_built = false, spins_set = false;
     bool field_valid[2] = {false, false};
+    bool spec_valid[2] = {false, false};  // FFT field: the cache holds the half-spectrum of colour c of the CURRENT spins
     float w0[4] = {0, 0, 0, 0};  // W(0) components (fp32, as stored)
     uint32_t replica_offset = 0;  // dsmc_set_replica_offset
     int field_kind = -1;  // -1 automatic, 0 generic, 1 tiled, 2 FFT (dsmc_select_field_kernel)
@@ -104,6 +106,7 @@ struct dsmc_ctx {
     cudaGraphExec_t sweep_graph = nullptr;
     uint64_t graph_seed = 0;
     int graph_kind = -1, graph_flags = -1, graph_every = -1;  // graph_every > 0: sweeps + record (dsmc_run_recorded)
+    int graph_spec_in = -1, graph_spec_out = -1;  // spec_valid (bit c) the capture started from / ended with
     uint64_t graph_launches = 0;
     // one stride-l pass (field + flip + pass counter += 1) for dsmc_sublattice_run
     cudaGraphExec_t pass_graph = nullptr;
@@ -122,6 +125,7 @@ struct dsmc_ctx {
     float *Hpart() const { return (float *)(ws + lay.off_Hpart); }
     float *M() const { return (float *)(ws + lay.off_M); }
     void *Z() const { return (void *)(ws + lay.off_Z); }
+    void *C() const { return (void *)(ws + lay.off_C); }
     float *stage() const { return (float *)(ws + lay.off_stage); }
     float *invT() const { return (float *)(ws + lay.off_T); }
     float *K2d() const { return invT() + R; }
@@ -159,11 +163,13 @@ cudaError_t launch_field_generic(const float *S, const float *Wc, float *H, int 
 bool dsmc_fft_supported(int L, int R);
 size_t dsmc_fft_m_floats(int L);
 size_t dsmc_fft_scratch_bytes(int L, int R);
+size_t dsmc_fft_cache_bytes(int L, int R);
 cudaError_t launch_make_fft_table(const float *Wc, float *M, void *scratch, int L, cudaStream_t st,
                                   uint64_t *launches);
-// colour = -1 writes both colours of H with one convolution
-cudaError_t launch_field_fft(const float *S, const float *M, void *scratch, float *H, int L, int R, int colour,
-                             bool *configured, cudaStream_t st, uint64_t *launches);
+// colour = -1 writes both colours of H.  valid[2]: which colours' half-spectra in `cache` are those of the current
+// spins; updated here (a colour transformed forward becomes valid), cleared by the caller when a colour's spins change
+cudaError_t launch_field_fft(const float *S, const float *AB, void *scratch, void *cache, float *H, int L, int R, int colour,
+                             bool *valid, bool *configured, cudaStream_t st, uint64_t *launches);
 // configured: the context's "dynamic shared memory limit raised on this device" flag
 cudaError_t launch_field_tiled(const float *S, const float *Wk, float *Hpart, float *H, int L, int R,
                                int colour, int sm_count, bool *configured, cudaStream_t st, uint64_t *launches);

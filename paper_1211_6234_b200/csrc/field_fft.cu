@@ -1,25 +1,33 @@
 // field_fft.cu -- a1, spectral route ("more efficient
-// parallelization of the dipole sum"): the dipole field as a batched circular convolution by FFT.
+// parallelization of the dipole sum"): the dipole field as a batched circular convolution by FFT,
+// organised around the checkerboard: every transform is a HALF-size transform of one colour.
 //
-//   h_n^a = sum_m W^{ab}(m - n) s_m^b  =  (w' (*) s)(n),  w'(d) = W(-d)
-//   => h^ = M . s^,   M^{ab}(k) = sum_rho W^{ab}(rho) e^{+i k.rho}
+//   h_n^a = sum_m W^{ab}(m - n) s_m^b  =>  h^(k) = M(k) s^(k),  M^{ab}(k) = sum_rho W^{ab}(rho) e^{+i k.rho}
 //
-// W is real, so F^-1[ M F[a + i b] ] = w' (*) a + i w' (*) b for real fields a, b: two replicas ride
-// through one complex transform as real and imaginary part.  In the [q][c][a][r] layout replicas
-// r, r+1 are adjacent floats, i.e. the spin array already IS an array of complex "replica pairs";
-// no packing, no Hermitian bookkeeping, and M may be complex (W need not be even).
+// Colour c = (x + y) & 1 holds the sites x = 2 i + p_c(y), p_c(y) = (y + c) & 1, i in [0, L/2): the dense array
+// S[c][a][y L/2 + i][r] of the internal layout.  Its transform
+//   S^_c(kx, ky) = sum_y e^{-2 pi i ky y / L} e^{-2 pi i kx p_c(y) / L} G_{c,y}(kx),   G_{c,y} = (L/2)-point FFT of row y over i,
+// obeys S^_c(kx + L/2, ky) = (-1)^c S^_c(kx, ky + L/2), so kx in [0, L/2) carries everything ("half-spectrum": N/2 values),
+// and the field at the sites of colour t needs only the folded spectrum
+//   H^_t(kx, ky) = h^(kx, ky) + (-1)^t h^(kx + L/2, ky + L/2) = A(kx, ky) S^_t(kx, ky) + B(kx, ky) S^_{1-t}(kx, ky),
+//   A = M(k) + M(k + (L/2, L/2))  (displacements of even parity: same colour),  B = M(k) - M(k + (L/2, L/2))  (odd parity),
+//   h_t(i, y) = (1/N) sum_{kx < L/2} e^{2 pi i kx i / (L/2)} e^{+2 pi i kx p_t(y) / L} sum_ky H^_t(kx, ky) e^{2 pi i ky y / L}.
+// A checkerboard half-sweep of colour t changes only colour t, so in a running sweep the half-spectrum of the colour
+// that was just updated is the only thing to recompute: S^_t from the half-sweep before last is still valid and is kept
+// in a cache (C).  One field = three kernels, each a half-size pass:
+//   fftc_x_forward   rows of the updated colour: (L/2)-point FFT over i, row phase, -> Z[a][slot_x][pb][y][lane]
+//   fftc_y           columns kx < L/2: L-point FFT over y -> S^_{1-t} (stored to the cache), H^_t = A S^_t + B S^_{1-t},
+//                    inverse L-point FFT over ky, in place in Z
+//   fftc_x_inverse   rows of the target colour: row phase, inverse (L/2)-point FFT -> H (colour t only, dense)
+// i.e. 2 half-size 2-D transforms per field where the full-lattice formulation needs 1 full forward + 1 full inverse.
 //
-// Three kernels per field, all fp32, every global access a contiguous run over replica pairs:
-//   fft_x_forward   (row y, component c): gather the row from the two colour arrays, length-L FFT
-//                    along x, write Z[c][y][slot_x][pair]
-//   fft_y_multiply  (column slot_x, 16 pairs): FFT along y, multiply by M (mixing x and y
-//                    components), inverse FFT along y, in place in Z
-//   fft_x_inverse   (row y, component c): inverse FFT along x, scatter to H (only the colour asked)
-// A length-L transform (L = 16 * N2, N2 in {2,...,32}) is the four-step algorithm: 16-point FFTs in
-// registers over the stride-N2 sub-sequences, twiddle, one pass through shared memory, N2-point
-// FFTs in registers.  The spectrum is left in "slot order" slot(k) = N2 * (k mod 16) + k div 16;
-// the inverse runs the same steps backwards, so no bit/digit reversal pass exists anywhere and M
-// is simply tabulated in slot order.  The 1/N of the inverse transform is folded into M.
+// W is real, so the whole map s -> h is a real linear operator and two replicas ride through every complex transform as
+// real and imaginary part: replicas r, r+1 are adjacent floats of the [c][a][site][r] layout, i.e. the spin array already
+// IS an array of complex "replica pairs".  M may be complex (W need not be even).
+// A length-n transform (n = 16 * N2) is the four-step algorithm: 16-point FFTs in registers over the stride-N2
+// sub-sequences, twiddle, one pass through shared memory, N2-point FFTs in registers; spectra stay in "slot order"
+// slot(k) = N2 (k mod 16) + k div 16 and the inverse runs the steps backwards, so no reordering pass exists anywhere and
+// A, B are tabulated in slot order with the 1/N of the inverse folded in.
 #include "dsmc_internal.cuh"
 
 namespace {
@@ -123,26 +131,27 @@ __device__ __forceinline__ void fft_reg(float2 (&v)[N]) {
     }
 }
 
-// ---- the four steps of a length L = 16 * N2 transform --------------------------------------
+// ---- the four steps of a length n = 16 * N2 transform --------------------------------------
 // buf[sidx(k1, n2) * LN + lane] is the CTA's shared line buffer (LN = replica pairs per CTA): slot
-// N2 k1 + n2 with one pad row per block of N2 slots, so that the two blocks a 16-lane warp touches in
-// step 2 fall on different banks.  tw[j] = (cos, sin)(2 pi j / L).  Threads are (lane, t), t in [0, 16).
+// N2 k1 + n2 with one pad row per block of N2 slots, so that blocks k1, k1 + 1 of a warp fall on different banks when
+// LN < 16.  tw[j] = (cos, sin)(2 pi j / L) with L the LATTICE size: a length-L line uses stride TS = 1, a length-L/2 line
+// TS = 2.  Threads are (lane, t).
 template <int N2>
 __device__ __forceinline__ int sidx(int k1, int n2) { return (N2 + 1) * k1 + n2; }
 template <int N2>
 __host__ __device__ constexpr int line_rows() { return (N2 + 1) * 16; }
 
-// forward step 1: v[n1] = x[N2 n1 + n2]  ->  A[k1][n2] * W_L^{n2 k1}  at slot N2 k1 + n2
-template <int N2>
+// forward step 1: v[n1] = x[N2 n1 + n2]  ->  A[k1][n2] * W_n^{n2 k1}  at slot N2 k1 + n2
+template <int N2, int TS>
 __device__ __forceinline__ void fwd_step1(float2 (&v)[16], int n2, const float2 *tw, float2 *buf, int LN, int lane) {
     fft_reg<16, false>(v);
 #pragma unroll
     for (int k1 = 0; k1 < 16; ++k1) {
-        const float2 w = tw[n2 * k1];
+        const float2 w = tw[TS * n2 * k1];
         buf[sidx<N2>(k1, n2) * LN + lane] = cmul(v[bitrev<16>(k1)], make_float2(w.x, -w.y));
     }
 }
-// forward step 2: the thread's block k1 -> u[k2] = X[k1 + 16 k2] in natural k2 order
+// forward step 2: block k1 -> u[k2] = X[k1 + 16 k2] in natural k2 order
 template <int N2>
 __device__ __forceinline__ void fwd_step2(float2 (&u)[N2], int k1, const float2 *buf, int LN, int lane) {
     float2 t[N2];
@@ -152,12 +161,12 @@ __device__ __forceinline__ void fwd_step2(float2 (&u)[N2], int k1, const float2 
 #pragma unroll
     for (int k2 = 0; k2 < N2; ++k2) u[k2] = t[bitrev<N2>(k2)];
 }
-// inverse step 2: u[k2] = Y[k1 + 16 k2]  ->  B[k1][n2] * conj(W_L^{n2 k1})  at slot N2 k1 + n2
-template <int N2>
+// inverse step 2: u[k2] = Y[k1 + 16 k2]  ->  B[k1][n2] * conj(W_n^{n2 k1})  at slot N2 k1 + n2
+template <int N2, int TS>
 __device__ __forceinline__ void inv_step2(float2 (&u)[N2], int k1, const float2 *tw, float2 *buf, int LN, int lane) {
     fft_reg<N2, true>(u);
 #pragma unroll
-    for (int n2 = 0; n2 < N2; ++n2) buf[sidx<N2>(k1, n2) * LN + lane] = cmul(u[bitrev<N2>(n2)], tw[n2 * k1]);
+    for (int n2 = 0; n2 < N2; ++n2) buf[sidx<N2>(k1, n2) * LN + lane] = cmul(u[bitrev<N2>(n2)], tw[TS * n2 * k1]);
 }
 // inverse step 1: slots N2 k1 + n2 (k1 = 0..15)  ->  v[n1] = x[N2 n1 + n2]
 template <int N2>
@@ -179,213 +188,219 @@ __device__ __forceinline__ void fill_twiddles(float2 *tw, int L) {
     }
 }
 
-struct FftParams {
-    const float *S;   // spins, internal layout
-    float *H;         // field, internal layout
-    float2 *Z;        // spectrum scratch Z[c][y][slot_x][pair]
-    const float4 *M;  // M[slot_x][slot_y][2]: (xx.re, xx.im, xy.re, xy.im), (yy.re, yy.im, zz.re, zz.im), scaled 1/N
-    int L, P;         // P = R / 2 complex replica pairs
-    int colour;       // which targets fft_x_inverse writes: -1 both colours, 0, 1
+// Z and the two caches share one layout: [a][slot_x][pb][row][lane], a = component, slot_x < L/2, pb = block of LN replica
+// pairs, row = y (Z after the x pass / before the x-inverse pass) or slot_y (spectra), lane = pair within the block.
+struct FcParams {
+    const float *S;    // spins, internal layout
+    float *H;          // field, internal layout
+    float2 *Z;         // scratch lines of the field being computed
+    float2 *Cnew;      // cache of the half-spectrum of colour `colour` (y pass: written unless FC_COMBINE)
+    const float2 *Ctgt;  // cache of the half-spectrum of the target colour 1 - colour (FC_FUSED) or ... see fftc_y_kernel
+    const float4 *AB;  // AB[slot_x][slot_y][4]: (Axx, Axy), (Ayy, Bxx), (Bxy, Byy), (Azz, Bzz), each complex, scaled 1/N
+    int L, P;          // P = R / 2 complex replica pairs
+    int PB;            // blocks of LN pairs (P = PB * LN)
+    int colour;        // x passes: the colour of the rows; y pass: the colour whose lines sit in Z (FC_FWD_ONLY, FC_FUSED)
 };
 
-// grid (P / LN, L, 3), block (LN, 16)
-template <int N2>
-__global__ void __launch_bounds__(512) fft_x_forward_kernel(const FftParams p) {
-    extern __shared__ __align__(16) float2 fsm[];
-    const int L = 16 * N2, Lh = L / 2, LN = blockDim.x;
-    float2 *tw = fsm, *buf = fsm + L;
-    const int lane = threadIdx.x, t = threadIdx.y;
-    const int pair = blockIdx.x * LN + lane, y = blockIdx.y, c = blockIdx.z;
-    const size_t planeP = (size_t)L * Lh * p.P;
-    const float2 *S2 = reinterpret_cast<const float2 *>(p.S);
-    auto load_line = [&](float2 (&v)[16], int n2) {
-#pragma unroll
-        for (int n1 = 0; n1 < 16; ++n1) {
-            const int x = N2 * n1 + n2, q = (x + y) & 1;
-            v[n1] = __ldg(S2 + (size_t)(q * 3 + c) * planeP + (size_t)(y * Lh + (x >> 1)) * p.P + pair);
-        }
-    };
-    // the twiddles do not depend on the spins: they are computed while the kernel that writes the spins may still run
-    // the first sub-sequence's loads are issued before the twiddles are computed: they do not depend on them
-    pdl_wait();                                            // the spins come from the Metropolis kernel before
-    float2 v0[16];
-    if (t < N2) load_line(v0, t);
-    fill_twiddles(tw, L);
-    __syncthreads();
-    if (t < N2) fwd_step1<N2>(v0, t, tw, buf, LN, lane);
-    for (int n2 = t + 16; n2 < N2; n2 += 16) {
-        float2 v[16];
-        load_line(v, n2);
-        fwd_step1<N2>(v, n2, tw, buf, LN, lane);
-    }
-    __syncthreads();
-    pdl_trigger();                                         // late: a successor resident earlier only takes room (section 5.2b)
-    float2 u[N2];
-    fwd_step2<N2>(u, t, buf, LN, lane);
-    float2 *dst = p.Z + ((size_t)(c * L + y) * L + N2 * t) * p.P + pair;
-#pragma unroll
-    for (int k2 = 0; k2 < N2; ++k2) dst[(size_t)k2 * p.P] = u[k2];
+__device__ __forceinline__ size_t line_base(const FcParams &p, int a, int sx, int pb, int LN) {
+    return ((((size_t)a * (p.L >> 1) + sx) * p.PB + pb) * p.L) * LN;
 }
 
-// grid (P / LN, L, 3), block (LN, 16)
-template <int N2>
-__global__ void __launch_bounds__(512) fft_x_inverse_kernel(const FftParams p) {
+// x forward, colour p.colour: grid (PB, L rows, 3 components), block (LN, TL), TL = min(16, N2X) threads per line.
+template <int N2X>
+__global__ void __launch_bounds__(512) fftc_x_forward_kernel(const FcParams p) {
     extern __shared__ __align__(16) float2 fsm[];
-    const int L = 16 * N2, Lh = L / 2, LN = blockDim.x;
+    constexpr int Lh = 16 * N2X, L = 2 * Lh;
+    const int LN = blockDim.x, TL = blockDim.y;
     float2 *tw = fsm, *buf = fsm + L;
     const int lane = threadIdx.x, t = threadIdx.y;
-    const int pair = blockIdx.x * LN + lane, y = blockIdx.y, c = blockIdx.z;
-    float2 u[N2];
-    const float2 *src = p.Z + ((size_t)(c * L + y) * L + N2 * t) * p.P + pair;
-    pdl_wait();                                            // the spectrum comes from the y pass
+    const int pb = blockIdx.x, pair = pb * LN + lane, y = blockIdx.y, a = blockIdx.z, c = p.colour;
+    const size_t planeP = (size_t)L * Lh * p.P;
+    const float2 *src = reinterpret_cast<const float2 *>(p.S) + (size_t)(c * 3 + a) * planeP + (size_t)y * Lh * p.P + pair;
+    pdl_wait();                                            // the spins come from the Metropolis kernel before
+    float2 v[16];
 #pragma unroll
-    for (int k2 = 0; k2 < N2; ++k2) u[k2] = src[(size_t)k2 * p.P];
+    for (int n1 = 0; n1 < 16; ++n1) v[n1] = __ldg(src + (size_t)(N2X * n1 + t) * p.P);   // t < N2X by construction
+    fill_twiddles(tw, L);                                  // while the loads are in flight
+    __syncthreads();
+    fwd_step1<N2X, 2>(v, t, tw, buf, LN, lane);
+    __syncthreads();
+    pdl_trigger();                                         // late: a successor resident earlier only takes room
+    const bool odd_row = (y + c) & 1;                      // sites x = 2 i + 1: row phase e^{-2 pi i kx / L}
+    float2 *dst = p.Z + line_base(p, a, 0, pb, LN) + (size_t)y * LN + lane;
+    const size_t sx_stride = (size_t)p.PB * L * LN;
+    for (int k1 = t; k1 < 16; k1 += TL) {
+        float2 u[N2X];
+        fwd_step2<N2X>(u, k1, buf, LN, lane);
+#pragma unroll
+        for (int k2 = 0; k2 < N2X; ++k2) {
+            float2 r = u[k2];
+            if (odd_row) {
+                const float2 w = tw[k1 + 16 * k2];
+                r = cmul(r, make_float2(w.x, -w.y));
+            }
+            dst[(size_t)(N2X * k1 + k2) * sx_stride] = r;
+        }
+    }
+}
+
+// x inverse, target colour p.colour: grid (PB, L rows, 3 components), block (LN, TL).
+template <int N2X>
+__global__ void __launch_bounds__(512) fftc_x_inverse_kernel(const FcParams p) {
+    extern __shared__ __align__(16) float2 fsm[];
+    constexpr int Lh = 16 * N2X, L = 2 * Lh;
+    const int LN = blockDim.x, TL = blockDim.y;
+    float2 *tw = fsm, *buf = fsm + L;
+    const int lane = threadIdx.x, t = threadIdx.y;
+    const int pb = blockIdx.x, pair = pb * LN + lane, y = blockIdx.y, a = blockIdx.z, c = p.colour;
+    const float2 *src = p.Z + line_base(p, a, 0, pb, LN) + (size_t)y * LN + lane;
+    const size_t sx_stride = (size_t)p.PB * L * LN;
+    constexpr int NK = N2X >= 16 ? 1 : 16 / N2X;           // blocks k1 per thread
+    pdl_wait();                                            // the lines come from the y pass
+    float2 u[NK][N2X];
+#pragma unroll
+    for (int j = 0; j < NK; ++j)
+#pragma unroll
+        for (int k2 = 0; k2 < N2X; ++k2) u[j][k2] = src[(size_t)(N2X * (t + j * TL) + k2) * sx_stride];
     fill_twiddles(tw, L);
     __syncthreads();
-    bool folded = false;
-    if constexpr (N2 == 16) {
-        // One colour wanted: of the N2 outputs n2 of inverse step 2 only those of parity par = (colour + y) & 1 are
-        // used below, so the step is an 8-point transform of the folded input (the same radix-2 step by hand as in the
-        // last step; par is uniform over the CTA)
-        if (p.colour >= 0) {
-            const int par = (p.colour + y) & 1;
-            float2 a[8];
+    const bool odd_row = (y + c) & 1;                      // row phase e^{+2 pi i kx / L}
 #pragma unroll
-            for (int k = 0; k < 8; ++k) {
-                if (par) {
-                    const float2 d = csub(u[k], u[k + 8]);
-                    a[k] = k == 0 ? d : k == 4 ? make_float2(-d.y, d.x) : cmul(d, make_float2(kTw32.c[2 * k], kTw32.s[2 * k]));
-                } else {
-                    a[k] = cadd(u[k], u[k + 8]);
-                }
-            }
-            fft_reg<8, true>(a);
+    for (int j = 0; j < NK; ++j) {
+        const int k1 = t + j * TL;
+        if (odd_row) {
 #pragma unroll
-            for (int j = 0; j < 8; ++j) {
-                const int n2 = par + 2 * j;
-                buf[sidx<N2>(t, n2) * LN + lane] = cmul(a[bitrev<8>(j)], tw[n2 * t]);
-            }
-            folded = true;
+            for (int k2 = 0; k2 < N2X; ++k2) u[j][k2] = cmul(u[j][k2], tw[k1 + 16 * k2]);
         }
+        inv_step2<N2X, 2>(u[j], k1, tw, buf, LN, lane);
     }
-    if (!folded) inv_step2<N2>(u, t, tw, buf, LN, lane);
     pdl_trigger();
     __syncthreads();
+    float2 v[16];
+    inv_step1<N2X>(v, t, buf, LN, lane);
     const size_t planeP = (size_t)L * Lh * p.P;
-    float2 *H2 = reinterpret_cast<float2 *>(p.H);
-    if constexpr (N2 == 16) {
-        // One colour wanted: only the 8 sub-sequences n2 of the right parity are transformed, which would leave every
-        // second t idle.  Instead the 16 t share them in pairs, t < 8 taking the even and t >= 8 the odd outputs n1 of
-        // sub-sequence n2 = par + 2 (t & 7) (a warp holds two consecutive t, so neither half diverges): one radix-2
-        // step by hand, x[2j] = F8^-1[t_k + t_{k+8}](j), x[2j+1] = F8^-1[(t_k - t_{k+8}) w^k](j), w = e^{2 pi i / 16}.
-        if (p.colour >= 0) {
-            const int par = (p.colour + y) & 1, n2 = par + 2 * (t & 7), odd = t >> 3;
-            float2 a[8];
+    float2 *dst = reinterpret_cast<float2 *>(p.H) + (size_t)(c * 3 + a) * planeP + (size_t)y * Lh * p.P + pair;
 #pragma unroll
-            for (int k = 0; k < 8; ++k) {
-                const float2 lo = buf[sidx<N2>(k, n2) * LN + lane], hi = buf[sidx<N2>(k + 8, n2) * LN + lane];
-                if (odd) {
-                    const float2 d = csub(lo, hi);
-                    a[k] = k == 0 ? d : k == 4 ? make_float2(-d.y, d.x) : cmul(d, make_float2(kTw32.c[2 * k], kTw32.s[2 * k]));
-                } else {
-                    a[k] = cadd(lo, hi);
-                }
-            }
-            fft_reg<8, true>(a);
-#pragma unroll
-            for (int j = 0; j < 8; ++j) {
-                const int x = N2 * (2 * j + odd) + n2;                 // parity of n2: colour p.colour
-                H2[(size_t)(p.colour * 3 + c) * planeP + (size_t)(y * Lh + (x >> 1)) * p.P + pair] = a[bitrev<8>(j)];
-            }
-            return;
-        }
-    }
-    for (int n2 = t; n2 < N2; n2 += 16) {
-        if (p.colour >= 0 && ((n2 + y) & 1) != p.colour) continue;   // x = N2 n1 + n2 has the parity of n2
-        float2 v[16];
-        inv_step1<N2>(v, n2, buf, LN, lane);
-#pragma unroll
-        for (int n1 = 0; n1 < 16; ++n1) {
-            const int x = N2 * n1 + n2, q = (x + y) & 1;
-            H2[(size_t)(q * 3 + c) * planeP + (size_t)(y * Lh + (x >> 1)) * p.P + pair] = v[n1];
-        }
-    }
+    for (int n1 = 0; n1 < 16; ++n1) dst[(size_t)(N2X * n1 + t) * p.P] = v[n1];
 }
 
 __device__ __forceinline__ float2 cmac(float2 acc, float2 a, float2 m) {  // acc + a * m
     return make_float2(fmaf(a.x, m.x, fmaf(-a.y, m.y, acc.x)), fmaf(a.x, m.y, fmaf(a.y, m.x, acc.y)));
 }
 
-// grid (P / LN, L slots), block (LN, 16); shared: twiddles + 3 line buffers
-template <int N2>
-__global__ void __launch_bounds__(256, 2) fft_y_multiply_kernel(const FftParams p) {
+// The y pass, column slot_x of the half-spectrum, LN pairs: grid (PB, L/2 slots), block (LN, 16).
+//   FC_FWD_ONLY  Z holds the x-transformed rows of colour c = p.colour: forward L-point FFT over y -> S^_c -> Cnew.
+//   FC_FUSED     the same, then H^_t = A S^_t + B S^_c with t = 1 - c and S^_t read from Ctgt, inverse FFT over ky -> Z.
+//   FC_COMBINE   nothing to transform forward: S^_c is read from Cnew as well (both caches valid); t = 1 - c.
+// The three modes run the same arithmetic on the same values, so a field does not depend on which of them produced it.
+enum { FC_FWD_ONLY = 0, FC_FUSED = 1, FC_COMBINE = 2 };
+
+template <int N2, int MODE>
+__global__ void __launch_bounds__(256, 2) fftc_y_kernel(const FcParams p) {
     extern __shared__ __align__(16) float2 fsm[];
-    const int L = 16 * N2, LN = blockDim.x;
+    constexpr int L = 16 * N2;
+    const int LN = blockDim.x;
     float2 *tw = fsm;
-    float4 *Msm = reinterpret_cast<float4 *>(fsm + L);     // this column's multiplier, 2 float4 per slot_y
-    float2 *b0 = fsm + L + 4 * L;
+    float2 *b0 = fsm + L;
     float2 *buf[3] = {b0, b0 + (size_t)line_rows<N2>() * LN, b0 + 2 * (size_t)line_rows<N2>() * LN};
     const int lane = threadIdx.x, t = threadIdx.y;
-    const int pair = blockIdx.x * LN + lane, sx = blockIdx.y;
+    const int pb = blockIdx.x, sx = blockIdx.y;
     fill_twiddles(tw, L);
-    for (int j = t * LN + lane; j < 2 * L; j += 16 * LN) Msm[j] = __ldg(p.M + (size_t)sx * L * 2 + j);  // constant table
-    pdl_wait();                                            // the spectrum comes from the x pass
+    pdl_wait();                                            // Z comes from the x pass, the caches from earlier y passes
     __syncthreads();
-    const size_t rowP = (size_t)L * p.P;                   // one y step in Z
-    float2 *col = p.Z + (size_t)sx * p.P + pair;           // + (c * L + y) * rowP
+    const size_t a_stride = (size_t)(L >> 1) * p.PB * L * LN;   // one component
+    const size_t base = line_base(p, 0, sx, pb, LN) + lane;
+    float2 *col = p.Z + base;                              // + a * a_stride + row * LN
+    float2 *cnew = p.Cnew + base;
+    const float2 *ctgt = p.Ctgt + base;
+    if (MODE != FC_COMBINE) {
 #pragma unroll 1
-    for (int c = 0; c < 3; ++c)
-        for (int n2 = t; n2 < N2; n2 += 16) {
-            float2 v[16];
+        for (int a = 0; a < 3; ++a)
+            for (int n2 = t; n2 < N2; n2 += 16) {
+                float2 v[16];
 #pragma unroll
-            for (int n1 = 0; n1 < 16; ++n1) v[n1] = col[(size_t)(c * L + N2 * n1 + n2) * rowP];
-            fwd_step1<N2>(v, n2, tw, buf[c], LN, lane);
-        }
-    __syncthreads();
+                for (int n1 = 0; n1 < 16; ++n1) v[n1] = col[a * a_stride + (size_t)(N2 * n1 + n2) * LN];
+                fwd_step1<N2, 1>(v, n2, tw, buf[a], LN, lane);
+            }
+        __syncthreads();
+    }
+    // The thread owns block t (slots N2 t + k2) of all three components.
+    const size_t row0 = (size_t)(N2 * t) * LN;
+    float2 u[N2];
+    float2 *bx = buf[0] + sidx<N2>(t, 0) * LN + lane;      // the x spectrum waits in the thread's own shared block
+    if (MODE != FC_COMBINE) {
+        fwd_step2<N2>(u, t, buf[0], LN, lane);
+#pragma unroll
+        for (int k2 = 0; k2 < N2; ++k2) cnew[row0 + (size_t)k2 * LN] = u[k2];
+    } else {
+#pragma unroll
+        for (int k2 = 0; k2 < N2; ++k2) u[k2] = cnew[row0 + (size_t)k2 * LN];
+    }
+    if (MODE != FC_FWD_ONLY) {
+#pragma unroll
+        for (int k2 = 0; k2 < N2; ++k2) bx[k2 * LN] = u[k2];
+    }
+    if (MODE != FC_COMBINE) {
+        fwd_step2<N2>(u, t, buf[1], LN, lane);             // u now holds the y component
+#pragma unroll
+        for (int k2 = 0; k2 < N2; ++k2) cnew[a_stride + row0 + (size_t)k2 * LN] = u[k2];
+    } else {
+#pragma unroll
+        for (int k2 = 0; k2 < N2; ++k2) u[k2] = cnew[a_stride + row0 + (size_t)k2 * LN];
+    }
+    if (MODE == FC_FWD_ONLY) {
+        fwd_step2<N2>(u, t, buf[2], LN, lane);
+#pragma unroll
+        for (int k2 = 0; k2 < N2; ++k2) cnew[2 * a_stride + row0 + (size_t)k2 * LN] = u[k2];
+        pdl_trigger();
+        return;
+    }
     {
-        const float4 *Mrow = Msm + (N2 * t) * 2;
-        // The thread owns block t of all three components, so the x spectrum can wait in its own
-        // shared-memory block (natural k2 order) while the y spectrum is transformed: at most one
-        // block lives in registers at a time.
-        float2 ux[N2];
-        float2 *bx = buf[0] + sidx<N2>(t, 0) * LN + lane;
-        fwd_step2<N2>(ux, t, buf[0], LN, lane);
-#pragma unroll
-        for (int k2 = 0; k2 < N2; ++k2) bx[k2 * LN] = ux[k2];
-        fwd_step2<N2>(ux, t, buf[1], LN, lane);            // ux now holds the y component
+        // this column's tables: a constant array read through the read-only path (the lanes of a half-warp share an address)
+        const float4 *tab = p.AB + ((size_t)sx * L + N2 * t) * 4;
 #pragma unroll
         for (int k2 = 0; k2 < N2; ++k2) {
-            const float4 m0 = Mrow[2 * k2], m1 = Mrow[2 * k2 + 1];
-            const float2 xx = make_float2(m0.x, m0.y), xy = make_float2(m0.z, m0.w), yy = make_float2(m1.x, m1.y);
-            const float2 zx = bx[k2 * LN], zy = ux[k2];
-            bx[k2 * LN] = cmac(cmul(zx, xx), zy, xy);
-            ux[k2] = cmac(cmul(zx, xy), zy, yy);
+            const float4 m0 = __ldg(tab + 4 * k2), m1 = __ldg(tab + 4 * k2 + 1), m2 = __ldg(tab + 4 * k2 + 2);
+            const float2 Axx = make_float2(m0.x, m0.y), Axy = make_float2(m0.z, m0.w), Ayy = make_float2(m1.x, m1.y);
+            const float2 Bxx = make_float2(m1.z, m1.w), Bxy = make_float2(m2.x, m2.y), Byy = make_float2(m2.z, m2.w);
+            const float2 tx = ctgt[row0 + (size_t)k2 * LN], ty = ctgt[a_stride + row0 + (size_t)k2 * LN];
+            const float2 ox = bx[k2 * LN], oy = u[k2];
+            bx[k2 * LN] = cmac(cmac(cmac(cmul(tx, Axx), ty, Axy), ox, Bxx), oy, Bxy);
+            u[k2] = cmac(cmac(cmac(cmul(tx, Axy), ty, Ayy), ox, Bxy), oy, Byy);
         }
-        inv_step2<N2>(ux, t, tw, buf[1], LN, lane);
+        inv_step2<N2, 1>(u, t, tw, buf[1], LN, lane);
 #pragma unroll
-        for (int k2 = 0; k2 < N2; ++k2) ux[k2] = bx[k2 * LN];
-        inv_step2<N2>(ux, t, tw, buf[0], LN, lane);
-        fwd_step2<N2>(ux, t, buf[2], LN, lane);            // ux reused for the z component
+        for (int k2 = 0; k2 < N2; ++k2) u[k2] = bx[k2 * LN];
+        inv_step2<N2, 1>(u, t, tw, buf[0], LN, lane);
+        if (MODE != FC_COMBINE) {
+            fwd_step2<N2>(u, t, buf[2], LN, lane);         // u reused for the z component
+#pragma unroll
+            for (int k2 = 0; k2 < N2; ++k2) cnew[2 * a_stride + row0 + (size_t)k2 * LN] = u[k2];
+        } else {
+#pragma unroll
+            for (int k2 = 0; k2 < N2; ++k2) u[k2] = cnew[2 * a_stride + row0 + (size_t)k2 * LN];
+        }
 #pragma unroll
         for (int k2 = 0; k2 < N2; ++k2) {
-            const float4 m1 = Mrow[2 * k2 + 1];
-            ux[k2] = cmul(ux[k2], make_float2(m1.z, m1.w));
+            const float4 m3 = __ldg(tab + 4 * k2 + 3);
+            const float2 tz = ctgt[2 * a_stride + row0 + (size_t)k2 * LN];
+            u[k2] = cmac(cmul(tz, make_float2(m3.x, m3.y)), u[k2], make_float2(m3.z, m3.w));
         }
-        inv_step2<N2>(ux, t, tw, buf[2], LN, lane);
+        inv_step2<N2, 1>(u, t, tw, buf[2], LN, lane);
     }
     __syncthreads();
     pdl_trigger();
 #pragma unroll 1
-    for (int c = 0; c < 3; ++c)
+    for (int a = 0; a < 3; ++a)
         for (int n2 = t; n2 < N2; n2 += 16) {
             float2 v[16];
-            inv_step1<N2>(v, n2, buf[c], LN, lane);
+            inv_step1<N2>(v, n2, buf[a], LN, lane);
 #pragma unroll
-            for (int n1 = 0; n1 < 16; ++n1) col[(size_t)(c * L + N2 * n1 + n2) * rowP] = v[n1];
+            for (int n1 = 0; n1 < 16; ++n1) col[a * a_stride + (size_t)(N2 * n1 + n2) * LN] = v[n1];
         }
 }
 
-// ---- M = transform of W, fp64, once per tensor ------------------------------------------------
+// ---- A, B = folded transform of W, fp64, once per tensor --------------------------------------
 // T1[c][rho_y][kx] = sum_{rho_x} W[c][rho_y][rho_x] e^{+2 pi i kx rho_x / L}
 __global__ void wq_pass1_kernel(const float *__restrict__ Wc, double2 *__restrict__ T1, int L) {
     const size_t N = (size_t)L * L;
@@ -403,25 +418,34 @@ __global__ void wq_pass1_kernel(const float *__restrict__ Wc, double2 *__restric
     }
     T1[id] = make_double2(re, im);
 }
-// M[slot(kx)][slot(ky)][c] = (1/N) sum_{rho_y} T1[c][rho_y][kx] e^{+2 pi i ky rho_y / L}
-__global__ void wq_pass2_kernel(const double2 *__restrict__ T1, float *__restrict__ M, int L) {
-    const size_t N = (size_t)L * L;
+// M(kx, ky) = sum_{rho_y} T1[c][rho_y][kx] e^{+2 pi i ky rho_y / L};  M' = M(kx + L/2, ky + L/2) (the (-1)^{rho_y} sum over
+// the shifted column);  A = (M + M') / N,  B = (M - M') / N  at  AB[slot_x(kx)][slot_y(ky)],  kx < L/2.
+__global__ void wq_pass2_kernel(const double2 *__restrict__ T1, float *__restrict__ AB, int L) {
+    const int Lh = L >> 1;
     const size_t id = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (id >= 4 * N) return;
-    const int kx = (int)(id % L), ky = (int)((id / L) % L), c = (int)(id / N);
-    double re = 0.0, im = 0.0;
+    if (id >= 4 * (size_t)Lh * L) return;
+    const int kx = (int)(id % Lh), ky = (int)((id / Lh) % L), c = (int)(id / ((size_t)Lh * L));
+    double re = 0.0, im = 0.0, re2 = 0.0, im2 = 0.0;
     for (int ry = 0; ry < L; ++ry) {
         double s, cs;
         sincospi(2.0 * (double)((ky * ry) % L) / (double)L, &s, &cs);
-        const double2 t = T1[((size_t)c * L + ry) * L + kx];
-        re += t.x * cs - t.y * s;
-        im += t.x * s + t.y * cs;
+        const double2 a = T1[((size_t)c * L + ry) * L + kx], b = T1[((size_t)c * L + ry) * L + kx + Lh];
+        const double sg = (ry & 1) ? -1.0 : 1.0;
+        re += a.x * cs - a.y * s;
+        im += a.x * s + a.y * cs;
+        re2 += sg * (b.x * cs - b.y * s);
+        im2 += sg * (b.x * s + b.y * cs);
     }
-    const int N2 = L / 16;
-    const int sx = N2 * (kx & 15) + (kx >> 4), sy = N2 * (ky & 15) + (ky >> 4);
-    float *dst = M + ((size_t)sx * L + sy) * 8 + 2 * c;
-    dst[0] = (float)(re / (double)N);
-    dst[1] = (float)(im / (double)N);
+    const int N2 = L / 16, N2X = Lh >= 16 ? Lh / 16 : 1;
+    const int sx = N2X * (kx & 15) + (kx >> 4), sy = N2 * (ky & 15) + (ky >> 4);
+    const double inv = 1.0 / ((double)L * (double)L);
+    // floats of one (slot_x, slot_y): Axx 0-1, Axy 2-3, Ayy 4-5, Bxx 6-7, Bxy 8-9, Byy 10-11, Azz 12-13, Bzz 14-15
+    const int ia = c == 3 ? 12 : 2 * c, ib = c == 3 ? 14 : 6 + 2 * c;
+    float *dst = AB + ((size_t)sx * L + sy) * 16;
+    dst[ia] = (float)((re + re2) * inv);
+    dst[ia + 1] = (float)((im + im2) * inv);
+    dst[ib] = (float)((re - re2) * inv);
+    dst[ib + 1] = (float)((im - im2) * inv);
 }
 
 int pairs_per_cta(int P, int cap) {
@@ -431,24 +455,74 @@ int pairs_per_cta(int P, int cap) {
 }
 
 template <int N2>
-cudaError_t launch_fft_n2(const FftParams &p, bool *configured, cudaStream_t st, uint64_t *launches) {
-    const int L = 16 * N2;
-    // 16 replica pairs per CTA: 128-byte runs in HBM, and enough CTAs (half rows / half columns) that
-    // the last wave over 148 SMs stays full
-    const int LNX = pairs_per_cta(p.P, 16), LNY = pairs_per_cta(p.P, 16);
-    const size_t smx = sizeof(float2) * (L + (size_t)line_rows<N2>() * LNX);
-    const size_t smy = sizeof(float2) * (L + 4 * L + 3 * (size_t)line_rows<N2>() * LNY);
+size_t y_smem_bytes(int LN) {
+    return sizeof(float2) * (16 * N2 + 3 * (size_t)line_rows<N2>() * LN);
+}
+
+// one field of colour `colour` (0 / 1), or of both (-1); valid[c] = "the cache holds the half-spectrum of colour c of the
+// current spins" (kept by the caller across calls; a Metropolis update of colour c clears valid[c])
+template <int N2>
+cudaError_t launch_fftc(FcParams p, float2 *C, size_t cache_elems, int colour, bool *valid, bool *configured, cudaStream_t st,
+                        uint64_t *launches) {
+    constexpr int L = 16 * N2, N2X = N2 / 2 > 0 ? N2 / 2 : 1;
+    static_assert(N2 >= 2, "L >= 32");
+    // 16 replica pairs per CTA: 128-byte runs in HBM; fewer when the y pass would not fit its line buffers (L = 512)
+    int cap = 16;
+    while (cap > 1 && y_smem_bytes<N2>(cap) > 220 * 1024) cap >>= 1;
+    const int LN = pairs_per_cta(p.P, cap);
+    p.PB = p.P / LN;
+    const int TL = N2X < 16 ? N2X : 16;
+    const size_t smx = sizeof(float2) * (L + (size_t)line_rows<N2X>() * LN);
     if (!*configured) {
         cudaError_t e;
-        if ((e = cudaFuncSetAttribute(fft_x_forward_kernel<N2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)) != cudaSuccess) return e;
-        if ((e = cudaFuncSetAttribute(fft_x_inverse_kernel<N2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)) != cudaSuccess) return e;
-        if ((e = cudaFuncSetAttribute(fft_y_multiply_kernel<N2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024)) != cudaSuccess) return e;
+        if ((e = cudaFuncSetAttribute(fftc_y_kernel<N2, FC_FWD_ONLY>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024)) != cudaSuccess) return e;
+        if ((e = cudaFuncSetAttribute(fftc_y_kernel<N2, FC_FUSED>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024)) != cudaSuccess) return e;
+        if ((e = cudaFuncSetAttribute(fftc_y_kernel<N2, FC_COMBINE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024)) != cudaSuccess) return e;
+        if ((e = cudaFuncSetAttribute(fftc_x_forward_kernel<N2X>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024)) != cudaSuccess) return e;
+        if ((e = cudaFuncSetAttribute(fftc_x_inverse_kernel<N2X>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024)) != cudaSuccess) return e;
         *configured = true;
     }
-    cudaError_t e = launch_pdl(fft_x_forward_kernel<N2>, dim3(p.P / LNX, L, 3), dim3(LNX, 16), smx, st, p);
-    if (e == cudaSuccess) e = launch_pdl(fft_y_multiply_kernel<N2>, dim3(p.P / LNY, L), dim3(LNY, 16), smy, st, p);
-    if (e == cudaSuccess) e = launch_pdl(fft_x_inverse_kernel<N2>, dim3(p.P / LNX, L, 3), dim3(LNX, 16), smx, st, p);
-    *launches += 3;
+    const dim3 gx(p.PB, L, 3), bx(LN, TL), gy(p.PB, L / 2), by(LN, 16);
+    cudaError_t e = cudaSuccess;
+    auto x_forward = [&](int c) {
+        FcParams q = p;
+        q.colour = c;
+        ++*launches;
+        return launch_pdl(fftc_x_forward_kernel<N2X>, gx, bx, smx, st, q);
+    };
+    auto y_pass = [&](int mode, int c) {                   // c = the colour transformed forward / "new" colour
+        FcParams q = p;
+        q.colour = c;
+        q.Cnew = C + (size_t)c * cache_elems;
+        q.Ctgt = C + (size_t)(1 - c) * cache_elems;
+        ++*launches;
+        if (mode == FC_FWD_ONLY) return launch_pdl(fftc_y_kernel<N2, FC_FWD_ONLY>, gy, by, y_smem_bytes<N2>(LN), st, q);
+        if (mode == FC_FUSED) return launch_pdl(fftc_y_kernel<N2, FC_FUSED>, gy, by, y_smem_bytes<N2>(LN), st, q);
+        return launch_pdl(fftc_y_kernel<N2, FC_COMBINE>, gy, by, y_smem_bytes<N2>(LN), st, q);
+    };
+    auto x_inverse = [&](int c) {
+        FcParams q = p;
+        q.colour = c;
+        ++*launches;
+        return launch_pdl(fftc_x_inverse_kernel<N2X>, gx, bx, smx, st, q);
+    };
+    for (int tc = 0; tc < 2 && e == cudaSuccess; ++tc) {
+        if (colour >= 0 && colour != tc) continue;
+        const int oc = 1 - tc;
+        if (!valid[tc]) {                                  // the target colour's own half-spectrum is stale: refresh it alone
+            if ((e = x_forward(tc)) != cudaSuccess) break;
+            if ((e = y_pass(FC_FWD_ONLY, tc)) != cudaSuccess) break;
+            valid[tc] = true;
+        }
+        if (!valid[oc]) {                                  // the running-sweep case: only the colour just updated is stale
+            if ((e = x_forward(oc)) != cudaSuccess) break;
+            if ((e = y_pass(FC_FUSED, oc)) != cudaSuccess) break;
+            valid[oc] = true;
+        } else {
+            if ((e = y_pass(FC_COMBINE, oc)) != cudaSuccess) break;
+        }
+        e = x_inverse(tc);
+    }
     return e != cudaSuccess ? e : cudaGetLastError();
 }
 
@@ -457,38 +531,43 @@ cudaError_t launch_fft_n2(const FftParams &p, bool *configured, cudaStream_t st,
 bool dsmc_fft_supported(int L, int R) {
     return (R % 2 == 0) && (L == 32 || L == 64 || L == 128 || L == 256 || L == 512);
 }
-size_t dsmc_fft_m_floats(int L) { return 8 * (size_t)L * L; }
+size_t dsmc_fft_m_floats(int L) { return 8 * (size_t)L * L; }                 // AB: (L/2) L slots of 16 floats
+size_t dsmc_fft_cache_elems(int L, int R) { return 3 * (size_t)(L / 2) * L * (size_t)(R / 2); }   // float2 per colour
 size_t dsmc_fft_scratch_bytes(int L, int R) {
     const size_t N = (size_t)L * L;
-    const size_t z = sizeof(float) * 3 * N * R, t1 = sizeof(double2) * 4 * N;
+    const size_t z = sizeof(float2) * dsmc_fft_cache_elems(L, R), t1 = sizeof(double2) * 4 * N;
     return z > t1 ? z : t1;
 }
+size_t dsmc_fft_cache_bytes(int L, int R) { return 2 * sizeof(float2) * dsmc_fft_cache_elems(L, R); }
 
-cudaError_t launch_make_fft_table(const float *Wc, float *M, void *scratch, int L, cudaStream_t st, uint64_t *launches) {
+cudaError_t launch_make_fft_table(const float *Wc, float *AB, void *scratch, int L, cudaStream_t st, uint64_t *launches) {
     const size_t total = 4 * (size_t)L * L;
-    const unsigned grid = (unsigned)((total + 127) / 128);
-    wq_pass1_kernel<<<grid, 128, 0, st>>>(Wc, (double2 *)scratch, L);
-    wq_pass2_kernel<<<grid, 128, 0, st>>>((const double2 *)scratch, M, L);
+    wq_pass1_kernel<<<(unsigned)((total + 127) / 128), 128, 0, st>>>(Wc, (double2 *)scratch, L);
+    wq_pass2_kernel<<<(unsigned)((total / 2 + 127) / 128), 128, 0, st>>>((const double2 *)scratch, AB, L);
     *launches += 2;
     return cudaGetLastError();
 }
 
-cudaError_t launch_field_fft(const float *S, const float *M, void *scratch, float *H, int L, int R, int colour,
-                             bool *configured, cudaStream_t st, uint64_t *launches) {
-    FftParams p;
+cudaError_t launch_field_fft(const float *S, const float *AB, void *scratch, void *cache, float *H, int L, int R, int colour,
+                             bool *valid, bool *configured, cudaStream_t st, uint64_t *launches) {
+    FcParams p;
     p.S = S;
     p.H = H;
     p.Z = (float2 *)scratch;
-    p.M = (const float4 *)M;
+    p.Cnew = nullptr;
+    p.Ctgt = nullptr;
+    p.AB = (const float4 *)AB;
     p.L = L;
     p.P = R / 2;
-    p.colour = colour;
+    p.PB = 1;
+    p.colour = 0;
+    const size_t ce = dsmc_fft_cache_elems(L, R);
     switch (L / 16) {
-        case 2: return launch_fft_n2<2>(p, configured, st, launches);
-        case 4: return launch_fft_n2<4>(p, configured, st, launches);
-        case 8: return launch_fft_n2<8>(p, configured, st, launches);
-        case 16: return launch_fft_n2<16>(p, configured, st, launches);
-        case 32: return launch_fft_n2<32>(p, configured, st, launches);
+        case 2: return launch_fftc<2>(p, (float2 *)cache, ce, colour, valid, configured, st, launches);
+        case 4: return launch_fftc<4>(p, (float2 *)cache, ce, colour, valid, configured, st, launches);
+        case 8: return launch_fftc<8>(p, (float2 *)cache, ce, colour, valid, configured, st, launches);
+        case 16: return launch_fftc<16>(p, (float2 *)cache, ce, colour, valid, configured, st, launches);
+        case 32: return launch_fftc<32>(p, (float2 *)cache, ce, colour, valid, configured, st, launches);
     }
     return cudaErrorInvalidValue;
 }

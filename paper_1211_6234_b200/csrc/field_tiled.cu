@@ -71,7 +71,6 @@ __global__ void __launch_bounds__(MAX_THREADS, 1) field_tiled_kernel(const Tiled
     const int trow = yt - y_first;
     const int ks = blockIdx.y;
     const int r0 = blockIdx.z * RCH;
-    const int j0 = ks * p.rows_per_chunk;
     const int nseg = Lh / SEG;
     const int nstages = p.rows_per_chunk * 2 * nseg;
 
@@ -90,10 +89,12 @@ __global__ void __launch_bounds__(MAX_THREADS, 1) field_tiled_kernel(const Tiled
         const int q = rem / nseg, seg = rem - q * nseg;
         const int i0 = seg * SEG;
         // Source rows in the order far -> near (relative to the CTA's first target row): entry j of the sequence
-        // d = -L/2, +(L/2-1), -(L/2-1), ..., +1, -1, 0.  The big terms of the sum (|d| small, W ~ 1/r^3) then arrive
-        // last and only in the last chunk, so every accumulator stays small while the many small far-field terms
-        // are added: the rounding error of an fp32 add scales with the accumulator.
-        const int j = j0 + rr, mm = (j + 1) >> 1;
+        // d = -L/2, +(L/2-1), -(L/2-1), ..., +1, -1, 0, dealt out to the KS chunks in turn (chunk ks takes j = ks,
+        // ks + KS, ...).  Every chunk then adds its many small far-field terms while its accumulators are still small
+        // -- the rounding error of an fp32 add scales with the accumulator, and a term below half an ulp of it is
+        // lost altogether -- and ends with ONE of the near rows, so no accumulator ever holds more than one row's
+        // worth (<= 2 zeta(3) = 2.4) of the 9.03 the z-aligned state sums to.
+        const int j = ks + (int)gridDim.y * rr, mm = (j + 1) >> 1;
         const int d = j == 0 ? -(L >> 1) : ((j & 1) ? (L >> 1) - mm : mm - (L >> 1));
         int ys = y_first + d;
         ys += ys < 0 ? L : 0;

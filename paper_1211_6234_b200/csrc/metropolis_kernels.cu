@@ -99,12 +99,17 @@ __device__ __forceinline__ void ld2(const float4 *ptr, f2 &lo, f2 &hi) {
 // do not depend on them and run while they are in flight.  HOOKS = parity outputs requested.
 // FLIP: 0 = uniform-sphere trial, 1 = Ising reversal (App. B), 2 = decided at run time from p.flip (parity-hook
 // variant only: a run-time branch here splits the block the scheduler interleaves the two pairs in, +5 %)
-template <bool HOOKS, bool DEVSTEP, int FLIP>
-__global__ void __launch_bounds__(128, 7) metropolis4_kernel(const MetropolisArgs p, const RoundKeys rk) {
+// TY = lattice rows per CTA: the 128 threads are TY groups of 128 / TY consecutive (i, replica quad) entries, one group
+// per row y0 .. y0 + TY - 1.  The neighbour rows of adjacent update rows coincide (row y + 1 of the other colour is
+// "north" for row y, "same row" for row y + 1 and "south" for row y + 2), so with TY > 1 those loads hit in L1
+// instead of going to L2 three times.  MINB = CTAs per SM the register allocation is held to.
+template <bool HOOKS, bool DEVSTEP, int FLIP, int TY, int MINB>
+__global__ void __launch_bounds__(128, MINB) metropolis4_kernel(const MetropolisArgs p, const RoundKeys rk) {
+    constexpr int EX = 128 / TY;
     const int Lh = p.L >> 1, RQ = p.R >> 2;
-    const int y = blockIdx.y;
+    const int y = blockIdx.y * TY + (TY > 1 ? (int)(threadIdx.x / EX) : 0);
     const uint32_t row4 = (uint32_t)(Lh * RQ);
-    const uint32_t e = blockIdx.x * blockDim.x + threadIdx.x;   // (i, replica quad) within the row
+    const uint32_t e = blockIdx.x * EX + (TY > 1 ? threadIdx.x % EX : threadIdx.x);   // (i, replica quad) within the row
     if (!p.pdl_late) pdl_trigger();
     if (e >= row4) return;
     pdl_wait();                                                 // spins, field and step counter come from earlier kernels
@@ -279,15 +284,18 @@ cudaError_t launch_metropolis(const MetropolisArgs &a, cudaStream_t st, uint64_t
             while ((1 << b.rq_shift) < RQ) ++b.rq_shift;
         }
         const unsigned per_row = (unsigned)((a.L / 2) * RQ);
-        dim3 grid((per_row + 127) / 128, a.L);
+        // two lattice rows per CTA (L is even): measured at config 5 over 24 cold launches, 18.6 us for one row per CTA,
+        // 18.4 for two, 18.45 for four; 64 registers for 8 CTAs per SM spill and lose (19.3-19.8 us)
+        constexpr int TY = 2, MINB = 7;
+        dim3 grid((per_row + 128 / TY - 1) / (128 / TY), a.L / TY);
         // measured: a one-wave grid gains from triggering its successor late (L = 128, R = 4:
         // 18.9 -> 20.8 k sweeps/s), a many-wave grid from triggering at the top (L = 256, R = 64)
         b.pdl_late = (size_t)grid.x * grid.y <= 1024 ? 1 : 0;
-        if (a.accept_out || a.margin_out) err = launch_pdl(metropolis4_kernel<true, false, 2>, grid, dim3(128), 0, st, b, rk);
-        else if (a.step_dev && a.flip) err = launch_pdl(metropolis4_kernel<false, true, 1>, grid, dim3(128), 0, st, b, rk);
-        else if (a.step_dev) err = launch_pdl(metropolis4_kernel<false, true, 0>, grid, dim3(128), 0, st, b, rk);
-        else if (a.flip) err = launch_pdl(metropolis4_kernel<false, false, 1>, grid, dim3(128), 0, st, b, rk);
-        else err = launch_pdl(metropolis4_kernel<false, false, 0>, grid, dim3(128), 0, st, b, rk);
+        if (a.accept_out || a.margin_out) err = launch_pdl(metropolis4_kernel<true, false, 2, TY, MINB>, grid, dim3(128), 0, st, b, rk);
+        else if (a.step_dev && a.flip) err = launch_pdl(metropolis4_kernel<false, true, 1, TY, MINB>, grid, dim3(128), 0, st, b, rk);
+        else if (a.step_dev) err = launch_pdl(metropolis4_kernel<false, true, 0, TY, MINB>, grid, dim3(128), 0, st, b, rk);
+        else if (a.flip) err = launch_pdl(metropolis4_kernel<false, false, 1, TY, MINB>, grid, dim3(128), 0, st, b, rk);
+        else err = launch_pdl(metropolis4_kernel<false, false, 0, TY, MINB>, grid, dim3(128), 0, st, b, rk);
         if (err == cudaSuccess) err = cudaGetLastError();
     } else {
         const size_t total = (size_t)a.L * (a.L / 2) * a.R;

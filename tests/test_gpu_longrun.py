@@ -86,15 +86,17 @@ def test_long_run_config2_full(dsmc_mod, oracle_runs):
     """BASELINE config 2 as written: L = 32, R = 8, T = 0.2 ... 1.6, random start, 2 000 sweeps, observables every
     sweep; the direct-sum (tiled) field kernel."""
     gpu, cpu, z = _run_config(dsmc_mod, 2, oracle_runs, None)
-    # the runs are not trivially frozen or trivially random: the cold end orders along z, the hot end does not
-    assert np.abs(gpu[:, 0, 1]).mean() > 0.3 and np.abs(gpu[:, -1, 1]).mean() < 0.2
+    # the runs are neither frozen nor trivially random: the cold end orders (in the plane: the dipolar shape anisotropy
+    # (g/2)(9.03 + 4.52) = 0.68 outweighs K2 = 0.6), the hot end does not
+    assert gpu[:, 0, 2].mean() > 0.3 and gpu[:, -1, 2].mean() < 0.15 and np.abs(gpu[:, -1, 1]).mean() < 0.15
 
 
 def test_long_run_config3_full(dsmc_mod, oracle_runs):
     """BASELINE config 3 as written: L = 64, R = 16 (K4 = -0.2 / +0.2, T = 0.2 ... 1.6 each), all +z start, 5 000
     sweeps; the direct-sum (tiled) field kernel.  The z-aligned start is the fp32 field's worst case."""
     gpu, cpu, z = _run_config(dsmc_mod, 3, oracle_runs, None)
-    assert gpu[:, 0, 1].mean() > 0.8 and gpu[:, 8, 1].mean() > 0.8       # the T = 0.2 replicas stay ordered
+    # not vacuous: the cold K4 = +0.2 replica keeps the z order it started in, the hot ends are disordered
+    assert gpu[:, 8, 1].mean() > 0.8 and gpu[:, 7, 2].mean() < 0.1 and np.abs(gpu[:, 15, 1]).mean() < 0.1
 
 
 def test_long_run_config4_full(dsmc_mod, oracle_runs):
