@@ -29,6 +29,7 @@
 // slot(k) = N2 (k mod 16) + k div 16 and the inverse runs the steps backwards, so no reordering pass exists anywhere and
 // A, B are tabulated in slot order with the 1/N of the inverse folded in.
 #include "dsmc_internal.cuh"
+#include "bulk_copy.cuh"
 
 namespace {
 
@@ -188,22 +189,28 @@ __device__ __forceinline__ void fill_twiddles(float2 *tw, int L) {
     }
 }
 
-// Z and the two caches share one layout: [a][slot_x][pb][row][lane], a = component, slot_x < L/2, pb = block of LN replica
-// pairs, row = y (Z after the x pass / before the x-inverse pass) or slot_y (spectra), lane = pair within the block.
+// Z and the two caches share one layout: [a][slot_x][pb][row'][lane], a = component, slot_x < L/2, pb = block of LZ
+// replica pairs (LZ <= 8), row = y (Z after the x pass / before the x-inverse pass) or slot_y (spectra), lane = pair
+// within the block.  One (a, slot_x, pb) line is L * LZ contiguous complex numbers: one TMA bulk copy moves it between
+// global and shared memory, where the y pass transforms it in place.  row' = row ^ ((row >> 4) & 1): with 8-byte
+// elements and LZ = 8 a row is 64 bytes = 16 banks, rows of equal parity share banks, and the second step of the
+// four-step transform has the threads of a half-warp read rows 16 apart; the swap of neighbouring rows in every other
+// block of 16 puts them on different banks (the first step reads runs of consecutive rows either way).
 struct FcParams {
     const float *S;    // spins, internal layout
     float *H;          // field, internal layout
     float2 *Z;         // scratch lines of the field being computed
-    float2 *Cnew;      // cache of the half-spectrum of colour `colour` (y pass: written unless FC_COMBINE)
-    const float2 *Ctgt;  // cache of the half-spectrum of the target colour 1 - colour (FC_FUSED) or ... see fftc_y_kernel
+    float2 *Cnew;      // y pass: cache of the half-spectrum of colour `colour` (written unless FC_COMBINE, then read)
+    const float2 *Ctgt;  // y pass: cache of the half-spectrum of the target colour 1 - colour
     const float4 *AB;  // AB[slot_x][slot_y][4]: (Axx, Axy), (Ayy, Bxx), (Bxy, Byy), (Azz, Bzz), each complex, scaled 1/N
     int L, P;          // P = R / 2 complex replica pairs
-    int PB;            // blocks of LN pairs (P = PB * LN)
-    int colour;        // x passes: the colour of the rows; y pass: the colour whose lines sit in Z (FC_FWD_ONLY, FC_FUSED)
+    int LZ, PBZ;       // lanes per line and line blocks: P = PBZ * LZ
+    int colour;        // x passes: the colour of the rows; y pass: the colour whose lines sit in Z / in Cnew
 };
 
-__device__ __forceinline__ size_t line_base(const FcParams &p, int a, int sx, int pb, int LN) {
-    return ((((size_t)a * (p.L >> 1) + sx) * p.PB + pb) * p.L) * LN;
+__device__ __forceinline__ int swz(int row) { return row ^ ((row >> 4) & 1); }
+__device__ __forceinline__ size_t line_base(const FcParams &p, int a, int sx, int pb) {
+    return ((((size_t)a * (p.L >> 1) + sx) * p.PBZ + pb) * p.L) * p.LZ;
 }
 
 // x forward, colour p.colour: grid (PB, L rows, 3 components), block (LN, TL), TL = min(16, N2X) threads per line.
@@ -227,8 +234,8 @@ __global__ void __launch_bounds__(512) fftc_x_forward_kernel(const FcParams p) {
     __syncthreads();
     pdl_trigger();                                         // late: a successor resident earlier only takes room
     const bool odd_row = (y + c) & 1;                      // sites x = 2 i + 1: row phase e^{-2 pi i kx / L}
-    float2 *dst = p.Z + line_base(p, a, 0, pb, LN) + (size_t)y * LN + lane;
-    const size_t sx_stride = (size_t)p.PB * L * LN;
+    float2 *dst = p.Z + line_base(p, a, 0, pair / p.LZ) + (size_t)swz(y) * p.LZ + pair % p.LZ;
+    const size_t sx_stride = (size_t)p.PBZ * L * p.LZ;
     for (int k1 = t; k1 < 16; k1 += TL) {
         float2 u[N2X];
         fwd_step2<N2X>(u, k1, buf, LN, lane);
@@ -253,8 +260,8 @@ __global__ void __launch_bounds__(512) fftc_x_inverse_kernel(const FcParams p) {
     float2 *tw = fsm, *buf = fsm + L;
     const int lane = threadIdx.x, t = threadIdx.y;
     const int pb = blockIdx.x, pair = pb * LN + lane, y = blockIdx.y, a = blockIdx.z, c = p.colour;
-    const float2 *src = p.Z + line_base(p, a, 0, pb, LN) + (size_t)y * LN + lane;
-    const size_t sx_stride = (size_t)p.PB * L * LN;
+    const float2 *src = p.Z + line_base(p, a, 0, pair / p.LZ) + (size_t)swz(y) * p.LZ + pair % p.LZ;
+    const size_t sx_stride = (size_t)p.PBZ * L * p.LZ;
     constexpr int NK = N2X >= 16 ? 1 : 16 / N2X;           // blocks k1 per thread
     pdl_wait();                                            // the lines come from the y pass
     float2 u[NK][N2X];
@@ -284,11 +291,64 @@ __global__ void __launch_bounds__(512) fftc_x_inverse_kernel(const FcParams p) {
     for (int n1 = 0; n1 < 16; ++n1) dst[(size_t)(N2X * n1 + t) * p.P] = v[n1];
 }
 
+
+// In-place four-step transforms of one shared-memory line B[row' * LZ + lane] (rows = y or slot_y, see FcParams).
+// Forward: natural order in, slot order out; inverse: slot order in, natural order out.  Step 1 works on the rows
+// {N2 n1 + n2 : n1} = {N2 k1 + n2 : k1} of a sub-sequence n2, step 2 on the rows {N2 t + k} of block t: both write back
+// exactly the rows they read, so each half needs no barrier of its own (the caller puts one between the halves).
+template <int N2>
+__device__ __forceinline__ void line_fwd_step1(float2 *B, const float2 *tw, int LZ, int lane, int t) {
+    for (int n2 = t; n2 < N2; n2 += 16) {
+        float2 v[16];
+#pragma unroll
+        for (int n1 = 0; n1 < 16; ++n1) v[n1] = B[swz(N2 * n1 + n2) * LZ + lane];
+        fft_reg<16, false>(v);
+#pragma unroll
+        for (int k1 = 0; k1 < 16; ++k1) {
+            const float2 w = tw[n2 * k1];
+            B[swz(N2 * k1 + n2) * LZ + lane] = cmul(v[bitrev<16>(k1)], make_float2(w.x, -w.y));
+        }
+    }
+}
+template <int N2>
+__device__ __forceinline__ void line_fwd_step2(float2 *B, int LZ, int lane, int t) {
+    float2 v[N2];
+#pragma unroll
+    for (int n2 = 0; n2 < N2; ++n2) v[n2] = B[swz(N2 * t + n2) * LZ + lane];
+    fft_reg<N2, false>(v);
+#pragma unroll
+    for (int k2 = 0; k2 < N2; ++k2) B[swz(N2 * t + k2) * LZ + lane] = v[bitrev<N2>(k2)];
+}
+template <int N2>
+__device__ __forceinline__ void line_inv_step2(float2 *B, const float2 *tw, int LZ, int lane, int t) {
+    float2 u[N2];
+#pragma unroll
+    for (int k2 = 0; k2 < N2; ++k2) u[k2] = B[swz(N2 * t + k2) * LZ + lane];
+    fft_reg<N2, true>(u);
+#pragma unroll
+    for (int n2 = 0; n2 < N2; ++n2) B[swz(N2 * t + n2) * LZ + lane] = cmul(u[bitrev<N2>(n2)], tw[n2 * t]);
+}
+template <int N2>
+__device__ __forceinline__ void line_inv_step1(float2 *B, int LZ, int lane, int t) {
+    for (int n2 = t; n2 < N2; n2 += 16) {
+        float2 v[16];
+#pragma unroll
+        for (int k1 = 0; k1 < 16; ++k1) v[k1] = B[swz(N2 * k1 + n2) * LZ + lane];
+        fft_reg<16, true>(v);
+#pragma unroll
+        for (int n1 = 0; n1 < 16; ++n1) B[swz(N2 * n1 + n2) * LZ + lane] = v[bitrev<16>(n1)];
+    }
+}
+
 __device__ __forceinline__ float2 cmac(float2 acc, float2 a, float2 m) {  // acc + a * m
     return make_float2(fmaf(a.x, m.x, fmaf(-a.y, m.y, acc.x)), fmaf(a.x, m.y, fmaf(a.y, m.x, acc.y)));
 }
 
-// The y pass, column slot_x of the half-spectrum, LN pairs: grid (PB, L/2 slots), block (LN, 16).
+// The y pass.  A CTA owns two lines of LZ replica pairs and transforms them in place in shared memory; every byte it
+// moves to or from global memory goes by TMA bulk copy (one contiguous line each), issued by one thread at the top, so
+// no warp ever waits on a global load: while one CTA's lines are in flight the other CTAs of the SM compute.
+//   grid (PBZ, L/2 + L/4), block (LZ, 16).  blockIdx.y < L/2: the x and y lines of column slot_x = blockIdx.y (they mix
+//   through W^xy); else the z lines of the two columns 2 (blockIdx.y - L/2) and + 1: every CTA has the same size.
 //   FC_FWD_ONLY  Z holds the x-transformed rows of colour c = p.colour: forward L-point FFT over y -> S^_c -> Cnew.
 //   FC_FUSED     the same, then H^_t = A S^_t + B S^_c with t = 1 - c and S^_t read from Ctgt, inverse FFT over ky -> Z.
 //   FC_COMBINE   nothing to transform forward: S^_c is read from Cnew as well (both caches valid); t = 1 - c.
@@ -296,108 +356,97 @@ __device__ __forceinline__ float2 cmac(float2 acc, float2 a, float2 m) {  // acc
 enum { FC_FWD_ONLY = 0, FC_FUSED = 1, FC_COMBINE = 2 };
 
 template <int N2, int MODE>
-__global__ void __launch_bounds__(256, 2) fftc_y_kernel(const FcParams p) {
-    extern __shared__ __align__(16) float2 fsm[];
-    constexpr int L = 16 * N2;
-    const int LN = blockDim.x;
-    float2 *tw = fsm;
-    float2 *b0 = fsm + L;
-    float2 *buf[3] = {b0, b0 + (size_t)line_rows<N2>() * LN, b0 + 2 * (size_t)line_rows<N2>() * LN};
-    const int lane = threadIdx.x, t = threadIdx.y;
-    const int pb = blockIdx.x, sx = blockIdx.y;
+__global__ void __launch_bounds__(128, 3) fftc_y_kernel(const FcParams p) {
+    extern __shared__ __align__(128) unsigned char ysm_raw[];
+    constexpr int L = 16 * N2, Lh = L / 2;
+    const int LZ = blockDim.x;
+    const uint32_t line_elems = (uint32_t)(L * LZ), line_bytes = line_elems * (uint32_t)sizeof(float2);
+    float2 *B0 = reinterpret_cast<float2 *>(ysm_raw), *B1 = B0 + line_elems, *B2 = B1 + line_elems, *B3 = B2 + line_elems;
+    float2 *tw = B0 + (MODE == FC_FWD_ONLY ? 2 : 4) * (size_t)line_elems;
+    uint64_t *bars = reinterpret_cast<uint64_t *>(tw + L);
+    const int lane = threadIdx.x, t = threadIdx.y, tid = t * LZ + lane;
+    const int pb = blockIdx.x;
+    const bool is_z = (int)blockIdx.y >= Lh;
+    const int sx0 = is_z ? 2 * ((int)blockIdx.y - Lh) : (int)blockIdx.y;
+    const int sx1 = is_z ? sx0 + 1 : sx0;
+    const size_t off0 = line_base(p, is_z ? 2 : 0, sx0, pb), off1 = line_base(p, is_z ? 2 : 1, sx1, pb);
+    if (tid == 0) {
+        mbar_init(&bars[0], 1);
+        mbar_init(&bars[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
     fill_twiddles(tw, L);
-    pdl_wait();                                            // Z comes from the x pass, the caches from earlier y passes
     __syncthreads();
-    const size_t a_stride = (size_t)(L >> 1) * p.PB * L * LN;   // one component
-    const size_t base = line_base(p, 0, sx, pb, LN) + lane;
-    float2 *col = p.Z + base;                              // + a * a_stride + row * LN
-    float2 *cnew = p.Cnew + base;
-    const float2 *ctgt = p.Ctgt + base;
+    pdl_wait();                                            // Z comes from the x pass, the caches from earlier y passes
+    if (tid == 0) {
+        const float2 *in = MODE == FC_COMBINE ? p.Cnew : p.Z;
+        mbar_expect_tx(&bars[0], 2 * line_bytes);
+        bulk_g2s(B0, in + off0, line_bytes, &bars[0]);
+        bulk_g2s(B1, in + off1, line_bytes, &bars[0]);
+        if (MODE != FC_FWD_ONLY) {
+            mbar_expect_tx(&bars[1], 2 * line_bytes);
+            bulk_g2s(B2, p.Ctgt + off0, line_bytes, &bars[1]);
+            bulk_g2s(B3, p.Ctgt + off1, line_bytes, &bars[1]);
+        }
+    }
+    mbar_wait(&bars[0], 0);
     if (MODE != FC_COMBINE) {
-#pragma unroll 1
-        for (int a = 0; a < 3; ++a)
-            for (int n2 = t; n2 < N2; n2 += 16) {
-                float2 v[16];
-#pragma unroll
-                for (int n1 = 0; n1 < 16; ++n1) v[n1] = col[a * a_stride + (size_t)(N2 * n1 + n2) * LN];
-                fwd_step1<N2, 1>(v, n2, tw, buf[a], LN, lane);
-            }
+        line_fwd_step1<N2>(B0, tw, LZ, lane, t);
+        line_fwd_step1<N2>(B1, tw, LZ, lane, t);
         __syncthreads();
+        line_fwd_step2<N2>(B0, LZ, lane, t);
+        line_fwd_step2<N2>(B1, LZ, lane, t);
+        fence_async_smem();                                // the spectra go to the cache straight from shared memory
+        __syncthreads();
+        if (tid == 0) {
+            bulk_s2g(p.Cnew + off0, B0, line_bytes);
+            bulk_s2g(p.Cnew + off1, B1, line_bytes);
+            bulk_commit();
+        }
+        if (MODE == FC_FWD_ONLY) {
+            pdl_trigger();
+            if (tid == 0) bulk_wait_all();
+            return;
+        }
     }
-    // The thread owns block t (slots N2 t + k2) of all three components.
-    const size_t row0 = (size_t)(N2 * t) * LN;
-    float2 u[N2];
-    float2 *bx = buf[0] + sidx<N2>(t, 0) * LN + lane;      // the x spectrum waits in the thread's own shared block
-    if (MODE != FC_COMBINE) {
-        fwd_step2<N2>(u, t, buf[0], LN, lane);
-#pragma unroll
-        for (int k2 = 0; k2 < N2; ++k2) cnew[row0 + (size_t)k2 * LN] = u[k2];
-    } else {
-#pragma unroll
-        for (int k2 = 0; k2 < N2; ++k2) u[k2] = cnew[row0 + (size_t)k2 * LN];
-    }
-    if (MODE != FC_FWD_ONLY) {
-#pragma unroll
-        for (int k2 = 0; k2 < N2; ++k2) bx[k2 * LN] = u[k2];
-    }
-    if (MODE != FC_COMBINE) {
-        fwd_step2<N2>(u, t, buf[1], LN, lane);             // u now holds the y component
-#pragma unroll
-        for (int k2 = 0; k2 < N2; ++k2) cnew[a_stride + row0 + (size_t)k2 * LN] = u[k2];
-    } else {
-#pragma unroll
-        for (int k2 = 0; k2 < N2; ++k2) u[k2] = cnew[a_stride + row0 + (size_t)k2 * LN];
-    }
-    if (MODE == FC_FWD_ONLY) {
-        fwd_step2<N2>(u, t, buf[2], LN, lane);
-#pragma unroll
-        for (int k2 = 0; k2 < N2; ++k2) cnew[2 * a_stride + row0 + (size_t)k2 * LN] = u[k2];
-        pdl_trigger();
-        return;
-    }
-    {
-        // this column's tables: a constant array read through the read-only path (the lanes of a half-warp share an address)
-        const float4 *tab = p.AB + ((size_t)sx * L + N2 * t) * 4;
-#pragma unroll
+    mbar_wait(&bars[1], 0);
+    // H^ = A S^_t + B S^_c, rows N2 t + k2 (the rows this thread wrote in step 2), result over S^_t in B2, B3
+    if (!is_z) {
+        const float4 *tab = p.AB + ((size_t)sx0 * L + N2 * t) * 4;   // constant table, read-only path
+#pragma unroll 4
         for (int k2 = 0; k2 < N2; ++k2) {
             const float4 m0 = __ldg(tab + 4 * k2), m1 = __ldg(tab + 4 * k2 + 1), m2 = __ldg(tab + 4 * k2 + 2);
             const float2 Axx = make_float2(m0.x, m0.y), Axy = make_float2(m0.z, m0.w), Ayy = make_float2(m1.x, m1.y);
             const float2 Bxx = make_float2(m1.z, m1.w), Bxy = make_float2(m2.x, m2.y), Byy = make_float2(m2.z, m2.w);
-            const float2 tx = ctgt[row0 + (size_t)k2 * LN], ty = ctgt[a_stride + row0 + (size_t)k2 * LN];
-            const float2 ox = bx[k2 * LN], oy = u[k2];
-            bx[k2 * LN] = cmac(cmac(cmac(cmul(tx, Axx), ty, Axy), ox, Bxx), oy, Bxy);
-            u[k2] = cmac(cmac(cmac(cmul(tx, Axy), ty, Ayy), ox, Bxy), oy, Byy);
+            const int r = swz(N2 * t + k2) * LZ + lane;
+            const float2 ox = B0[r], oy = B1[r], tx = B2[r], ty = B3[r];
+            B2[r] = cmac(cmac(cmac(cmul(tx, Axx), ty, Axy), ox, Bxx), oy, Bxy);
+            B3[r] = cmac(cmac(cmac(cmul(tx, Axy), ty, Ayy), ox, Bxy), oy, Byy);
         }
-        inv_step2<N2, 1>(u, t, tw, buf[1], LN, lane);
-#pragma unroll
-        for (int k2 = 0; k2 < N2; ++k2) u[k2] = bx[k2 * LN];
-        inv_step2<N2, 1>(u, t, tw, buf[0], LN, lane);
-        if (MODE != FC_COMBINE) {
-            fwd_step2<N2>(u, t, buf[2], LN, lane);         // u reused for the z component
-#pragma unroll
-            for (int k2 = 0; k2 < N2; ++k2) cnew[2 * a_stride + row0 + (size_t)k2 * LN] = u[k2];
-        } else {
-#pragma unroll
-            for (int k2 = 0; k2 < N2; ++k2) u[k2] = cnew[2 * a_stride + row0 + (size_t)k2 * LN];
-        }
-#pragma unroll
+    } else {
+        const float4 *tab0 = p.AB + ((size_t)sx0 * L + N2 * t) * 4 + 3, *tab1 = p.AB + ((size_t)sx1 * L + N2 * t) * 4 + 3;
+#pragma unroll 4
         for (int k2 = 0; k2 < N2; ++k2) {
-            const float4 m3 = __ldg(tab + 4 * k2 + 3);
-            const float2 tz = ctgt[2 * a_stride + row0 + (size_t)k2 * LN];
-            u[k2] = cmac(cmul(tz, make_float2(m3.x, m3.y)), u[k2], make_float2(m3.z, m3.w));
+            const float4 ma = __ldg(tab0 + 4 * k2), mb = __ldg(tab1 + 4 * k2);
+            const int r = swz(N2 * t + k2) * LZ + lane;
+            B2[r] = cmac(cmul(B2[r], make_float2(ma.x, ma.y)), B0[r], make_float2(ma.z, ma.w));
+            B3[r] = cmac(cmul(B3[r], make_float2(mb.x, mb.y)), B1[r], make_float2(mb.z, mb.w));
         }
-        inv_step2<N2, 1>(u, t, tw, buf[2], LN, lane);
     }
+    line_inv_step2<N2>(B2, tw, LZ, lane, t);
+    line_inv_step2<N2>(B3, tw, LZ, lane, t);
+    __syncthreads();
+    line_inv_step1<N2>(B2, LZ, lane, t);
+    line_inv_step1<N2>(B3, LZ, lane, t);
+    fence_async_smem();
     __syncthreads();
     pdl_trigger();
-#pragma unroll 1
-    for (int a = 0; a < 3; ++a)
-        for (int n2 = t; n2 < N2; n2 += 16) {
-            float2 v[16];
-            inv_step1<N2>(v, n2, buf[a], LN, lane);
-#pragma unroll
-            for (int n1 = 0; n1 < 16; ++n1) col[a * a_stride + (size_t)(N2 * n1 + n2) * LN] = v[n1];
-        }
+    if (tid == 0) {
+        bulk_s2g(p.Z + off0, B2, line_bytes);
+        bulk_s2g(p.Z + off1, B3, line_bytes);
+        bulk_commit();
+        bulk_wait_all();                                   // shared memory must outlive the copies; the next kernel reads Z
+    }
 }
 
 // ---- A, B = folded transform of W, fp64, once per tensor --------------------------------------
@@ -455,8 +504,8 @@ int pairs_per_cta(int P, int cap) {
 }
 
 template <int N2>
-size_t y_smem_bytes(int LN) {
-    return sizeof(float2) * (16 * N2 + 3 * (size_t)line_rows<N2>() * LN);
+size_t y_smem_bytes(int LZ, int lines) {
+    return sizeof(float2) * ((size_t)lines * 16 * N2 * LZ + 16 * N2) + 64;
 }
 
 // one field of colour `colour` (0 / 1), or of both (-1); valid[c] = "the cache holds the half-spectrum of colour c of the
@@ -466,23 +515,25 @@ cudaError_t launch_fftc(FcParams p, float2 *C, size_t cache_elems, int colour, b
                         uint64_t *launches) {
     constexpr int L = 16 * N2, N2X = N2 / 2 > 0 ? N2 / 2 : 1;
     static_assert(N2 >= 2, "L >= 32");
-    // 16 replica pairs per CTA: 128-byte runs in HBM; fewer when the y pass would not fit its line buffers (L = 512)
-    int cap = 16;
-    while (cap > 1 && y_smem_bytes<N2>(cap) > 220 * 1024) cap >>= 1;
-    const int LN = pairs_per_cta(p.P, cap);
-    p.PB = p.P / LN;
+    // lines of 8 replica pairs (64-byte runs): four of them are 64 KB of shared memory at L = 256, three CTAs per SM
+    int capz = 8;
+    while (capz > 1 && y_smem_bytes<N2>(capz, 4) > 200 * 1024) capz >>= 1;
+    p.LZ = pairs_per_cta(p.P, capz);
+    p.PBZ = p.P / p.LZ;
+    const int LNX = pairs_per_cta(p.P, 16);               // the x passes: 16 pairs per CTA = 128-byte runs of the spin arrays
     const int TL = N2X < 16 ? N2X : 16;
-    const size_t smx = sizeof(float2) * (L + (size_t)line_rows<N2X>() * LN);
+    const size_t smx = sizeof(float2) * (L + (size_t)line_rows<N2X>() * LNX);
+    const size_t smy2 = y_smem_bytes<N2>(p.LZ, 2), smy4 = y_smem_bytes<N2>(p.LZ, 4);
     if (!*configured) {
         cudaError_t e;
-        if ((e = cudaFuncSetAttribute(fftc_y_kernel<N2, FC_FWD_ONLY>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024)) != cudaSuccess) return e;
-        if ((e = cudaFuncSetAttribute(fftc_y_kernel<N2, FC_FUSED>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024)) != cudaSuccess) return e;
-        if ((e = cudaFuncSetAttribute(fftc_y_kernel<N2, FC_COMBINE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024)) != cudaSuccess) return e;
+        if ((e = cudaFuncSetAttribute(fftc_y_kernel<N2, FC_FWD_ONLY>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)) != cudaSuccess) return e;
+        if ((e = cudaFuncSetAttribute(fftc_y_kernel<N2, FC_FUSED>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)) != cudaSuccess) return e;
+        if ((e = cudaFuncSetAttribute(fftc_y_kernel<N2, FC_COMBINE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)) != cudaSuccess) return e;
         if ((e = cudaFuncSetAttribute(fftc_x_forward_kernel<N2X>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024)) != cudaSuccess) return e;
         if ((e = cudaFuncSetAttribute(fftc_x_inverse_kernel<N2X>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024)) != cudaSuccess) return e;
         *configured = true;
     }
-    const dim3 gx(p.PB, L, 3), bx(LN, TL), gy(p.PB, L / 2), by(LN, 16);
+    const dim3 gx(p.P / LNX, L, 3), bx(LNX, TL), gy(p.PBZ, L / 2 + L / 4), by(p.LZ, 16);
     cudaError_t e = cudaSuccess;
     auto x_forward = [&](int c) {
         FcParams q = p;
@@ -496,9 +547,9 @@ cudaError_t launch_fftc(FcParams p, float2 *C, size_t cache_elems, int colour, b
         q.Cnew = C + (size_t)c * cache_elems;
         q.Ctgt = C + (size_t)(1 - c) * cache_elems;
         ++*launches;
-        if (mode == FC_FWD_ONLY) return launch_pdl(fftc_y_kernel<N2, FC_FWD_ONLY>, gy, by, y_smem_bytes<N2>(LN), st, q);
-        if (mode == FC_FUSED) return launch_pdl(fftc_y_kernel<N2, FC_FUSED>, gy, by, y_smem_bytes<N2>(LN), st, q);
-        return launch_pdl(fftc_y_kernel<N2, FC_COMBINE>, gy, by, y_smem_bytes<N2>(LN), st, q);
+        if (mode == FC_FWD_ONLY) return launch_pdl(fftc_y_kernel<N2, FC_FWD_ONLY>, gy, by, smy2, st, q);
+        if (mode == FC_FUSED) return launch_pdl(fftc_y_kernel<N2, FC_FUSED>, gy, by, smy4, st, q);
+        return launch_pdl(fftc_y_kernel<N2, FC_COMBINE>, gy, by, smy4, st, q);
     };
     auto x_inverse = [&](int c) {
         FcParams q = p;
@@ -559,7 +610,8 @@ cudaError_t launch_field_fft(const float *S, const float *AB, void *scratch, voi
     p.AB = (const float4 *)AB;
     p.L = L;
     p.P = R / 2;
-    p.PB = 1;
+    p.LZ = 1;
+    p.PBZ = 1;
     p.colour = 0;
     const size_t ce = dsmc_fft_cache_elems(L, R);
     switch (L / 16) {
