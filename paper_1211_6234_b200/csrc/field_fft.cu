@@ -30,6 +30,7 @@
 // A, B are tabulated in slot order with the 1/N of the inverse folded in.
 #include "dsmc_internal.cuh"
 #include "bulk_copy.cuh"
+#include "packed_f32x2.cuh"
 
 namespace {
 
@@ -133,28 +134,47 @@ __device__ __forceinline__ void fft_reg(float2 (&v)[N]) {
 }
 
 // ---- the four steps of a length n = 16 * N2 transform --------------------------------------
-// buf[sidx(k1, n2) * LN + lane] is the CTA's shared line buffer (LN = replica pairs per CTA): slot
-// N2 k1 + n2 with one pad row per block of N2 slots, so that blocks k1, k1 + 1 of a warp fall on different banks when
-// LN < 16.  tw[j] = (cos, sin)(2 pi j / L) with L the LATTICE size: a length-L line uses stride TS = 1, a length-L/2 line
-// TS = 2.  Threads are (lane, t).
+// Twiddles come from two tables of L entries (L = the LATTICE size; a length-L line uses stride TS = 1, a length-L/2 line
+// TS = 2): twf[j] = (c, -s) = e^{-2 pi i j / L} (forward transforms), twi[j] = (c, s) (inverse transforms), read with
+// 64-bit shared loads (128-bit entries holding both operand pairs of the packed multiply were measured slower: a
+// broadcast LDS.128 still takes four passes, and the x passes became bound by the shared-memory queue).
+// a * (x + i y) = a.x (x, y) + a.y (-y, x): one sign flip (integer pipe), one FMUL2 and one FFMA2 with the scalars as
+// broadcast operands.
+__device__ __forceinline__ float2 cmul_tw(float2 a, float2 w) {
+    f2 r = f2_mul(f2_bc(a.x), f2_make(w.x, w.y));
+    r = f2_fma(f2_bc(a.y), f2_make(__uint_as_float(__float_as_uint(w.y) ^ 0x80000000u), w.x), r);
+    float2 o;
+    f2_split(r, o.x, o.y);
+    return o;
+}
+
+// LNC = lanes (replica pairs) per line as a compile-time constant, 0 = blockDim.x (small replica counts)
+template <int LNC>
+__device__ __forceinline__ int nlanes() { return LNC ? LNC : (int)blockDim.x; }
+
+// x passes: buf[sidx(k1, n2) * LN + lane] is the CTA's shared line buffer: slot N2 k1 + n2 with one pad row per block of
+// N2 slots, so that blocks k1, k1 + 1 of a warp fall on different banks when LN < 16.  Threads are (lane, t).
 template <int N2>
 __device__ __forceinline__ int sidx(int k1, int n2) { return (N2 + 1) * k1 + n2; }
 template <int N2>
 __host__ __device__ constexpr int line_rows() { return (N2 + 1) * 16; }
 
 // forward step 1: v[n1] = x[N2 n1 + n2]  ->  A[k1][n2] * W_n^{n2 k1}  at slot N2 k1 + n2
-template <int N2, int TS>
-__device__ __forceinline__ void fwd_step1(float2 (&v)[16], int n2, const float2 *tw, float2 *buf, int LN, int lane) {
+template <int N2, int TS, int LNC>
+__device__ __forceinline__ void fwd_step1(float2 (&v)[16], int n2, const float2 *twf, float2 *buf, int lane) {
+    const int LN = nlanes<LNC>();
+    float2 w[16];                                          // all twiddles first: the loads go out as one batch
+#pragma unroll
+    for (int k1 = 1; k1 < 16; ++k1) w[k1] = twf[TS * n2 * k1];
     fft_reg<16, false>(v);
 #pragma unroll
-    for (int k1 = 0; k1 < 16; ++k1) {
-        const float2 w = tw[TS * n2 * k1];
-        buf[sidx<N2>(k1, n2) * LN + lane] = cmul(v[bitrev<16>(k1)], make_float2(w.x, -w.y));
-    }
+    for (int k1 = 0; k1 < 16; ++k1)
+        buf[sidx<N2>(k1, n2) * LN + lane] = k1 == 0 ? v[0] : cmul_tw(v[bitrev<16>(k1)], w[k1]);
 }
 // forward step 2: block k1 -> u[k2] = X[k1 + 16 k2] in natural k2 order
-template <int N2>
-__device__ __forceinline__ void fwd_step2(float2 (&u)[N2], int k1, const float2 *buf, int LN, int lane) {
+template <int N2, int LNC>
+__device__ __forceinline__ void fwd_step2(float2 (&u)[N2], int k1, const float2 *buf, int lane) {
+    const int LN = nlanes<LNC>();
     float2 t[N2];
 #pragma unroll
     for (int n2 = 0; n2 < N2; ++n2) t[n2] = buf[sidx<N2>(k1, n2) * LN + lane];
@@ -163,30 +183,27 @@ __device__ __forceinline__ void fwd_step2(float2 (&u)[N2], int k1, const float2 
     for (int k2 = 0; k2 < N2; ++k2) u[k2] = t[bitrev<N2>(k2)];
 }
 // inverse step 2: u[k2] = Y[k1 + 16 k2]  ->  B[k1][n2] * conj(W_n^{n2 k1})  at slot N2 k1 + n2
-template <int N2, int TS>
-__device__ __forceinline__ void inv_step2(float2 (&u)[N2], int k1, const float2 *tw, float2 *buf, int LN, int lane) {
+template <int N2, int TS, int LNC>
+__device__ __forceinline__ void inv_step2(float2 (&u)[N2], int k1, const float2 *twi, float2 *buf, int lane) {
+    const int LN = nlanes<LNC>();
+    float2 w[N2];
+#pragma unroll
+    for (int n2 = 1; n2 < N2; ++n2) w[n2] = twi[TS * n2 * k1];
     fft_reg<N2, true>(u);
 #pragma unroll
-    for (int n2 = 0; n2 < N2; ++n2) buf[sidx<N2>(k1, n2) * LN + lane] = cmul(u[bitrev<N2>(n2)], tw[TS * n2 * k1]);
+    for (int n2 = 0; n2 < N2; ++n2)
+        buf[sidx<N2>(k1, n2) * LN + lane] = n2 == 0 ? u[0] : cmul_tw(u[bitrev<N2>(n2)], w[n2]);
 }
 // inverse step 1: slots N2 k1 + n2 (k1 = 0..15)  ->  v[n1] = x[N2 n1 + n2]
-template <int N2>
-__device__ __forceinline__ void inv_step1(float2 (&v)[16], int n2, const float2 *buf, int LN, int lane) {
+template <int N2, int LNC>
+__device__ __forceinline__ void inv_step1(float2 (&v)[16], int n2, const float2 *buf, int lane) {
+    const int LN = nlanes<LNC>();
     float2 t[16];
 #pragma unroll
     for (int k1 = 0; k1 < 16; ++k1) t[k1] = buf[sidx<N2>(k1, n2) * LN + lane];
     fft_reg<16, true>(t);
 #pragma unroll
     for (int n1 = 0; n1 < 16; ++n1) v[n1] = t[bitrev<16>(n1)];
-}
-
-__device__ __forceinline__ void fill_twiddles(float2 *tw, int L) {
-    const int tid = threadIdx.y * blockDim.x + threadIdx.x, nt = blockDim.x * blockDim.y;
-    for (int j = tid; j < L; j += nt) {
-        float s, c;
-        sincospif(2.0f * (float)j / (float)L, &s, &c);   // exact argument: j / L is a dyadic fraction
-        tw[j] = make_float2(c, s);
-    }
 }
 
 // Z and the two caches share one layout: [a][slot_x][pb][row'][lane], a = component, slot_x < L/2, pb = block of LZ
@@ -203,6 +220,7 @@ struct FcParams {
     float2 *Cnew;      // y pass: cache of the half-spectrum of colour `colour` (written unless FC_COMBINE, then read)
     const float2 *Ctgt;  // y pass: cache of the half-spectrum of the target colour 1 - colour
     const float4 *AB;  // AB[slot_x][slot_y][4]: (Axx, Axy), (Ayy, Bxx), (Bxy, Byy), (Azz, Bzz), each complex, scaled 1/N
+    const float2 *twf, *twi;  // twiddle tables, L entries each (behind AB in the workspace)
     int L, P;          // P = R / 2 complex replica pairs
     int LZ, PBZ;       // lanes per line and line blocks: P = PBZ * LZ
     int colour;        // x passes: the colour of the rows; y pass: the colour whose lines sit in Z / in Cnew
@@ -213,105 +231,107 @@ __device__ __forceinline__ size_t line_base(const FcParams &p, int a, int sx, in
     return ((((size_t)a * (p.L >> 1) + sx) * p.PBZ + pb) * p.L) * p.LZ;
 }
 
-// x forward, colour p.colour: grid (PB, L rows, 3 components), block (LN, TL), TL = min(16, N2X) threads per line.
-template <int N2X>
-__global__ void __launch_bounds__(512) fftc_x_forward_kernel(const FcParams p) {
+// x forward, colour p.colour: grid (P / LN, L rows, 3 components), block (LN, TL), TL = min(16, N2X) threads per line.
+template <int N2X, int LNC>
+__global__ void __launch_bounds__(256) fftc_x_forward_kernel(const FcParams p) {
     extern __shared__ __align__(16) float2 fsm[];
     constexpr int Lh = 16 * N2X, L = 2 * Lh;
-    const int LN = blockDim.x, TL = blockDim.y;
-    float2 *tw = fsm, *buf = fsm + L;
-    const int lane = threadIdx.x, t = threadIdx.y;
-    const int pb = blockIdx.x, pair = pb * LN + lane, y = blockIdx.y, a = blockIdx.z, c = p.colour;
+    const int LN = nlanes<LNC>(), TL = blockDim.y;
+    float2 *twf = fsm, *buf = fsm + L;
+    const int lane = threadIdx.x, t = threadIdx.y, tid = t * LN + lane;
+    const int pair = blockIdx.x * LN + lane, y = blockIdx.y, a = blockIdx.z, c = p.colour;
+    for (int j = tid; j < L; j += LN * TL) twf[j] = __ldg(p.twf + j);   // a constant table: before the wait
     const size_t planeP = (size_t)L * Lh * p.P;
     const float2 *src = reinterpret_cast<const float2 *>(p.S) + (size_t)(c * 3 + a) * planeP + (size_t)y * Lh * p.P + pair;
+    const unsigned ld_stride = (unsigned)(N2X * p.P);
     pdl_wait();                                            // the spins come from the Metropolis kernel before
     float2 v[16];
+    src += (unsigned)t * p.P;                              // t < N2X by construction
 #pragma unroll
-    for (int n1 = 0; n1 < 16; ++n1) v[n1] = __ldg(src + (size_t)(N2X * n1 + t) * p.P);   // t < N2X by construction
-    fill_twiddles(tw, L);                                  // while the loads are in flight
+    for (int n1 = 0; n1 < 16; ++n1) v[n1] = __ldg(src + n1 * ld_stride);
     __syncthreads();
-    fwd_step1<N2X, 2>(v, t, tw, buf, LN, lane);
+    fwd_step1<N2X, 2, LNC>(v, t, twf, buf, lane);
     __syncthreads();
     pdl_trigger();                                         // late: a successor resident earlier only takes room
     const bool odd_row = (y + c) & 1;                      // sites x = 2 i + 1: row phase e^{-2 pi i kx / L}
-    float2 *dst = p.Z + line_base(p, a, 0, pair / p.LZ) + (size_t)swz(y) * p.LZ + pair % p.LZ;
-    const size_t sx_stride = (size_t)p.PBZ * L * p.LZ;
+    const int lz = LNC ? (LNC < 8 ? LNC : 8) : p.LZ;       // LNC = 16 goes with lines of 8 pairs
+    float2 *dst = p.Z + line_base(p, a, 0, pair / lz) + (size_t)swz(y) * lz + pair % lz;
+    const unsigned sx_stride = (unsigned)(p.PBZ * L * lz);
     for (int k1 = t; k1 < 16; k1 += TL) {
-        float2 u[N2X];
-        fwd_step2<N2X>(u, k1, buf, LN, lane);
+        float2 u[N2X], w[N2X];
 #pragma unroll
-        for (int k2 = 0; k2 < N2X; ++k2) {
-            float2 r = u[k2];
-            if (odd_row) {
-                const float2 w = tw[k1 + 16 * k2];
-                r = cmul(r, make_float2(w.x, -w.y));
-            }
-            dst[(size_t)(N2X * k1 + k2) * sx_stride] = r;
-        }
+        for (int k2 = 0; k2 < N2X; ++k2) w[k2] = twf[odd_row ? k1 + 16 * k2 : 0];   // twf[0] = 1: no branch
+        fwd_step2<N2X, LNC>(u, k1, buf, lane);
+#pragma unroll
+        for (int k2 = 0; k2 < N2X; ++k2) dst[(unsigned)(N2X * k1 + k2) * sx_stride] = cmul_tw(u[k2], w[k2]);
     }
 }
 
-// x inverse, target colour p.colour: grid (PB, L rows, 3 components), block (LN, TL).
-template <int N2X>
-__global__ void __launch_bounds__(512) fftc_x_inverse_kernel(const FcParams p) {
+// x inverse, target colour p.colour: grid (P / LN, L rows, 3 components), block (LN, TL).
+template <int N2X, int LNC>
+__global__ void __launch_bounds__(256) fftc_x_inverse_kernel(const FcParams p) {
     extern __shared__ __align__(16) float2 fsm[];
     constexpr int Lh = 16 * N2X, L = 2 * Lh;
-    const int LN = blockDim.x, TL = blockDim.y;
-    float2 *tw = fsm, *buf = fsm + L;
-    const int lane = threadIdx.x, t = threadIdx.y;
-    const int pb = blockIdx.x, pair = pb * LN + lane, y = blockIdx.y, a = blockIdx.z, c = p.colour;
-    const float2 *src = p.Z + line_base(p, a, 0, pair / p.LZ) + (size_t)swz(y) * p.LZ + pair % p.LZ;
-    const size_t sx_stride = (size_t)p.PBZ * L * p.LZ;
+    const int LN = nlanes<LNC>(), TL = blockDim.y;
+    float2 *twi = fsm, *buf = fsm + L;
+    const int lane = threadIdx.x, t = threadIdx.y, tid = t * LN + lane;
+    const int pair = blockIdx.x * LN + lane, y = blockIdx.y, a = blockIdx.z, c = p.colour;
+    for (int j = tid; j < L; j += LN * TL) twi[j] = __ldg(p.twi + j);
+    const int lz = LNC ? (LNC < 8 ? LNC : 8) : p.LZ;
+    const float2 *src = p.Z + line_base(p, a, 0, pair / lz) + (size_t)swz(y) * lz + pair % lz;
+    const unsigned sx_stride = (unsigned)(p.PBZ * L * lz);
     constexpr int NK = N2X >= 16 ? 1 : 16 / N2X;           // blocks k1 per thread
     pdl_wait();                                            // the lines come from the y pass
     float2 u[NK][N2X];
 #pragma unroll
     for (int j = 0; j < NK; ++j)
 #pragma unroll
-        for (int k2 = 0; k2 < N2X; ++k2) u[j][k2] = src[(size_t)(N2X * (t + j * TL) + k2) * sx_stride];
-    fill_twiddles(tw, L);
+        for (int k2 = 0; k2 < N2X; ++k2) u[j][k2] = src[(unsigned)(N2X * (t + j * TL) + k2) * sx_stride];
     __syncthreads();
     const bool odd_row = (y + c) & 1;                      // row phase e^{+2 pi i kx / L}
 #pragma unroll
     for (int j = 0; j < NK; ++j) {
         const int k1 = t + j * TL;
-        if (odd_row) {
+        float2 w[N2X];
 #pragma unroll
-            for (int k2 = 0; k2 < N2X; ++k2) u[j][k2] = cmul(u[j][k2], tw[k1 + 16 * k2]);
-        }
-        inv_step2<N2X, 2>(u[j], k1, tw, buf, LN, lane);
+        for (int k2 = 0; k2 < N2X; ++k2) w[k2] = twi[odd_row ? k1 + 16 * k2 : 0];   // twi[0] = 1: no branch
+#pragma unroll
+        for (int k2 = 0; k2 < N2X; ++k2) u[j][k2] = cmul_tw(u[j][k2], w[k2]);
+        inv_step2<N2X, 2, LNC>(u[j], k1, twi, buf, lane);
     }
     pdl_trigger();
     __syncthreads();
     float2 v[16];
-    inv_step1<N2X>(v, t, buf, LN, lane);
+    inv_step1<N2X, LNC>(v, t, buf, lane);
     const size_t planeP = (size_t)L * Lh * p.P;
-    float2 *dst = reinterpret_cast<float2 *>(p.H) + (size_t)(c * 3 + a) * planeP + (size_t)y * Lh * p.P + pair;
+    float2 *dst = reinterpret_cast<float2 *>(p.H) + (size_t)(c * 3 + a) * planeP + (size_t)y * Lh * p.P + pair + (unsigned)t * p.P;
+    const unsigned st_stride = (unsigned)(N2X * p.P);
 #pragma unroll
-    for (int n1 = 0; n1 < 16; ++n1) dst[(size_t)(N2X * n1 + t) * p.P] = v[n1];
+    for (int n1 = 0; n1 < 16; ++n1) dst[n1 * st_stride] = v[n1];
 }
-
 
 // In-place four-step transforms of one shared-memory line B[row' * LZ + lane] (rows = y or slot_y, see FcParams).
 // Forward: natural order in, slot order out; inverse: slot order in, natural order out.  Step 1 works on the rows
 // {N2 n1 + n2 : n1} = {N2 k1 + n2 : k1} of a sub-sequence n2, step 2 on the rows {N2 t + k} of block t: both write back
 // exactly the rows they read, so each half needs no barrier of its own (the caller puts one between the halves).
-template <int N2>
-__device__ __forceinline__ void line_fwd_step1(float2 *B, const float2 *tw, int LZ, int lane, int t) {
+template <int N2, int LZC>
+__device__ __forceinline__ void line_fwd_step1(float2 *B, const float2 *twf, int lane, int t) {
+    const int LZ = nlanes<LZC>();
     for (int n2 = t; n2 < N2; n2 += 16) {
-        float2 v[16];
+        float2 v[16], w[16];
 #pragma unroll
         for (int n1 = 0; n1 < 16; ++n1) v[n1] = B[swz(N2 * n1 + n2) * LZ + lane];
+#pragma unroll
+        for (int k1 = 1; k1 < 16; ++k1) w[k1] = twf[n2 * k1];
         fft_reg<16, false>(v);
 #pragma unroll
-        for (int k1 = 0; k1 < 16; ++k1) {
-            const float2 w = tw[n2 * k1];
-            B[swz(N2 * k1 + n2) * LZ + lane] = cmul(v[bitrev<16>(k1)], make_float2(w.x, -w.y));
-        }
+        for (int k1 = 0; k1 < 16; ++k1)
+            B[swz(N2 * k1 + n2) * LZ + lane] = k1 == 0 ? v[0] : cmul_tw(v[bitrev<16>(k1)], w[k1]);
     }
 }
-template <int N2>
-__device__ __forceinline__ void line_fwd_step2(float2 *B, int LZ, int lane, int t) {
+template <int N2, int LZC>
+__device__ __forceinline__ void line_fwd_step2(float2 *B, int lane, int t) {
+    const int LZ = nlanes<LZC>();
     float2 v[N2];
 #pragma unroll
     for (int n2 = 0; n2 < N2; ++n2) v[n2] = B[swz(N2 * t + n2) * LZ + lane];
@@ -319,17 +339,22 @@ __device__ __forceinline__ void line_fwd_step2(float2 *B, int LZ, int lane, int 
 #pragma unroll
     for (int k2 = 0; k2 < N2; ++k2) B[swz(N2 * t + k2) * LZ + lane] = v[bitrev<N2>(k2)];
 }
-template <int N2>
-__device__ __forceinline__ void line_inv_step2(float2 *B, const float2 *tw, int LZ, int lane, int t) {
-    float2 u[N2];
+template <int N2, int LZC>
+__device__ __forceinline__ void line_inv_step2(float2 *B, const float2 *twi, int lane, int t) {
+    const int LZ = nlanes<LZC>();
+    float2 u[N2], w[N2];
 #pragma unroll
     for (int k2 = 0; k2 < N2; ++k2) u[k2] = B[swz(N2 * t + k2) * LZ + lane];
+#pragma unroll
+    for (int n2 = 1; n2 < N2; ++n2) w[n2] = twi[n2 * t];
     fft_reg<N2, true>(u);
 #pragma unroll
-    for (int n2 = 0; n2 < N2; ++n2) B[swz(N2 * t + n2) * LZ + lane] = cmul(u[bitrev<N2>(n2)], tw[n2 * t]);
+    for (int n2 = 0; n2 < N2; ++n2)
+        B[swz(N2 * t + n2) * LZ + lane] = n2 == 0 ? u[0] : cmul_tw(u[bitrev<N2>(n2)], w[n2]);
 }
-template <int N2>
-__device__ __forceinline__ void line_inv_step1(float2 *B, int LZ, int lane, int t) {
+template <int N2, int LZC>
+__device__ __forceinline__ void line_inv_step1(float2 *B, int lane, int t) {
+    const int LZ = nlanes<LZC>();
     for (int n2 = t; n2 < N2; n2 += 16) {
         float2 v[16];
 #pragma unroll
@@ -340,14 +365,24 @@ __device__ __forceinline__ void line_inv_step1(float2 *B, int LZ, int lane, int 
     }
 }
 
-__device__ __forceinline__ float2 cmac(float2 acc, float2 a, float2 m) {  // acc + a * m
-    return make_float2(fmaf(a.x, m.x, fmaf(-a.y, m.y, acc.x)), fmaf(a.x, m.y, fmaf(a.y, m.x, acc.y)));
+// packed complex arithmetic of the spectral multiply: (a.x, a.y) as one 64-bit operand, m * a = m.x (a.x, a.y) + m.y (-a.y, a.x)
+__device__ __forceinline__ f2 c_pack(float2 a) { return f2_make(a.x, a.y); }
+__device__ __forceinline__ f2 c_rot(float2 a) { return f2_make(-a.y, a.x); }     // i * a
+__device__ __forceinline__ f2 c_mac(f2 acc, float mre, float mim, f2 a, f2 ia) {  // acc + m * a
+    return f2_fma(f2_bc(mim), ia, f2_fma(f2_bc(mre), a, acc));
+}
+__device__ __forceinline__ f2 c_mul(float mre, float mim, f2 a, f2 ia) { return f2_fma(f2_bc(mim), ia, f2_mul(f2_bc(mre), a)); }
+__device__ __forceinline__ float2 c_unpack(f2 v) {
+    float2 o;
+    f2_split(v, o.x, o.y);
+    return o;
 }
 
-// The y pass.  A CTA owns two lines of LZ replica pairs and transforms them in place in shared memory; every byte it
-// moves to or from global memory goes by TMA bulk copy (one contiguous line each), issued by one thread at the top, so
-// no warp ever waits on a global load: while one CTA's lines are in flight the other CTAs of the SM compute.
-//   grid (PBZ, L/2 + L/4), block (LZ, 16).  blockIdx.y < L/2: the x and y lines of column slot_x = blockIdx.y (they mix
+// The y pass.  A CTA owns two lines of LZ replica pairs, one per half of its threads, and transforms them in place in
+// shared memory; every byte it moves to or from global memory goes by TMA bulk copy (one contiguous line each, the
+// twiddle tables too), issued by one thread at the top, so no warp ever waits on a global load except for the few
+// table values of the spectral multiply.
+//   grid (PBZ, L/2 + L/4), block (LZ, 16, 2).  blockIdx.y < L/2: the x and y lines of column slot_x = blockIdx.y (they mix
 //   through W^xy); else the z lines of the two columns 2 (blockIdx.y - L/2) and + 1: every CTA has the same size.
 //   FC_FWD_ONLY  Z holds the x-transformed rows of colour c = p.colour: forward L-point FFT over y -> S^_c -> Cnew.
 //   FC_FUSED     the same, then H^_t = A S^_t + B S^_c with t = 1 - c and S^_t read from Ctgt, inverse FFT over ky -> Z.
@@ -355,16 +390,17 @@ __device__ __forceinline__ float2 cmac(float2 acc, float2 a, float2 m) {  // acc
 // The three modes run the same arithmetic on the same values, so a field does not depend on which of them produced it.
 enum { FC_FWD_ONLY = 0, FC_FUSED = 1, FC_COMBINE = 2 };
 
-template <int N2, int MODE>
-__global__ void __launch_bounds__(128, 3) fftc_y_kernel(const FcParams p) {
+template <int N2, int MODE, int LZC>
+__global__ void __launch_bounds__(256, 3) fftc_y_kernel(const FcParams p) {
     extern __shared__ __align__(128) unsigned char ysm_raw[];
     constexpr int L = 16 * N2, Lh = L / 2;
-    const int LZ = blockDim.x;
+    const int LZ = nlanes<LZC>();
     const uint32_t line_elems = (uint32_t)(L * LZ), line_bytes = line_elems * (uint32_t)sizeof(float2);
+    constexpr uint32_t tw_bytes = (uint32_t)(L * sizeof(float2));
     float2 *B0 = reinterpret_cast<float2 *>(ysm_raw), *B1 = B0 + line_elems, *B2 = B1 + line_elems, *B3 = B2 + line_elems;
-    float2 *tw = B0 + (MODE == FC_FWD_ONLY ? 2 : 4) * (size_t)line_elems;
-    uint64_t *bars = reinterpret_cast<uint64_t *>(tw + L);
-    const int lane = threadIdx.x, t = threadIdx.y, tid = t * LZ + lane;
+    float2 *twf = B0 + (MODE == FC_FWD_ONLY ? 2 : 4) * (size_t)line_elems, *twi = twf + L;
+    uint64_t *bars = reinterpret_cast<uint64_t *>(twi + L);
+    const int lane = threadIdx.x, t = threadIdx.y, j = threadIdx.z, tid = (j * 16 + t) * LZ + lane;
     const int pb = blockIdx.x;
     const bool is_z = (int)blockIdx.y >= Lh;
     const int sx0 = is_z ? 2 * ((int)blockIdx.y - Lh) : (int)blockIdx.y;
@@ -375,27 +411,27 @@ __global__ void __launch_bounds__(128, 3) fftc_y_kernel(const FcParams p) {
         mbar_init(&bars[1], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    fill_twiddles(tw, L);
     __syncthreads();
     pdl_wait();                                            // Z comes from the x pass, the caches from earlier y passes
     if (tid == 0) {
         const float2 *in = MODE == FC_COMBINE ? p.Cnew : p.Z;
-        mbar_expect_tx(&bars[0], 2 * line_bytes);
+        mbar_expect_tx(&bars[0], 2 * line_bytes + (MODE == FC_COMBINE ? 0 : tw_bytes));
+        if (MODE != FC_COMBINE) bulk_g2s(twf, p.twf, tw_bytes, &bars[0]);
         bulk_g2s(B0, in + off0, line_bytes, &bars[0]);
         bulk_g2s(B1, in + off1, line_bytes, &bars[0]);
         if (MODE != FC_FWD_ONLY) {
-            mbar_expect_tx(&bars[1], 2 * line_bytes);
+            mbar_expect_tx(&bars[1], 2 * line_bytes + tw_bytes);
+            bulk_g2s(twi, p.twi, tw_bytes, &bars[1]);
             bulk_g2s(B2, p.Ctgt + off0, line_bytes, &bars[1]);
             bulk_g2s(B3, p.Ctgt + off1, line_bytes, &bars[1]);
         }
     }
     mbar_wait(&bars[0], 0);
     if (MODE != FC_COMBINE) {
-        line_fwd_step1<N2>(B0, tw, LZ, lane, t);
-        line_fwd_step1<N2>(B1, tw, LZ, lane, t);
+        float2 *Bj = j ? B1 : B0;                          // the two lines side by side, one per half of the threads
+        line_fwd_step1<N2, LZC>(Bj, twf, lane, t);
         __syncthreads();
-        line_fwd_step2<N2>(B0, LZ, lane, t);
-        line_fwd_step2<N2>(B1, LZ, lane, t);
+        line_fwd_step2<N2, LZC>(Bj, lane, t);
         fence_async_smem();                                // the spectra go to the cache straight from shared memory
         __syncthreads();
         if (tid == 0) {
@@ -410,34 +446,46 @@ __global__ void __launch_bounds__(128, 3) fftc_y_kernel(const FcParams p) {
         }
     }
     mbar_wait(&bars[1], 0);
-    // H^ = A S^_t + B S^_c, rows N2 t + k2 (the rows this thread wrote in step 2), result over S^_t in B2, B3
+    // H^ = A S^_t + B S^_c on the rows N2 t + k2 (half of the k2 for each half of the threads), result over S^_t in B2, B3
+    constexpr int KH = N2 / 2;
     if (!is_z) {
-        const float4 *tab = p.AB + ((size_t)sx0 * L + N2 * t) * 4;   // constant table, read-only path
+        const float4 *tab = p.AB + ((size_t)sx0 * L + N2 * t + KH * j) * 4;   // constant table, read-only path
 #pragma unroll 4
-        for (int k2 = 0; k2 < N2; ++k2) {
+        for (int k2 = 0; k2 < KH; ++k2) {
             const float4 m0 = __ldg(tab + 4 * k2), m1 = __ldg(tab + 4 * k2 + 1), m2 = __ldg(tab + 4 * k2 + 2);
-            const float2 Axx = make_float2(m0.x, m0.y), Axy = make_float2(m0.z, m0.w), Ayy = make_float2(m1.x, m1.y);
-            const float2 Bxx = make_float2(m1.z, m1.w), Bxy = make_float2(m2.x, m2.y), Byy = make_float2(m2.z, m2.w);
-            const int r = swz(N2 * t + k2) * LZ + lane;
+            const int r = swz(N2 * t + KH * j + k2) * LZ + lane;
             const float2 ox = B0[r], oy = B1[r], tx = B2[r], ty = B3[r];
-            B2[r] = cmac(cmac(cmac(cmul(tx, Axx), ty, Axy), ox, Bxx), oy, Bxy);
-            B3[r] = cmac(cmac(cmac(cmul(tx, Axy), ty, Ayy), ox, Bxy), oy, Byy);
+            const f2 pox = c_pack(ox), poy = c_pack(oy), ptx = c_pack(tx), pty = c_pack(ty);
+            const f2 iox = c_rot(ox), ioy = c_rot(oy), itx = c_rot(tx), ity = c_rot(ty);
+            // (Axx, Axy) = m0, (Ayy, Bxx) = m1, (Bxy, Byy) = m2
+            f2 hx = c_mul(m0.x, m0.y, ptx, itx);
+            hx = c_mac(hx, m0.z, m0.w, pty, ity);
+            hx = c_mac(hx, m1.z, m1.w, pox, iox);
+            hx = c_mac(hx, m2.x, m2.y, poy, ioy);
+            f2 hy = c_mul(m0.z, m0.w, ptx, itx);
+            hy = c_mac(hy, m1.x, m1.y, pty, ity);
+            hy = c_mac(hy, m2.x, m2.y, pox, iox);
+            hy = c_mac(hy, m2.z, m2.w, poy, ioy);
+            B2[r] = c_unpack(hx);
+            B3[r] = c_unpack(hy);
         }
     } else {
-        const float4 *tab0 = p.AB + ((size_t)sx0 * L + N2 * t) * 4 + 3, *tab1 = p.AB + ((size_t)sx1 * L + N2 * t) * 4 + 3;
+        const float4 *tab0 = p.AB + ((size_t)sx0 * L + N2 * t + KH * j) * 4 + 3;
+        const float4 *tab1 = p.AB + ((size_t)sx1 * L + N2 * t + KH * j) * 4 + 3;
 #pragma unroll 4
-        for (int k2 = 0; k2 < N2; ++k2) {
-            const float4 ma = __ldg(tab0 + 4 * k2), mb = __ldg(tab1 + 4 * k2);
-            const int r = swz(N2 * t + k2) * LZ + lane;
-            B2[r] = cmac(cmul(B2[r], make_float2(ma.x, ma.y)), B0[r], make_float2(ma.z, ma.w));
-            B3[r] = cmac(cmul(B3[r], make_float2(mb.x, mb.y)), B1[r], make_float2(mb.z, mb.w));
+        for (int k2 = 0; k2 < KH; ++k2) {
+            const float4 ma = __ldg(tab0 + 4 * k2), mb = __ldg(tab1 + 4 * k2);   // (Azz, Bzz) of the two columns
+            const int r = swz(N2 * t + KH * j + k2) * LZ + lane;
+            const float2 o0 = B0[r], o1 = B1[r], t0 = B2[r], t1 = B3[r];
+            B2[r] = c_unpack(c_mac(c_mul(ma.x, ma.y, c_pack(t0), c_rot(t0)), ma.z, ma.w, c_pack(o0), c_rot(o0)));
+            B3[r] = c_unpack(c_mac(c_mul(mb.x, mb.y, c_pack(t1), c_rot(t1)), mb.z, mb.w, c_pack(o1), c_rot(o1)));
         }
     }
-    line_inv_step2<N2>(B2, tw, LZ, lane, t);
-    line_inv_step2<N2>(B3, tw, LZ, lane, t);
     __syncthreads();
-    line_inv_step1<N2>(B2, LZ, lane, t);
-    line_inv_step1<N2>(B3, LZ, lane, t);
+    float2 *Bj = j ? B3 : B2;
+    line_inv_step2<N2, LZC>(Bj, twi, lane, t);
+    __syncthreads();
+    line_inv_step1<N2, LZC>(Bj, lane, t);
     fence_async_smem();
     __syncthreads();
     pdl_trigger();
@@ -497,6 +545,17 @@ __global__ void wq_pass2_kernel(const double2 *__restrict__ T1, float *__restric
     dst[ib + 1] = (float)((im - im2) * inv);
 }
 
+// twf[j] = (c, -s), twi[j] = (c, s) with (c, s) = (cos, sin)(2 pi j / L), j < L, rounded from fp64
+__global__ void twiddle_table_kernel(float2 *__restrict__ twf, float2 *__restrict__ twi, int L) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= L) return;
+    double s, c;
+    sincospi(2.0 * (double)j / (double)L, &s, &c);
+    const float cf = (float)c, sf = (float)s;
+    twf[j] = make_float2(cf, -sf);
+    twi[j] = make_float2(cf, sf);
+}
+
 int pairs_per_cta(int P, int cap) {
     int ln = 1;
     while (ln * 2 <= cap && P % (ln * 2) == 0) ln *= 2;
@@ -505,8 +564,18 @@ int pairs_per_cta(int P, int cap) {
 
 template <int N2>
 size_t y_smem_bytes(int LZ, int lines) {
-    return sizeof(float2) * ((size_t)lines * 16 * N2 * LZ + 16 * N2) + 64;
+    return sizeof(float2) * ((size_t)lines * 16 * N2 * LZ) + 2 * sizeof(float2) * 16 * N2 + 64;
 }
+
+template <int N2, int LZC>
+cudaError_t launch_y(int mode, const FcParams &q, dim3 gy, dim3 by, size_t smy2, size_t smy4, cudaStream_t st) {
+    if (mode == FC_FWD_ONLY) return launch_pdl(fftc_y_kernel<N2, FC_FWD_ONLY, LZC>, gy, by, smy2, st, q);
+    if (mode == FC_FUSED) return launch_pdl(fftc_y_kernel<N2, FC_FUSED, LZC>, gy, by, smy4, st, q);
+    return launch_pdl(fftc_y_kernel<N2, FC_COMBINE, LZC>, gy, by, smy4, st, q);
+}
+
+template <typename K>
+cudaError_t raise_smem(K kern) { return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024); }
 
 // one field of colour `colour` (0 / 1), or of both (-1); valid[c] = "the cache holds the half-spectrum of colour c of the
 // current spins" (kept by the caller across calls; a Metropolis update of colour c clears valid[c])
@@ -521,25 +590,32 @@ cudaError_t launch_fftc(FcParams p, float2 *C, size_t cache_elems, int colour, b
     p.LZ = pairs_per_cta(p.P, capz);
     p.PBZ = p.P / p.LZ;
     const int LNX = pairs_per_cta(p.P, 16);               // the x passes: 16 pairs per CTA = 128-byte runs of the spin arrays
+    const bool fast = LNX == 16 && p.LZ == 8;             // lane counts known at compile time (config 5)
     const int TL = N2X < 16 ? N2X : 16;
     const size_t smx = sizeof(float2) * (L + (size_t)line_rows<N2X>() * LNX);
     const size_t smy2 = y_smem_bytes<N2>(p.LZ, 2), smy4 = y_smem_bytes<N2>(p.LZ, 4);
     if (!*configured) {
         cudaError_t e;
-        if ((e = cudaFuncSetAttribute(fftc_y_kernel<N2, FC_FWD_ONLY>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)) != cudaSuccess) return e;
-        if ((e = cudaFuncSetAttribute(fftc_y_kernel<N2, FC_FUSED>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)) != cudaSuccess) return e;
-        if ((e = cudaFuncSetAttribute(fftc_y_kernel<N2, FC_COMBINE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)) != cudaSuccess) return e;
-        if ((e = cudaFuncSetAttribute(fftc_x_forward_kernel<N2X>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024)) != cudaSuccess) return e;
-        if ((e = cudaFuncSetAttribute(fftc_x_inverse_kernel<N2X>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024)) != cudaSuccess) return e;
+        if ((e = raise_smem(fftc_y_kernel<N2, FC_FWD_ONLY, 0>)) != cudaSuccess) return e;
+        if ((e = raise_smem(fftc_y_kernel<N2, FC_FUSED, 0>)) != cudaSuccess) return e;
+        if ((e = raise_smem(fftc_y_kernel<N2, FC_COMBINE, 0>)) != cudaSuccess) return e;
+        if ((e = raise_smem(fftc_y_kernel<N2, FC_FWD_ONLY, 8>)) != cudaSuccess) return e;
+        if ((e = raise_smem(fftc_y_kernel<N2, FC_FUSED, 8>)) != cudaSuccess) return e;
+        if ((e = raise_smem(fftc_y_kernel<N2, FC_COMBINE, 8>)) != cudaSuccess) return e;
+        if ((e = raise_smem(fftc_x_forward_kernel<N2X, 0>)) != cudaSuccess) return e;
+        if ((e = raise_smem(fftc_x_inverse_kernel<N2X, 0>)) != cudaSuccess) return e;
+        if ((e = raise_smem(fftc_x_forward_kernel<N2X, 16>)) != cudaSuccess) return e;
+        if ((e = raise_smem(fftc_x_inverse_kernel<N2X, 16>)) != cudaSuccess) return e;
         *configured = true;
     }
-    const dim3 gx(p.P / LNX, L, 3), bx(LNX, TL), gy(p.PBZ, L / 2 + L / 4), by(p.LZ, 16);
+    const dim3 gx(p.P / LNX, L, 3), bx(LNX, TL), gy(p.PBZ, L / 2 + L / 4), by(p.LZ, 16, 2);
     cudaError_t e = cudaSuccess;
     auto x_forward = [&](int c) {
         FcParams q = p;
         q.colour = c;
         ++*launches;
-        return launch_pdl(fftc_x_forward_kernel<N2X>, gx, bx, smx, st, q);
+        return fast ? launch_pdl(fftc_x_forward_kernel<N2X, 16>, gx, bx, smx, st, q)
+                    : launch_pdl(fftc_x_forward_kernel<N2X, 0>, gx, bx, smx, st, q);
     };
     auto y_pass = [&](int mode, int c) {                   // c = the colour transformed forward / "new" colour
         FcParams q = p;
@@ -547,15 +623,14 @@ cudaError_t launch_fftc(FcParams p, float2 *C, size_t cache_elems, int colour, b
         q.Cnew = C + (size_t)c * cache_elems;
         q.Ctgt = C + (size_t)(1 - c) * cache_elems;
         ++*launches;
-        if (mode == FC_FWD_ONLY) return launch_pdl(fftc_y_kernel<N2, FC_FWD_ONLY>, gy, by, smy2, st, q);
-        if (mode == FC_FUSED) return launch_pdl(fftc_y_kernel<N2, FC_FUSED>, gy, by, smy4, st, q);
-        return launch_pdl(fftc_y_kernel<N2, FC_COMBINE>, gy, by, smy4, st, q);
+        return fast ? launch_y<N2, 8>(mode, q, gy, by, smy2, smy4, st) : launch_y<N2, 0>(mode, q, gy, by, smy2, smy4, st);
     };
     auto x_inverse = [&](int c) {
         FcParams q = p;
         q.colour = c;
         ++*launches;
-        return launch_pdl(fftc_x_inverse_kernel<N2X>, gx, bx, smx, st, q);
+        return fast ? launch_pdl(fftc_x_inverse_kernel<N2X, 16>, gx, bx, smx, st, q)
+                    : launch_pdl(fftc_x_inverse_kernel<N2X, 0>, gx, bx, smx, st, q);
     };
     for (int tc = 0; tc < 2 && e == cudaSuccess; ++tc) {
         if (colour >= 0 && colour != tc) continue;
@@ -582,7 +657,7 @@ cudaError_t launch_fftc(FcParams p, float2 *C, size_t cache_elems, int colour, b
 bool dsmc_fft_supported(int L, int R) {
     return (R % 2 == 0) && (L == 32 || L == 64 || L == 128 || L == 256 || L == 512);
 }
-size_t dsmc_fft_m_floats(int L) { return 8 * (size_t)L * L; }                 // AB: (L/2) L slots of 16 floats
+size_t dsmc_fft_m_floats(int L) { return 8 * (size_t)L * L + 4 * (size_t)L; }   // AB: (L/2) L slots of 16 floats; twf, twi
 size_t dsmc_fft_cache_elems(int L, int R) { return 3 * (size_t)(L / 2) * L * (size_t)(R / 2); }   // float2 per colour
 size_t dsmc_fft_scratch_bytes(int L, int R) {
     const size_t N = (size_t)L * L;
@@ -595,7 +670,9 @@ cudaError_t launch_make_fft_table(const float *Wc, float *AB, void *scratch, int
     const size_t total = 4 * (size_t)L * L;
     wq_pass1_kernel<<<(unsigned)((total + 127) / 128), 128, 0, st>>>(Wc, (double2 *)scratch, L);
     wq_pass2_kernel<<<(unsigned)((total / 2 + 127) / 128), 128, 0, st>>>((const double2 *)scratch, AB, L);
-    *launches += 2;
+    float2 *tw = reinterpret_cast<float2 *>(AB + 8 * (size_t)L * L);
+    twiddle_table_kernel<<<(L + 127) / 128, 128, 0, st>>>(tw, tw + L, L);
+    *launches += 3;
     return cudaGetLastError();
 }
 
@@ -608,6 +685,8 @@ cudaError_t launch_field_fft(const float *S, const float *AB, void *scratch, voi
     p.Cnew = nullptr;
     p.Ctgt = nullptr;
     p.AB = (const float4 *)AB;
+    p.twf = reinterpret_cast<const float2 *>(AB + 8 * (size_t)L * L);
+    p.twi = p.twf + L;
     p.L = L;
     p.P = R / 2;
     p.LZ = 1;
