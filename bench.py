@@ -142,13 +142,20 @@ def paper_schedule(m, inputs, dev):
     per replica pair, one kernel for the whole run) and, for comparison, through the two-launches-per-pass path."""
     import torch
     L, out = 64, {}
-    for name, R, l, flags in (("resident", 16, 32, 0), ("resident_R296", 296, 32, 0), ("resident_l16_R296", 296, 16, 0),
-                              ("two_launch_graph", 16, 32, m.DSMC_NO_RESIDENT)):
+    # T = 0.2 ... 1.6 is the ladder of the BASELINE configs; "cold" = script-T 0.2 ... 2 of the paper's production run
+    # (T = script-T g / 2, DESIGN.md R7), where few moves are accepted and the incremental field update pays
+    for name, R, l, flags, Trange in (("resident", 16, 32, 0, (0.2, 1.6)), ("resident_R296", 296, 32, 0, (0.2, 1.6)),
+                                      ("resident_l16_R296", 296, 16, 0, (0.2, 1.6)),
+                                      ("resident_cold", 16, 32, 0, (0.022, 0.22)),
+                                      ("incremental", 16, 32, m.DSMC_INCREMENTAL, (0.2, 1.6)),
+                                      ("incremental_cold", 16, 32, m.DSMC_INCREMENTAL, (0.022, 0.22)),
+                                      ("incremental_cold_R296", 296, 32, m.DSMC_INCREMENTAL, (0.022, 0.22)),
+                                      ("two_launch_graph", 16, 32, m.DSMC_NO_RESIDENT, (0.2, 1.6))):
         npass = l * l
         ctx = m.Dsmc(L, R, J=1.0, g=0.2247, K2=1.685, K4=0.0, device=dev)
         ctx.build_tensor(m.DSMC_W_EWALD)
         ctx.set_spins(inputs.random_spins(L, R, 1))
-        T = np.linspace(0.2, 1.6, R).astype(np.float32)
+        T = np.linspace(Trange[0], Trange[1], R).astype(np.float32)
         ctx.sublattice_run(T, 1, 0, npass, l, flags=flags)
         torch.cuda.synchronize(dev)
         reps = 4
@@ -158,7 +165,8 @@ def paper_schedule(m, inputs, dev):
         e1.record()
         torch.cuda.synchronize(dev)
         ms = e0.elapsed_time(e1) / reps
-        out[name] = {"R": R, "l": l, "us_per_pass": ms * 1e3 / npass, "ms_per_mc_step": ms, "updates_per_s": L * L * R / (ms * 1e-3)}
+        out[name] = {"R": R, "l": l, "T": list(Trange), "us_per_pass": ms * 1e3 / npass, "ms_per_mc_step": ms,
+                     "updates_per_s": L * L * R / (ms * 1e-3)}
         ctx.close()
     # resident kernel: one CTA = one SM sums 4 targets x 4096 sources x 5 FMA x 2 replicas per pass
     fma_clk = 4 * L * L * 5 * 2 / 128.0

@@ -59,8 +59,9 @@ enum {
                              the same colour (for timing the Metropolis kernel alone)         */
     DSMC_TRIAL_FLIP = 2,  /* the trial is the reversed spin s' = -s instead of a point uniform on
                              S^2: the Ising move of App. B; u is drawn as usual   */
-    DSMC_NO_RESIDENT = 4  /* dsmc_sublattice_pass / _run only: do not use the kernel that keeps the
+    DSMC_NO_RESIDENT = 4, /* dsmc_sublattice_pass / _run only: do not use the kernel that keeps the
                              lattice in shared memory (two launches per pass instead)            */
+    DSMC_INCREMENTAL = 8  /* dsmc_sublattice_run only: incremental field update (see there)         */
 };
 
 /* dsmc_init_spins modes */
@@ -129,6 +130,10 @@ int dsmc_init_spins(dsmc_ctx *ctx, int mode, uint64_t seed);
  * kept in the context for the next half-sweep of that colour.  h_out (nullable) receives the
  * canonical h[R][3][L][L]; entries of inactive targets are left untouched.                     */
 int dsmc_dipole_field(dsmc_ctx *ctx, int colour, float *h_out, int where);
+/* The field array as the context keeps it, canonical h[R][3][L][L], WITHOUT recomputing it: what the last
+ * dsmc_dipole_field(colour = -1) left, or the incrementally updated field after a DSMC_INCREMENTAL run.
+ * DSMC_ESTATE unless a field of both colours is kept.  To HOST synchronises.                       */
+int dsmc_get_field(dsmc_ctx *ctx, float *h_out, int where);
 
 /* a2. One checkerboard Metropolis half-sweep (PAPER.md:60-72 eq. 7; :98; :102-118; R11-R14):
  *   colour c = step & 1.  (i) h <- dipole field of colour c from the state at entry (frozen for
@@ -166,6 +171,23 @@ int dsmc_sublattice_pass(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t 
  * the offset from a pass counter on the device.                                                    */
 int dsmc_sublattice_run(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_pass, uint64_t n_passes, int l,
                         int flags);
+/* DSMC_INCREMENTAL (section 3.2, eq. 8 read the other way round): after a pass
+ * only the accepted update sites have changed, so the field of EVERY site changes by exactly
+ *   h_t += sum over accepted c of W(c - t) . (s'_c - s_c).
+ * The run keeps the field of all N sites of a replica pair in the registers of one CTA and applies these rank-n
+ * updates instead of summing over all N sources for the n update sites of every pass: work only for accepted moves
+ * (the paper's low-temperature regime), no reduction, a pass without acceptance costs two barriers.  Same schedule,
+ * same random numbers and the same decisions as the plain run up to the rounding of the field: the field is
+ * recomputed from scratch by a field kernel at entry and every 4096 passes, between which it drifts by at most a few
+ * 1e-6 relative (tested); it is therefore NOT bit-identical to pass-by-pass calls -- the parity contract is the
+ * lock-step one (decisions identical outside |dE/T + ln u| < 1e-4).  On return the field array holds the field of
+ * the final state (dsmc_dipole_field semantics).  Needs L / l in {1, 2, 4} and L * L <= 4096 (DSMC_EINVAL otherwise);
+ * flags: DSMC_INCREMENTAL | optionally DSMC_TRIAL_FLIP.
+ * dsmc_sublattice_run_ex: margin_log (nullable, DEVICE, [n_passes][R][(L/l)^2] floats, only with DSMC_INCREMENTAL)
+ * receives dE/T + ln u of every trial, update sites in the order b (rows) outer, a inner: the parity hook of a run
+ * that cannot be stopped between passes.                                                              */
+int dsmc_sublattice_run_ex(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_pass, uint64_t n_passes, int l,
+                           int flags, float *margin_log);
 
 /* n_half consecutive half-sweeps (steps first_step .. first_step + n_half - 1) without returning
  * to the caller in between.  Long runs are replayed from a CUDA graph of 8 sweeps (each: field +

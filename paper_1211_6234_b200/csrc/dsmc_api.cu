@@ -109,10 +109,10 @@ int field_kind(const dsmc_ctx *ctx) {
     return dsmc_tiled_supported(ctx->L, ctx->R) ? 1 : 0;
 }
 
-// colour = -1: both colours
-int run_field(dsmc_ctx *ctx, int colour) {
+// colour = -1: both colours; kind_override >= 0 runs that field kernel whatever the selection
+int run_field(dsmc_ctx *ctx, int colour, int kind_override = -1) {
     cudaError_t e = cudaSuccess;
-    const int kind = field_kind(ctx);
+    const int kind = kind_override >= 0 ? kind_override : field_kind(ctx);
     if (kind == 2) {
         e = launch_field_fft(ctx->S(), ctx->M(), ctx->Z(), ctx->C(), ctx->H(), ctx->L, ctx->R, colour, ctx->spec_valid,
                              &ctx->fft_configured, ctx->stream, &ctx->launches);
@@ -571,6 +571,21 @@ int dsmc_dipole_field(dsmc_ctx *ctx, int colour, float *h_out, int where) {
     return DSMC_OK;
 }
 
+int dsmc_get_field(dsmc_ctx *ctx, float *h_out, int where) {
+    ENTER_BOUND(ctx);
+    if (!h_out) return fail(ctx, DSMC_EINVAL, "null argument");
+    if (!ctx->field_valid[0] || !ctx->field_valid[1]) return fail(ctx, DSMC_ESTATE, "no field of both colours is kept");
+    float *dst = where == DSMC_HOST ? ctx->stage() : h_out;
+    CU(launch_internal_to_canon(ctx->H(), dst, ctx->L, ctx->R, -1, ctx->stream, &ctx->launches), "get field");
+    if (where == DSMC_HOST) {
+        CU(cudaMemcpyAsync(h_out, dst, sizeof(float) * 3 * (size_t)ctx->L * ctx->L * ctx->R, cudaMemcpyDeviceToHost,
+                           ctx->stream),
+           "h D2H");
+        CU(cudaStreamSynchronize(ctx->stream), "h D2H sync");
+    }
+    return DSMC_OK;
+}
+
 int dsmc_halfsweep_ex(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t step, int flags, uint8_t *accept_out,
                       float *margin_out) {
     ENTER_BOUND(ctx);
@@ -615,7 +630,37 @@ int dsmc_sublattice_pass(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t 
 
 int dsmc_sublattice_run(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_pass, uint64_t n_passes, int l,
                         int flags) {
+    return dsmc_sublattice_run_ex(ctx, T, seed, first_pass, n_passes, l, flags, nullptr);
+}
+
+int dsmc_sublattice_run_ex(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_pass, uint64_t n_passes, int l,
+                           int flags, float *margin_log) {
     ENTER_BOUND(ctx);
+    if (flags & DSMC_INCREMENTAL) {
+        if (flags & ~(DSMC_TRIAL_FLIP | DSMC_INCREMENTAL)) return fail(ctx, DSMC_EINVAL, "unknown flag");
+        if (!ctx->tensor_built) return fail(ctx, DSMC_ESTATE, "tensor not built");
+        if (!ctx->spins_set) return fail(ctx, DSMC_ESTATE, "spins not set");
+        if (l < 2 || ctx->L % l || !dsmc_incremental_supported(ctx->L, l))
+            return fail(ctx, DSMC_EINVAL, "DSMC_INCREMENTAL needs L / l in {1, 2, 4} and L * L <= 4096");
+        if (int rc = upload_params(ctx, T)) return rc;
+        // the field of every site from a field kernel (the FFT one when the shape allows: microseconds), then up to
+        // DSMC_INCREMENTAL_REFRESH passes of rank-n updates in registers; the refresh bounds the rounding drift
+        const int kind = dsmc_fft_supported(ctx->L, ctx->R) ? 2 : (dsmc_tiled_supported(ctx->L, ctx->R) ? 1 : 0);
+        for (uint64_t done = 0; done < n_passes;) {
+            const uint64_t chunk = n_passes - done < DSMC_INCREMENTAL_REFRESH ? n_passes - done : DSMC_INCREMENTAL_REFRESH;
+            if (int rc = run_field(ctx, -1, kind)) return rc;
+            const MetropolisArgs a = metropolis_args(ctx, 0, seed, first_pass + done, flags, nullptr, nullptr);
+            CU(launch_sublattice_incremental(a, ctx->Wc(), ctx->H(), l, first_pass + done, chunk,
+                                             margin_log ? margin_log + done * (uint64_t)ctx->R * (uint64_t)((ctx->L / l) * (ctx->L / l)) : nullptr,
+                                             ctx->stream, &ctx->launches),
+               "incremental run launch");
+            ctx->spec_valid[0] = ctx->spec_valid[1] = false;
+            done += chunk;
+        }
+        ctx->field_valid[0] = ctx->field_valid[1] = true;      // H holds the (incrementally updated) field of the final state
+        return DSMC_OK;
+    }
+    if (margin_log) return fail(ctx, DSMC_EINVAL, "margin_log needs DSMC_INCREMENTAL");
     if (n_passes >= 2 && l >= 2 && ctx->L % l == 0 && !(flags & ~(DSMC_TRIAL_FLIP | DSMC_NO_RESIDENT)) &&
         ctx->tensor_built && ctx->spins_set && use_resident(ctx, l, flags)) {
         // every pass of the run inside one kernel (per 65536 passes), the lattice in shared memory

@@ -205,6 +205,12 @@ cudaError_t launch_sublattice_pass(const MetropolisArgs &a, const float *Wc, flo
 bool dsmc_resident_supported(int L, int l);
 cudaError_t launch_sublattice_resident(const MetropolisArgs &a, const float *Wc, int l, uint64_t first_pass, uint64_t n_passes,
                                        cudaStream_t st, uint64_t *launches);
+// the same schedule with the field of all sites kept in registers and updated by the accepted moves (NEXT-4): H holds the
+// field of the current spins at entry and at exit; margin_log: nullable device [n_passes][R][(L/l)^2]
+#define DSMC_INCREMENTAL_REFRESH 4096  // passes between two recomputations of the field from scratch (rounding drift)
+bool dsmc_incremental_supported(int L, int l);
+cudaError_t launch_sublattice_incremental(const MetropolisArgs &a, const float *Wc, float *H, int l, uint64_t first_pass,
+                                          uint64_t n_passes, float *margin_log, cudaStream_t st, uint64_t *launches);
 // *step = value (add = 0) or *step += value (add = 1): one thread, stream-ordered
 cudaError_t launch_step_update(unsigned long long *step, unsigned long long value, int add, cudaStream_t st,
                                uint64_t *launches);

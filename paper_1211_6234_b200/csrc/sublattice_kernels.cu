@@ -431,6 +431,217 @@ __global__ void __launch_bounds__(kResThreads, 1) sublattice_resident_kernel(con
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// The same schedule with an INCREMENTAL field (section 3.2, eq. 8 read the
+// other way round): after a pass only the accepted update sites have changed, so the dipole field of EVERY site
+// changes by exactly  h_t += W(c - t) . delta_c  summed over the accepted sites c (delta = s' - s).  One CTA owns a
+// replica pair as in sublattice_resident_kernel, but the 256 field threads keep the field of all N sites in registers
+// (site t = tid + 256 j, j < 16: 48 packed values per thread) instead of summing over all N sources for the n update
+// sites of every pass:
+//   pass:  owners publish h of the n update sites  | the drawing warp draws (Philox) as before
+//          -- barrier --  the drawing warp decides and publishes delta_c (zero when rejected)
+//          -- barrier --  every field thread adds W(c - t) delta_c to its 16 sites, for the c that were accepted
+// Work per pass is 5 n N FMAs per replica pair only for accepted moves (the full sum costs 5 n N always), there is
+// no reduction across threads, and a pass in which nothing was accepted costs two barriers.  The field is taken from
+// the field array H at entry (the caller computes it with a field kernel) and written back at exit; rounding
+// accumulates with every update, so the caller refreshes H every few thousand passes (dsmc_api.cu).
+// Needs N <= 4096 (16 sites per thread) and L / l in {1, 2, 4}.
+constexpr int kIncThreads = 256;
+constexpr int kIncSpt = 16;       // sites per field thread
+
+__host__ __device__ constexpr size_t incremental_smem_bytes(int L, int NL) {
+    return (size_t)40 * L * L + 16 + 2 * sizeof(f2) * NL * NL * 3 + 64;
+}
+
+template <int NL, int LC>
+__global__ void __launch_bounds__(kIncThreads + 32, 1) sublattice_incremental_kernel(const MetropolisArgs p, const RoundKeys rk,
+                                                                                  const float *__restrict__ Wc,
+                                                                                  float *__restrict__ Hio, int l_arg,
+                                                                                  unsigned long long first_pass,
+                                                                                  unsigned n_passes,
+                                                                                  float *__restrict__ margin_log) {
+    constexpr int NN = NL * NL;
+    extern __shared__ __align__(16) unsigned char rsm[];
+    const int L = LC > 0 ? LC : p.L, l = LC > 0 ? LC / NL : l_arg, Lh = L >> 1, R = p.R, N = L * L;
+    float4 *Wsm = reinterpret_cast<float4 *>(rsm);                     // [N + 1]  (xx, xy, yy, zz) at rho = ry L + rx
+    f2 *Ssm = reinterpret_cast<f2 *>(rsm + (size_t)16 * (N + 1));      // [N][3]  replicas (r0, r1) of site n = y L + x
+    float *Sf = reinterpret_cast<float *>(Ssm);
+    f2 *hpub = Ssm + 3 * (size_t)N;                                    // [NN][3] field of the update sites
+    float *dlf = reinterpret_cast<float *>(hpub + NN * 3);             // [NN][3][2] delta of the update sites (0 = rejected)
+    int *off = reinterpret_cast<int *>(dlf + NN * 6);                  // [2][2]: offsets of this and the next pass
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int r0 = 2 * blockIdx.x, r1 = min(r0 + 1, R - 1);            // odd R: the last CTA carries its replica twice
+    const size_t plane = (size_t)L * Lh * R;
+
+    for (int n = tid; n < N; n += kIncThreads + 32) {
+        Wsm[n] = make_float4(__ldg(Wc + n), __ldg(Wc + (size_t)N + n), __ldg(Wc + 2 * (size_t)N + n),
+                             __ldg(Wc + 3 * (size_t)N + n));
+        const int x = n % L, y = n / L;
+        int q;
+        const float *src = p.S + site_index(x, y, Lh, R, plane, q);
+        Ssm[3 * n] = f2_make(src[r0], src[r1]);
+        Ssm[3 * n + 1] = f2_make(src[plane + r0], src[plane + r1]);
+        Ssm[3 * n + 2] = f2_make(src[2 * plane + r0], src[2 * plane + r1]);
+    }
+    // the field of this thread's sites, from the field array
+    f2 h[kIncSpt][3];
+    int txy[kIncSpt];                                                  // x | y << 16 of the sites (-1: none)
+#pragma unroll
+    for (int j = 0; j < kIncSpt; ++j) {
+        const int n = tid + kIncThreads * j;
+        txy[j] = -1;
+        h[j][0] = h[j][1] = h[j][2] = f2_bc(0.0f);
+        if (tid < kIncThreads && n < N) {
+            const int x = n % L, y = n / L;
+            txy[j] = x | (y << 16);
+            int q;
+            const float *src = Hio + site_index(x, y, Lh, R, plane, q);
+            h[j][0] = f2_make(src[r0], src[r1]);
+            h[j][1] = f2_make(src[plane + r0], src[plane + r1]);
+            h[j][2] = f2_make(src[2 * plane + r0], src[2 * plane + r1]);
+        }
+    }
+    if (tid == 0) pass_offset(rk, first_pass, l, off[0], off[1]);
+    __syncthreads();
+
+    const bool drawer = warp == kIncThreads / 32;
+    const bool flipper = drawer && lane < 2 * NN;
+    const int fk = lane >> 1, rb = lane & 1, fr = rb ? r1 : r0;
+    float invT = 0.0f, K2 = 0.0f, K4 = 0.0f;
+    if (flipper) invT = p.invT[fr], K2 = p.K2[fr], K4 = p.K4[fr];
+    MetropolisArgs q = p;
+    q.step_dev = nullptr;
+
+    for (unsigned it = 0; it < n_passes; ++it) {
+        const unsigned long long pass = first_pass + it;
+        const int cur = (int)(it & 1u);
+        const int ox = off[2 * cur], oy = off[2 * cur + 1];
+        Draw dr;
+        float sx = 0.0f, sy = 0.0f, sz = 0.0f, nx = 0.0f, ny = 0.0f, nz = 0.0f;
+        int nt = 0;
+        if (!drawer) {
+            // the owners publish the field of the update sites (a register array cannot be indexed: compare and select)
+#pragma unroll
+            for (int k = 0; k < NN; ++k) {
+                const int nk = (oy + l * (k / NL)) * L + ox + l * (k % NL);
+                if ((nk % kIncThreads) == tid) {
+                    const int jj = nk / kIncThreads;
+                    f2 v0 = h[0][0], v1 = h[0][1], v2 = h[0][2];
+#pragma unroll
+                    for (int j = 1; j < kIncSpt; ++j)
+                        if (j == jj) v0 = h[j][0], v1 = h[j][1], v2 = h[j][2];
+                    hpub[3 * k] = v0, hpub[3 * k + 1] = v1, hpub[3 * k + 2] = v2;
+                }
+            }
+        } else {
+            const int xt = ox + l * (fk % NL), yt = oy + l * (fk / NL);
+            nt = yt * L + xt;
+            uint4 ctr = make_uint4((uint32_t)nt, (uint32_t)fr + p.r_off, (uint32_t)(pass & 0xFFFFFFFFull),
+                                   (uint32_t)(pass >> 32) & 0x7FFFFFFFu);
+            if (2 * NN < 32 && lane == 31)
+                ctr = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, (uint32_t)((pass + 1) & 0xFFFFFFFFull),
+                                 (uint32_t)((pass + 1) >> 32) & 0x7FFFFFFFu);
+            const uint4 rnd = philox4x32_10(ctr, rk);
+            if (2 * NN < 32 && lane == 31) {
+                off[2 * (cur ^ 1)] = (int)(rnd.x % (uint32_t)l);
+                off[2 * (cur ^ 1) + 1] = (int)(rnd.y % (uint32_t)l);
+            }
+            if constexpr (2 * NN >= 32) {
+                if (lane == 0) pass_offset(rk, pass + 1, l, off[2 * (cur ^ 1)], off[2 * (cur ^ 1) + 1]);
+            }
+            if (flipper) {
+                const int xe = xt + 1 == L ? 0 : xt + 1, xw = xt == 0 ? L - 1 : xt - 1;
+                const int yn = yt + 1 == L ? 0 : yt + 1, ys = yt == 0 ? L - 1 : yt - 1;
+                const float *sc = Sf + 6 * nt + rb, *se = Sf + 6 * (yt * L + xe) + rb, *sw = Sf + 6 * (yt * L + xw) + rb,
+                            *sn = Sf + 6 * (yn * L + xt) + rb, *ss = Sf + 6 * (ys * L + xt) + rb;
+                sx = sc[0], sy = sc[2], sz = sc[4];
+                nx = (se[0] + sw[0]) + (sn[0] + ss[0]);
+                ny = (se[2] + sw[2]) + (sn[2] + ss[2]);
+                nz = (se[4] + sw[4]) + (sn[4] + ss[4]);
+                dr = draw_from_words(q, rnd, sx, sy, sz);
+            }
+        }
+        __syncthreads();
+        if (flipper) {
+            const float *pf = reinterpret_cast<const float *>(hpub) + rb;
+            const Trial tr = decide_drawn(q, dr, sx, sy, sz, nx, ny, nz, pf[6 * fk], pf[6 * fk + 2], pf[6 * fk + 4], invT, K2, K4);
+            const bool live = r0 + rb < R;                             // the duplicate of an odd R's last replica stays silent
+            float dx = 0.0f, dy = 0.0f, dz = 0.0f;
+            if (tr.acc) {
+                dx = tr.tx - sx, dy = tr.ty - sy, dz = tr.tz - sz;
+                Sf[6 * nt + rb] = tr.tx;
+                Sf[6 * nt + 2 + rb] = tr.ty;
+                Sf[6 * nt + 4 + rb] = tr.tz;
+            }
+            dlf[6 * fk + rb] = dx, dlf[6 * fk + 2 + rb] = dy, dlf[6 * fk + 4 + rb] = dz;
+            if (live) {
+                if (p.accept_out) p.accept_out[(size_t)fr * N + nt] = tr.acc ? 1 : 0;
+                if (p.margin_out) p.margin_out[(size_t)fr * N + nt] = tr.margin;
+                if (margin_log) margin_log[((size_t)it * R + fr) * NN + fk] = tr.margin;
+            }
+        }
+        __syncthreads();
+        if (!drawer) {
+            // rank-n update of the field of this thread's sites: h_t += W(c - t) . delta_c for the accepted c
+            const f2 *dl = reinterpret_cast<const f2 *>(dlf);
+#pragma unroll 1
+            for (int k = 0; k < NN; ++k) {
+                const f2 dxp = dl[3 * k], dyp = dl[3 * k + 1], dzp = dl[3 * k + 2];
+                if ((dxp | dyp | dzp) == 0ull) continue;       // all six components +0: rejected in both replicas (uniform over the CTA)
+                const int xc = ox + l * (k % NL), yc = oy + l * (k / NL);
+                if constexpr (LC == 64) {
+                    // site j of this thread is (tid & 63, (tid >> 6) + 4 j): rho_x is the same for all of them and the
+                    // table index steps back by 4 rows = 256 entries from one to the next
+                    const int idx0 = (((yc - (tid >> 6)) & 63) << 6) | ((xc - tid) & 63);
+#pragma unroll
+                    for (int j = 0; j < kIncSpt; ++j) {
+                        const float4 w = Wsm[(idx0 - 256 * j) & 4095];
+                        h[j][0] = f2_fma(f2_bc(w.x), dxp, f2_fma(f2_bc(w.y), dyp, h[j][0]));
+                        h[j][1] = f2_fma(f2_bc(w.y), dxp, f2_fma(f2_bc(w.z), dyp, h[j][1]));
+                        h[j][2] = f2_fma(f2_bc(w.w), dzp, h[j][2]);
+                    }
+                } else {
+#pragma unroll
+                    for (int j = 0; j < kIncSpt; ++j) {
+                        if (txy[j] < 0) continue;
+                        int rx = xc - (txy[j] & 0xFFFF), ry = yc - (txy[j] >> 16);
+                        rx += rx < 0 ? L : 0;
+                        ry += ry < 0 ? L : 0;
+                        const float4 w = Wsm[ry * L + rx];
+                        h[j][0] = f2_fma(f2_bc(w.x), dxp, f2_fma(f2_bc(w.y), dyp, h[j][0]));
+                        h[j][1] = f2_fma(f2_bc(w.y), dxp, f2_fma(f2_bc(w.z), dyp, h[j][1]));
+                        h[j][2] = f2_fma(f2_bc(w.w), dzp, h[j][2]);
+                    }
+                }
+            }
+        }
+    }
+    __syncthreads();
+    for (int n = tid; n < N; n += kIncThreads + 32) {
+        const int x = n % L, y = n / L;
+        int qc;
+        float *dst = p.S + site_index(x, y, Lh, R, plane, qc);
+        float a0, a1, b0, b1, c0, c1;
+        f2_split(Ssm[3 * n], a0, a1);
+        f2_split(Ssm[3 * n + 1], b0, b1);
+        f2_split(Ssm[3 * n + 2], c0, c1);
+        dst[r0] = a0, dst[plane + r0] = b0, dst[2 * plane + r0] = c0;
+        if (r0 + 1 < R) dst[r1] = a1, dst[plane + r1] = b1, dst[2 * plane + r1] = c1;
+    }
+#pragma unroll
+    for (int j = 0; j < kIncSpt; ++j) {
+        if (txy[j] < 0) continue;
+        int qc;
+        float *dst = Hio + site_index(txy[j] & 0xFFFF, txy[j] >> 16, Lh, R, plane, qc);
+        float a0, a1, b0, b1, c0, c1;
+        f2_split(h[j][0], a0, a1);
+        f2_split(h[j][1], b0, b1);
+        f2_split(h[j][2], c0, c1);
+        dst[r0] = a0, dst[plane + r0] = b0, dst[2 * plane + r0] = c0;
+        if (r0 + 1 < R) dst[r1] = a1, dst[plane + r1] = b1, dst[2 * plane + r1] = c1;
+    }
+}
+
 }  // namespace
 
 void dsmc_sublattice_offset(uint64_t seed, uint64_t pass, int l, int *ox, int *oy) {
@@ -489,5 +700,25 @@ cudaError_t launch_sublattice_resident(const MetropolisArgs &a, const float *Wc,
         ++*launches;
         done += chunk;
     }
+    return cudaGetLastError();
+}
+
+bool dsmc_incremental_supported(int L, int l) {
+    const int nl = L / l;
+    return (nl == 1 || nl == 2 || nl == 4) && L * L <= kIncThreads * kIncSpt && incremental_smem_bytes(L, nl) <= 227 * 1024;
+}
+
+cudaError_t launch_sublattice_incremental(const MetropolisArgs &a, const float *Wc, float *H, int l, uint64_t first_pass,
+                                          uint64_t n_passes, float *margin_log, cudaStream_t st, uint64_t *launches) {
+    const RoundKeys rk = make_round_keys(a.seed_lo, a.seed_hi);
+    const int nl = a.L / l;
+    const size_t smem = incremental_smem_bytes(a.L, nl);
+    void (*kern)(const MetropolisArgs, const RoundKeys, const float *, float *, int, unsigned long long, unsigned, float *) = nullptr;
+    if (nl == 2) kern = a.L == 64 ? sublattice_incremental_kernel<2, 64> : sublattice_incremental_kernel<2, 0>;
+    else if (nl == 4) kern = a.L == 64 ? sublattice_incremental_kernel<4, 64> : sublattice_incremental_kernel<4, 0>;
+    else kern = a.L == 64 ? sublattice_incremental_kernel<1, 64> : sublattice_incremental_kernel<1, 0>;
+    if (cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024)) return e;
+    kern<<<(unsigned)((a.R + 1) / 2), kIncThreads + 32, smem, st>>>(a, rk, Wc, H, l, first_pass, (unsigned)n_passes, margin_log);
+    ++*launches;
     return cudaGetLastError();
 }

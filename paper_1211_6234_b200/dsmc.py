@@ -13,6 +13,7 @@ DSMC_W_IMAGE, DSMC_W_EWALD = 0, 1
 DSMC_REUSE_FIELD = 1
 DSMC_TRIAL_FLIP = 2
 DSMC_NO_RESIDENT = 4
+DSMC_INCREMENTAL = 8
 DSMC_INIT_RANDOM, DSMC_INIT_UP = 0, 1
 DSMC_FIELD_AUTO, DSMC_FIELD_GENERIC, DSMC_FIELD_TILED, DSMC_FIELD_FFT = -1, 0, 1, 2
 
@@ -35,6 +36,7 @@ ABI = [
     ("dsmc_get_spins", _i, [_vp, _vp, _i]),
     ("dsmc_init_spins", _i, [_vp, _i, _u64]),
     ("dsmc_dipole_field", _i, [_vp, _i, _vp, _i]),
+    ("dsmc_get_field", _i, [_vp, _vp, _i]),
     ("dsmc_halfsweep", _i, [_vp, _vp, _u64, _u64]),
     ("dsmc_halfsweep_ex", _i, [_vp, _vp, _u64, _u64, _i, _vp, _vp]),
     ("dsmc_run", _i, [_vp, _vp, _u64, _u64, _u64]),
@@ -42,6 +44,7 @@ ABI = [
     ("dsmc_run_recorded", _i, [_vp, _vp, _u64, _u64, _u64, _i, _i]),
     ("dsmc_sublattice_pass", _i, [_vp, _vp, _u64, _u64, _i, _i, _vp, _vp, _vp]),
     ("dsmc_sublattice_run", _i, [_vp, _vp, _u64, _u64, _u64, _i, _i]),
+    ("dsmc_sublattice_run_ex", _i, [_vp, _vp, _u64, _u64, _u64, _i, _i, _vp]),
     ("dsmc_observables", _i, [_vp, _vp]),
     ("dsmc_wall_observables", _i, [_vp, _vp, _vp]),
     ("dsmc_staggered_magnetisation", _i, [_vp, _vp]),
@@ -196,6 +199,14 @@ class Dsmc:
         self._check(self.lib.dsmc_dipole_field(self._h, colour, p, where))
         return out
 
+    def get_field(self, out=None):
+        """The field array as kept in the context (no recomputation), canonical [R][3][L][L]."""
+        if out is None:
+            out = np.zeros((self.R, 3, self.L, self.L), dtype=np.float32)
+        p, where = self._ptr(out)
+        self._check(self.lib.dsmc_get_field(self._h, p, where))
+        return out
+
     def _T(self, T):
         if T is None:
             return None, None
@@ -233,9 +244,13 @@ class Dsmc:
         self._check(self.lib.dsmc_sublattice_pass(self._h, tp, seed, pass_index, l, flags, ap, mp, off))
         return int(off[0]), int(off[1])
 
-    def sublattice_run(self, T, seed, first_pass, n_passes, l, flags=0):
+    def sublattice_run(self, T, seed, first_pass, n_passes, l, flags=0, margin_log=None):
         t, tp = self._T(T)
-        self._check(self.lib.dsmc_sublattice_run(self._h, tp, seed, first_pass, n_passes, l, flags))
+        if margin_log is None:
+            self._check(self.lib.dsmc_sublattice_run(self._h, tp, seed, first_pass, n_passes, l, flags))
+        else:
+            self._check(self.lib.dsmc_sublattice_run_ex(self._h, tp, seed, first_pass, n_passes, l, flags,
+                                                        self._ptr(margin_log)[0]))
 
     def observables(self):
         out = np.empty((self.R, 4), dtype=np.float64)

@@ -419,3 +419,77 @@ def test_checkerboard_is_unbiased_on_baseline_configs(dsmc_mod, cfg_id):
         print(name, "checkerboard", np.round(mc[:, q], 4))
         print(name, "single-spin ", np.round(ms[:, q], 4))
         assert np.all(d < tol), (name, d, tol)
+
+
+@pytest.mark.parametrize("L,R,l,passes", [(64, 16, 32, 160), (32, 8, 16, 128), (16, 6, 4, 64), (12, 5, 12, 96), (64, 3, 64, 64)])
+def test_incremental_run_lockstep(dsmc_mod, oracle, L, R, l, passes):
+    """DSMC_INCREMENTAL (eq. 8 in reverse): the field of all sites kept in
+    registers and corrected by W(c - t) . delta_c for the accepted moves only.  A run cannot be stopped between passes,
+    so the kernel logs the margin dE/T + ln u of every trial; the oracle replays the same passes from the same state
+    in fp64 (field from scratch every pass).  Every replica is its own chain: until its first decision inside the
+    |margin| < 1e-4 band, margins must agree to the lock-step tolerance plus the drift of the running field, decisions
+    must be identical and the final spins equal; at most a few chains may leave the comparison.  Finally the field the
+    kernel ends with is compared with the field of its final state computed from scratch."""
+    from paper_1211_6234_b200 import inputs
+    J, g, K2, K4 = 1.0, 0.25, 0.6, 0.1
+    n = (L // l) ** 2
+    ctx = dsmc_mod.Dsmc(L, R, J=J, g=g, K2=K2, K4=K4)
+    ctx.build_tensor(dsmc_mod.DSMC_W_EWALD)
+    W = oracle.build_tensor_ewald(L)
+    s0 = inputs.random_spins(L, R, 57)
+    ctx.set_spins(s0)
+    T = np.linspace(0.2, 1.6, R).astype(np.float32)
+    log = torch.zeros((passes, R, n), dtype=torch.float32, device="cuda")
+    ctx.sublattice_run(T, 0xABCD, 3, passes, l, flags=dsmc_mod.DSMC_INCREMENTAL, margin_log=log)
+    got = log.cpu().numpy()
+    s_gpu = ctx.get_spins()
+    h_gpu = ctx.get_field()
+    s = s0.astype(np.float64)
+    alive = np.ones(R, dtype=bool)
+    compared = accepted = 0
+    for k in range(passes):
+        ref = oracle.sublattice_pass(W, s, T, 0xABCD, 3 + k, l, J, g, K2, K4)
+        ox, oy = ref["offset"]
+        m_ref = np.stack([ref["margin"][:, oy + l * b, ox + l * a] for b in range(L // l) for a in range(L // l)], axis=1)
+        band = np.abs(m_ref) < BAND
+        ok = alive[:, None] & ~band
+        assert np.all(np.abs(got[k] - m_ref)[ok] <= 4e-5 + 3e-6 * np.abs(m_ref)[ok]), (k, np.abs(got[k] - m_ref)[ok].max())
+        assert np.array_equal((got[k] < 0)[ok], (m_ref < 0)[ok]), k
+        compared += int(ok.sum())
+        accepted += int((m_ref < 0)[ok].sum())
+        alive &= ~band.any(axis=1)                              # a chain with an ambiguous decision may have branched off
+    assert alive.sum() >= max(1, R - 2), alive
+    assert 0 < accepted < compared
+    assert np.max(np.abs(s_gpu[alive].astype(np.float64) - s[alive])) <= 1e-6
+    # the running field against the field of the final state from scratch (fp64 direct sum)
+    h_ref = oracle.dipole_field(W, s_gpu.astype(np.float64))
+    d = h_gpu.astype(np.float64) - h_ref
+    rel = np.sqrt((d ** 2).sum() / (h_ref ** 2).sum())
+    print(f"L={L} l={l}: {compared} trials compared, {accepted} accepted, running field rel L2 {rel:.2e} max abs {np.abs(d).max():.2e}")
+    assert rel <= 1e-5 and np.abs(d).max() <= 1e-4
+    ctx.close()
+
+
+def test_incremental_field_drift_and_refresh(dsmc_mod, oracle):
+    """A whole refresh period and beyond at the paper's L = 64, l = 32 (4096 + 1000 passes: one refresh inside): the
+    field the kernel carries stays within the field tolerances of the field of its own final state."""
+    from paper_1211_6234_b200 import inputs
+    L, R, l = 64, 8, 32
+    ctx = dsmc_mod.Dsmc(L, R, J=1.0, g=0.2247, K2=1.685, K4=0.0)
+    ctx.build_tensor(dsmc_mod.DSMC_W_EWALD)
+    ctx.set_spins(inputs.random_spins(L, R, 3))
+    T = np.linspace(0.2, 1.6, R).astype(np.float32)
+    W = oracle.build_tensor_ewald(L)
+    for n_passes in (4096, 5096):
+        ctx.sublattice_run(T, 9, 0, n_passes, l, flags=dsmc_mod.DSMC_INCREMENTAL)
+        h_ref = oracle.dipole_field(W, ctx.get_spins().astype(np.float64))
+        d = ctx.get_field().astype(np.float64) - h_ref
+        rel = np.sqrt((d ** 2).sum() / (h_ref ** 2).sum())
+        print(f"{n_passes} passes: running field rel L2 {rel:.2e} max abs {np.abs(d).max():.2e}")
+        assert rel <= 1e-5 and np.abs(d).max() <= 1e-4
+    with pytest.raises(dsmc_mod.DsmcError):                      # L * L > 4096
+        big = dsmc_mod.Dsmc(128, 2)
+        big.build_tensor()
+        big.set_spins(inputs.random_spins(128, 2, 1))
+        big.sublattice_run(np.ones(2, np.float32), 1, 0, 4, 64, flags=dsmc_mod.DSMC_INCREMENTAL)
+    ctx.close()
