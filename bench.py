@@ -156,17 +156,24 @@ def paper_schedule(m, inputs, dev):
         ctx.build_tensor(m.DSMC_W_EWALD)
         ctx.set_spins(inputs.random_spins(L, R, 1))
         T = np.linspace(Trange[0], Trange[1], R).astype(np.float32)
-        ctx.sublattice_run(T, 1, 0, npass, l, flags=flags)
+        # equilibrate first (the acceptance rate of the quench from a random state is not the ladder's)
+        ctx.sublattice_run(T, 1, 0, 40 * npass, l, flags=flags & ~m.DSMC_INCREMENTAL)
+        ctx.sublattice_run(T, 1, 40 * npass, npass, l, flags=flags)
         torch.cuda.synchronize(dev)
         reps = 4
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
-        ctx.sublattice_run(None, 1, npass, reps * npass, l, flags=flags)
+        ctx.sublattice_run(None, 1, 41 * npass, reps * npass, l, flags=flags)
         e1.record()
         torch.cuda.synchronize(dev)
         ms = e0.elapsed_time(e1) / reps
         out[name] = {"R": R, "l": l, "T": list(Trange), "us_per_pass": ms * 1e3 / npass, "ms_per_mc_step": ms,
                      "updates_per_s": L * L * R / (ms * 1e-3)}
+        if flags & m.DSMC_INCREMENTAL:                            # the acceptance rate the timing goes with
+            log = torch.zeros((npass, R, (L // l) ** 2), dtype=torch.float32, device=dev)
+            ctx.sublattice_run(None, 1, 45 * npass, npass, l, flags=flags, margin_log=log)
+            acc = (log < 0).float().mean(dim=(0, 2)).cpu().numpy()
+            out[name]["acceptance_coldest_hottest"] = [float(acc[0]), float(acc[-1])]
         ctx.close()
     # resident kernel: one CTA = one SM sums 4 targets x 4096 sources x 5 FMA x 2 replicas per pass
     fma_clk = 4 * L * L * 5 * 2 / 128.0

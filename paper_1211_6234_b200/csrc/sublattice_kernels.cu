@@ -438,9 +438,11 @@ __global__ void __launch_bounds__(kResThreads, 1) sublattice_resident_kernel(con
 // replica pair as in sublattice_resident_kernel, but the 256 field threads keep the field of all N sites in registers
 // (site t = tid + 256 j, j < 16: 48 packed values per thread) instead of summing over all N sources for the n update
 // sites of every pass:
-//   pass:  owners publish h of the n update sites  | the drawing warp draws (Philox) as before
-//          -- barrier --  the drawing warp decides and publishes delta_c (zero when rejected)
-//          -- barrier --  every field thread adds W(c - t) delta_c to its 16 sites, for the c that were accepted
+//   pass:  every field thread adds W(c - t) delta_c of the pass before to its 16 sites (for the c that were accepted),
+//          then the owners publish h of this pass's n update sites | one drawing warp reads its sites' neighbours
+//          -- barrier --  that warp decides and publishes delta_c (zero when rejected) | the OTHER drawing warp runs
+//                         Philox for the next pass (offset, trial spins, ln u: none of it depends on the state)
+//          -- barrier --
 // Work per pass is 5 n N FMAs per replica pair only for accepted moves (the full sum costs 5 n N always), there is
 // no reduction across threads, and a pass in which nothing was accepted costs two barriers.  The field is taken from
 // the field array H at entry (the caller computes it with a field kernel) and written back at exit; rounding
@@ -454,13 +456,14 @@ __host__ __device__ constexpr size_t incremental_smem_bytes(int L, int NL) {
 }
 
 template <int NL, int LC>
-__global__ void __launch_bounds__(kIncThreads + 32, 1) sublattice_incremental_kernel(const MetropolisArgs p, const RoundKeys rk,
+__global__ void __launch_bounds__(kIncThreads + 64, 1) sublattice_incremental_kernel(const MetropolisArgs p, const RoundKeys rk,
                                                                                   const float *__restrict__ Wc,
                                                                                   float *__restrict__ Hio, int l_arg,
                                                                                   unsigned long long first_pass,
                                                                                   unsigned n_passes,
                                                                                   float *__restrict__ margin_log) {
     constexpr int NN = NL * NL;
+    constexpr int NT = kIncThreads + 64;                               // 8 field warps + 2 drawing warps
     extern __shared__ __align__(16) unsigned char rsm[];
     const int L = LC > 0 ? LC : p.L, l = LC > 0 ? LC / NL : l_arg, Lh = L >> 1, R = p.R, N = L * L;
     float4 *Wsm = reinterpret_cast<float4 *>(rsm);                     // [N + 1]  (xx, xy, yy, zz) at rho = ry L + rx
@@ -473,7 +476,7 @@ __global__ void __launch_bounds__(kIncThreads + 32, 1) sublattice_incremental_ke
     const int r0 = 2 * blockIdx.x, r1 = min(r0 + 1, R - 1);            // odd R: the last CTA carries its replica twice
     const size_t plane = (size_t)L * Lh * R;
 
-    for (int n = tid; n < N; n += kIncThreads + 32) {
+    for (int n = tid; n < N; n += NT) {
         Wsm[n] = make_float4(__ldg(Wc + n), __ldg(Wc + (size_t)N + n), __ldg(Wc + 2 * (size_t)N + n),
                              __ldg(Wc + 3 * (size_t)N + n));
         const int x = n % L, y = n / L;
@@ -501,26 +504,77 @@ __global__ void __launch_bounds__(kIncThreads + 32, 1) sublattice_incremental_ke
             h[j][2] = f2_make(src[2 * plane + r0], src[2 * plane + r1]);
         }
     }
-    if (tid == 0) pass_offset(rk, first_pass, l, off[0], off[1]);
-    __syncthreads();
 
-    const bool drawer = warp == kIncThreads / 32;
+    // Two drawing warps take the passes in turn: while one decides pass k, the other already runs Philox for pass
+    // k + 1 (its offset, then the trial spin and ln u of its sites: none of that depends on the state), so the serial
+    // part of a pass is only "read the neighbours, dE, accept".  Lanes: update site fk = lane >> 1, replica rb = lane & 1.
+    const bool drawer = warp >= kIncThreads / 32;
+    const int dw = warp - kIncThreads / 32;
     const bool flipper = drawer && lane < 2 * NN;
     const int fk = lane >> 1, rb = lane & 1, fr = rb ? r1 : r0;
     float invT = 0.0f, K2 = 0.0f, K4 = 0.0f;
     if (flipper) invT = p.invT[fr], K2 = p.K2[fr], K4 = p.K4[fr];
     MetropolisArgs q = p;
     q.step_dev = nullptr;
+    q.flip = 0;                                                        // the reversal move is applied at decision time
+    Draw dr = {0.0f, 0.0f, 0.0f, 0.0f};
+    int my_ox = 0, my_oy = 0;
+    if (drawer && dw == 0) {                                           // the first pass's draw, before the loop
+        pass_offset(rk, first_pass, l, my_ox, my_oy);
+        if (lane == 0) off[0] = my_ox, off[1] = my_oy;
+        const int nt = (my_oy + l * (fk / NL)) * L + my_ox + l * (fk % NL);
+        const uint4 rnd = philox4x32_10(make_uint4((uint32_t)nt, (uint32_t)fr + p.r_off, (uint32_t)(first_pass & 0xFFFFFFFFull),
+                                                   (uint32_t)(first_pass >> 32) & 0x7FFFFFFFu), rk);
+        dr = draw_from_words(q, rnd, 0.0f, 0.0f, 0.0f);
+    }
+    __syncthreads();
 
+    // Barriers: A(it) = "h of this pass's sites is published", B(it) = "decisions and deltas of this pass are out".
+    // Named barriers 1..4 (A and B of even / odd passes) over all threads; the warp that pre-draws only ARRIVES (it
+    // has nothing to wait for), so its Philox work spans the whole pass instead of sitting between the two barriers.
+    int pox = 0, poy = 0;                                              // field threads: the offsets of the pass before
     for (unsigned it = 0; it < n_passes; ++it) {
         const unsigned long long pass = first_pass + it;
         const int cur = (int)(it & 1u);
-        const int ox = off[2 * cur], oy = off[2 * cur + 1];
-        Draw dr;
-        float sx = 0.0f, sy = 0.0f, sz = 0.0f, nx = 0.0f, ny = 0.0f, nz = 0.0f;
-        int nt = 0;
+        const int idA = 1 + 2 * cur, idB = 2 + 2 * cur;
         if (!drawer) {
-            // the owners publish the field of the update sites (a register array cannot be indexed: compare and select)
+            const int ox = off[2 * cur], oy = off[2 * cur + 1];
+            if (it > 0) {
+                // rank-n update of the field of this thread's sites by the moves of the pass before:
+                // h_t += W(c - t) . delta_c for the accepted c
+                const f2 *dl = reinterpret_cast<const f2 *>(dlf);
+#pragma unroll 1
+                for (int k = 0; k < NN; ++k) {
+                    const f2 dxp = dl[3 * k], dyp = dl[3 * k + 1], dzp = dl[3 * k + 2];
+                    if ((dxp | dyp | dzp) == 0ull) continue;       // all six components +0: rejected in both replicas (uniform over the CTA)
+                    const int xc = pox + l * (k % NL), yc = poy + l * (k / NL);
+                    if constexpr (LC == 64) {
+                        // site j of this thread is (tid & 63, (tid >> 6) + 4 j): rho_x is the same for all of them and
+                        // the table index steps back by 4 rows = 256 entries from one to the next
+                        const int idx0 = (((yc - (tid >> 6)) & 63) << 6) | ((xc - tid) & 63);
+#pragma unroll
+                        for (int j = 0; j < kIncSpt; ++j) {
+                            const float4 w = Wsm[(idx0 - 256 * j) & 4095];
+                            h[j][0] = f2_fma(f2_bc(w.x), dxp, f2_fma(f2_bc(w.y), dyp, h[j][0]));
+                            h[j][1] = f2_fma(f2_bc(w.y), dxp, f2_fma(f2_bc(w.z), dyp, h[j][1]));
+                            h[j][2] = f2_fma(f2_bc(w.w), dzp, h[j][2]);
+                        }
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < kIncSpt; ++j) {
+                            if (txy[j] < 0) continue;
+                            int rx = xc - (txy[j] & 0xFFFF), ry = yc - (txy[j] >> 16);
+                            rx += rx < 0 ? L : 0;
+                            ry += ry < 0 ? L : 0;
+                            const float4 w = Wsm[ry * L + rx];
+                            h[j][0] = f2_fma(f2_bc(w.x), dxp, f2_fma(f2_bc(w.y), dyp, h[j][0]));
+                            h[j][1] = f2_fma(f2_bc(w.y), dxp, f2_fma(f2_bc(w.z), dyp, h[j][1]));
+                            h[j][2] = f2_fma(f2_bc(w.w), dzp, h[j][2]);
+                        }
+                    }
+                }
+            }
+            // the owners publish the field of this pass's update sites (a register array cannot be indexed: compare and select)
 #pragma unroll
             for (int k = 0; k < NN; ++k) {
                 const int nk = (oy + l * (k / NL)) * L + ox + l * (k % NL);
@@ -533,91 +587,84 @@ __global__ void __launch_bounds__(kIncThreads + 32, 1) sublattice_incremental_ke
                     hpub[3 * k] = v0, hpub[3 * k + 1] = v1, hpub[3 * k + 2] = v2;
                 }
             }
-        } else {
-            const int xt = ox + l * (fk % NL), yt = oy + l * (fk / NL);
-            nt = yt * L + xt;
-            uint4 ctr = make_uint4((uint32_t)nt, (uint32_t)fr + p.r_off, (uint32_t)(pass & 0xFFFFFFFFull),
-                                   (uint32_t)(pass >> 32) & 0x7FFFFFFFu);
-            if (2 * NN < 32 && lane == 31)
-                ctr = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, (uint32_t)((pass + 1) & 0xFFFFFFFFull),
-                                 (uint32_t)((pass + 1) >> 32) & 0x7FFFFFFFu);
-            const uint4 rnd = philox4x32_10(ctr, rk);
-            if (2 * NN < 32 && lane == 31) {
-                off[2 * (cur ^ 1)] = (int)(rnd.x % (uint32_t)l);
-                off[2 * (cur ^ 1) + 1] = (int)(rnd.y % (uint32_t)l);
-            }
-            if constexpr (2 * NN >= 32) {
-                if (lane == 0) pass_offset(rk, pass + 1, l, off[2 * (cur ^ 1)], off[2 * (cur ^ 1) + 1]);
-            }
+            pox = ox, poy = oy;
+            asm volatile("bar.sync %0, %1;" ::"r"(idA), "r"(NT) : "memory");
+            asm volatile("bar.sync %0, %1;" ::"r"(idB), "r"(NT) : "memory");
+        } else if (dw == cur) {
+            // the deciding warp: everything that depends on the state, after the barrier that orders it behind the pass before
+            asm volatile("bar.sync %0, %1;" ::"r"(idA), "r"(NT) : "memory");
             if (flipper) {
+                const int xt = my_ox + l * (fk % NL), yt = my_oy + l * (fk / NL);
+                const int nt = yt * L + xt;
                 const int xe = xt + 1 == L ? 0 : xt + 1, xw = xt == 0 ? L - 1 : xt - 1;
                 const int yn = yt + 1 == L ? 0 : yt + 1, ys = yt == 0 ? L - 1 : yt - 1;
                 const float *sc = Sf + 6 * nt + rb, *se = Sf + 6 * (yt * L + xe) + rb, *sw = Sf + 6 * (yt * L + xw) + rb,
                             *sn = Sf + 6 * (yn * L + xt) + rb, *ss = Sf + 6 * (ys * L + xt) + rb;
-                sx = sc[0], sy = sc[2], sz = sc[4];
-                nx = (se[0] + sw[0]) + (sn[0] + ss[0]);
-                ny = (se[2] + sw[2]) + (sn[2] + ss[2]);
-                nz = (se[4] + sw[4]) + (sn[4] + ss[4]);
-                dr = draw_from_words(q, rnd, sx, sy, sz);
-            }
-        }
-        __syncthreads();
-        if (flipper) {
-            const float *pf = reinterpret_cast<const float *>(hpub) + rb;
-            const Trial tr = decide_drawn(q, dr, sx, sy, sz, nx, ny, nz, pf[6 * fk], pf[6 * fk + 2], pf[6 * fk + 4], invT, K2, K4);
-            const bool live = r0 + rb < R;                             // the duplicate of an odd R's last replica stays silent
-            float dx = 0.0f, dy = 0.0f, dz = 0.0f;
-            if (tr.acc) {
-                dx = tr.tx - sx, dy = tr.ty - sy, dz = tr.tz - sz;
-                Sf[6 * nt + rb] = tr.tx;
-                Sf[6 * nt + 2 + rb] = tr.ty;
-                Sf[6 * nt + 4 + rb] = tr.tz;
-            }
-            dlf[6 * fk + rb] = dx, dlf[6 * fk + 2 + rb] = dy, dlf[6 * fk + 4 + rb] = dz;
-            if (live) {
-                if (p.accept_out) p.accept_out[(size_t)fr * N + nt] = tr.acc ? 1 : 0;
-                if (p.margin_out) p.margin_out[(size_t)fr * N + nt] = tr.margin;
-                if (margin_log) margin_log[((size_t)it * R + fr) * NN + fk] = tr.margin;
-            }
-        }
-        __syncthreads();
-        if (!drawer) {
-            // rank-n update of the field of this thread's sites: h_t += W(c - t) . delta_c for the accepted c
-            const f2 *dl = reinterpret_cast<const f2 *>(dlf);
-#pragma unroll 1
-            for (int k = 0; k < NN; ++k) {
-                const f2 dxp = dl[3 * k], dyp = dl[3 * k + 1], dzp = dl[3 * k + 2];
-                if ((dxp | dyp | dzp) == 0ull) continue;       // all six components +0: rejected in both replicas (uniform over the CTA)
-                const int xc = ox + l * (k % NL), yc = oy + l * (k / NL);
-                if constexpr (LC == 64) {
-                    // site j of this thread is (tid & 63, (tid >> 6) + 4 j): rho_x is the same for all of them and the
-                    // table index steps back by 4 rows = 256 entries from one to the next
-                    const int idx0 = (((yc - (tid >> 6)) & 63) << 6) | ((xc - tid) & 63);
-#pragma unroll
-                    for (int j = 0; j < kIncSpt; ++j) {
-                        const float4 w = Wsm[(idx0 - 256 * j) & 4095];
-                        h[j][0] = f2_fma(f2_bc(w.x), dxp, f2_fma(f2_bc(w.y), dyp, h[j][0]));
-                        h[j][1] = f2_fma(f2_bc(w.y), dxp, f2_fma(f2_bc(w.z), dyp, h[j][1]));
-                        h[j][2] = f2_fma(f2_bc(w.w), dzp, h[j][2]);
-                    }
-                } else {
-#pragma unroll
-                    for (int j = 0; j < kIncSpt; ++j) {
-                        if (txy[j] < 0) continue;
-                        int rx = xc - (txy[j] & 0xFFFF), ry = yc - (txy[j] >> 16);
-                        rx += rx < 0 ? L : 0;
-                        ry += ry < 0 ? L : 0;
-                        const float4 w = Wsm[ry * L + rx];
-                        h[j][0] = f2_fma(f2_bc(w.x), dxp, f2_fma(f2_bc(w.y), dyp, h[j][0]));
-                        h[j][1] = f2_fma(f2_bc(w.y), dxp, f2_fma(f2_bc(w.z), dyp, h[j][1]));
-                        h[j][2] = f2_fma(f2_bc(w.w), dzp, h[j][2]);
-                    }
+                const float sx = sc[0], sy = sc[2], sz = sc[4];
+                const float nx = (se[0] + sw[0]) + (sn[0] + ss[0]);
+                const float ny = (se[2] + sw[2]) + (sn[2] + ss[2]);
+                const float nz = (se[4] + sw[4]) + (sn[4] + ss[4]);
+                if (p.flip) dr.tx = -sx, dr.ty = -sy, dr.tz = -sz;     // Ising move of App. B: complete reversal
+                const float *pf = reinterpret_cast<const float *>(hpub) + rb;
+                const Trial tr = decide_drawn(q, dr, sx, sy, sz, nx, ny, nz, pf[6 * fk], pf[6 * fk + 2], pf[6 * fk + 4], invT, K2, K4);
+                const bool live = r0 + rb < R;                         // the duplicate of an odd R's last replica stays silent
+                float dx = 0.0f, dy = 0.0f, dz = 0.0f;
+                if (tr.acc) {
+                    dx = tr.tx - sx, dy = tr.ty - sy, dz = tr.tz - sz;
+                    Sf[6 * nt + rb] = tr.tx;
+                    Sf[6 * nt + 2 + rb] = tr.ty;
+                    Sf[6 * nt + 4 + rb] = tr.tz;
                 }
+                dlf[6 * fk + rb] = dx, dlf[6 * fk + 2 + rb] = dy, dlf[6 * fk + 4 + rb] = dz;
+                if (live) {
+                    if (p.accept_out) p.accept_out[(size_t)fr * N + nt] = tr.acc ? 1 : 0;
+                    if (p.margin_out) p.margin_out[(size_t)fr * N + nt] = tr.margin;
+                    if (margin_log) margin_log[((size_t)it * R + fr) * NN + fk] = tr.margin;
+                }
+            }
+            asm volatile("bar.sync %0, %1;" ::"r"(idB), "r"(NT) : "memory");
+        } else {
+            // the pre-drawing warp: Philox for the next pass; its offset has to be out before B(it)
+            asm volatile("bar.arrive %0, %1;" ::"r"(idA), "r"(NT) : "memory");
+            const bool more = it + 1 < n_passes;
+            if (more) {
+                pass_offset(rk, pass + 1, l, my_ox, my_oy);            // every lane computes the (same) offset: no divergence
+                if (lane == 0) off[2 * (cur ^ 1)] = my_ox, off[2 * (cur ^ 1) + 1] = my_oy;
+                __threadfence_block();
+            }
+            asm volatile("bar.arrive %0, %1;" ::"r"(idB), "r"(NT) : "memory");
+            if (more) {
+                const int nt = (my_oy + l * (fk / NL)) * L + my_ox + l * (fk % NL);
+                const unsigned long long np = pass + 1;
+                const uint4 rnd = philox4x32_10(make_uint4((uint32_t)nt, (uint32_t)fr + p.r_off, (uint32_t)(np & 0xFFFFFFFFull),
+                                                           (uint32_t)(np >> 32) & 0x7FFFFFFFu), rk);
+                dr = draw_from_words(q, rnd, 0.0f, 0.0f, 0.0f);
+            }
+        }
+    }
+    // the moves of the last pass are still to be applied to the field that is handed back
+    if (!drawer && n_passes > 0) {
+        const f2 *dl = reinterpret_cast<const f2 *>(dlf);
+#pragma unroll 1
+        for (int k = 0; k < NN; ++k) {
+            const f2 dxp = dl[3 * k], dyp = dl[3 * k + 1], dzp = dl[3 * k + 2];
+            if ((dxp | dyp | dzp) == 0ull) continue;
+            const int xc = pox + l * (k % NL), yc = poy + l * (k / NL);
+#pragma unroll
+            for (int j = 0; j < kIncSpt; ++j) {
+                if (txy[j] < 0) continue;
+                int rx = xc - (txy[j] & 0xFFFF), ry = yc - (txy[j] >> 16);
+                rx += rx < 0 ? L : 0;
+                ry += ry < 0 ? L : 0;
+                const float4 w = Wsm[ry * L + rx];
+                h[j][0] = f2_fma(f2_bc(w.x), dxp, f2_fma(f2_bc(w.y), dyp, h[j][0]));
+                h[j][1] = f2_fma(f2_bc(w.y), dxp, f2_fma(f2_bc(w.z), dyp, h[j][1]));
+                h[j][2] = f2_fma(f2_bc(w.w), dzp, h[j][2]);
             }
         }
     }
     __syncthreads();
-    for (int n = tid; n < N; n += kIncThreads + 32) {
+    for (int n = tid; n < N; n += NT) {
         const int x = n % L, y = n / L;
         int qc;
         float *dst = p.S + site_index(x, y, Lh, R, plane, qc);
@@ -718,7 +765,7 @@ cudaError_t launch_sublattice_incremental(const MetropolisArgs &a, const float *
     else if (nl == 4) kern = a.L == 64 ? sublattice_incremental_kernel<4, 64> : sublattice_incremental_kernel<4, 0>;
     else kern = a.L == 64 ? sublattice_incremental_kernel<1, 64> : sublattice_incremental_kernel<1, 0>;
     if (cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024)) return e;
-    kern<<<(unsigned)((a.R + 1) / 2), kIncThreads + 32, smem, st>>>(a, rk, Wc, H, l, first_pass, (unsigned)n_passes, margin_log);
+    kern<<<(unsigned)((a.R + 1) / 2), kIncThreads + 64, smem, st>>>(a, rk, Wc, H, l, first_pass, (unsigned)n_passes, margin_log);
     ++*launches;
     return cudaGetLastError();
 }
