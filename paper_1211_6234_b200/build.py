@@ -18,6 +18,7 @@ def _deps():
     d.append(os.path.join(CSRC, "bulk_copy.cuh"))
     d.append(os.path.join(CSRC, "packed_f32x2.cuh"))
     d.append(os.path.join(CSRC, "metropolis_common.cuh"))
+    d.append(os.path.join(CSRC, "metropolis_pair.cuh"))
     d.append(os.path.join(HERE, "..", "include", "dsmc.h"))
     return d
 

@@ -115,7 +115,7 @@ int run_field(dsmc_ctx *ctx, int colour, int kind_override = -1) {
     const int kind = kind_override >= 0 ? kind_override : field_kind(ctx);
     if (kind == 2) {
         e = launch_field_fft(ctx->S(), ctx->M(), ctx->Z(), ctx->C(), ctx->H(), ctx->L, ctx->R, colour, ctx->spec_valid,
-                             &ctx->fft_configured, ctx->stream, &ctx->launches);
+                             &ctx->zline, nullptr, &ctx->fft_configured, ctx->stream, &ctx->launches);
     } else {
         for (int q = 0; q < 2 && e == cudaSuccess; ++q) {
             if (colour >= 0 && colour != q) continue;
@@ -147,7 +147,7 @@ int after_tensor_change(dsmc_ctx *ctx) {
     CU(cudaStreamSynchronize(ctx->stream), "tensor sync");
     ctx->tensor_built = true;
     ctx->field_valid[0] = ctx->field_valid[1] = false;
-    ctx->spec_valid[0] = ctx->spec_valid[1] = false;
+    ctx->spec_valid[0] = ctx->spec_valid[1] = false, ctx->zline = -1;
     drop_sweep_graph(ctx);  // W(0) is baked into the captured kernel parameters
     return DSMC_OK;
 }
@@ -184,6 +184,39 @@ MetropolisArgs metropolis_args(dsmc_ctx *ctx, int colour, uint64_t seed, uint64_
     return a;
 }
 
+// One half-sweep: field of `colour` + Metropolis on it.  With the FFT field on a shape the fused row kernel supports, and no
+// parity hooks, timing or field reuse asked for, the Metropolis decision rides in the field's last pass (field_fft.cu:
+// two launches per half-sweep, h never written to global memory); otherwise field kernel(s) + metropolis kernel.  Both
+// routes take bit-identical decisions (tests/test_gpu_parity.py::test_benchmarked_metropolis_instantiation_is_the_tested_one).
+int enqueue_halfsweep(dsmc_ctx *ctx, const MetropolisArgs &a, int flags) {
+    const int colour = a.colour;
+    const bool fused = field_kind(ctx) == 2 && dsmc_fft_fused_supported(ctx->L, ctx->R) && !a.accept_out && !a.margin_out &&
+                       !ctx->timing && !(flags & DSMC_REUSE_FIELD) && !ctx->no_fuse;
+    if (fused) {
+        const cudaError_t e = launch_field_fft(ctx->S(), ctx->M(), ctx->Z(), ctx->C(), ctx->H(), ctx->L, ctx->R, colour,
+                                               ctx->spec_valid, &ctx->zline, &a, &ctx->fft_configured, ctx->stream,
+                                               &ctx->launches);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "fused FFT half-sweep launch");
+        ctx->field_valid[colour] = false;                       // h of this half-sweep never reached the field array
+        return DSMC_OK;
+    }
+    if (ctx->timing) CU(cudaEventRecord(ctx->ev[0], ctx->stream), "event");
+    if (!(flags & DSMC_REUSE_FIELD)) {
+        if (int rc = run_field(ctx, colour)) return rc;
+    } else if (!ctx->field_valid[colour]) {
+        return fail(ctx, DSMC_ESTATE, "DSMC_REUSE_FIELD without a field of this colour");
+    }
+    if (ctx->timing) CU(cudaEventRecord(ctx->ev[1], ctx->stream), "event");
+    CU(launch_metropolis(a, ctx->stream, &ctx->launches), "metropolis launch");
+    if (ctx->timing) {
+        CU(cudaEventRecord(ctx->ev[2], ctx->stream), "event");
+        ctx->ev_recorded = true;
+    }
+    ctx->spec_valid[colour] = false;                            // the cached half-spectrum of this colour is stale now
+    if (ctx->zline == colour) ctx->zline = -1;
+    return DSMC_OK;
+}
+
 void drop_sweep_graph(dsmc_ctx *ctx) {
     if (ctx->sweep_graph) cudaGraphExecDestroy(ctx->sweep_graph);
     ctx->sweep_graph = nullptr;
@@ -213,7 +246,7 @@ int enqueue_pass(dsmc_ctx *ctx, uint64_t seed, uint64_t pass, int l, int flags, 
         const MetropolisArgs a = metropolis_args(ctx, 0, seed, pass, flags, accept_out, margin_out);
         CU(launch_sublattice_resident(a, ctx->Wc(), l, pass, 1, ctx->stream, &ctx->launches), "resident pass launch");
         ctx->field_valid[0] = ctx->field_valid[1] = false;
-        ctx->spec_valid[0] = ctx->spec_valid[1] = false;
+        ctx->spec_valid[0] = ctx->spec_valid[1] = false, ctx->zline = -1;
         return DSMC_OK;
     }
     if (fft)
@@ -223,7 +256,7 @@ int enqueue_pass(dsmc_ctx *ctx, uint64_t seed, uint64_t pass, int l, int flags, 
     CU(launch_sublattice_pass(a, ctx->Wc(), ctx->stage(), ctx->sm_count, l, ox, oy, fft, ctx->stream, &ctx->launches),
        "sub-lattice pass launch");
     ctx->field_valid[0] = ctx->field_valid[1] = false;
-    ctx->spec_valid[0] = ctx->spec_valid[1] = false;
+    ctx->spec_valid[0] = ctx->spec_valid[1] = false, ctx->zline = -1;
     return DSMC_OK;
 }
 
@@ -294,7 +327,7 @@ int build_sweep_graph(dsmc_ctx *ctx, uint64_t seed, int flags, int record_every)
     const int kind = field_kind(ctx);
     // the kernels a field call enqueues depend on which half-spectra are current (FFT field): a graph is only valid
     // from the state it was captured in, and must leave that state behind to be replayed back to back
-    const int spec_in = (ctx->spec_valid[0] ? 1 : 0) | (ctx->spec_valid[1] ? 2 : 0);
+    const int spec_in = (ctx->spec_valid[0] ? 1 : 0) | (ctx->spec_valid[1] ? 2 : 0) | ((ctx->zline + 1) << 2);
     if (ctx->sweep_graph && ctx->graph_seed == seed && ctx->graph_kind == kind && ctx->graph_flags == flags &&
         ctx->graph_every == record_every && ctx->graph_spec_in == spec_in)
         return DSMC_OK;
@@ -311,14 +344,10 @@ int build_sweep_graph(dsmc_ctx *ctx, uint64_t seed, int flags, int record_every)
         const int n_sweeps = record_every > 0 ? record_every : DSMC_GRAPH_UNROLL;
         for (int rep = 0; rep < n_sweeps && rc == DSMC_OK && e == cudaSuccess; ++rep) {
             for (int colour = 0; colour < 2 && rc == DSMC_OK; ++colour) {
-                rc = run_field(ctx, colour);
-                if (rc != DSMC_OK) break;
                 MetropolisArgs a = metropolis_args(ctx, colour, seed, 0, flags, nullptr, nullptr);
                 a.step_dev = ctx->step_dev();
                 a.step_off = (uint32_t)(2 * rep + colour);  // the counter moves once per graph, not once per sweep
-                e = launch_metropolis(a, ctx->stream, &ctx->launches);
-                if (e != cudaSuccess) break;
-                ctx->spec_valid[colour] = false;
+                rc = enqueue_halfsweep(ctx, a, flags);
             }
         }
         if (e == cudaSuccess && rc == DSMC_OK)
@@ -330,9 +359,10 @@ int build_sweep_graph(dsmc_ctx *ctx, uint64_t seed, int flags, int record_every)
     ctx->stream = saved;
     ctx->graph_launches = ctx->launches - l0;
     ctx->launches = l0;
-    const int spec_out = (ctx->spec_valid[0] ? 1 : 0) | (ctx->spec_valid[1] ? 2 : 0);
+    const int spec_out = (ctx->spec_valid[0] ? 1 : 0) | (ctx->spec_valid[1] ? 2 : 0) | ((ctx->zline + 1) << 2);
     ctx->spec_valid[0] = spec_in & 1;                           // nothing has run: back to the state before the capture
     ctx->spec_valid[1] = (spec_in & 2) != 0;
+    ctx->zline = (spec_in >> 2) - 1;
     if (rc == DSMC_OK && e == cudaSuccess && spec_out != spec_in) {
         if (graph) cudaGraphDestroy(graph);
         return fail(ctx, DSMC_ESTATE, "internal: a captured sweep does not return to the spectrum state it started from");
@@ -406,6 +436,7 @@ int dsmc_create(dsmc_ctx **out, int L, int R, float J, float g, float K2, float 
     c->K4.assign(R, K4);
     c->T.assign(R, 0.0f);
     c->lay = dsmc_make_layout(L, R);
+    if (const char *v = getenv("DSMC_NO_FUSE")) c->no_fuse = v[0] && v[0] != '0';
     *out = c;
     return DSMC_OK;
 }
@@ -448,7 +479,7 @@ int dsmc_bind(dsmc_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_strea
     ctx->stream = (cudaStream_t)cuda_stream;
     ctx->tensor_built = ctx->spins_set = false;
     ctx->field_valid[0] = ctx->field_valid[1] = false;
-    ctx->spec_valid[0] = ctx->spec_valid[1] = false;
+    ctx->spec_valid[0] = ctx->spec_valid[1] = false, ctx->zline = -1;
     ctx->T_valid = false;
     ctx->aniso_dirty = true;
     for (int i = 0; i < 3; ++i)
@@ -503,7 +534,7 @@ int dsmc_set_spins(dsmc_ctx *ctx, const float *s, int where) {
     }
     CU(launch_canon_to_internal(src, ctx->S(), ctx->L, ctx->R, ctx->stream, &ctx->launches), "set spins");
     ctx->field_valid[0] = ctx->field_valid[1] = false;
-    ctx->spec_valid[0] = ctx->spec_valid[1] = false;
+    ctx->spec_valid[0] = ctx->spec_valid[1] = false, ctx->zline = -1;
     if (ctx->debug) {
         // |s| = 1 is the caller's contract, checked to 1e-5 when debugging is on (one reduction kernel and
         // one synchronisation; the default path pays nothing)
@@ -544,7 +575,7 @@ int dsmc_init_spins(dsmc_ctx *ctx, int mode, uint64_t seed) {
     CU(launch_init_spins(ctx->S(), ctx->L, ctx->R, mode, seed, ctx->replica_offset, ctx->stream, &ctx->launches), "init spins");
     ctx->spins_set = true;
     ctx->field_valid[0] = ctx->field_valid[1] = false;
-    ctx->spec_valid[0] = ctx->spec_valid[1] = false;
+    ctx->spec_valid[0] = ctx->spec_valid[1] = false, ctx->zline = -1;
     return DSMC_OK;
 }
 
@@ -594,23 +625,10 @@ int dsmc_halfsweep_ex(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t ste
     if (flags & ~(DSMC_REUSE_FIELD | DSMC_TRIAL_FLIP)) return fail(ctx, DSMC_EINVAL, "unknown flag");
     if (int rc = upload_params(ctx, T)) return rc;
     const int colour = (int)(step & 1u);
-    if (ctx->timing) CU(cudaEventRecord(ctx->ev[0], ctx->stream), "event");
-    if (!(flags & DSMC_REUSE_FIELD)) {
-        if (int rc = run_field(ctx, colour)) return rc;
-    } else if (!ctx->field_valid[colour]) {
-        return fail(ctx, DSMC_ESTATE, "DSMC_REUSE_FIELD without a field of this colour");
-    }
-    if (ctx->timing) CU(cudaEventRecord(ctx->ev[1], ctx->stream), "event");
     const MetropolisArgs a = metropolis_args(ctx, colour, seed, step, flags, accept_out, margin_out);
-    CU(launch_metropolis(a, ctx->stream, &ctx->launches), "metropolis launch");
-    ctx->spec_valid[colour] = false;                            // the cached half-spectrum of this colour is stale now
-    if (ctx->timing) {
-        CU(cudaEventRecord(ctx->ev[2], ctx->stream), "event");
-        ctx->ev_recorded = true;
-    }
     // field_valid only records that H holds a field of that colour computed since the spins were
     // last set (what DSMC_REUSE_FIELD needs for timing); observables always recompute both colours
-    return DSMC_OK;
+    return enqueue_halfsweep(ctx, a, flags);
 }
 
 int dsmc_halfsweep(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t step) {
@@ -654,7 +672,7 @@ int dsmc_sublattice_run_ex(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_
                                              margin_log ? margin_log + done * (uint64_t)ctx->R * (uint64_t)((ctx->L / l) * (ctx->L / l)) : nullptr,
                                              ctx->stream, &ctx->launches),
                "incremental run launch");
-            ctx->spec_valid[0] = ctx->spec_valid[1] = false;
+            ctx->spec_valid[0] = ctx->spec_valid[1] = false, ctx->zline = -1;
             done += chunk;
         }
         ctx->field_valid[0] = ctx->field_valid[1] = true;      // H holds the (incrementally updated) field of the final state
@@ -669,7 +687,7 @@ int dsmc_sublattice_run_ex(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_
         CU(launch_sublattice_resident(a, ctx->Wc(), l, first_pass, n_passes, ctx->stream, &ctx->launches),
            "resident run launch");
         ctx->field_valid[0] = ctx->field_valid[1] = false;
-        ctx->spec_valid[0] = ctx->spec_valid[1] = false;
+        ctx->spec_valid[0] = ctx->spec_valid[1] = false, ctx->zline = -1;
         return DSMC_OK;
     }
     uint64_t k = 0;
@@ -720,6 +738,7 @@ int dsmc_run_ex(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_ste
             ctx->field_valid[0] = ctx->field_valid[1] = true;
             ctx->spec_valid[0] = ctx->graph_spec_out & 1;           // (= the state the graph started from)
             ctx->spec_valid[1] = (ctx->graph_spec_out & 2) != 0;
+            ctx->zline = (ctx->graph_spec_out >> 2) - 1;
             k += 2 * DSMC_GRAPH_UNROLL * reps;
         }
     }
@@ -845,6 +864,7 @@ int dsmc_run_recorded(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t fir
         ctx->field_valid[0] = ctx->field_valid[1] = true;
         ctx->spec_valid[0] = ctx->graph_spec_out & 1;
         ctx->spec_valid[1] = (ctx->graph_spec_out & 2) != 0;
+        ctx->zline = (ctx->graph_spec_out >> 2) - 1;
         ctx->ensemble_n += reps;
         done += reps;
     }

@@ -92,10 +92,12 @@ struct dsmc_ctx {
     bool tensor_built = false, spins_set = false;
     bool field_valid[2] = {false, false};
     bool spec_valid[2] = {false, false};  // FFT field: the cache holds the half-spectrum of colour c of the CURRENT spins
+    int zline = -1;  // FFT field: the colour whose forward-transformed rows (of the CURRENT spins) sit in the scratch Z, or -1
     float w0[4] = {0, 0, 0, 0};  // W(0) components (fp32, as stored)
     uint32_t replica_offset = 0;  // dsmc_set_replica_offset
     int field_kind = -1;  // -1 automatic, 0 generic, 1 tiled, 2 FFT (dsmc_select_field_kernel)
     int timing = 0;
+    int no_fuse = 0;  // DSMC_NO_FUSE=1 in the environment at dsmc_create: never fuse the Metropolis decision into the FFT field (A/B)
     int debug = 0;  // dsmc_set_debug: argument checks that cost a kernel (|s| = 1 in dsmc_set_spins)
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
     bool ev_recorded = false;
@@ -168,8 +170,14 @@ cudaError_t launch_make_fft_table(const float *Wc, float *M, void *scratch, int 
                                   uint64_t *launches);
 // colour = -1 writes both colours of H.  valid[2]: which colours' half-spectra in `cache` are those of the current
 // spins; updated here (a colour transformed forward becomes valid), cleared by the caller when a colour's spins change
+// zline: which colour's forward-transformed rows the scratch Z holds (-1 none).  fuse != null (colour 0 / 1, shape
+// dsmc_fft_fused_supported): the last pass also takes the Metropolis decision of the half-sweep and
+// transforms the updated rows forward: H is NOT written, the spins of `colour` change
+struct MetropolisArgs;
+bool dsmc_fft_fused_supported(int L, int R);
 cudaError_t launch_field_fft(const float *S, const float *AB, void *scratch, void *cache, float *H, int L, int R, int colour,
-                             bool *valid, bool *configured, cudaStream_t st, uint64_t *launches);
+                             bool *valid, int *zline, const MetropolisArgs *fuse, bool *configured, cudaStream_t st,
+                             uint64_t *launches);
 // configured: the context's "dynamic shared memory limit raised on this device" flag
 cudaError_t launch_field_tiled(const float *S, const float *Wk, float *Hpart, float *H, int L, int R,
                                int colour, int sm_count, bool *configured, cudaStream_t st, uint64_t *launches);

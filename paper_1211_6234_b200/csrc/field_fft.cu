@@ -28,9 +28,8 @@
 // sub-sequences, twiddle, one pass through shared memory, N2-point FFTs in registers; spectra stay in "slot order"
 // slot(k) = N2 (k mod 16) + k div 16 and the inverse runs the steps backwards, so no reordering pass exists anywhere and
 // A, B are tabulated in slot order with the 1/N of the inverse folded in.
-#include "dsmc_internal.cuh"
+#include "metropolis_pair.cuh"
 #include "bulk_copy.cuh"
-#include "packed_f32x2.cuh"
 
 namespace {
 
@@ -310,6 +309,138 @@ __global__ void __launch_bounds__(256) fftc_x_inverse_kernel(const FcParams p) {
     for (int n1 = 0; n1 < 16; ++n1) dst[n1 * st_stride] = v[n1];
 }
 
+// The fused row kernel of a running FFT sweep: everything a half-sweep of colour t does to one lattice row, in one launch.
+//   A. x inverse of the three components (as fftc_x_inverse_kernel), the field h of the row left in shared memory;
+//   B. the Metropolis decision of every site of the row (metropolis_pair.cuh: the arithmetic of metropolis4_kernel, pair by
+//      pair, on the same inputs in the same order -- bit-identical decisions), new spins to the spin array and to shared
+//      memory;
+//   C. x forward of the UPDATED row (as fftc_x_forward_kernel), written over the row's entries of Z: the lines the next
+//      field's y pass needs (colour t is then the colour that was just updated).
+// A half-sweep is then two launches (y pass, this kernel) instead of four, h is never written to or read from global
+// memory, and the updated spins are transformed while they are on the chip.
+//   grid (P / LN, L rows), block (LN, TL, 3 components); LN = the line width LZ (8 at config 5).
+// Phase B's items (site i, pair) are spread over all threads; every other phase works on component threadIdx.z.
+template <int N2X, int LNC, bool DEVSTEP, int FLIP>
+__global__ void __launch_bounds__(384) fftc_row_update_kernel(const FcParams p, const MetropolisArgs ma, const RoundKeys rk) {
+    extern __shared__ __align__(16) float2 fsm[];
+    constexpr int Lh = 16 * N2X, L = 2 * Lh;
+    const int LN = nlanes<LNC>(), TL = blockDim.y;
+    float2 *twi = fsm, *twf = fsm + L;
+    const int lane = threadIdx.x, t = threadIdx.y, a = threadIdx.z;
+    const int nthr = LN * TL * 3, tid = (a * TL + t) * LN + lane;
+    float2 *X0 = fsm + 2 * L;                              // three exchange buffers, also h / spins of the row by site
+    const int xstride = line_rows<N2X>() * LN;
+    float2 *buf = X0 + a * xstride;
+    const int pb = blockIdx.x, pair = pb * LN + lane, y = blockIdx.y, c = p.colour;
+    for (int j = tid; j < L; j += nthr) twi[j] = __ldg(p.twi + j), twf[j] = __ldg(p.twf + j);   // constant tables
+    float2 *zline = p.Z + line_base(p, a, 0, pb) + (size_t)swz(y) * LN + lane;   // LN == p.LZ
+    const unsigned sx_stride = (unsigned)(p.PBZ * L * LN);
+    constexpr int NK = N2X >= 16 ? 1 : 16 / N2X;           // blocks k1 per thread
+    const bool odd_row = (y + c) & 1;
+    pdl_wait();                                            // the lines come from the y pass, the spins from earlier kernels
+    // ---- A: x inverse -> h(i) of this component in buf[i * LN + lane]
+    {
+        float2 u[NK][N2X];
+#pragma unroll
+        for (int j = 0; j < NK; ++j)
+#pragma unroll
+            for (int k2 = 0; k2 < N2X; ++k2) u[j][k2] = zline[(unsigned)(N2X * (t + j * TL) + k2) * sx_stride];
+        __syncthreads();
+#pragma unroll
+        for (int j = 0; j < NK; ++j) {
+            const int k1 = t + j * TL;
+            float2 w[N2X];
+#pragma unroll
+            for (int k2 = 0; k2 < N2X; ++k2) w[k2] = twi[odd_row ? k1 + 16 * k2 : 0];
+#pragma unroll
+            for (int k2 = 0; k2 < N2X; ++k2) u[j][k2] = cmul_tw(u[j][k2], w[k2]);
+            inv_step2<N2X, 2, LNC>(u[j], k1, twi, buf, lane);
+        }
+        __syncthreads();
+        float2 v[16];
+        inv_step1<N2X, LNC>(v, t, buf, lane);
+        __syncthreads();                                   // everybody has read the exchange layout: reuse it by site
+#pragma unroll
+        for (int n1 = 0; n1 < 16; ++n1) buf[(N2X * n1 + t) * LN + lane] = v[n1];
+    }
+    __syncthreads();
+    // ---- B: Metropolis on the row (eq. 7; the half-sweep's frozen field is the h just computed)
+    {
+        const int P = p.P;
+        const size_t planeP = (size_t)L * Lh * P;
+        f2 *S2 = reinterpret_cast<f2 *>(ma.S);
+        const f2 *X2 = reinterpret_cast<const f2 *>(X0);
+        f2 *X2w = reinterpret_cast<f2 *>(X0);
+        const int yn = (y + 1 == L) ? 0 : y + 1, ys = (y == 0) ? L - 1 : y - 1;
+        const size_t own0 = (size_t)c * 3 * planeP + (size_t)y * Lh * P, oth = (size_t)(1 - c) * 3 * planeP;
+        const size_t o0 = oth + (size_t)y * Lh * P, on = oth + (size_t)yn * Lh * P, os = oth + (size_t)ys * Lh * P;
+        uint32_t step_lo = ma.step_lo, step_hi = ma.step_hi;
+        if (DEVSTEP) step_words(ma, step_lo, step_hi);
+        for (int item = tid; item < Lh * LN; item += nthr) {
+            const int i = item / LN, ln = item - i * LN, pr = pb * LN + ln;
+            const int i1 = odd_row ? (i + 1 == Lh ? 0 : i + 1) : (i == 0 ? Lh - 1 : i - 1);
+            const unsigned e = (unsigned)(i * P + pr), e1 = (unsigned)(i1 * P + pr);
+            f2 s[3], nb[3], h[3];
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                s[k] = S2[own0 + k * planeP + e];
+                const f2 va = __ldg(S2 + o0 + k * planeP + e), vb = __ldg(S2 + o0 + k * planeP + e1);
+                const f2 vc = __ldg(S2 + on + k * planeP + e), vd = __ldg(S2 + os + k * planeP + e);
+                nb[k] = f2_add(f2_add(va, vb), f2_add(vc, vd));
+                h[k] = X2[k * xstride + item];
+            }
+            const f2 invT = __ldg(reinterpret_cast<const f2 *>(ma.invT) + pr), K2 = __ldg(reinterpret_cast<const f2 *>(ma.K2) + pr),
+                     K4 = __ldg(reinterpret_cast<const f2 *>(ma.K4) + pr);
+            const uint32_t n = (uint32_t)(y * L + 2 * i + (odd_row ? 1 : 0));
+            const uint32_t r = 2u * (uint32_t)pr + ma.r_off;
+            const uint4 ra = philox4x32_10(make_uint4(n, r, step_lo, step_hi), rk);
+            const uint4 rb = philox4x32_10(make_uint4(n, r + 1u, step_lo, step_hi), rk);
+            Trial2 tr = trial2(ra, rb);
+            if (FLIP) {                                    // Ising move of App. B: complete reversal
+                tr.tx = f2_mul(s[0], f2_bc(-1.0f));
+                tr.ty = f2_mul(s[1], f2_bc(-1.0f));
+                tr.tz = f2_mul(s[2], f2_bc(-1.0f));
+            }
+            const f2 margin = margin2(ma, tr, s[0], s[1], s[2], nb[0], nb[1], nb[2], h[0], h[1], h[2], invT, K2, K4);
+            float m0, m1;
+            f2_split(margin, m0, m1);
+            const bool acc0 = m0 < 0.0f, acc1 = m1 < 0.0f;
+            const f2 tv[3] = {tr.tx, tr.ty, tr.tz};
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                float a0, a1, b0, b1;
+                f2_split(tv[k], a0, a1);
+                f2_split(s[k], b0, b1);
+                s[k] = f2_make(acc0 ? a0 : b0, acc1 ? a1 : b1);
+                X2w[k * xstride + item] = s[k];            // the row after the update, for phase C
+            }
+            if (acc0 | acc1) {
+#pragma unroll
+                for (int k = 0; k < 3; ++k) S2[own0 + k * planeP + e] = s[k];
+            }
+        }
+    }
+    __syncthreads();
+    // ---- C: x forward of the updated row -> the row's entries of Z
+    {
+        float2 v[16];
+#pragma unroll
+        for (int n1 = 0; n1 < 16; ++n1) v[n1] = buf[(N2X * n1 + t) * LN + lane];
+        __syncthreads();
+        fwd_step1<N2X, 2, LNC>(v, t, twf, buf, lane);
+        __syncthreads();
+        pdl_trigger();
+        for (int k1 = t; k1 < 16; k1 += TL) {
+            float2 u[N2X], w[N2X];
+#pragma unroll
+            for (int k2 = 0; k2 < N2X; ++k2) w[k2] = twf[odd_row ? k1 + 16 * k2 : 0];
+            fwd_step2<N2X, LNC>(u, k1, buf, lane);
+#pragma unroll
+            for (int k2 = 0; k2 < N2X; ++k2) zline[(unsigned)(N2X * k1 + k2) * sx_stride] = cmul_tw(u[k2], w[k2]);
+        }
+    }
+}
+
 // In-place four-step transforms of one shared-memory line B[row' * LZ + lane] (rows = y or slot_y, see FcParams).
 // Forward: natural order in, slot order out; inverse: slot order in, natural order out.  Step 1 works on the rows
 // {N2 n1 + n2 : n1} = {N2 k1 + n2 : k1} of a sub-sequence n2, step 2 on the rows {N2 t + k} of block t: both write back
@@ -579,9 +710,20 @@ cudaError_t raise_smem(K kern) { return cudaFuncSetAttribute(kern, cudaFuncAttri
 
 // one field of colour `colour` (0 / 1), or of both (-1); valid[c] = "the cache holds the half-spectrum of colour c of the
 // current spins" (kept by the caller across calls; a Metropolis update of colour c clears valid[c])
+template <int N2X>
+cudaError_t launch_row_update(const FcParams &q, const MetropolisArgs &ma, dim3 grid, dim3 block, size_t smem, cudaStream_t st) {
+    const RoundKeys rk = make_round_keys(ma.seed_lo, ma.seed_hi);
+    if (ma.step_dev && ma.flip) return launch_pdl(fftc_row_update_kernel<N2X, 8, true, 1>, grid, block, smem, st, q, ma, rk);
+    if (ma.step_dev) return launch_pdl(fftc_row_update_kernel<N2X, 8, true, 0>, grid, block, smem, st, q, ma, rk);
+    if (ma.flip) return launch_pdl(fftc_row_update_kernel<N2X, 8, false, 1>, grid, block, smem, st, q, ma, rk);
+    return launch_pdl(fftc_row_update_kernel<N2X, 8, false, 0>, grid, block, smem, st, q, ma, rk);
+}
+
+// fuse != null (and colour 0 / 1): the x-inverse pass is replaced by the fused row kernel, which also takes the Metropolis
+// decision of the half-sweep and leaves the forward-transformed rows of the updated colour in Z (*zline = that colour)
 template <int N2>
-cudaError_t launch_fftc(FcParams p, float2 *C, size_t cache_elems, int colour, bool *valid, bool *configured, cudaStream_t st,
-                        uint64_t *launches) {
+cudaError_t launch_fftc(FcParams p, float2 *C, size_t cache_elems, int colour, bool *valid, int *zline, const MetropolisArgs *fuse,
+                        bool *configured, cudaStream_t st, uint64_t *launches) {
     constexpr int L = 16 * N2, N2X = N2 / 2 > 0 ? N2 / 2 : 1;
     static_assert(N2 >= 2, "L >= 32");
     // lines of 8 replica pairs (64-byte runs): four of them are 64 KB of shared memory at L = 256, three CTAs per SM
@@ -606,6 +748,10 @@ cudaError_t launch_fftc(FcParams p, float2 *C, size_t cache_elems, int colour, b
         if ((e = raise_smem(fftc_x_inverse_kernel<N2X, 0>)) != cudaSuccess) return e;
         if ((e = raise_smem(fftc_x_forward_kernel<N2X, 16>)) != cudaSuccess) return e;
         if ((e = raise_smem(fftc_x_inverse_kernel<N2X, 16>)) != cudaSuccess) return e;
+        if ((e = raise_smem(fftc_row_update_kernel<N2X, 8, false, 0>)) != cudaSuccess) return e;
+        if ((e = raise_smem(fftc_row_update_kernel<N2X, 8, false, 1>)) != cudaSuccess) return e;
+        if ((e = raise_smem(fftc_row_update_kernel<N2X, 8, true, 0>)) != cudaSuccess) return e;
+        if ((e = raise_smem(fftc_row_update_kernel<N2X, 8, true, 1>)) != cudaSuccess) return e;
         *configured = true;
     }
     const dim3 gx(p.P / LNX, L, 3), bx(LNX, TL), gy(p.PBZ, L / 2 + L / 4), by(p.LZ, 16, 2);
@@ -636,18 +782,30 @@ cudaError_t launch_fftc(FcParams p, float2 *C, size_t cache_elems, int colour, b
         if (colour >= 0 && colour != tc) continue;
         const int oc = 1 - tc;
         if (!valid[tc]) {                                  // the target colour's own half-spectrum is stale: refresh it alone
-            if ((e = x_forward(tc)) != cudaSuccess) break;
+            if (*zline != tc && (e = x_forward(tc)) != cudaSuccess) break;
             if ((e = y_pass(FC_FWD_ONLY, tc)) != cudaSuccess) break;
             valid[tc] = true;
+            *zline = -1;
         }
         if (!valid[oc]) {                                  // the running-sweep case: only the colour just updated is stale
-            if ((e = x_forward(oc)) != cudaSuccess) break;
+            if (*zline != oc && (e = x_forward(oc)) != cudaSuccess) break;   // (the fused row kernel has left its lines in Z)
             if ((e = y_pass(FC_FUSED, oc)) != cudaSuccess) break;
             valid[oc] = true;
         } else {
             if ((e = y_pass(FC_COMBINE, oc)) != cudaSuccess) break;
         }
-        e = x_inverse(tc);
+        *zline = -1;
+        if (fuse) {
+            FcParams q = p;
+            q.colour = tc;
+            ++*launches;
+            const size_t smu = sizeof(float2) * (2 * L + 3 * (size_t)line_rows<N2X>() * p.LZ);
+            e = launch_row_update<N2X>(q, *fuse, dim3(p.PBZ, L), dim3(p.LZ, TL, 3), smu, st);
+            valid[tc] = false;                             // the spins of colour tc have changed ...
+            *zline = tc;                                   // ... and their forward-transformed rows are in Z already
+        } else {
+            e = x_inverse(tc);
+        }
     }
     return e != cudaSuccess ? e : cudaGetLastError();
 }
@@ -676,8 +834,12 @@ cudaError_t launch_make_fft_table(const float *Wc, float *AB, void *scratch, int
     return cudaGetLastError();
 }
 
+bool dsmc_fft_fused_supported(int L, int R) { return dsmc_fft_supported(L, R) && R % 16 == 0; }
+
 cudaError_t launch_field_fft(const float *S, const float *AB, void *scratch, void *cache, float *H, int L, int R, int colour,
-                             bool *valid, bool *configured, cudaStream_t st, uint64_t *launches) {
+                             bool *valid, int *zline, const MetropolisArgs *fuse, bool *configured, cudaStream_t st,
+                             uint64_t *launches) {
+    if (fuse && (colour < 0 || !dsmc_fft_fused_supported(L, R))) return cudaErrorInvalidValue;
     FcParams p;
     p.S = S;
     p.H = H;
@@ -694,11 +856,11 @@ cudaError_t launch_field_fft(const float *S, const float *AB, void *scratch, voi
     p.colour = 0;
     const size_t ce = dsmc_fft_cache_elems(L, R);
     switch (L / 16) {
-        case 2: return launch_fftc<2>(p, (float2 *)cache, ce, colour, valid, configured, st, launches);
-        case 4: return launch_fftc<4>(p, (float2 *)cache, ce, colour, valid, configured, st, launches);
-        case 8: return launch_fftc<8>(p, (float2 *)cache, ce, colour, valid, configured, st, launches);
-        case 16: return launch_fftc<16>(p, (float2 *)cache, ce, colour, valid, configured, st, launches);
-        case 32: return launch_fftc<32>(p, (float2 *)cache, ce, colour, valid, configured, st, launches);
+        case 2: return launch_fftc<2>(p, (float2 *)cache, ce, colour, valid, zline, fuse, configured, st, launches);
+        case 4: return launch_fftc<4>(p, (float2 *)cache, ce, colour, valid, zline, fuse, configured, st, launches);
+        case 8: return launch_fftc<8>(p, (float2 *)cache, ce, colour, valid, zline, fuse, configured, st, launches);
+        case 16: return launch_fftc<16>(p, (float2 *)cache, ce, colour, valid, zline, fuse, configured, st, launches);
+        case 32: return launch_fftc<32>(p, (float2 *)cache, ce, colour, valid, zline, fuse, configured, st, launches);
     }
     return cudaErrorInvalidValue;
 }
