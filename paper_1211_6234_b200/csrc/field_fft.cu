@@ -321,7 +321,7 @@ __global__ void __launch_bounds__(256) fftc_x_inverse_kernel(const FcParams p) {
 //   grid (P / LN, L rows), block (LN, TL, 3 components); LN = the line width LZ (8 at config 5).
 // Phase B's items (site i, pair) are spread over all threads; every other phase works on component threadIdx.z.
 template <int N2X, int LNC, bool DEVSTEP, int FLIP>
-__global__ void __launch_bounds__(384) fftc_row_update_kernel(const FcParams p, const MetropolisArgs ma, const RoundKeys rk) {
+__global__ void __launch_bounds__(N2X >= 16 ? 384 : 192, N2X >= 16 ? 2 : 4) fftc_row_update_kernel(const FcParams p, const MetropolisArgs ma, const RoundKeys rk) {
     extern __shared__ __align__(16) float2 fsm[];
     constexpr int Lh = 16 * N2X, L = 2 * Lh;
     const int LN = nlanes<LNC>(), TL = blockDim.y;

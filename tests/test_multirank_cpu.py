@@ -34,7 +34,7 @@ def _worker(rank, world, port, out):
     allrows = multirank.gather_replica_rows(rows, 5)
     assert allrows.shape == (5, 8) and np.array_equal(allrows[:, 0], np.arange(5) + 0.25)
     dist.barrier()
-    out.put((rank, got, multirank.rank_seed(0x12116234, rank)))
+    out.put((rank, got, multirank.rank_seed(0x12116234, rank), multirank.rank_replica_offset(64, rank)))
     dist.destroy_process_group()
 
 
@@ -51,6 +51,9 @@ def test_two_ranks_max_and_seeds():
         assert p.exitcode == 0
     assert res[0][1] == res[1][1] == [15.0, 3.0]                 # max over ranks, identical everywhere
     assert res[0][2] != res[1][2]                                # independent chains per rank
+    assert (res[0][2] & 0xFFFFFFFF) == (res[1][2] & 0xFFFFFFFF) == 0x12116234   # ... that differ in the high word only
+    assert multirank.rank_seed(1000, 1) != multirank.rank_seed(2000, 0)          # no collision between base seeds
+    assert [res[0][3], res[1][3]] == [0, 64]                     # bench.py: one seed, disjoint replica indices
     # weak scaling: value = world x per-rank units / max time
     assert multirank.whole_job_rate(4_194_304, world, 0.015) == 2 * 4_194_304 / 0.015
 
