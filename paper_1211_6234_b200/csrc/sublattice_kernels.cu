@@ -451,19 +451,20 @@ __global__ void __launch_bounds__(kResThreads, 1) sublattice_resident_kernel(con
 constexpr int kIncThreads = 256;
 constexpr int kIncSpt = 16;       // sites per field thread
 
+constexpr int kIncDraw = 3;      // drawing warps
 __host__ __device__ constexpr size_t incremental_smem_bytes(int L, int NL) {
-    return (size_t)40 * L * L + 16 + 2 * sizeof(f2) * NL * NL * 3 + 64;
+    return (size_t)40 * L * L + 16 + 2 * sizeof(f2) * NL * NL * 3 + 64 * 2 * sizeof(int) + 64;
 }
 
 template <int NL, int LC>
-__global__ void __launch_bounds__(kIncThreads + 64, 1) sublattice_incremental_kernel(const MetropolisArgs p, const RoundKeys rk,
+__global__ void __launch_bounds__(kIncThreads + 32 * kIncDraw, 1) sublattice_incremental_kernel(const MetropolisArgs p, const RoundKeys rk,
                                                                                   const float *__restrict__ Wc,
                                                                                   float *__restrict__ Hio, int l_arg,
                                                                                   unsigned long long first_pass,
                                                                                   unsigned n_passes,
                                                                                   float *__restrict__ margin_log) {
     constexpr int NN = NL * NL;
-    constexpr int NT = kIncThreads + 64;                               // 8 field warps + 2 drawing warps
+    constexpr int NT = kIncThreads + 32 * kIncDraw;                    // 8 field warps + 3 drawing warps
     extern __shared__ __align__(16) unsigned char rsm[];
     const int L = LC > 0 ? LC : p.L, l = LC > 0 ? LC / NL : l_arg, Lh = L >> 1, R = p.R, N = L * L;
     float4 *Wsm = reinterpret_cast<float4 *>(rsm);                     // [N + 1]  (xx, xy, yy, zz) at rho = ry L + rx
@@ -471,7 +472,7 @@ __global__ void __launch_bounds__(kIncThreads + 64, 1) sublattice_incremental_ke
     float *Sf = reinterpret_cast<float *>(Ssm);
     f2 *hpub = Ssm + 3 * (size_t)N;                                    // [NN][3] field of the update sites
     float *dlf = reinterpret_cast<float *>(hpub + NN * 3);             // [NN][3][2] delta of the update sites (0 = rejected)
-    int *off = reinterpret_cast<int *>(dlf + NN * 6);                  // [2][2]: offsets of this and the next pass
+    int *offtab = reinterpret_cast<int *>(dlf + NN * 6);               // [64][2]: offsets of the passes it .. it + 63, slot it & 63
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int r0 = 2 * blockIdx.x, r1 = min(r0 + 1, R - 1);            // odd R: the last CTA carries its replica twice
     const size_t plane = (size_t)L * Lh * R;
@@ -505,9 +506,14 @@ __global__ void __launch_bounds__(kIncThreads + 64, 1) sublattice_incremental_ke
         }
     }
 
-    // Two drawing warps take the passes in turn: while one decides pass k, the other already runs Philox for pass
-    // k + 1 (its offset, then the trial spin and ln u of its sites: none of that depends on the state), so the serial
-    // part of a pass is only "read the neighbours, dE, accept".  Lanes: update site fk = lane >> 1, replica rb = lane & 1.
+    // Three drawing warps take the passes in turn.  The warp that decides pass k then has two whole passes to run Philox
+    // for pass k + 3 (the trial spins and ln u of its sites: none of that depends on the state); the offsets of the next
+    // 32-64 passes come from a table that one warp refills 32 at a time (one pass per lane), so the serial part of a
+    // pass is only "read the neighbours, dE, accept".  Lanes: update site fk = lane >> 1, replica rb = lane & 1.
+    // Barriers: A(it) = "h of this pass's sites is published", B(it) = "decisions and deltas of this pass are out":
+    // named barriers 1..8 (A and B of pass it & 3) over all threads.  A drawing warp syncs on the barriers of its own
+    // passes and only ARRIVES at those of the two passes in between (it has nothing to wait for there); four phases of
+    // barrier ids keep an early arrival from ever landing in a phase that is still open.
     const bool drawer = warp >= kIncThreads / 32;
     const int dw = warp - kIncThreads / 32;
     const bool flipper = drawer && lane < 2 * NN;
@@ -517,28 +523,30 @@ __global__ void __launch_bounds__(kIncThreads + 64, 1) sublattice_incremental_ke
     MetropolisArgs q = p;
     q.step_dev = nullptr;
     q.flip = 0;                                                        // the reversal move is applied at decision time
+    auto fill_offsets = [&](unsigned it0) {                            // passes it0 .. it0 + 31, one per lane
+        int ox, oy;
+        pass_offset(rk, first_pass + it0 + lane, l, ox, oy);
+        offtab[2 * ((it0 + lane) & 63)] = ox, offtab[2 * ((it0 + lane) & 63) + 1] = oy;
+    };
+    if (drawer && dw == 0) fill_offsets(0), fill_offsets(32);
+    __syncthreads();
     Draw dr = {0.0f, 0.0f, 0.0f, 0.0f};
     int my_ox = 0, my_oy = 0;
-    if (drawer && dw == 0) {                                           // the first pass's draw, before the loop
-        pass_offset(rk, first_pass, l, my_ox, my_oy);
-        if (lane == 0) off[0] = my_ox, off[1] = my_oy;
+    auto predraw = [&](unsigned it) {                                  // trial spins and ln u of pass `it`
+        my_ox = offtab[2 * (it & 63)], my_oy = offtab[2 * (it & 63) + 1];
+        const unsigned long long ps = first_pass + it;
         const int nt = (my_oy + l * (fk / NL)) * L + my_ox + l * (fk % NL);
-        const uint4 rnd = philox4x32_10(make_uint4((uint32_t)nt, (uint32_t)fr + p.r_off, (uint32_t)(first_pass & 0xFFFFFFFFull),
-                                                   (uint32_t)(first_pass >> 32) & 0x7FFFFFFFu), rk);
+        const uint4 rnd = philox4x32_10(make_uint4((uint32_t)nt, (uint32_t)fr + p.r_off, (uint32_t)(ps & 0xFFFFFFFFull),
+                                                   (uint32_t)(ps >> 32) & 0x7FFFFFFFu), rk);
         dr = draw_from_words(q, rnd, 0.0f, 0.0f, 0.0f);
-    }
-    __syncthreads();
+    };
+    auto bar_sync = [&](int id) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(NT) : "memory"); };
+    auto bar_arrive = [&](int id) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(NT) : "memory"); };
 
-    // Barriers: A(it) = "h of this pass's sites is published", B(it) = "decisions and deltas of this pass are out".
-    // Named barriers 1..4 (A and B of even / odd passes) over all threads; the warp that pre-draws only ARRIVES (it
-    // has nothing to wait for), so its Philox work spans the whole pass instead of sitting between the two barriers.
-    int pox = 0, poy = 0;                                              // field threads: the offsets of the pass before
-    for (unsigned it = 0; it < n_passes; ++it) {
-        const unsigned long long pass = first_pass + it;
-        const int cur = (int)(it & 1u);
-        const int idA = 1 + 2 * cur, idB = 2 + 2 * cur;
-        if (!drawer) {
-            const int ox = off[2 * cur], oy = off[2 * cur + 1];
+    if (!drawer) {
+        int pox = 0, poy = 0;                                          // the offsets of the pass before
+        for (unsigned it = 0; it < n_passes; ++it) {
+            const int ox = offtab[2 * (it & 63)], oy = offtab[2 * (it & 63) + 1];
             if (it > 0) {
                 // rank-n update of the field of this thread's sites by the moves of the pass before:
                 // h_t += W(c - t) . delta_c for the accepted c
@@ -588,11 +596,37 @@ __global__ void __launch_bounds__(kIncThreads + 64, 1) sublattice_incremental_ke
                 }
             }
             pox = ox, poy = oy;
-            asm volatile("bar.sync %0, %1;" ::"r"(idA), "r"(NT) : "memory");
-            asm volatile("bar.sync %0, %1;" ::"r"(idB), "r"(NT) : "memory");
-        } else if (dw == cur) {
+            bar_sync(1 + 2 * (int)(it & 3u));
+            bar_sync(2 + 2 * (int)(it & 3u));
+        }
+        // the moves of the last pass are still to be applied to the field that is handed back
+        if (n_passes > 0) {
+            const f2 *dl = reinterpret_cast<const f2 *>(dlf);
+#pragma unroll 1
+            for (int k = 0; k < NN; ++k) {
+                const f2 dxp = dl[3 * k], dyp = dl[3 * k + 1], dzp = dl[3 * k + 2];
+                if ((dxp | dyp | dzp) == 0ull) continue;
+                const int xc = pox + l * (k % NL), yc = poy + l * (k / NL);
+#pragma unroll
+                for (int j = 0; j < kIncSpt; ++j) {
+                    if (txy[j] < 0) continue;
+                    int rx = xc - (txy[j] & 0xFFFF), ry = yc - (txy[j] >> 16);
+                    rx += rx < 0 ? L : 0;
+                    ry += ry < 0 ? L : 0;
+                    const float4 w = Wsm[ry * L + rx];
+                    h[j][0] = f2_fma(f2_bc(w.x), dxp, f2_fma(f2_bc(w.y), dyp, h[j][0]));
+                    h[j][1] = f2_fma(f2_bc(w.y), dxp, f2_fma(f2_bc(w.z), dyp, h[j][1]));
+                    h[j][2] = f2_fma(f2_bc(w.w), dzp, h[j][2]);
+                }
+            }
+        }
+    } else {
+        // the passes before this warp's first one: nothing to wait for
+        for (unsigned it = 0; it < (unsigned)dw && it < n_passes; ++it) bar_arrive(1 + 2 * (int)(it & 3u)), bar_arrive(2 + 2 * (int)(it & 3u));
+        if ((unsigned)dw < n_passes) predraw((unsigned)dw);
+        for (unsigned it = (unsigned)dw; it < n_passes; it += kIncDraw) {
+            bar_sync(1 + 2 * (int)(it & 3u));
             // the deciding warp: everything that depends on the state, after the barrier that orders it behind the pass before
-            asm volatile("bar.sync %0, %1;" ::"r"(idA), "r"(NT) : "memory");
             if (flipper) {
                 const int xt = my_ox + l * (fk % NL), yt = my_oy + l * (fk / NL);
                 const int nt = yt * L + xt;
@@ -622,45 +656,16 @@ __global__ void __launch_bounds__(kIncThreads + 64, 1) sublattice_incremental_ke
                     if (margin_log) margin_log[((size_t)it * R + fr) * NN + fk] = tr.margin;
                 }
             }
-            asm volatile("bar.sync %0, %1;" ::"r"(idB), "r"(NT) : "memory");
-        } else {
-            // the pre-drawing warp: Philox for the next pass; its offset has to be out before B(it)
-            asm volatile("bar.arrive %0, %1;" ::"r"(idA), "r"(NT) : "memory");
-            const bool more = it + 1 < n_passes;
-            if (more) {
-                pass_offset(rk, pass + 1, l, my_ox, my_oy);            // every lane computes the (same) offset: no divergence
-                if (lane == 0) off[2 * (cur ^ 1)] = my_ox, off[2 * (cur ^ 1) + 1] = my_oy;
+            bar_sync(2 + 2 * (int)(it & 3u));
+            // the two passes the other drawing warps decide
+            for (unsigned j = it + 1; j < it + kIncDraw && j < n_passes; ++j) bar_arrive(1 + 2 * (int)(j & 3u)), bar_arrive(2 + 2 * (int)(j & 3u));
+            // refill duty: whoever decided the first pass of a block of 32 computes the offsets of the block after the next
+            // (the table holds passes it .. it + 63 then; the slots it overwrites belong to passes that are done)
+            if ((it & 31u) == 0u && it > 0u) {
+                fill_offsets(it + 32u);
                 __threadfence_block();
             }
-            asm volatile("bar.arrive %0, %1;" ::"r"(idB), "r"(NT) : "memory");
-            if (more) {
-                const int nt = (my_oy + l * (fk / NL)) * L + my_ox + l * (fk % NL);
-                const unsigned long long np = pass + 1;
-                const uint4 rnd = philox4x32_10(make_uint4((uint32_t)nt, (uint32_t)fr + p.r_off, (uint32_t)(np & 0xFFFFFFFFull),
-                                                           (uint32_t)(np >> 32) & 0x7FFFFFFFu), rk);
-                dr = draw_from_words(q, rnd, 0.0f, 0.0f, 0.0f);
-            }
-        }
-    }
-    // the moves of the last pass are still to be applied to the field that is handed back
-    if (!drawer && n_passes > 0) {
-        const f2 *dl = reinterpret_cast<const f2 *>(dlf);
-#pragma unroll 1
-        for (int k = 0; k < NN; ++k) {
-            const f2 dxp = dl[3 * k], dyp = dl[3 * k + 1], dzp = dl[3 * k + 2];
-            if ((dxp | dyp | dzp) == 0ull) continue;
-            const int xc = pox + l * (k % NL), yc = poy + l * (k / NL);
-#pragma unroll
-            for (int j = 0; j < kIncSpt; ++j) {
-                if (txy[j] < 0) continue;
-                int rx = xc - (txy[j] & 0xFFFF), ry = yc - (txy[j] >> 16);
-                rx += rx < 0 ? L : 0;
-                ry += ry < 0 ? L : 0;
-                const float4 w = Wsm[ry * L + rx];
-                h[j][0] = f2_fma(f2_bc(w.x), dxp, f2_fma(f2_bc(w.y), dyp, h[j][0]));
-                h[j][1] = f2_fma(f2_bc(w.y), dxp, f2_fma(f2_bc(w.z), dyp, h[j][1]));
-                h[j][2] = f2_fma(f2_bc(w.w), dzp, h[j][2]);
-            }
+            if (it + kIncDraw < n_passes) predraw(it + kIncDraw);
         }
     }
     __syncthreads();
@@ -765,7 +770,7 @@ cudaError_t launch_sublattice_incremental(const MetropolisArgs &a, const float *
     else if (nl == 4) kern = a.L == 64 ? sublattice_incremental_kernel<4, 64> : sublattice_incremental_kernel<4, 0>;
     else kern = a.L == 64 ? sublattice_incremental_kernel<1, 64> : sublattice_incremental_kernel<1, 0>;
     if (cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024)) return e;
-    kern<<<(unsigned)((a.R + 1) / 2), kIncThreads + 64, smem, st>>>(a, rk, Wc, H, l, first_pass, (unsigned)n_passes, margin_log);
+    kern<<<(unsigned)((a.R + 1) / 2), kIncThreads + 32 * kIncDraw, smem, st>>>(a, rk, Wc, H, l, first_pass, (unsigned)n_passes, margin_log);
     ++*launches;
     return cudaGetLastError();
 }
