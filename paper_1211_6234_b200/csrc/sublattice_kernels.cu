@@ -520,9 +520,6 @@ __global__ void __launch_bounds__(kIncThreads + 32 * kIncDraw, 1) sublattice_inc
     const int fk = lane >> 1, rb = lane & 1, fr = rb ? r1 : r0;
     float invT = 0.0f, K2 = 0.0f, K4 = 0.0f;
     if (flipper) invT = p.invT[fr], K2 = p.K2[fr], K4 = p.K4[fr];
-    MetropolisArgs q = p;
-    q.step_dev = nullptr;
-    q.flip = 0;                                                        // the reversal move is applied at decision time
     auto fill_offsets = [&](unsigned it0) {                            // passes it0 .. it0 + 31, one per lane
         int ox, oy;
         pass_offset(rk, first_pass + it0 + lane, l, ox, oy);
@@ -538,7 +535,8 @@ __global__ void __launch_bounds__(kIncThreads + 32 * kIncDraw, 1) sublattice_inc
         const int nt = (my_oy + l * (fk / NL)) * L + my_ox + l * (fk % NL);
         const uint4 rnd = philox4x32_10(make_uint4((uint32_t)nt, (uint32_t)fr + p.r_off, (uint32_t)(ps & 0xFFFFFFFFull),
                                                    (uint32_t)(ps >> 32) & 0x7FFFFFFFu), rk);
-        dr = draw_from_words(q, rnd, 0.0f, 0.0f, 0.0f);
+        sphere_point(rnd.x, rnd.y, dr.tx, dr.ty, dr.tz);              // (the reversal move replaces it at decision time)
+        dr.lnu = __logf(unit24(rnd.z));
     };
     auto bar_sync = [&](int id) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(NT) : "memory"); };
     auto bar_arrive = [&](int id) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(NT) : "memory"); };
@@ -640,7 +638,7 @@ __global__ void __launch_bounds__(kIncThreads + 32 * kIncDraw, 1) sublattice_inc
                 const float nz = (se[4] + sw[4]) + (sn[4] + ss[4]);
                 if (p.flip) dr.tx = -sx, dr.ty = -sy, dr.tz = -sz;     // Ising move of App. B: complete reversal
                 const float *pf = reinterpret_cast<const float *>(hpub) + rb;
-                const Trial tr = decide_drawn(q, dr, sx, sy, sz, nx, ny, nz, pf[6 * fk], pf[6 * fk + 2], pf[6 * fk + 4], invT, K2, K4);
+                const Trial tr = decide_drawn(p, dr, sx, sy, sz, nx, ny, nz, pf[6 * fk], pf[6 * fk + 2], pf[6 * fk + 4], invT, K2, K4);
                 const bool live = r0 + rb < R;                         // the duplicate of an odd R's last replica stays silent
                 float dx = 0.0f, dy = 0.0f, dz = 0.0f;
                 if (tr.acc) {
