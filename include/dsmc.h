@@ -270,6 +270,26 @@ int dsmc_field_kernel_supported(dsmc_ctx *ctx, int kind);
  * bench.py reports beside the derived SMs x 128 lanes x 2 x clock figure.  Synchronises.          */
 int dsmc_fp32_fma_peak(dsmc_ctx *ctx, double *tflops_out);
 
+/* The domain-wall counts of eq. 14 (the counts_out of dsmc_wall_observables, bit for bit) for callers
+ * that cannot allocate device memory: code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc.  Context-free: no dsmc_ctx, no workspace, no cudaMalloc / cudaFree / allocating library call.
+ *   s_dev       DEVICE, canonical s[R][3][L][L] fp32 (read only; the caller's)
+ *   counts_dev  DEVICE, [R][6] long long = n_h^x, n_v^x, n_h^y, n_v^y, n_h^z, n_v^z (written; the caller's)
+ *   cuda_stream a cudaStream_t passed as void* (NULL = default stream); the call is asynchronous on it
+ *   err         nullable HOST buffer of err_len bytes that receives the message of a refused call
+ * Both pointers must be memory of the CURRENT device (else DSMC_EINVAL).  The per-CTA partial sums of the reduction
+ * live in a static device array inside the library (1 MiB + 4 KiB on every GPU that loads it, held until the process
+ * exits), which sets the limits: R <= DSMC_NOALLOC_MAX_R, L even, 4 <= L <= DSMC_NOALLOC_MAX_L; anything larger is
+ * refused with DSMC_EINVAL and a message, nothing is launched.  Every call on a GPU shares that one array (it keeps the
+ * last call's contents; the call clears what must start at zero with a memset node on the stream): calls that OVERLAP on
+ * the same GPU -- two streams, two threads -- race and give wrong counts; calls ordered on one stream, or otherwise
+ * serialised, are safe.  The first call with a given device current looks the array's device address up
+ * (cudaGetSymbolAddress); make that call outside stream capture.                                            */
+#define DSMC_NOALLOC_MAX_R 1024
+#define DSMC_NOALLOC_MAX_L 4096
+int dsmc_wall_counts_noalloc(const float *s_dev, int L, int R, long long *counts_dev, void *cuda_stream, char *err,
+                             size_t err_len);
+
 int dsmc_destroy(dsmc_ctx *ctx);
 const char *dsmc_last_error(dsmc_ctx *ctx);
 const char *dsmc_version(void);

@@ -7,7 +7,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdsmc.so")
 SOURCES = ["dsmc_api.cu", "tensor_kernels.cu", "state_kernels.cu", "metropolis_kernels.cu", "sublattice_kernels.cu",
-           "field_generic.cu", "field_tiled.cu", "field_fft.cu", "peak_kernels.cu"]
+           "field_generic.cu", "field_tiled.cu", "field_fft.cu", "peak_kernels.cu", "wall_counts_noalloc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--shared", "-cudart", "static", "--threads", "0"]
 

@@ -59,6 +59,7 @@ ABI = [
     ("dsmc_select_field_kernel", _i, [_vp, _i]),
     ("dsmc_field_kernel_supported", _i, [_vp, _i]),
     ("dsmc_fp32_fma_peak", _i, [_vp, _vp]),
+    ("dsmc_wall_counts_noalloc", _i, [_vp, _i, _i, _vp, _vp, ctypes.c_char_p, _sz]),
     ("dsmc_destroy", _i, [_vp]),
     ("dsmc_last_error", ctypes.c_char_p, [_vp]),
     ("dsmc_version", ctypes.c_char_p, []),
@@ -93,6 +94,28 @@ def _np_f32(a, shape=None):
     if shape is not None and tuple(a.shape) != tuple(shape):
         raise ValueError(f"expected shape {shape}, got {a.shape}")
     return a
+
+
+def wall_counts_noalloc(s, counts, stream=None):
+    """dsmc_wall_counts_noalloc: eq. 14 wall counts of s (torch CUDA float32 [R][3][L][L]) into counts (torch CUDA
+    int64 [R][6]) with no device allocation anywhere in the call (scratch = a static device array in the library;
+    limits DSMC_NOALLOC_MAX_R / _L in include/dsmc.h).  Asynchronous on `stream` (default: torch's current stream);
+    calls that overlap on one GPU race."""
+    import torch
+    lib = load_library()
+    if not (isinstance(s, torch.Tensor) and s.is_cuda and s.is_contiguous() and s.dtype == torch.float32 and s.dim() == 4
+            and s.shape[1] == 3 and s.shape[2] == s.shape[3]):
+        raise TypeError("s: expected a contiguous CUDA float32 tensor [R][3][L][L]")
+    R, L = int(s.shape[0]), int(s.shape[2])
+    if not (isinstance(counts, torch.Tensor) and counts.is_cuda and counts.is_contiguous() and counts.dtype == torch.int64
+            and tuple(counts.shape) == (R, 6) and counts.device == s.device):
+        raise TypeError(f"counts: expected a contiguous CUDA int64 tensor [{R}][6] on {s.device}")
+    err = ctypes.create_string_buffer(256)
+    with torch.cuda.device(s.device):
+        st = stream if stream is not None else torch.cuda.current_stream(s.device)
+        rc = lib.dsmc_wall_counts_noalloc(s.data_ptr(), L, R, counts.data_ptr(), st.cuda_stream, err, len(err))
+    if rc != 0:
+        raise DsmcError(f"dsmc error {rc}: {err.value.decode()}")
 
 
 class Dsmc:
