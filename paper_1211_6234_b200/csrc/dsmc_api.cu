@@ -115,7 +115,7 @@ int run_field(dsmc_ctx *ctx, int colour, int kind_override = -1) {
     const int kind = kind_override >= 0 ? kind_override : field_kind(ctx);
     if (kind == 2) {
         e = launch_field_fft(ctx->S(), ctx->M(), ctx->Z(), ctx->C(), ctx->H(), ctx->L, ctx->R, colour, ctx->spec_valid,
-                             &ctx->zline, nullptr, &ctx->fft_configured, ctx->stream, &ctx->launches);
+                             &ctx->zline, nullptr, 0, 0, nullptr, &ctx->fft_configured, ctx->stream, &ctx->launches);
     } else {
         for (int q = 0; q < 2 && e == cudaSuccess; ++q) {
             if (colour >= 0 && colour != q) continue;
@@ -194,8 +194,8 @@ int enqueue_halfsweep(dsmc_ctx *ctx, const MetropolisArgs &a, int flags) {
                        !ctx->timing && !(flags & DSMC_REUSE_FIELD) && !ctx->no_fuse;
     if (fused) {
         const cudaError_t e = launch_field_fft(ctx->S(), ctx->M(), ctx->Z(), ctx->C(), ctx->H(), ctx->L, ctx->R, colour,
-                                               ctx->spec_valid, &ctx->zline, &a, &ctx->fft_configured, ctx->stream,
-                                               &ctx->launches);
+                                               ctx->spec_valid, &ctx->zline, &a, ctx->fft_pb0, ctx->fft_npb, ctx->fft_SG,
+                                               &ctx->fft_configured, ctx->stream, &ctx->launches);
         if (e != cudaSuccess) return cuda_fail(ctx, e, "fused FFT half-sweep launch");
         ctx->field_valid[colour] = false;                       // h of this half-sweep never reached the field array
         return DSMC_OK;
@@ -220,6 +220,11 @@ int enqueue_halfsweep(dsmc_ctx *ctx, const MetropolisArgs &a, int flags) {
 void drop_sweep_graph(dsmc_ctx *ctx) {
     if (ctx->sweep_graph) cudaGraphExecDestroy(ctx->sweep_graph);
     ctx->sweep_graph = nullptr;
+    for (int b = 0; b < DSMC_MAX_BRANCHES - 1; ++b) {
+        if (ctx->branch_graph[b]) cudaGraphExecDestroy(ctx->branch_graph[b]);
+        ctx->branch_graph[b] = nullptr;
+    }
+    ctx->graph_branches = 1;
     if (ctx->pass_graph) cudaGraphExecDestroy(ctx->pass_graph);
     ctx->pass_graph = nullptr;
 }
@@ -334,52 +339,86 @@ int build_sweep_graph(dsmc_ctx *ctx, uint64_t seed, int flags, int record_every)
     drop_sweep_graph(ctx);
     if (!ctx->capture_stream)
         CU(cudaStreamCreateWithFlags(&ctx->capture_stream, cudaStreamNonBlocking), "capture stream");
+    // Fused FFT path in its running state (y pass + fused row kernel per half-sweep): the line blocks of 16 replicas
+    // never exchange data, so the sweeps are captured as up to DSMC_MAX_BRANCHES independent chains, one graph each with
+    // its own step counter, which dsmc_run replays side by side on streams of the context's own between a fork and a
+    // join event.  A chain's y pass (bound by L2 traffic) then overlaps another chain's row kernel (bound by instruction
+    // issue) and no launch waits for the tail of a grid it does not depend on.  Same kernels on the same data: the
+    // trajectory does not change.  (One graph with parallel branches was measured too and gained a third of what
+    // separate graphs on separate streams gain.)
+    const int blocks = dsmc_fft_line_blocks(ctx->L, ctx->R);
+    int branches = 1;
+    // (measured: a gain from L = 64 up -- 10-20 % where the working set fits the L2 -- and a loss of 5 % at L = 32)
+    if (kind == 2 && blocks > 1 && ctx->L >= 64 && record_every == 0 && !ctx->no_fuse && !ctx->timing && ctx->zline >= 0 &&
+        ctx->spec_valid[1 - ctx->zline] && !ctx->spec_valid[ctx->zline])
+        for (int b = 2; b <= ctx->max_branches; ++b)
+            if (blocks % b == 0) branches = b;
+    for (int b = 0; b + 1 < branches; ++b) {
+        if (!ctx->branch_stream[b])
+            CU(cudaStreamCreateWithFlags(&ctx->branch_stream[b], cudaStreamNonBlocking), "branch stream");
+        if (!ctx->ev_join[b]) CU(cudaEventCreateWithFlags(&ctx->ev_join[b], cudaEventDisableTiming), "join event");
+    }
+    if (branches > 1 && !ctx->ev_fork) CU(cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming), "fork event");
     cudaStream_t saved = ctx->stream;
     const uint64_t l0 = ctx->launches;
-    ctx->stream = ctx->capture_stream;
-    cudaGraph_t graph = nullptr;
-    cudaError_t e = cudaStreamBeginCapture(ctx->capture_stream, cudaStreamCaptureModeThreadLocal);
+    const int n_sweeps = record_every > 0 ? record_every : DSMC_GRAPH_UNROLL;
+    int spec_out = spec_in;
     int rc = DSMC_OK;
-    if (e == cudaSuccess) {
-        const int n_sweeps = record_every > 0 ? record_every : DSMC_GRAPH_UNROLL;
-        for (int rep = 0; rep < n_sweeps && rc == DSMC_OK && e == cudaSuccess; ++rep) {
-            for (int colour = 0; colour < 2 && rc == DSMC_OK; ++colour) {
-                MetropolisArgs a = metropolis_args(ctx, colour, seed, 0, flags, nullptr, nullptr);
-                a.step_dev = ctx->step_dev();
-                a.step_off = (uint32_t)(2 * rep + colour);  // the counter moves once per graph, not once per sweep
-                rc = enqueue_halfsweep(ctx, a, flags);
-            }
+    cudaError_t e = cudaSuccess;
+    const char *what = "sweep graph capture";
+    for (int b = 0; b < branches && rc == DSMC_OK && e == cudaSuccess; ++b) {
+        ctx->stream = ctx->capture_stream;
+        ctx->spec_valid[0] = spec_in & 1;                       // every chain starts from the state before the capture
+        ctx->spec_valid[1] = (spec_in & 2) != 0;
+        ctx->zline = (spec_in >> 2) - 1;
+        if (branches > 1) {
+            ctx->fft_pb0 = b * (blocks / branches);
+            ctx->fft_npb = blocks / branches;
+            ctx->fft_SG = ctx->stage();                         // the chains work on the block-major copy (replay_sweep_graph)
         }
-        if (e == cudaSuccess && rc == DSMC_OK)
-            e = launch_step_update(ctx->step_dev(), 2 * (uint64_t)n_sweeps, 1, ctx->stream, &ctx->launches);
-        if (e == cudaSuccess && rc == DSMC_OK && record_every > 0) rc = enqueue_record(ctx);
-        cudaError_t e2 = cudaStreamEndCapture(ctx->capture_stream, &graph);
-        if (e == cudaSuccess) e = e2;
+        cudaGraph_t graph = nullptr;
+        e = cudaStreamBeginCapture(ctx->capture_stream, cudaStreamCaptureModeThreadLocal);
+        if (e == cudaSuccess) {
+            for (int rep = 0; rep < n_sweeps && rc == DSMC_OK; ++rep) {
+                for (int colour = 0; colour < 2 && rc == DSMC_OK; ++colour) {
+                    MetropolisArgs a = metropolis_args(ctx, colour, seed, 0, flags, nullptr, nullptr);
+                    a.step_dev = ctx->step_dev() + b;
+                    a.step_off = (uint32_t)(2 * rep + colour);  // the counter moves once per graph, not once per sweep
+                    rc = enqueue_halfsweep(ctx, a, flags);
+                }
+            }
+            if (rc == DSMC_OK)
+                e = launch_step_update(ctx->step_dev() + b, 2 * (uint64_t)n_sweeps, 1, ctx->stream, &ctx->launches);
+            if (e == cudaSuccess && rc == DSMC_OK && record_every > 0) rc = enqueue_record(ctx);
+            cudaError_t e2 = cudaStreamEndCapture(ctx->capture_stream, &graph);
+            if (e == cudaSuccess) e = e2;
+        }
+        spec_out = (ctx->spec_valid[0] ? 1 : 0) | (ctx->spec_valid[1] ? 2 : 0) | ((ctx->zline + 1) << 2);
+        if (rc == DSMC_OK && e == cudaSuccess) {
+            what = "sweep graph instantiate";
+            e = cudaGraphInstantiate(b == 0 ? &ctx->sweep_graph : &ctx->branch_graph[b - 1], graph, 0);
+        }
+        if (graph) cudaGraphDestroy(graph);
     }
     ctx->stream = saved;
+    ctx->fft_pb0 = ctx->fft_npb = 0;
+    ctx->fft_SG = nullptr;
     ctx->graph_launches = ctx->launches - l0;
     ctx->launches = l0;
-    const int spec_out = (ctx->spec_valid[0] ? 1 : 0) | (ctx->spec_valid[1] ? 2 : 0) | ((ctx->zline + 1) << 2);
     ctx->spec_valid[0] = spec_in & 1;                           // nothing has run: back to the state before the capture
     ctx->spec_valid[1] = (spec_in & 2) != 0;
     ctx->zline = (spec_in >> 2) - 1;
     if (rc == DSMC_OK && e == cudaSuccess && spec_out != spec_in) {
-        if (graph) cudaGraphDestroy(graph);
+        drop_sweep_graph(ctx);
         return fail(ctx, DSMC_ESTATE, "internal: a captured sweep does not return to the spectrum state it started from");
     }
     if (rc != DSMC_OK) {
-        if (graph) cudaGraphDestroy(graph);
+        drop_sweep_graph(ctx);
         return rc;
     }
     if (e != cudaSuccess) {
-        if (graph) cudaGraphDestroy(graph);
-        return cuda_fail(ctx, e, "sweep graph capture");
-    }
-    e = cudaGraphInstantiate(&ctx->sweep_graph, graph, 0);
-    cudaGraphDestroy(graph);
-    if (e != cudaSuccess) {
-        ctx->sweep_graph = nullptr;
-        return cuda_fail(ctx, e, "sweep graph instantiate");
+        drop_sweep_graph(ctx);
+        return cuda_fail(ctx, e, what);
     }
     ctx->graph_seed = seed;
     ctx->graph_kind = kind;
@@ -387,6 +426,37 @@ int build_sweep_graph(dsmc_ctx *ctx, uint64_t seed, int flags, int record_every)
     ctx->graph_every = record_every;
     ctx->graph_spec_in = spec_in;
     ctx->graph_spec_out = spec_out;
+    ctx->graph_branches = branches;
+    return DSMC_OK;
+}
+
+// replay the captured sweeps `reps` times from step `step`: one chain on the context's stream, or the chains of the fused
+// FFT path side by side (build_sweep_graph) -- the others on the context's branch streams, forked from and joined back
+// into its stream, so that the call keeps plain stream order towards everything before and after it
+int replay_sweep_graph(dsmc_ctx *ctx, uint64_t step, uint64_t reps) {
+    const int nb = ctx->graph_branches;
+    for (int b = 0; b < nb; ++b)
+        CU(launch_step_update(ctx->step_dev() + b, step, 0, ctx->stream, &ctx->launches), "step counter");
+    // The chains work on a block-major copy of the spins (in the host-transfer staging area, idle during a run): a chain's
+    // 16 replicas are 64 bytes of every 256-byte site record of S, and chains that drift apart would fetch and write back
+    // half cache lines at different times; in the copy every chain's spins are dense.  Measured at config 5, four chains:
+    // 101.0 us per sweep on S, 91.3 on the copy (one chain: 103.6 either way).
+    if (nb > 1) {
+        CU(launch_spin_blocks(ctx->S(), ctx->stage(), ctx->L, ctx->R, true, ctx->stream, &ctx->launches), "spins to blocks");
+        CU(cudaEventRecord(ctx->ev_fork, ctx->stream), "fork event");
+    }
+    for (int b = 1; b < nb; ++b) CU(cudaStreamWaitEvent(ctx->branch_stream[b - 1], ctx->ev_fork, 0), "fork wait");
+    for (uint64_t j = 0; j < reps; ++j)
+        for (int b = 0; b < nb; ++b)
+            CU(cudaGraphLaunch(b == 0 ? ctx->sweep_graph : ctx->branch_graph[b - 1], b == 0 ? ctx->stream : ctx->branch_stream[b - 1]),
+               "sweep graph launch");
+    for (int b = 1; b < nb; ++b) {
+        CU(cudaEventRecord(ctx->ev_join[b - 1], ctx->branch_stream[b - 1]), "join event");
+        CU(cudaStreamWaitEvent(ctx->stream, ctx->ev_join[b - 1], 0), "join wait");
+    }
+    if (nb > 1)
+        CU(launch_spin_blocks(ctx->S(), ctx->stage(), ctx->L, ctx->R, false, ctx->stream, &ctx->launches), "blocks to spins");
+    ctx->launches += reps * ctx->graph_launches;
     return DSMC_OK;
 }
 
@@ -437,6 +507,10 @@ int dsmc_create(dsmc_ctx **out, int L, int R, float J, float g, float K2, float 
     c->T.assign(R, 0.0f);
     c->lay = dsmc_make_layout(L, R);
     if (const char *v = getenv("DSMC_NO_FUSE")) c->no_fuse = v[0] && v[0] != '0';
+    if (const char *v = getenv("DSMC_BRANCHES")) {
+        const int n = atoi(v);
+        if (n >= 1 && n <= DSMC_MAX_BRANCHES) c->max_branches = n;
+    }
     *out = c;
     return DSMC_OK;
 }
@@ -732,9 +806,7 @@ int dsmc_run_ex(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t first_ste
         const uint64_t reps = (n_half - k) / (2 * DSMC_GRAPH_UNROLL);
         if (reps >= 1) {
             if (int rc = build_sweep_graph(ctx, seed, flags, 0)) return rc;
-            CU(launch_step_update(ctx->step_dev(), first_step + k, 0, ctx->stream, &ctx->launches), "step counter");
-            for (uint64_t j = 0; j < reps; ++j) CU(cudaGraphLaunch(ctx->sweep_graph, ctx->stream), "sweep graph launch");
-            ctx->launches += reps * ctx->graph_launches;
+            if (int rc = replay_sweep_graph(ctx, first_step + k, reps)) return rc;
             ctx->field_valid[0] = ctx->field_valid[1] = true;
             ctx->spec_valid[0] = ctx->graph_spec_out & 1;           // (= the state the graph started from)
             ctx->spec_valid[1] = (ctx->graph_spec_out & 2) != 0;
@@ -857,10 +929,7 @@ int dsmc_run_recorded(dsmc_ctx *ctx, const float *T, uint64_t seed, uint64_t fir
     if (every <= 2 * DSMC_GRAPH_UNROLL && n_records - done >= 4 && !ctx->timing) {
         if (int rc = build_sweep_graph(ctx, seed, flags, every)) return rc;
         const uint64_t reps = n_records - done;
-        CU(launch_step_update(ctx->step_dev(), first_step + 2 * (uint64_t)every * done, 0, ctx->stream, &ctx->launches),
-           "step counter");
-        for (uint64_t j = 0; j < reps; ++j) CU(cudaGraphLaunch(ctx->sweep_graph, ctx->stream), "record graph launch");
-        ctx->launches += reps * ctx->graph_launches;
+        if (int rc = replay_sweep_graph(ctx, first_step + 2 * (uint64_t)every * done, reps)) return rc;
         ctx->field_valid[0] = ctx->field_valid[1] = true;
         ctx->spec_valid[0] = ctx->graph_spec_out & 1;
         ctx->spec_valid[1] = (ctx->graph_spec_out & 2) != 0;
@@ -946,6 +1015,11 @@ int dsmc_destroy(dsmc_ctx *ctx) {
         if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
     drop_sweep_graph(ctx);
     if (ctx->capture_stream) cudaStreamDestroy(ctx->capture_stream);
+    for (int b = 0; b < DSMC_MAX_BRANCHES - 1; ++b) {
+        if (ctx->branch_stream[b]) cudaStreamDestroy(ctx->branch_stream[b]);
+        if (ctx->ev_join[b]) cudaEventDestroy(ctx->ev_join[b]);
+    }
+    if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
     delete ctx;
     return DSMC_OK;
 }

@@ -21,6 +21,7 @@
 // ---------------------------------------------------------------------------------------------
 
 #define DSMC_GRAPH_UNROLL 8  // sweeps (dsmc_run) or passes (dsmc_sublattice_run) per captured CUDA graph
+#define DSMC_MAX_BRANCHES 8  // independent chains of replica groups in the sweep graph of the fused FFT path
 #define DSMC_KS_MAX 16  // maximum source split (partial-field slabs) of the tiled field kernel
 #define DSMC_TILED_MAX_L 1024  // largest lattice the tiled kernel accepts: the size up to which its fp32 accumulation is
                                // tested to meet the field tolerances (include/dsmc.h, dsmc_select_field_kernel)
@@ -76,7 +77,7 @@ struct DsmcLayout {
     size_t off_stats;  // R*8*2 doubles: ensemble sums of x and x^2
     size_t off_opart;  // per-CTA partial sums of the observable walks (state_kernels.cu: deterministic reductions)
     size_t off_ticket; // 4 arrival counters of those walks (zero between launches)
-    size_t off_step;   // one 64-bit step counter (dsmc_run's graph replay)
+    size_t off_step;   // 64-bit step counters of dsmc_run's graph replay, one per chain (a 256-byte slot: DSMC_MAX_BRANCHES <= 32)
     size_t total;
 };
 
@@ -105,7 +106,14 @@ struct dsmc_ctx {
     uint64_t ensemble_n = 0;  // snapshots accumulated since dsmc_ensemble_reset
     // one sweep (2 x [field + Metropolis] + step advance) captured as a CUDA graph for dsmc_run
     cudaStream_t capture_stream = nullptr;
-    cudaGraphExec_t sweep_graph = nullptr;
+    // the fused FFT path replays its sweeps as up to DSMC_MAX_BRANCHES independent chains of line blocks (build_sweep_graph)
+    cudaStream_t branch_stream[DSMC_MAX_BRANCHES - 1] = {};
+    cudaEvent_t ev_fork = nullptr, ev_join[DSMC_MAX_BRANCHES - 1] = {};
+    int fft_pb0 = 0, fft_npb = 0;  // line-block range the next fused half-sweep is enqueued for (0, 0 = all)
+    float *fft_SG = nullptr;       // ... on the block-major copy of the spins (null: on S)
+    int graph_branches = 1;        // chains the captured sweeps consist of (sweep_graph, branch_graph[])
+    int max_branches = DSMC_MAX_BRANCHES;  // DSMC_BRANCHES=n in the environment at dsmc_create (A/B timing; 1 = one chain)
+    cudaGraphExec_t sweep_graph = nullptr, branch_graph[DSMC_MAX_BRANCHES - 1] = {};
     uint64_t graph_seed = 0;
     int graph_kind = -1, graph_flags = -1, graph_every = -1;  // graph_every > 0: sweeps + record (dsmc_run_recorded)
     int graph_spec_in = -1, graph_spec_out = -1;  // spec_valid (bit c) the capture started from / ended with
@@ -176,8 +184,13 @@ cudaError_t launch_make_fft_table(const float *Wc, float *M, void *scratch, int 
 struct MetropolisArgs;
 bool dsmc_fft_fused_supported(int L, int R);
 cudaError_t launch_field_fft(const float *S, const float *AB, void *scratch, void *cache, float *H, int L, int R, int colour,
-                             bool *valid, int *zline, const MetropolisArgs *fuse, bool *configured, cudaStream_t st,
-                             uint64_t *launches);
+                             bool *valid, int *zline, const MetropolisArgs *fuse, int pb0, int npb, float *SG, bool *configured,
+                             cudaStream_t st, uint64_t *launches);
+// pb0, npb: with fuse, only the line blocks (16 replicas each) pb0 .. pb0 + npb - 1; npb = 0: all of them.  SG (only with a
+// proper sub-range): the spins are read and written in the block-major copy SG[pb][q][c][a][16 replicas] instead of S
+int dsmc_fft_line_blocks(int L, int R);
+// S -> SG (to_blocks) or SG -> S, all line blocks; R % 16 == 0
+cudaError_t launch_spin_blocks(float *S, float *SG, int L, int R, bool to_blocks, cudaStream_t st, uint64_t *launches);
 // configured: the context's "dynamic shared memory limit raised on this device" flag
 cudaError_t launch_field_tiled(const float *S, const float *Wk, float *Hpart, float *H, int L, int R,
                                int colour, int sm_count, bool *configured, cudaStream_t st, uint64_t *launches);

@@ -222,6 +222,8 @@ struct FcParams {
     const float2 *twf, *twi;  // twiddle tables, L entries each (behind AB in the workspace)
     int L, P;          // P = R / 2 complex replica pairs
     int LZ, PBZ;       // lanes per line and line blocks: P = PBZ * LZ
+    int pb0;           // y pass and fused row kernel: first line block of this launch (grid.x = line blocks it covers)
+    float *SG;         // fused row kernel: null, or the block-major copy of the spins SG[pb][q][c][a][lane] to work on
     int colour;        // x passes: the colour of the rows; y pass: the colour whose lines sit in Z / in Cnew
 };
 
@@ -331,7 +333,7 @@ __global__ void __launch_bounds__(N2X >= 16 ? 384 : 192, N2X >= 16 ? 2 : 4) fftc
     float2 *X0 = fsm + 2 * L;                              // three exchange buffers, also h / spins of the row by site
     const int xstride = line_rows<N2X>() * LN;
     float2 *buf = X0 + a * xstride;
-    const int pb = blockIdx.x, pair = pb * LN + lane, y = blockIdx.y, c = p.colour;
+    const int pb = blockIdx.x + p.pb0, y = blockIdx.y, c = p.colour;
     for (int j = tid; j < L; j += nthr) twi[j] = __ldg(p.twi + j), twf[j] = __ldg(p.twf + j);   // constant tables
     float2 *zline = p.Z + line_base(p, a, 0, pb) + (size_t)swz(y) * LN + lane;   // LN == p.LZ
     const unsigned sx_stride = (unsigned)(p.PBZ * L * LN);
@@ -366,20 +368,23 @@ __global__ void __launch_bounds__(N2X >= 16 ? 384 : 192, N2X >= 16 ? 2 : 4) fftc
     __syncthreads();
     // ---- B: Metropolis on the row (eq. 7; the half-sweep's frozen field is the h just computed)
     {
-        const int P = p.P;
-        const size_t planeP = (size_t)L * Lh * P;
-        f2 *S2 = reinterpret_cast<f2 *>(ma.S);
+        // the spins: the internal array (replica pairs of all line blocks side by side: runs of LN pairs = 64 bytes, P pairs
+        // apart) or, for a chain of the branched replay, the chain's line block in the block-major copy SG (dense)
+        const bool dense = p.SG != nullptr;
+        const int Pe = dense ? LN : p.P;
+        const size_t planeP = (size_t)L * Lh * Pe;
+        f2 *S2 = dense ? reinterpret_cast<f2 *>(p.SG) + (size_t)pb * 6 * planeP : reinterpret_cast<f2 *>(ma.S);
         const f2 *X2 = reinterpret_cast<const f2 *>(X0);
         f2 *X2w = reinterpret_cast<f2 *>(X0);
         const int yn = (y + 1 == L) ? 0 : y + 1, ys = (y == 0) ? L - 1 : y - 1;
-        const size_t own0 = (size_t)c * 3 * planeP + (size_t)y * Lh * P, oth = (size_t)(1 - c) * 3 * planeP;
-        const size_t o0 = oth + (size_t)y * Lh * P, on = oth + (size_t)yn * Lh * P, os = oth + (size_t)ys * Lh * P;
+        const size_t own0 = (size_t)c * 3 * planeP + (size_t)y * Lh * Pe, oth = (size_t)(1 - c) * 3 * planeP;
+        const size_t o0 = oth + (size_t)y * Lh * Pe, on = oth + (size_t)yn * Lh * Pe, os = oth + (size_t)ys * Lh * Pe;
         uint32_t step_lo = ma.step_lo, step_hi = ma.step_hi;
         if (DEVSTEP) step_words(ma, step_lo, step_hi);
         for (int item = tid; item < Lh * LN; item += nthr) {
             const int i = item / LN, ln = item - i * LN, pr = pb * LN + ln;
             const int i1 = odd_row ? (i + 1 == Lh ? 0 : i + 1) : (i == 0 ? Lh - 1 : i - 1);
-            const unsigned e = (unsigned)(i * P + pr), e1 = (unsigned)(i1 * P + pr);
+            const unsigned e = (unsigned)(i * Pe) + (dense ? ln : pr), e1 = (unsigned)(i1 * Pe) + (dense ? ln : pr);
             f2 s[3], nb[3], h[3];
 #pragma unroll
             for (int k = 0; k < 3; ++k) {
@@ -532,7 +537,7 @@ __global__ void __launch_bounds__(256, 3) fftc_y_kernel(const FcParams p) {
     float2 *twf = B0 + (MODE == FC_FWD_ONLY ? 2 : 4) * (size_t)line_elems, *twi = twf + L;
     uint64_t *bars = reinterpret_cast<uint64_t *>(twi + L);
     const int lane = threadIdx.x, t = threadIdx.y, j = threadIdx.z, tid = (j * 16 + t) * LZ + lane;
-    const int pb = blockIdx.x;
+    const int pb = blockIdx.x + p.pb0;
     const bool is_z = (int)blockIdx.y >= Lh;
     const int sx0 = is_z ? 2 * ((int)blockIdx.y - Lh) : (int)blockIdx.y;
     const int sx1 = is_z ? sx0 + 1 : sx0;
@@ -687,6 +692,19 @@ __global__ void twiddle_table_kernel(float2 *__restrict__ twf, float2 *__restric
     twi[j] = make_float2(cf, sf);
 }
 
+// The spins between the internal layout S[qc][a][P pairs] and the block-major copy SG[pb][qc][a][8 pairs] a chain of the
+// branched replay works on (dsmc_api.cu: replay_sweep_graph).  One thread per replica pair of one site.
+template <bool TO_BLOCKS>
+__global__ void __launch_bounds__(256) spin_blocks_kernel(float2 *__restrict__ S, float2 *__restrict__ SG, size_t sites6, int P) {
+    const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= sites6 * (size_t)P) return;
+    const size_t qa = t / (size_t)P;                            // (qc, a) flattened: qc * Nh + a
+    const int pair = (int)(t - qa * (size_t)P), pb = pair >> 3, ln = pair & 7;
+    float2 *blk = SG + ((size_t)pb * sites6 + qa) * 8 + ln;
+    if (TO_BLOCKS) *blk = S[t];
+    else S[t] = *blk;
+}
+
 int pairs_per_cta(int P, int cap) {
     int ln = 1;
     while (ln * 2 <= cap && P % (ln * 2) == 0) ln *= 2;
@@ -723,7 +741,7 @@ cudaError_t launch_row_update(const FcParams &q, const MetropolisArgs &ma, dim3 
 // decision of the half-sweep and leaves the forward-transformed rows of the updated colour in Z (*zline = that colour)
 template <int N2>
 cudaError_t launch_fftc(FcParams p, float2 *C, size_t cache_elems, int colour, bool *valid, int *zline, const MetropolisArgs *fuse,
-                        bool *configured, cudaStream_t st, uint64_t *launches) {
+                        int pb0, int npb, bool *configured, cudaStream_t st, uint64_t *launches) {
     constexpr int L = 16 * N2, N2X = N2 / 2 > 0 ? N2 / 2 : 1;
     static_assert(N2 >= 2, "L >= 32");
     // lines of 8 replica pairs (64-byte runs): four of them are 64 KB of shared memory at L = 256, three CTAs per SM
@@ -754,7 +772,23 @@ cudaError_t launch_fftc(FcParams p, float2 *C, size_t cache_elems, int colour, b
         if ((e = raise_smem(fftc_row_update_kernel<N2X, 8, true, 1>)) != cudaSuccess) return e;
         *configured = true;
     }
-    const dim3 gx(p.P / LNX, L, 3), bx(LNX, TL), gy(p.PBZ, L / 2 + L / 4), by(p.LZ, 16, 2);
+    // npb > 0: only the line blocks pb0 .. pb0 + npb - 1 (16 replicas each).  Line blocks never exchange data, so a
+    // running sweep can be cut into independent chains of launches (dsmc_api.cu: the branches of the sweep graph); the x
+    // passes have no such cut, so this needs the running-sweep state (y pass FC_FUSED + fused row kernel only).
+    const bool part = npb > 0 && !(pb0 == 0 && npb == p.PBZ);
+    if (fuse && p.LZ != 8) return cudaErrorInvalidValue;    // the fused row kernel is built for lines of 8 pairs
+    if (part) {
+        const int tc = colour, oc = 1 - colour;
+        if (!fuse || colour < 0 || pb0 < 0 || pb0 + npb > p.PBZ || !valid[tc] || valid[oc] || *zline != oc)
+            return cudaErrorInvalidValue;
+    }
+    if (p.SG && !part) return cudaErrorInvalidValue;        // the block-major spins are the chains' business only
+    if (part) {
+        p.pb0 = pb0;
+    } else {
+        npb = p.PBZ;
+    }
+    const dim3 gx(p.P / LNX, L, 3), bx(LNX, TL), gy(npb, L / 2 + L / 4), by(p.LZ, 16, 2);
     cudaError_t e = cudaSuccess;
     auto x_forward = [&](int c) {
         FcParams q = p;
@@ -800,7 +834,7 @@ cudaError_t launch_fftc(FcParams p, float2 *C, size_t cache_elems, int colour, b
             q.colour = tc;
             ++*launches;
             const size_t smu = sizeof(float2) * (2 * L + 3 * (size_t)line_rows<N2X>() * p.LZ);
-            e = launch_row_update<N2X>(q, *fuse, dim3(p.PBZ, L), dim3(p.LZ, TL, 3), smu, st);
+            e = launch_row_update<N2X>(q, *fuse, dim3(npb, L), dim3(p.LZ, TL, 3), smu, st);
             valid[tc] = false;                             // the spins of colour tc have changed ...
             *zline = tc;                                   // ... and their forward-transformed rows are in Z already
         } else {
@@ -835,10 +869,21 @@ cudaError_t launch_make_fft_table(const float *Wc, float *AB, void *scratch, int
 }
 
 bool dsmc_fft_fused_supported(int L, int R) { return dsmc_fft_supported(L, R) && R % 16 == 0; }
+// line blocks (16 replicas each) of the fused path: the units a running sweep can be cut into (launch_field_fft: pb0, npb)
+int dsmc_fft_line_blocks(int L, int R) { return dsmc_fft_fused_supported(L, R) ? R / 16 : 0; }
+
+cudaError_t launch_spin_blocks(float *S, float *SG, int L, int R, bool to_blocks, cudaStream_t st, uint64_t *launches) {
+    const size_t sites6 = 6 * (size_t)L * (L / 2), total = sites6 * (size_t)(R / 2);
+    const unsigned grid = (unsigned)((total + 255) / 256);
+    if (to_blocks) spin_blocks_kernel<true><<<grid, 256, 0, st>>>((float2 *)S, (float2 *)SG, sites6, R / 2);
+    else spin_blocks_kernel<false><<<grid, 256, 0, st>>>((float2 *)S, (float2 *)SG, sites6, R / 2);
+    ++*launches;
+    return cudaGetLastError();
+}
 
 cudaError_t launch_field_fft(const float *S, const float *AB, void *scratch, void *cache, float *H, int L, int R, int colour,
-                             bool *valid, int *zline, const MetropolisArgs *fuse, bool *configured, cudaStream_t st,
-                             uint64_t *launches) {
+                             bool *valid, int *zline, const MetropolisArgs *fuse, int pb0, int npb, float *SG, bool *configured,
+                             cudaStream_t st, uint64_t *launches) {
     if (fuse && (colour < 0 || !dsmc_fft_fused_supported(L, R))) return cudaErrorInvalidValue;
     FcParams p;
     p.S = S;
@@ -853,14 +898,16 @@ cudaError_t launch_field_fft(const float *S, const float *AB, void *scratch, voi
     p.P = R / 2;
     p.LZ = 1;
     p.PBZ = 1;
+    p.pb0 = 0;
+    p.SG = SG;
     p.colour = 0;
     const size_t ce = dsmc_fft_cache_elems(L, R);
     switch (L / 16) {
-        case 2: return launch_fftc<2>(p, (float2 *)cache, ce, colour, valid, zline, fuse, configured, st, launches);
-        case 4: return launch_fftc<4>(p, (float2 *)cache, ce, colour, valid, zline, fuse, configured, st, launches);
-        case 8: return launch_fftc<8>(p, (float2 *)cache, ce, colour, valid, zline, fuse, configured, st, launches);
-        case 16: return launch_fftc<16>(p, (float2 *)cache, ce, colour, valid, zline, fuse, configured, st, launches);
-        case 32: return launch_fftc<32>(p, (float2 *)cache, ce, colour, valid, zline, fuse, configured, st, launches);
+        case 2: return launch_fftc<2>(p, (float2 *)cache, ce, colour, valid, zline, fuse, pb0, npb, configured, st, launches);
+        case 4: return launch_fftc<4>(p, (float2 *)cache, ce, colour, valid, zline, fuse, pb0, npb, configured, st, launches);
+        case 8: return launch_fftc<8>(p, (float2 *)cache, ce, colour, valid, zline, fuse, pb0, npb, configured, st, launches);
+        case 16: return launch_fftc<16>(p, (float2 *)cache, ce, colour, valid, zline, fuse, pb0, npb, configured, st, launches);
+        case 32: return launch_fftc<32>(p, (float2 *)cache, ce, colour, valid, zline, fuse, pb0, npb, configured, st, launches);
     }
     return cudaErrorInvalidValue;
 }
