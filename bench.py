@@ -492,6 +492,12 @@ def run_cuda(args):
             "speedup_vs_direct_sum": ms_per_step / fft["run_ms_per_step"],
             "e2e": {"value": world * updates_per_step / fft["e2e_s"], "unit": "updates/s",
                     "h2d_bytes_per_step": int(s_host.numel() * 4), "d2h_bytes_per_step": int(out_host.numel() * 4)},
+            "sweep_roofline": {
+                "what": "the whole sweep of this path (field and decision fused) against the bytes a sweep must move: per "
+                        "half-sweep read every spin (12 B x N x R) and write the updated colour (12 B x N/2 x R)",
+                "bound": "hbm", "bytes_per_step": 2 * fft_bytes, "unit": "GB/s", "peak": hbm_peak, "peak_kind": hbm_kind,
+                "achieved": 2 * fft_bytes / (fft["run_ms_per_step"] * 1e-3) / 1e9,
+                "frac": 2 * fft_bytes / (fft["run_ms_per_step"] * 1e-3) / 1e9 / hbm_peak},
             "roofline": {"kernel": "fftc_x_forward + fftc_y + fftc_x_inverse", "bound": "hbm", "achieved": gbs,
                          "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak, "peak_kind": hbm_kind,
                          "ms_per_launch_group": fft["field_ms_per_launch_group"], "bytes_per_launch_group": fft_bytes,
