@@ -139,7 +139,7 @@ def run_reference(args):
     print(json.dumps(line))
 
 
-def metropolis_roofline(nbytes, in_sweep_ms, b2b_ms, n_b2b, hbm_peak, hbm_kind, updates):
+def metropolis_roofline(nbytes, in_sweep_ms, b2b_ms, n_b2b, hbm_peak, hbm_kind, updates, stream_ms):
     """The Metropolis kernel against HBM bandwidth by every timing there is: `frac` is the
     conservative one -- algorithmic bytes over the CUDA-event time of the launch where it really runs, inside a sweep,
     which includes the exposed launch latency (the event between the field kernel and this launch rules out the
@@ -157,6 +157,11 @@ def metropolis_roofline(nbytes, in_sweep_ms, b2b_ms, n_b2b, hbm_peak, hbm_kind, 
             "back_to_back": dict(both(b2b), ms_per_launch=b2b_ms, launches_timed=n_b2b,
                                  what="24 dependent launches over 3 contexts (300 MB: every launch finds its data "
                                       "evicted from L2), one event pair around the batch"),
+            "stream_same_footprint": dict(both(nbytes / (stream_ms * 1e-3) / 1e9), ms_per_launch=stream_ms,
+                                          metropolis_over_stream=stream_ms / b2b_ms,
+                                          what="dsmc_stream_footprint in the same rotation: the Metropolis kernel's grid, "
+                                               "loads and addresses, every thread's spins written back, no arithmetic -- "
+                                               "what the memory system delivers for this footprint"),
             "ncu": dict(algorithmic_bytes_over_ncu_time=both(nbytes / (ncu["time_us"] * 1e-6) / 1e9),
                         dram_bytes_over_ncu_time=both(ncu["dram_bytes"] / (ncu["time_us"] * 1e-6) / 1e9),
                         gpu__time_duration_us=ncu["time_us"], dram_bytes=ncu["dram_bytes"], profile=ncu["profile"],
@@ -370,6 +375,16 @@ def run_cuda(args):
     torch.cuda.synchronize(dev)
     metro_cold_ms = m0.elapsed_time(m1) / (rounds * len(ring))
     launches_metro = rounds * len(ring)
+    # the same rotation with the kernel that moves a half-sweep's bytes without its arithmetic (dsmc_stream_footprint):
+    # what the memory system delivers for this footprint, grid and access pattern -- the measured denominator
+    ring[0].dipole_field(1, want_output=False)
+    m0.record()
+    for k in range(rounds):
+        for cj in ring:
+            cj.stream_footprint(1)
+    m1.record()
+    torch.cuda.synchronize(dev)
+    stream_ms = m0.elapsed_time(m1) / (rounds * len(ring))
     for cj in others:
         cj.close()
     del others, ring
@@ -471,7 +486,7 @@ def run_cuda(args):
                      "ms_per_launch": field_ms, "flop_per_launch": flop_per_field},
         "dipole_field_gflops": field_tflops * 1e3,
         "roofline_metropolis": metropolis_roofline(metro_bytes, metro_ms, metro_cold_ms, launches_metro, hbm_peak, hbm_kind,
-                                                   (N // 2) * R),
+                                                   (N // 2) * R, stream_ms),
     }
     if fft is not None:
         # algorithmic HBM bytes of one half-sweep field by FFT: read every spin (12 B per site and replica),

@@ -270,6 +270,14 @@ int dsmc_field_kernel_supported(dsmc_ctx *ctx, int kind);
  * bench.py reports beside the derived SMs x 128 lanes x 2 x clock figure.  Synchronises.          */
 int dsmc_fp32_fma_peak(dsmc_ctx *ctx, double *tflops_out);
 
+/* Measured denominator of the Metropolis kernel's HBM roofline: one launch that moves the bytes of a checkerboard
+ * half-sweep of `colour` without its arithmetic -- the grid, the 18 128-bit loads per thread (own spins, h, four
+ * neighbours) and the addresses of the 4-replica Metropolis kernel, the thread's own spins always written back
+ * (unchanged bits: the state is not modified), no Philox, no trial, no dE.  Reads whatever the field array holds.
+ * Asynchronous; the caller times it (bench.py: in the same rotation over three contexts as the Metropolis kernel).
+ * Needs R % 4 == 0 (DSMC_EINVAL) and spins (DSMC_ESTATE).                                                    */
+int dsmc_stream_footprint(dsmc_ctx *ctx, int colour);
+
 /* The domain-wall counts of eq. 14 (the counts_out of dsmc_wall_observables, bit for bit) for callers
  * that cannot allocate device memory: code under CUDA graph capture, tight serving loops, harnesses that forbid
  * cudaMalloc.  Context-free: no dsmc_ctx, no workspace, no cudaMalloc / cudaFree / allocating library call.

@@ -969,6 +969,16 @@ int dsmc_set_debug(dsmc_ctx *ctx, int on) {
     return DSMC_OK;
 }
 
+int dsmc_stream_footprint(dsmc_ctx *ctx, int colour) {
+    ENTER_BOUND(ctx);
+    if (colour != 0 && colour != 1) return fail(ctx, DSMC_EINVAL, "colour must be 0 or 1");
+    if (!ctx->spins_set) return fail(ctx, DSMC_ESTATE, "spins not set");
+    if (ctx->R % 4 != 0) return fail(ctx, DSMC_EINVAL, "needs R % 4 == 0 (the shape of the 4-replica Metropolis kernel)");
+    const MetropolisArgs a = metropolis_args(ctx, colour, 0, 0, 0, nullptr, nullptr);
+    CU(launch_metropolis_stream(a, ctx->stream, &ctx->launches), "stream footprint launch");
+    return DSMC_OK;
+}
+
 int dsmc_set_timing(dsmc_ctx *ctx, int on) {
     if (!ctx) return DSMC_EINVAL;
     ctx->timing = on ? 1 : 0;

@@ -215,6 +215,8 @@ struct MetropolisArgs {
                    // random numbers (grids of at most one wave), 0 = at its top (larger grids)
 };
 cudaError_t launch_metropolis(const MetropolisArgs &a, cudaStream_t st, uint64_t *launches);
+// the loads and stores of metropolis4_kernel without its arithmetic (R % 4 == 0)
+cudaError_t launch_metropolis_stream(const MetropolisArgs &a, cudaStream_t st, uint64_t *launches);
 // the paper's stride-l sub-lattice pass: offset (ox, oy) in [0, l)^2, n = (L/l)^2 update sites
 void dsmc_sublattice_offset(uint64_t seed, uint64_t pass, int l, int *ox, int *oy);
 // scratch: 3 N R floats for the per-slab partial fields (the staging buffer)

@@ -123,6 +123,59 @@ __global__ void __launch_bounds__(128, MINB) metropolis4_kernel(const Metropolis
     }
 }
 
+// The memory traffic of metropolis4_kernel without its arithmetic (dsmc_stream_footprint: the measured denominator of
+// that kernel's roofline): same grid, same 18 128-bit loads per thread at the same addresses, the 3 stores of the
+// thread's own spins (unchanged bits) ALWAYS issued -- so it moves at least the bytes of a half-sweep in which every
+// move is accepted -- and no Philox, trial or dE.  The store is guarded by a condition on the loaded values that is never
+// false for finite inputs, which keeps the loads alive.
+template <int TY, int MINB>
+__global__ void __launch_bounds__(128, MINB) metropolis_stream_kernel(const MetropolisArgs p) {
+    constexpr int EX = 128 / TY;
+    const int Lh = p.L >> 1, RQ = p.R >> 2;
+    const int y = blockIdx.y * TY + (TY > 1 ? (int)(threadIdx.x / EX) : 0);
+    const uint32_t row4 = (uint32_t)(Lh * RQ);
+    const uint32_t e = blockIdx.x * EX + (TY > 1 ? threadIdx.x % EX : threadIdx.x);
+    pdl_trigger();
+    if (e >= row4) return;
+    pdl_wait();
+    const int i = (int)(e / (uint32_t)RQ), rq = (int)e - i * RQ;
+    const int par = (y + p.colour) & 1;
+    const size_t plane4 = ((size_t)p.L * Lh * p.R) >> 2;
+    const int yn = (y + 1 == p.L) ? 0 : y + 1, ys = (y == 0) ? p.L - 1 : y - 1;
+    const int i1 = par ? (i + 1 == Lh ? 0 : i + 1) : (i == 0 ? Lh - 1 : i - 1);
+    const uint32_t e1 = (uint32_t)(i1 * RQ + rq);
+    float4 *const Se = reinterpret_cast<float4 *>(p.S) + e;
+    const float4 *const He = reinterpret_cast<const float4 *>(p.H) + e;
+    const float4 *const Se1 = reinterpret_cast<const float4 *>(p.S) + e1;
+    const size_t u_own = (size_t)p.colour * 3 * plane4 + (size_t)y * row4;
+    const size_t u_oth = (size_t)(1 - p.colour) * 3 * plane4;
+    const size_t u_o0 = u_oth + (size_t)y * row4, u_on = u_oth + (size_t)yn * row4, u_os = u_oth + (size_t)ys * row4;
+    float4 *own = Se + u_own;
+    const float4 *hf = He + u_own, *o0 = Se + u_o0, *o1 = Se1 + u_o0, *on = Se + u_on, *os = Se + u_os;
+    f2 s[3][2], h[3][2], a[3][2], b[3][2], c[3][2], d[3][2];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        ld2(own + k * plane4, s[k][0], s[k][1]);
+        ld2(hf + k * plane4, h[k][0], h[k][1]);
+        ld2(o0 + k * plane4, a[k][0], a[k][1]);
+        ld2(o1 + k * plane4, b[k][0], b[k][1]);
+        ld2(on + k * plane4, c[k][0], c[k][1]);
+        ld2(os + k * plane4, d[k][0], d[k][1]);
+    }
+    f2 sum = f2_bc(0.0f);
+#pragma unroll
+    for (int k = 0; k < 3; ++k)
+#pragma unroll
+        for (int j = 0; j < 2; ++j) sum = f2_add(f2_add(sum, h[k][j]), f2_add(f2_add(a[k][j], b[k][j]), f2_add(c[k][j], d[k][j])));
+    float s0, s1;
+    f2_split(sum, s0, s1);
+    if (s0 + s1 != 1.2345678e30f) {
+#pragma unroll
+        for (int k = 0; k < 3; ++k)
+            *reinterpret_cast<ulonglong2 *>(own + k * plane4) = make_ulonglong2(s[k][0], s[k][1]);
+    }
+}
+
 // any R: one thread per (active site, replica), replica fastest
 __global__ void __launch_bounds__(256) metropolis1_kernel(const MetropolisArgs p, const RoundKeys rk) {
     const int Lh = p.L >> 1;
@@ -222,6 +275,16 @@ cudaError_t launch_metropolis(const MetropolisArgs &a, cudaStream_t st, uint64_t
     }
     ++*launches;
     return err;
+}
+
+cudaError_t launch_metropolis_stream(const MetropolisArgs &a, cudaStream_t st, uint64_t *launches) {
+    if (a.R % 4 != 0 || a.L > 65535) return cudaErrorInvalidValue;
+    constexpr int TY = 2, MINB = 7;                             // the launch shape of launch_metropolis
+    const unsigned per_row = (unsigned)((a.L / 2) * (a.R / 4));
+    dim3 grid((per_row + 128 / TY - 1) / (128 / TY), a.L / TY);
+    cudaError_t err = launch_pdl(metropolis_stream_kernel<TY, MINB>, grid, dim3(128), 0, st, a);
+    ++*launches;
+    return err != cudaSuccess ? err : cudaGetLastError();
 }
 
 cudaError_t launch_init_spins(float *S, int L, int R, int mode, uint64_t seed, uint32_t r_off, cudaStream_t st,

@@ -59,6 +59,7 @@ ABI = [
     ("dsmc_select_field_kernel", _i, [_vp, _i]),
     ("dsmc_field_kernel_supported", _i, [_vp, _i]),
     ("dsmc_fp32_fma_peak", _i, [_vp, _vp]),
+    ("dsmc_stream_footprint", _i, [_vp, _i]),
     ("dsmc_wall_counts_noalloc", _i, [_vp, _i, _i, _vp, _vp, ctypes.c_char_p, _sz]),
     ("dsmc_destroy", _i, [_vp]),
     ("dsmc_last_error", ctypes.c_char_p, [_vp]),
@@ -331,6 +332,10 @@ class Dsmc:
         out = ctypes.c_double(0.0)
         self._check(self.lib.dsmc_fp32_fma_peak(self._h, ctypes.addressof(out)))
         return float(out.value)
+
+    def stream_footprint(self, colour):
+        """One launch that moves a Metropolis half-sweep's bytes without its arithmetic (roofline denominator)."""
+        self._check(self.lib.dsmc_stream_footprint(self._h, int(colour)))
 
     def set_replica_offset(self, first_replica):
         """This context holds replicas first_replica ... of a larger ladder (bit-reproducible sharding)."""
