@@ -801,3 +801,34 @@ def test_run_recorded_matches_separate_calls(dsmc_mod, L, R, every, fft):
         a.run_recorded(None, 17, 0, 2, 0)          # every < 1
     a.close()
     b.close()
+
+
+@pytest.mark.gpu
+def test_stream_footprint_leaves_the_state_alone(dsmc_mod):
+    """dsmc_stream_footprint (bench.py's measured denominator of the Metropolis roofline) rewrites every spin of the
+    colour with the bits it read: the state, and a run continued from it, must not change."""
+    from paper_1211_6234_b200 import inputs
+    L, R = 64, 16
+    T = np.linspace(0.3, 1.5, R).astype(np.float32)
+    a = dsmc_mod.Dsmc(L, R, J=1.0, g=0.2, K2=0.5, K4=0.1)
+    b = dsmc_mod.Dsmc(L, R, J=1.0, g=0.2, K2=0.5, K4=0.1)
+    a.build_tensor(dsmc_mod.DSMC_W_EWALD)
+    b.set_tensor(a.get_tensor())
+    s0 = inputs.random_spins(L, R, 77)
+    for c in (a, b):
+        c.set_spins(s0)
+        c.halfsweep(T, 5, 0)
+    for colour in (0, 1, 1, 0):
+        a.stream_footprint(colour)
+    assert np.array_equal(a.get_spins(), b.get_spins())
+    for c in (a, b):
+        c.halfsweep(T, 5, 1)
+    assert np.array_equal(a.get_spins(), b.get_spins())
+    with pytest.raises(dsmc_mod.DsmcError):
+        a.stream_footprint(2)
+    c5 = dsmc_mod.Dsmc(12, 5)
+    c5.set_spins(inputs.random_spins(12, 5, 1))
+    with pytest.raises(dsmc_mod.DsmcError):
+        c5.stream_footprint(0)                                  # R % 4 != 0
+    for c in (a, b, c5):
+        c.close()
