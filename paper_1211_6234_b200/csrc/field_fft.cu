@@ -372,6 +372,7 @@ __global__ void __launch_bounds__(N2X >= 16 ? 384 : 192, N2X >= 16 ? 2 : 4) fftc
         // apart) or, for a chain of the branched replay, the chain's line block in the block-major copy SG (dense)
         const bool dense = p.SG != nullptr;
         const int Pe = dense ? LN : p.P;
+        const int pr_sub = dense ? pb * LN : 0;               // pair index within the spin record: pr, or the lane in the block's copy
         const size_t planeP = (size_t)L * Lh * Pe;
         f2 *S2 = dense ? reinterpret_cast<f2 *>(p.SG) + (size_t)pb * 6 * planeP : reinterpret_cast<f2 *>(ma.S);
         const f2 *X2 = reinterpret_cast<const f2 *>(X0);
@@ -384,7 +385,7 @@ __global__ void __launch_bounds__(N2X >= 16 ? 384 : 192, N2X >= 16 ? 2 : 4) fftc
         for (int item = tid; item < Lh * LN; item += nthr) {
             const int i = item / LN, ln = item - i * LN, pr = pb * LN + ln;
             const int i1 = odd_row ? (i + 1 == Lh ? 0 : i + 1) : (i == 0 ? Lh - 1 : i - 1);
-            const unsigned e = (unsigned)(i * Pe) + (dense ? ln : pr), e1 = (unsigned)(i1 * Pe) + (dense ? ln : pr);
+            const unsigned e = (unsigned)(i * Pe + pr - pr_sub), e1 = (unsigned)(i1 * Pe + pr - pr_sub);
             f2 s[3], nb[3], h[3];
 #pragma unroll
             for (int k = 0; k < 3; ++k) {
