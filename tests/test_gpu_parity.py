@@ -527,7 +527,7 @@ def test_field_parity_tiled_large_L(dsmc_mod, oracle, L, R):
     big.close()
 
 
-@pytest.mark.parametrize("L,R", [(256, 64), (32, 8), (64, 16), (32, 16), (512, 16), (64, 48), (32, 128)])
+@pytest.mark.parametrize("L,R", [(256, 64), (32, 8), (64, 16), (32, 16), (512, 16), (64, 48), (64, 128), (32, 64)])
 @pytest.mark.parametrize("flip", [False, True])
 def test_benchmarked_metropolis_instantiation_is_the_tested_one(dsmc_mod, L, R, flip):
     """The lock-step tests pass accept_out / margin_out, which selects the hooked instantiation of the 4-replica
@@ -537,8 +537,9 @@ def test_benchmarked_metropolis_instantiation_is_the_tested_one(dsmc_mod, L, R, 
     closes the chain oracle -> hooked kernel -> production kernels (eq. 7).  With the FFT field and
     R % 16 == 0 the production path is the FUSED one (the decision taken inside the field's last pass, field_fft.cu:
     fftc_row_update_kernel), the hooked path field kernels + metropolis4_kernel: the same test ties those together.
-    From R = 32 up the replayed graph of that path runs the groups of 16 replicas as 2, 3 or 4 independent chains of
-    launches (dsmc_api.cu: build_sweep_graph; R = 64, 48, 128 here), the plain calls as one."""
+    From R = 32 and L = 64 up dsmc_run replays that path as independent chains of launches, one per group (or several
+    groups) of 16 replicas, on a block-major copy of the spins (dsmc_api.cu: build_sweep_graph, replay_sweep_graph): 4
+    chains at (256, 64), 3 at (64, 48), 8 at (64, 128), one at (32, 64); the plain calls always run as one."""
     from paper_1211_6234_b200 import inputs
     T = np.linspace(0.1, 2.0, R).astype(np.float32)
     flags = dsmc_mod.DSMC_TRIAL_FLIP if flip else 0
