@@ -664,7 +664,7 @@ def test_ensemble_statistics_parity(dsmc_mod, oracle, fft):
 
 
 @pytest.mark.parametrize("L,R,kind,flip", [(32, 8, 1, False), (32, 8, 2, False), (12, 5, 0, False), (64, 16, 2, False),
-                                           (32, 8, 2, True), (12, 5, 0, True)])
+                                           (32, 8, 2, True), (12, 5, 0, True), (64, 32, 2, False), (64, 32, 2, True)])
 def test_run_graph_replay_is_bit_identical(dsmc_mod, L, R, kind, flip):
     """dsmc_run / dsmc_run_ex replay a captured CUDA graph of 8 sweeps with the step counter on the device: the
     trajectory must be bit-identical to calling dsmc_halfsweep step by step (odd first step, ragged
