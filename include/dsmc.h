@@ -24,8 +24,10 @@
  *   E = -J sum_bonds s.s - sum_n (K2 s_z^2 + K4 s_z^4) + (g/2) sum_n s_n.h_n
  *
  * Error behaviour: every int-returning call returns DSMC_OK (0) or a negative
- * code; no exceptions, no abort, no global state.  dsmc_last_error() returns a
- * message owned by the context (valid until the next call on that context).
+ * code; no exceptions, no abort, no global state (the one exception is the static
+ * scratch array of the context-free dsmc_wall_counts_noalloc, documented there).
+ * dsmc_last_error() returns a message owned by the context (valid until the next
+ * call on that context).
  */
 #ifndef DSMC_H
 #define DSMC_H
